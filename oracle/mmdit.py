@@ -1,0 +1,190 @@
+"""Oracle: the Qwen-Image-shaped MMDiT forward pass in fp64 (TEST INFRASTRUCTURE).
+
+"each [denoising step] requiring a full forward pass through the DiT backbone"
+(PAPER.md:59); model = "Qwen-Image 20B".  The paper gives no block
+definition; this file is reading S4-S7 of DESIGN.md written out
+step by step, one sequence at a time, no blocking, fusion or reordering.
+
+All Linear layers are y = x W^T + b with W [out, in].  Joint sequence order is text tokens
+first, then image tokens.  Inputs are fp64 arrays holding the (already dtype-rounded) values
+the CUDA path receives.
+
+Matmul back ends: "blas" = numpy @ (OpenBLAS dgemm); "einsum" = numpy's own C loops with
+optimize=False (no BLAS).  Tests cross-check the two and brute-force tiny cases in Python.
+"""
+from __future__ import annotations
+
+import math
+from typing import Dict, List, Sequence, Tuple
+
+import numpy as np
+
+Array = np.ndarray
+
+
+def linear(x: Array, w: Array, b: Array | None, mode: str = "blas") -> Array:
+    """y = x W^T + b ; x [n, in], W [out, in]."""
+    if mode == "blas":
+        y = x @ w.T
+    elif mode == "einsum":
+        y = np.einsum("ni,oi->no", x, w, optimize=False)
+    else:
+        raise ValueError(mode)
+    return y if b is None else y + b
+
+
+def silu(x: Array) -> Array:
+    return x / (1.0 + np.exp(-x))
+
+
+def gelu_tanh(x: Array) -> Array:
+    """GELU_tanh(x) = x/2 (1 + tanh(sqrt(2/pi) (x + 0.044715 x^3)))  (reading S4)."""
+    return 0.5 * x * (1.0 + np.tanh(math.sqrt(2.0 / math.pi) * (x + 0.044715 * x ** 3)))
+
+
+def layer_norm(x: Array, eps: float) -> Array:
+    """LayerNorm over the last axis, biased variance, no affine (C5 step 2)."""
+    mu = x.mean(axis=-1, keepdims=True)
+    var = ((x - mu) ** 2).mean(axis=-1, keepdims=True)
+    return (x - mu) / np.sqrt(var + eps)
+
+
+def rms_norm(x: Array, gain: Array, eps: float) -> Array:
+    """x / sqrt(mean(x^2) + eps) * gain over the last axis (C5 step 4, C7)."""
+    ms = (x ** 2).mean(axis=-1, keepdims=True)
+    return x / np.sqrt(ms + eps) * gain
+
+
+def timestep_embedding(t: float) -> Array:
+    """Sinusoidal-256 (C4): a = 1000 t, f_i = exp(-ln(10000) i / 128), [cos(a f) ; sin(a f)]."""
+    a = 1000.0 * float(t)
+    f = np.exp(-math.log(10000.0) * np.arange(128, dtype=np.float64) / 128.0)
+    return np.concatenate([np.cos(a * f), np.sin(a * f)])
+
+
+def time_conditioning(t: float, g: Dict[str, Array], mode: str = "blas") -> Tuple[Array, Array]:
+    """temb = W2 SiLU(W1 e(t) + b1) + b2 ; c = SiLU(temb).  Returns (temb, c), each [D]."""
+    e = timestep_embedding(t)[None, :]
+    hid = silu(linear(e, g["time_w1"], g["time_b1"], mode))
+    temb = linear(hid, g["time_w2"], g["time_b2"], mode)[0]
+    return temb, silu(temb)
+
+
+def rope_positions(grid_h: int, grid_w: int, n_txt: int) -> Array:
+    """[S, 3] integer positions (t, h, w) of the joint sequence, text first (C6)."""
+    pos = np.zeros((n_txt + grid_h * grid_w, 3), dtype=np.float64)
+    base = max(grid_h // 2, grid_w // 2)
+    for j in range(n_txt):
+        pos[j, :] = base + j
+    for r in range(grid_h):
+        for c in range(grid_w):
+            pos[n_txt + r * grid_w + c] = (0, r - (grid_h + 1) // 2, c - (grid_w + 1) // 2)
+    return pos
+
+
+def rope_table(grid_h: int, grid_w: int, n_txt: int, rope_pairs: Sequence[int], theta: float,
+               shift: Tuple[int, int] = (0, 0)) -> Tuple[Array, Array]:
+    """cos, sin [S, d_h/2]: pair i belongs to axis a(i) (t pairs, then h, then w) with frequency
+    theta**(-i'/n_a), i' the index inside the axis; angle = pos_a * freq (C6).  `shift` moves the
+    image grid by (dr, dc) - used by the relative-position pin only."""
+    pos = rope_positions(grid_h, grid_w, n_txt)
+    pos[n_txt:, 1] += shift[0]
+    pos[n_txt:, 2] += shift[1]
+    cols = []
+    for axis, n_a in enumerate(rope_pairs):
+        freq = np.asarray([theta ** (-(i / n_a)) for i in range(n_a)], dtype=np.float64)
+        cols.append(pos[:, axis:axis + 1] * freq[None, :])
+    ang = np.concatenate(cols, axis=1)
+    return np.cos(ang), np.sin(ang)
+
+
+def apply_rope(x: Array, cos: Array, sin: Array) -> Array:
+    """x [S, H, d_h]; rotate interleaved pairs (2i, 2i+1) by the angle of (token s, pair i) (C5 step 5)."""
+    xe, xo = x[..., 0::2], x[..., 1::2]
+    c, s = cos[:, None, :], sin[:, None, :]
+    out = np.empty_like(x)
+    out[..., 0::2] = xe * c - xo * s
+    out[..., 1::2] = xe * s + xo * c
+    return out
+
+
+def attention(q: Array, k: Array, v: Array) -> Array:
+    """softmax(Q K^T / sqrt(d_h)) V per head, all S keys, no mask (C5 step 6). q,k,v [S, H, d_h]."""
+    S, H, dh = q.shape
+    out = np.empty_like(q)
+    for h in range(H):
+        logits = (q[:, h, :] @ k[:, h, :].T) / math.sqrt(dh)
+        logits = logits - logits.max(axis=1, keepdims=True)
+        p = np.exp(logits)
+        p = p / p.sum(axis=1, keepdims=True)
+        out[:, h, :] = p @ v[:, h, :]
+    return out
+
+
+def modulation(c: Array, w: Array, b: Array, mode: str = "blas") -> List[Array]:
+    """m = W_mod c + b in R^{6D}, split (shift1, scale1, gate1, shift2, scale2, gate2) (C5 step 1)."""
+    m = linear(c[None, :], w, b, mode)[0]
+    return list(m.reshape(6, -1))
+
+
+def block_forward(h_img: Array, h_txt: Array, c: Array, bw: Dict[str, Array], *, n_heads: int,
+                  cos: Array, sin: Array, ln_eps: float = 1e-6, rms_eps: float = 1e-6,
+                  mode: str = "blas", trace: Dict[str, Array] | None = None) -> Tuple[Array, Array]:
+    """One joint block for one sequence (C5 steps 1-8).  h_img [N_img, D], h_txt [N_txt, D], c = SiLU(temb) [D]."""
+    n_txt = h_txt.shape[0]
+    D = h_img.shape[1]
+    dh = D // n_heads
+    h = {"img": h_img, "txt": h_txt}
+    mod, q, k, v = {}, {}, {}, {}
+    for s in ("txt", "img"):
+        mod[s] = modulation(c, bw[f"{s}.mod_w"], bw[f"{s}.mod_b"], mode)
+        shift1, scale1 = mod[s][0], mod[s][1]
+        y = layer_norm(h[s], ln_eps) * (1.0 + scale1) + shift1
+        qkv = linear(y, bw[f"{s}.qkv_w"], bw[f"{s}.qkv_b"], mode)
+        n = qkv.shape[0]
+        q[s] = rms_norm(qkv[:, 0 * D:1 * D].reshape(n, n_heads, dh), bw[f"{s}.q_gain"], rms_eps)
+        k[s] = rms_norm(qkv[:, 1 * D:2 * D].reshape(n, n_heads, dh), bw[f"{s}.k_gain"], rms_eps)
+        v[s] = qkv[:, 2 * D:3 * D].reshape(n, n_heads, dh)
+        if trace is not None:
+            trace[f"{s}.y1"], trace[f"{s}.qkv"] = y, qkv
+    Q = apply_rope(np.concatenate([q["txt"], q["img"]], axis=0), cos, sin)
+    K = apply_rope(np.concatenate([k["txt"], k["img"]], axis=0), cos, sin)
+    V = np.concatenate([v["txt"], v["img"]], axis=0)
+    o = attention(Q, K, V).reshape(-1, D)
+    if trace is not None:
+        trace["Q"], trace["K"], trace["V"], trace["o"] = Q, K, V, o
+    o_s = {"txt": o[:n_txt], "img": o[n_txt:]}
+    out = {}
+    for s in ("txt", "img"):
+        _, _, gate1, shift2, scale2, gate2 = mod[s]
+        x = h[s] + gate1 * linear(o_s[s], bw[f"{s}.out_w"], bw[f"{s}.out_b"], mode)
+        y2 = layer_norm(x, ln_eps) * (1.0 + scale2) + shift2
+        u = gelu_tanh(linear(y2, bw[f"{s}.fc1_w"], bw[f"{s}.fc1_b"], mode))
+        out[s] = x + gate2 * linear(u, bw[f"{s}.fc2_w"], bw[f"{s}.fc2_b"], mode)
+        if trace is not None:
+            trace[f"{s}.h_attn"], trace[f"{s}.u"] = x, u
+    return out["img"], out["txt"]
+
+
+def text_input(text_emb: Array, g: Dict[str, Array], rms_eps: float = 1e-6, mode: str = "blas") -> Array:
+    """h_txt^0 = RMSNorm(text_emb; gain) W_txt^T + b, once per prompt (C7)."""
+    return linear(rms_norm(text_emb, g["txt_gain"], rms_eps), g["txt_in_w"], g["txt_in_b"], mode)
+
+
+def dit_velocity(x: Array, t: float, h_txt0: Array, g: Dict[str, Array], blocks: List[Dict[str, Array]], *,
+                 n_heads: int, cos: Array, sin: Array, ln_eps: float = 1e-6, rms_eps: float = 1e-6,
+                 mode: str = "blas", trace: List[Array] | None = None) -> Array:
+    """v = DiT(x, t, text) for one sequence.  x [N_img, C] -> v [N_img, C] (C7)."""
+    _, c = time_conditioning(t, g, mode)
+    h_img = linear(x, g["img_in_w"], g["img_in_b"], mode)
+    h_txt = h_txt0
+    for bw in blocks:
+        h_img, h_txt = block_forward(h_img, h_txt, c, bw, n_heads=n_heads, cos=cos, sin=sin,
+                                     ln_eps=ln_eps, rms_eps=rms_eps, mode=mode)
+        if trace is not None:
+            trace.append(h_img)
+    m_f = linear(c[None, :], g["final_mod_w"], g["final_mod_b"], mode)[0]
+    D = h_img.shape[1]
+    scale_f, shift_f = m_f[:D], m_f[D:]
+    y = layer_norm(h_img, ln_eps) * (1.0 + scale_f) + shift_f
+    return linear(y, g["proj_w"], g["proj_b"], mode)
