@@ -1,0 +1,175 @@
+/* spot.h - C ABI of the B200-native SPOTLIGHT seed-exploration rollout (libspot.so).
+ *
+ * What the library computes (PAPER.md = the paper text, arxiv 2606.19004):
+ *   PAPER.md:59  (s2.1) a DiT "starts from random Gaussian noise and refines a latent
+ *                representation over a fixed number of denoising steps ..., each requiring a full
+ *                forward pass through the DiT backbone";
+ *   PAPER.md:61  (s2.1) "K samples from each of P prompts by running denoising with K distinct noise
+ *                seeds ... Each sample is scored ..., yielding a per-sample scalar reward r_k";
+ *   PAPER.md:229 (s5)   "top-k/bottom-k strategy over per-prompt exploration rewards, retaining the
+ *                highest- and lowest-scoring seeds"; "top and bottom K/2 by reward";
+ *   PAPER.md:175 (s4.3.2) the per-prompt reward standard deviation sigma_g fed to the bandit planner.
+ * The paper fixes only this outer shape; every inner definition (Philox4x32-10 + Box-Muller, the
+ * Qwen-Image-shaped joint block, 2-D RoPE, Euler sampler, linear-probe reward) is a reading listed
+ * in DESIGN.md (S1-S16) that binds this library and the fp64 oracle alike.
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  All matrices are row-major;
+ *     every Linear is y = x W^T + b with W stored [out_features, in_features].
+ *   - Ownership: the caller owns every buffer.  The library allocates only inside spot_ctx (host
+ *     structs, a small device RoPE table, TMA descriptors) and frees it in spot_destroy.  Weights
+ *     are BORROWED for the life of the context.
+ *   - Errors: every call returns spot_status; nothing throws, aborts or prints.  Argument errors
+ *     are detected before any launch.  Launch failures map to SPOT_ERR_CUDA and the cudaError_t
+ *     is retrievable with spot_last_cuda_error().
+ *   - Asynchrony: device work is enqueued on the caller's stream (a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream).  Only spot_explore_host synchronises.
+ *   - Determinism: same inputs => bit-identical outputs run to run; the result for sequence b does
+ *     not depend on the batch size, its position in the batch, or the other sequences.
+ *   - There is no CPU fallback: on a machine without an sm_100 device every compute call returns
+ *     SPOT_ERR_ARCH.
+ */
+#ifndef SPOT_H_
+#define SPOT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SPOT_OK = 0,
+  SPOT_ERR_NULL = 1,          /* a required pointer is NULL */
+  SPOT_ERR_SHAPE = 2,         /* inconsistent or unsupported sizes */
+  SPOT_ERR_DTYPE = 3,         /* unknown spot_dtype */
+  SPOT_ERR_ALIGN = 4,         /* a pointer is not 16-byte aligned */
+  SPOT_ERR_WORKSPACE = 5,     /* workspace smaller than spot_workspace_bytes() */
+  SPOT_ERR_ARCH = 6,          /* no CUDA device of compute capability 10.x */
+  SPOT_ERR_CUDA = 7,          /* a CUDA call failed; see spot_last_cuda_error() */
+  SPOT_ERR_UNIMPLEMENTED = 8
+} spot_status;
+
+typedef enum { SPOT_F32 = 0, SPOT_BF16 = 1 } spot_dtype;
+
+/* Model/workload shape (plain data, copied at spot_create).  n_img = grid_h * grid_w image tokens,
+ * joint sequence S = n_txt + n_img with the text tokens FIRST.  hidden == n_heads * head_dim;
+ * rope_pairs (t, h, w) must sum to head_dim / 2; head_dim must be 64 or 128; hidden % 128 == 0;
+ * latent_ch % 4 == 0; txt_dim == hidden. */
+typedef struct {
+  int32_t n_blocks, hidden, n_heads, head_dim, mlp_hidden;
+  int32_t grid_h, grid_w, n_txt, latent_ch, txt_dim;
+  int32_t rope_pairs[3];
+  float rope_theta, ln_eps, rms_eps;
+  spot_dtype dtype;   /* of weights, biases, gains, text_emb and inter-kernel activations; latents,
+                         velocity, rewards, modulation vectors, the residual stream and all
+                         accumulators/statistics are always fp32 */
+} spot_config;
+
+/* Per-stream block weights, device pointers of `dtype`, 16-byte aligned. */
+typedef struct {
+  const void *mod_w, *mod_b;    /* [6D, D], [6D]: (shift1, scale1, gate1, shift2, scale2, gate2) */
+  const void *qkv_w, *qkv_b;    /* [3D, D], [3D]: rows q | k | v, head h owns rows h*d_h..(h+1)*d_h-1 */
+  const void *q_gain, *k_gain;  /* [d_h] each */
+  const void *out_w, *out_b;    /* [D, D], [D] */
+  const void *fc1_w, *fc1_b;    /* [F, D], [F] */
+  const void *fc2_w, *fc2_b;    /* [D, F], [D] */
+} spot_stream_weights;
+
+typedef struct { spot_stream_weights s[2]; } spot_block_weights;   /* [0] = image, [1] = text */
+
+typedef struct {
+  const void *time_w1, *time_b1, *time_w2, *time_b2;   /* [D,256], [D], [D,D], [D] */
+  const void *img_in_w, *img_in_b;                     /* [D,C], [D] */
+  const void *txt_gain, *txt_in_w, *txt_in_b;          /* [txt_dim], [D,txt_dim], [D] */
+  const spot_block_weights *blocks;                    /* HOST array of n_blocks structs (copied) */
+  const void *final_mod_w, *final_mod_b;               /* [2D,D], [2D]: (scale_f, shift_f) */
+  const void *proj_w, *proj_b;                         /* [C,D], [C] */
+} spot_weights;
+
+typedef struct spot_ctx spot_ctx;
+
+/* Options for spot_set_option. */
+typedef enum {
+  SPOT_OPT_GEMM_IMPL = 0,   /* 0 = auto (tcgen05 for bf16), 1 = force the SIMT FFMA GEMM */
+  SPOT_OPT_ATTN_IMPL = 1    /* 0 = auto (tcgen05 for bf16, d_h = 128), 1 = force the SIMT attention */
+} spot_option;
+
+/* Validates cfg and w, builds the RoPE table (S5) and returns a context.  max_seqs bounds
+ * n_seqs / n_prompts*seeds_per_prompt of later calls.  Does not synchronise. */
+spot_status spot_create(const spot_config *cfg, const spot_weights *w, int max_seqs, spot_ctx **out);
+spot_status spot_destroy(spot_ctx *ctx);
+spot_status spot_set_option(spot_ctx *ctx, spot_option opt, int value);
+/* Bytes of device workspace needed by spot_dit_block_forward / spot_dit_denoise / spot_explore*
+ * for n_seqs sequences and up to n_steps Euler steps (n_prompts <= n_seqs is assumed). */
+spot_status spot_workspace_bytes(const spot_ctx *ctx, int n_seqs, int n_steps, size_t *bytes);
+const char *spot_status_string(spot_status s);
+int spot_last_cuda_error(const spot_ctx *ctx);          /* cudaError_t of the last failed CUDA call */
+const char *spot_version(void);
+
+/* (1) Seeds -> N(0,1).  PAPER.md:59 "starts from random Gaussian noise", :61 "K distinct noise
+ * seeds", :251 "deterministic random seed" per sample.  DESIGN.md S1-S3: Philox4x32-10 with
+ * key = (lo32, hi32)(seed) and counter = (lo32(j), hi32(j), stream_id, 0) for the 4-element block
+ * j = e/4, then Box-Muller on 24-bit uniforms.  d_out[b*elems_per_seed + e], fp32.
+ * elems_per_seed must be a positive multiple of 4; d_out 16-byte aligned.  n_seeds == 0 is a no-op. */
+spot_status spot_noise_from_seeds(const uint64_t *d_seeds, int n_seeds, int64_t elems_per_seed,
+                                  uint32_t stream_id, float *d_out, void *cuda_stream);
+/* The raw Philox words of the same elements (u32 per element), for bit-exact checks. */
+spot_status spot_philox_words(const uint64_t *d_seeds, int n_seeds, int64_t elems_per_seed,
+                              uint32_t stream_id, uint32_t *d_out, void *cuda_stream);
+
+/* (2) One joint text+image block (S4-S6) for n_seqs sequences.
+ * d_h_img [n_seqs, n_img, D], d_h_txt [n_seqs, n_txt, D] of cfg.dtype; d_temb [D] fp32 is the
+ * PRE-SiLU conditioning vector (the block applies c = SiLU(temb) and its own modulation Linear).
+ * Outputs have the input shapes and dtype; in-place (out == in) is allowed. */
+spot_status spot_dit_block_forward(spot_ctx *ctx, int block, int n_seqs,
+                                   const void *d_h_img, const void *d_h_txt, const float *d_temb,
+                                   void *d_out_img, void *d_out_txt,
+                                   void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
+/* (3) n_steps flow-matching Euler steps x <- x + (t_{i+1} - t_i) v(x, t_i) (DESIGN.md
+ * S8).  d_latents [P*K, n_img, C] fp32, updated in place; sequence b belongs to prompt b / K.
+ * d_text_emb [P, n_txt, txt_dim] of cfg.dtype.  h_timesteps is a HOST array of n_steps + 1 floats
+ * (read before the call returns).  Resume: calling with h_timesteps + i and n_steps - i continues
+ * a run from the latents after step i (the paper's committed state "latent tensors and scheduler
+ * metadata"). */
+spot_status spot_dit_denoise(spot_ctx *ctx, int n_prompts, int seeds_per_prompt,
+                             float *d_latents, const void *d_text_emb,
+                             const float *h_timesteps, int n_steps,
+                             void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
+/* (4) Rewards and per-prompt statistics/selection (S9-S12).
+ * r_b = <probe, latents_b> / sqrt(n_img*C); per prompt: mean, population std; top-k by (reward
+ * descending, index ascending) and bottom-k by (reward ascending, index ascending); indices are
+ * positions 0..K-1 inside the prompt group.  argmax = d_top[p*k], argmin = d_bottom[p*k].
+ * Requires 0 <= 2*k_select <= K <= 1024.  d_top/d_bottom may be NULL when k_select == 0. */
+spot_status spot_seed_rewards(spot_ctx *ctx, int n_prompts, int seeds_per_prompt,
+                              const float *d_latents, const float *d_probe, int k_select,
+                              float *d_rewards /*[P*K]*/, float *d_stats /*[P,2] mean,std*/,
+                              int32_t *d_top /*[P,k]*/, int32_t *d_bottom /*[P,k]*/, void *cuda_stream);
+
+/* Whole exploration rollout on device buffers: (1) with stream_id 0 -> (3) with the reward
+ * reduction fused into the last Euler update -> selection of (4).  d_latents is an output. */
+spot_status spot_explore(spot_ctx *ctx, int n_prompts, int seeds_per_prompt,
+                         const uint64_t *d_seeds, const void *d_text_emb,
+                         const float *h_timesteps, int n_steps, const float *d_probe, int k_select,
+                         float *d_latents, float *d_rewards, float *d_stats,
+                         int32_t *d_top, int32_t *d_bottom,
+                         void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
+/* The same with HOST buffers: copies seeds, text_emb and probe to the device, runs spot_explore,
+ * copies rewards, stats, top/bottom (and the final latents if h_latents != NULL) back, and
+ * synchronises the stream.  Host buffers should be pinned for full copy bandwidth.  The staging
+ * area lives at the end of the workspace (accounted for by spot_workspace_bytes). */
+spot_status spot_explore_host(spot_ctx *ctx, int n_prompts, int seeds_per_prompt,
+                              const uint64_t *h_seeds, const void *h_text_emb,
+                              const float *h_timesteps, int n_steps, const float *h_probe, int k_select,
+                              float *h_latents, float *h_rewards, float *h_stats,
+                              int32_t *h_top, int32_t *h_bottom,
+                              void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPOT_H_ */

@@ -1,0 +1,61 @@
+/* spot_kernels.h - kernel-level entry points of libspot.so.
+ *
+ * The four north-star calls live in spot.h.  The calls below expose the individual kernels of the
+ * hot path so that the tests can compare each one with the oracle and
+ * bench.py can time each one against its roofline.  Same conventions as spot.h: device pointers,
+ * row-major, caller-owned buffers, asynchronous on `cuda_stream`, no CPU fallback.
+ */
+#ifndef SPOT_KERNELS_H_
+#define SPOT_KERNELS_H_
+
+#include "spot.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { SPOT_EPI_BIAS = 0, SPOT_EPI_BIAS_GELU = 1, SPOT_EPI_GATE_RESIDUAL = 2 } spot_epilogue;
+typedef enum { SPOT_IMPL_AUTO = 0, SPOT_IMPL_SIMT = 1, SPOT_IMPL_TCGEN05 = 2 } spot_impl;
+
+/* Linear layer y = x W^T + b with a fused epilogue (north_star (b); S4 steps 3, 7, 8).
+ *   d_a [M, K], d_w [N, K], d_bias [N] of `dtype`.
+ *   SPOT_EPI_BIAS:          d_out [M, N] (dtype)  = y
+ *   SPOT_EPI_BIAS_GELU:     d_out [M, N] (dtype)  = GELU_tanh(y)
+ *   SPOT_EPI_GATE_RESIDUAL: d_residual [M, N] fp32 += d_gate[N] (fp32) * y    (d_out unused)
+ * SPOT_IMPL_TCGEN05 requires dtype bf16, K % 8 == 0, N % 32 == 0 and returns SPOT_ERR_SHAPE otherwise;
+ * SPOT_IMPL_SIMT requires K % 16 == 0. */
+spot_status spot_linear(spot_dtype dtype, spot_impl impl, spot_epilogue epi, const void *d_a, int64_t M, int64_t K,
+                        const void *d_w, int64_t N, const void *d_bias, const float *d_gate, float *d_residual,
+                        void *d_out, void *cuda_stream);
+
+/* y = LayerNorm(h) * (1 + scale) + shift over the last axis, biased variance, no affine (S4
+ * step 2).  d_h [M, D] fp32 (residual stream), d_shift/d_scale [D] fp32, d_out [M, D] of `dtype`.
+ * D must be 128 * {1,2,4,8,12,16,24,32}. */
+spot_status spot_ln_modulate(spot_dtype dtype, const float *d_h, int64_t M, int64_t D, const float *d_shift,
+                             const float *d_scale, float eps, void *d_out, void *cuda_stream);
+
+/* In place on d_qkv [B, S, 3, H, d_h]: q <- RoPE(RMSNorm(q) * gain), k likewise; v untouched (north_star (c);
+ * DESIGN.md S4 steps 4-5).  Tokens s < n_txt use the text gains.  d_cos/d_sin [S, d_h/2] fp32. */
+spot_status spot_qk_norm_rope(spot_dtype dtype, void *d_qkv, int B, int S, int H, int head_dim, int n_txt,
+                              const void *d_q_gain_img, const void *d_k_gain_img, const void *d_q_gain_txt,
+                              const void *d_k_gain_txt, const float *d_cos, const float *d_sin, float eps,
+                              void *cuda_stream);
+
+/* O = softmax(Q K^T / sqrt(d_h)) V over all S keys per (sequence, head), no mask (north_star (d); DESIGN.md
+ * S4 step 6).  d_qkv [B, S, 3, H, d_h] -> d_out [B, S, H * d_h], both `dtype`.  SPOT_IMPL_TCGEN05 requires
+ * bf16, d_h = 128. */
+spot_status spot_attention(spot_dtype dtype, spot_impl impl, const void *d_qkv, void *d_out, int B, int S, int H,
+                           int head_dim, void *cuda_stream);
+
+/* x <- x + dt * v over [n_seqs, elems] fp32 (north_star (e); S8).  If d_probe != NULL also
+ * d_rewards[b] = <probe, x_b> / sqrt(elems) with d_partials [n_seqs, ceil(elems / 4096)] fp32 scratch. */
+spot_status spot_euler_update(float *d_x, const float *d_v, float dt, int n_seqs, int64_t elems, const float *d_probe,
+                              float *d_rewards, float *d_partials, void *cuda_stream);
+
+/* The RoPE table the context built at spot_create (S5): copies cos and sin [S, d_h/2] fp32 to HOST. */
+spot_status spot_rope_table(const spot_ctx *ctx, float *h_cos, float *h_sin);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPOT_KERNELS_H_ */

@@ -1,0 +1,344 @@
+"""Thin ctypes binding over libspot.so: argument marshalling only.
+
+Every function has the name of the C entry point it calls (include/spot.h, include/spot_kernels.h)
+and passes torch tensors as raw device (or host) pointers.  Nothing is computed here; if the shared
+library is missing or a call fails, an exception is raised - there is no fallback.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, List, Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libspot.so")
+_lib: Optional[C.CDLL] = None
+
+SPOT_F32, SPOT_BF16 = 0, 1
+EPI_BIAS, EPI_BIAS_GELU, EPI_GATE_RESIDUAL = 0, 1, 2
+IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05 = 0, 1, 2
+OPT_GEMM_IMPL, OPT_ATTN_IMPL = 0, 1
+STATUS_NAMES = ["SPOT_OK", "SPOT_ERR_NULL", "SPOT_ERR_SHAPE", "SPOT_ERR_DTYPE", "SPOT_ERR_ALIGN",
+                "SPOT_ERR_WORKSPACE", "SPOT_ERR_ARCH", "SPOT_ERR_CUDA", "SPOT_ERR_UNIMPLEMENTED"]
+
+
+class SpotError(RuntimeError):
+    def __init__(self, status: int, where: str, cuda_error: int = 0):
+        self.status = status
+        self.status_name = STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else str(status)
+        self.cuda_error = cuda_error
+        extra = f" (cudaError_t {cuda_error})" if cuda_error else ""
+        super().__init__(f"{where}: {self.status_name}{extra}")
+
+
+class SpotConfig(C.Structure):
+    _fields_ = [("n_blocks", C.c_int32), ("hidden", C.c_int32), ("n_heads", C.c_int32), ("head_dim", C.c_int32),
+                ("mlp_hidden", C.c_int32), ("grid_h", C.c_int32), ("grid_w", C.c_int32), ("n_txt", C.c_int32),
+                ("latent_ch", C.c_int32), ("txt_dim", C.c_int32), ("rope_pairs", C.c_int32 * 3),
+                ("rope_theta", C.c_float), ("ln_eps", C.c_float), ("rms_eps", C.c_float), ("dtype", C.c_int)]
+
+
+_STREAM_FIELDS = ["mod_w", "mod_b", "qkv_w", "qkv_b", "q_gain", "k_gain", "out_w", "out_b", "fc1_w", "fc1_b", "fc2_w", "fc2_b"]
+
+
+class SpotStreamWeights(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in _STREAM_FIELDS]
+
+
+class SpotBlockWeights(C.Structure):
+    _fields_ = [("s", SpotStreamWeights * 2)]
+
+
+class SpotWeights(C.Structure):
+    _fields_ = [("time_w1", C.c_void_p), ("time_b1", C.c_void_p), ("time_w2", C.c_void_p), ("time_b2", C.c_void_p),
+                ("img_in_w", C.c_void_p), ("img_in_b", C.c_void_p), ("txt_gain", C.c_void_p), ("txt_in_w", C.c_void_p),
+                ("txt_in_b", C.c_void_p), ("blocks", C.POINTER(SpotBlockWeights)), ("final_mod_w", C.c_void_p),
+                ("final_mod_b", C.c_void_p), ("proj_w", C.c_void_p), ("proj_b", C.c_void_p)]
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def load_library() -> C.CDLL:
+    """Loads libspot.so (built by paper_2606_19004_b200/build.py).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise FileNotFoundError(f"{_LIB_PATH} not found: run `python -m paper_2606_19004_b200.build` "
+                                "(or __graft_entry__.build()); there is no fallback path")
+    lib = C.CDLL(_LIB_PATH)
+    vp, i32, i64, u32, f32, sz = C.c_void_p, C.c_int, C.c_int64, C.c_uint32, C.c_float, C.c_size_t
+    sig = {
+        "spot_create": [C.POINTER(SpotConfig), C.POINTER(SpotWeights), i32, C.POINTER(vp)],
+        "spot_destroy": [vp],
+        "spot_set_option": [vp, i32, i32],
+        "spot_workspace_bytes": [vp, i32, i32, C.POINTER(sz)],
+        "spot_last_cuda_error": [vp],
+        "spot_noise_from_seeds": [vp, i32, i64, u32, vp, vp],
+        "spot_philox_words": [vp, i32, i64, u32, vp, vp],
+        "spot_dit_block_forward": [vp, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp],
+        "spot_dit_denoise": [vp, i32, i32, vp, vp, vp, i32, vp, sz, vp],
+        "spot_seed_rewards": [vp, i32, i32, vp, vp, i32, vp, vp, vp, vp, vp],
+        "spot_explore": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
+        "spot_explore_host": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
+        "spot_linear": [i32, i32, i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp],
+        "spot_ln_modulate": [i32, vp, i64, i64, vp, vp, f32, vp, vp],
+        "spot_qk_norm_rope": [i32, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, f32, vp],
+        "spot_attention": [i32, i32, vp, vp, i32, i32, i32, i32, vp],
+        "spot_euler_update": [vp, vp, f32, i32, i64, vp, vp, vp, vp],
+        "spot_rope_table": [vp, vp, vp],
+    }
+    for name, args in sig.items():
+        fn = getattr(lib, name)
+        fn.argtypes = args
+        fn.restype = C.c_int
+    lib.spot_status_string.argtypes = [C.c_int]
+    lib.spot_status_string.restype = C.c_char_p
+    lib.spot_version.argtypes = []
+    lib.spot_version.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
+    if t is None:
+        return None
+    assert t.is_contiguous(), "libspot takes dense row-major buffers"
+    return t.data_ptr()
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+
+
+def _dt(dtype: torch.dtype) -> int:
+    if dtype == torch.float32:
+        return SPOT_F32
+    if dtype == torch.bfloat16:
+        return SPOT_BF16
+    raise TypeError(f"unsupported dtype {dtype}")
+
+
+def _check(status: int, where: str, ctx: Optional["Context"] = None) -> None:
+    if status != 0:
+        ce = load_library().spot_last_cuda_error(ctx.handle) if (ctx is not None and status == 7) else 0
+        raise SpotError(status, where, ce)
+
+
+class Context:
+    """spot_ctx: validated config + borrowed weights (keeps the torch tensors alive)."""
+
+    def __init__(self, shape, weights: Dict[str, object], max_seqs: int):
+        lib = load_library()
+        self.shape = shape
+        self._keep = weights
+        cfg = SpotConfig(n_blocks=shape.n_blocks, hidden=shape.hidden, n_heads=shape.n_heads, head_dim=shape.head_dim,
+                         mlp_hidden=shape.mlp_hidden, grid_h=shape.grid_h, grid_w=shape.grid_w, n_txt=shape.n_txt,
+                         latent_ch=shape.latent_ch, txt_dim=shape.txt_dim, rope_pairs=(C.c_int32 * 3)(*shape.rope_pairs),
+                         rope_theta=shape.rope_theta, ln_eps=shape.ln_eps, rms_eps=shape.rms_eps, dtype=_dt(shape.dtype))
+        g = weights["global"]
+        blocks: List[Dict[str, torch.Tensor]] = weights["blocks"]
+        arr = (SpotBlockWeights * max(1, len(blocks)))()
+        for b, bw in enumerate(blocks):
+            for si, stream in enumerate(("img", "txt")):
+                for f in _STREAM_FIELDS:
+                    setattr(arr[b].s[si], f, _ptr(bw[f"{stream}.{f}"]))
+        w = SpotWeights(blocks=C.cast(arr, C.POINTER(SpotBlockWeights)))
+        for name in ("time_w1", "time_b1", "time_w2", "time_b2", "img_in_w", "img_in_b", "txt_gain", "txt_in_w",
+                     "txt_in_b", "final_mod_w", "final_mod_b", "proj_w", "proj_b"):
+            setattr(w, name, _ptr(g[name]))
+        self._cfg, self._w, self._arr = cfg, w, arr
+        self.cfg_struct = cfg
+        h = C.c_void_p()
+        _check(lib.spot_create(C.byref(cfg), C.byref(w), max_seqs, C.byref(h)), "spot_create")
+        self.handle = h
+        self.max_seqs = max_seqs
+        self._ws: Optional[torch.Tensor] = None
+
+    def close(self) -> None:
+        if getattr(self, "handle", None):
+            load_library().spot_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def workspace(self, n_seqs: int, n_steps: int) -> torch.Tensor:
+        n = spot_workspace_bytes(self, n_seqs, n_steps)
+        if self._ws is None or self._ws.numel() < n:
+            self._ws = None
+            self._ws = torch.empty(n, dtype=torch.uint8, device="cuda")
+        return self._ws
+
+
+def spot_version() -> str:
+    return load_library().spot_version().decode()
+
+
+def spot_set_option(ctx: Context, opt: int, value: int) -> None:
+    _check(load_library().spot_set_option(ctx.handle, opt, value), "spot_set_option", ctx)
+
+
+def spot_workspace_bytes(ctx: Context, n_seqs: int, n_steps: int) -> int:
+    out = C.c_size_t()
+    _check(load_library().spot_workspace_bytes(ctx.handle, n_seqs, n_steps, C.byref(out)), "spot_workspace_bytes", ctx)
+    return int(out.value)
+
+
+def spot_noise_from_seeds(seeds: torch.Tensor, elems_per_seed: int, stream_id: int = 0,
+                          out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    assert seeds.dtype in (torch.int64, torch.uint64)
+    n = seeds.numel()
+    if out is None:
+        out = torch.empty((n, elems_per_seed), dtype=torch.float32, device=seeds.device)
+    _check(load_library().spot_noise_from_seeds(_ptr(seeds), n, elems_per_seed, stream_id, _ptr(out), _stream()),
+           "spot_noise_from_seeds")
+    return out
+
+
+def spot_philox_words(seeds: torch.Tensor, elems_per_seed: int, stream_id: int = 0) -> torch.Tensor:
+    n = seeds.numel()
+    out = torch.empty((n, elems_per_seed), dtype=torch.int32, device=seeds.device)
+    _check(load_library().spot_philox_words(_ptr(seeds), n, elems_per_seed, stream_id, _ptr(out), _stream()),
+           "spot_philox_words")
+    return out
+
+
+def spot_dit_block_forward(ctx: Context, block: int, h_img: torch.Tensor, h_txt: torch.Tensor, temb: torch.Tensor,
+                           out_img: Optional[torch.Tensor] = None, out_txt: Optional[torch.Tensor] = None):
+    n_seqs = h_img.shape[0]
+    out_img = torch.empty_like(h_img) if out_img is None else out_img
+    out_txt = torch.empty_like(h_txt) if out_txt is None else out_txt
+    ws = ctx.workspace(n_seqs, 1)
+    _check(load_library().spot_dit_block_forward(ctx.handle, block, n_seqs, _ptr(h_img), _ptr(h_txt), _ptr(temb),
+                                                 _ptr(out_img), _ptr(out_txt), _ptr(ws), ws.numel(), _stream()),
+           "spot_dit_block_forward", ctx)
+    return out_img, out_txt
+
+
+def _timesteps(ts: Sequence[float]):
+    arr = (C.c_float * len(ts))(*[float(t) for t in ts])
+    return arr, len(ts) - 1
+
+
+def spot_dit_denoise(ctx: Context, latents: torch.Tensor, text_emb: torch.Tensor, timesteps: Sequence[float],
+                     n_prompts: int, seeds_per_prompt: int) -> torch.Tensor:
+    arr, T = _timesteps(timesteps)
+    ws = ctx.workspace(n_prompts * seeds_per_prompt, T)
+    _check(load_library().spot_dit_denoise(ctx.handle, n_prompts, seeds_per_prompt, _ptr(latents), _ptr(text_emb),
+                                           C.cast(arr, C.c_void_p), T, _ptr(ws), ws.numel(), _stream()),
+           "spot_dit_denoise", ctx)
+    return latents
+
+
+def spot_seed_rewards(ctx: Context, latents: torch.Tensor, probe: torch.Tensor, n_prompts: int, seeds_per_prompt: int,
+                      k_select: int):
+    dev = latents.device
+    rewards = torch.empty(n_prompts * seeds_per_prompt, dtype=torch.float32, device=dev)
+    stats = torch.empty((n_prompts, 2), dtype=torch.float32, device=dev)
+    top = torch.empty((n_prompts, max(k_select, 1)), dtype=torch.int32, device=dev)
+    bottom = torch.empty((n_prompts, max(k_select, 1)), dtype=torch.int32, device=dev)
+    _check(load_library().spot_seed_rewards(ctx.handle, n_prompts, seeds_per_prompt, _ptr(latents), _ptr(probe), k_select,
+                                            _ptr(rewards), _ptr(stats), _ptr(top), _ptr(bottom), _stream()),
+           "spot_seed_rewards", ctx)
+    return rewards, stats, top[:, :k_select], bottom[:, :k_select]
+
+
+def spot_explore(ctx: Context, seeds: torch.Tensor, text_emb: torch.Tensor, timesteps: Sequence[float],
+                 probe: torch.Tensor, n_prompts: int, seeds_per_prompt: int, k_select: int,
+                 out: Optional[dict] = None) -> dict:
+    """Device-buffer rollout.  `out` may carry preallocated latents/rewards/stats/top/bottom tensors."""
+    dev = seeds.device
+    B = n_prompts * seeds_per_prompt
+    s = ctx.shape
+    if out is None:
+        out = {"latents": torch.empty((B, s.n_img, s.latent_ch), dtype=torch.float32, device=dev),
+               "rewards": torch.empty(B, dtype=torch.float32, device=dev),
+               "stats": torch.empty((n_prompts, 2), dtype=torch.float32, device=dev),
+               "top": torch.empty((n_prompts, max(k_select, 1)), dtype=torch.int32, device=dev),
+               "bottom": torch.empty((n_prompts, max(k_select, 1)), dtype=torch.int32, device=dev)}
+    arr, T = _timesteps(timesteps)
+    ws = ctx.workspace(B, T)
+    _check(load_library().spot_explore(ctx.handle, n_prompts, seeds_per_prompt, _ptr(seeds), _ptr(text_emb),
+                                       C.cast(arr, C.c_void_p), T, _ptr(probe), k_select, _ptr(out["latents"]),
+                                       _ptr(out["rewards"]), _ptr(out["stats"]), _ptr(out["top"]), _ptr(out["bottom"]),
+                                       _ptr(ws), ws.numel(), _stream()), "spot_explore", ctx)
+    return out
+
+
+def spot_explore_host(ctx: Context, h_seeds: torch.Tensor, h_text_emb: torch.Tensor, timesteps: Sequence[float],
+                      h_probe: torch.Tensor, n_prompts: int, seeds_per_prompt: int, k_select: int, h_out: dict) -> dict:
+    """Host-buffer rollout: all tensors are (pinned) HOST tensors; synchronises the stream."""
+    arr, T = _timesteps(timesteps)
+    ws = ctx.workspace(n_prompts * seeds_per_prompt, T)
+    _check(load_library().spot_explore_host(ctx.handle, n_prompts, seeds_per_prompt, _ptr(h_seeds), _ptr(h_text_emb),
+                                            C.cast(arr, C.c_void_p), T, _ptr(h_probe), k_select,
+                                            _ptr(h_out.get("latents")), _ptr(h_out["rewards"]), _ptr(h_out["stats"]),
+                                            _ptr(h_out["top"]), _ptr(h_out["bottom"]), _ptr(ws), ws.numel(), _stream()),
+           "spot_explore_host", ctx)
+    return h_out
+
+
+# ---- kernel-level entry points (include/spot_kernels.h) -------------------------------------------
+def spot_linear(a: torch.Tensor, w: torch.Tensor, bias: torch.Tensor, epi: int = EPI_BIAS, impl: int = IMPL_AUTO,
+                gate: Optional[torch.Tensor] = None, residual: Optional[torch.Tensor] = None,
+                out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    M, K = a.shape
+    N = w.shape[0]
+    if epi != EPI_GATE_RESIDUAL and out is None:
+        out = torch.empty((M, N), dtype=a.dtype, device=a.device)
+    _check(load_library().spot_linear(_dt(w.dtype), impl, epi, _ptr(a), M, K, _ptr(w), N, _ptr(bias), _ptr(gate),
+                                      _ptr(residual), _ptr(out), _stream()), "spot_linear")
+    return residual if epi == EPI_GATE_RESIDUAL else out
+
+
+def spot_ln_modulate(h: torch.Tensor, shift: torch.Tensor, scale: torch.Tensor, eps: float, dtype: torch.dtype) -> torch.Tensor:
+    M, D = h.shape
+    out = torch.empty((M, D), dtype=dtype, device=h.device)
+    _check(load_library().spot_ln_modulate(_dt(dtype), _ptr(h), M, D, _ptr(shift), _ptr(scale), eps, _ptr(out), _stream()),
+           "spot_ln_modulate")
+    return out
+
+
+def spot_qk_norm_rope(qkv: torch.Tensor, n_txt: int, gains: Sequence[torch.Tensor], cos: torch.Tensor, sin: torch.Tensor,
+                      eps: float) -> torch.Tensor:
+    B, S, three, H, dh = qkv.shape
+    assert three == 3
+    _check(load_library().spot_qk_norm_rope(_dt(qkv.dtype), _ptr(qkv), B, S, H, dh, n_txt, _ptr(gains[0]), _ptr(gains[1]),
+                                            _ptr(gains[2]), _ptr(gains[3]), _ptr(cos), _ptr(sin), eps, _stream()),
+           "spot_qk_norm_rope")
+    return qkv
+
+
+def spot_attention(qkv: torch.Tensor, impl: int = IMPL_AUTO) -> torch.Tensor:
+    B, S, three, H, dh = qkv.shape
+    out = torch.empty((B, S, H * dh), dtype=qkv.dtype, device=qkv.device)
+    _check(load_library().spot_attention(_dt(qkv.dtype), impl, _ptr(qkv), _ptr(out), B, S, H, dh, _stream()), "spot_attention")
+    return out
+
+
+def spot_euler_update(x: torch.Tensor, v: torch.Tensor, dt: float, probe: Optional[torch.Tensor] = None):
+    B = x.shape[0]
+    E = x.numel() // B
+    rewards = partials = None
+    if probe is not None:
+        rewards = torch.empty(B, dtype=torch.float32, device=x.device)
+        partials = torch.empty((B, (E + 4095) // 4096), dtype=torch.float32, device=x.device)
+    _check(load_library().spot_euler_update(_ptr(x), _ptr(v), dt, B, E, _ptr(probe), _ptr(rewards), _ptr(partials), _stream()),
+           "spot_euler_update")
+    return x, rewards
+
+
+def spot_rope_table(ctx: Context):
+    s = ctx.shape
+    cos = torch.empty((s.seq, s.head_dim // 2), dtype=torch.float32)
+    sin = torch.empty_like(cos)
+    _check(load_library().spot_rope_table(ctx.handle, _ptr(cos), _ptr(sin)), "spot_rope_table", ctx)
+    return cos, sin

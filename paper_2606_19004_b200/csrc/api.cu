@@ -1,0 +1,708 @@
+// api.cu - the C ABI of libspot.so (include/spot.h, include/spot_kernels.h): argument validation,
+// workspace carving and the launch sequence of the exploration rollout.  Every step runs in the
+// kernels of this directory; there is no CPU or library fallback.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/spot_kernels.h"
+#include "kernels.h"
+
+struct spot_ctx {
+  spot_config cfg;
+  spot_weights w;
+  std::vector<spot_block_weights> blocks;
+  int max_seqs;
+  int num_sms;
+  int last_cuda;
+  int gemm_impl, attn_impl;      // 0 auto, 1 force SIMT
+  float* d_cos;                  // [S, d_h/2]
+  float* d_sin;
+  float* d_partials;             // [max_seqs, reward chunks]
+  int n_img() const { return cfg.grid_h * cfg.grid_w; }
+  int seq() const { return cfg.n_txt + n_img(); }
+};
+
+namespace {
+
+inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+inline size_t esize(spot_dtype d) { return d == SPOT_F32 ? 4 : 2; }
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+// 0 = unknown, 1 = ok (cc 10.x), -1 = no usable device
+int device_state() {
+  static int state = 0;
+  if (state == 0) {
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+      cudaGetLastError();
+      state = -1;
+    } else {
+      state = prop.major == 10 ? 1 : -1;
+    }
+  }
+  return state;
+}
+
+struct Workspace {
+  // all offsets in bytes from the workspace base
+  size_t t_dev, emb, hid, temb, cvec, mod, fmod, txt_norm, txt_h0, h_img, h_txt, ybuf, big, vel, stage, total;
+  size_t st_seeds, st_text, st_probe, st_lat, st_rew, st_stats, st_top, st_bot;
+};
+
+Workspace carve(const spot_ctx* c, int B, int T) {
+  const spot_config& g = c->cfg;
+  const size_t D = g.hidden, S = c->seq(), NI = c->n_img(), NT = g.n_txt, L = g.n_blocks, es = esize(g.dtype);
+  const size_t E = NI * g.latent_ch;
+  const size_t wide = (size_t)(3 * D > (size_t)g.mlp_hidden ? 3 * D : g.mlp_hidden);
+  Workspace w;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o += align_up(bytes); return r; };
+  const size_t Tp = T > 0 ? T : 1;
+  w.t_dev = take((Tp + 1) * 4);
+  w.emb = take(Tp * 256 * 4);
+  w.hid = take(Tp * D * 4);
+  w.temb = take(Tp * D * 4);
+  w.cvec = take(Tp * D * 4);
+  w.mod = take(Tp * L * 2 * 6 * D * 4);
+  w.fmod = take(Tp * 2 * D * 4);
+  w.txt_norm = take((size_t)B * NT * g.txt_dim * es);
+  w.txt_h0 = take((size_t)B * NT * D * 4);
+  w.h_img = take((size_t)B * NI * D * 4);
+  w.h_txt = take((size_t)B * NT * D * 4);
+  w.ybuf = take((size_t)B * S * D * es);
+  w.big = take((size_t)B * S * wide * es);
+  w.vel = take((size_t)B * E * 4);
+  w.stage = o;
+  w.st_seeds = take((size_t)B * 8);
+  w.st_text = take((size_t)B * NT * g.txt_dim * es);
+  w.st_probe = take(E * 4);
+  w.st_lat = take((size_t)B * E * 4);
+  w.st_rew = take((size_t)B * 4);
+  w.st_stats = take((size_t)B * 2 * 4);
+  w.st_top = take((size_t)B * 4);
+  w.st_bot = take((size_t)B * 4);
+  w.total = o;
+  return w;
+}
+
+#define CK(ctx, expr)                                  \
+  do {                                                 \
+    cudaError_t _e = (expr);                           \
+    if (_e != cudaSuccess) {                           \
+      (ctx)->last_cuda = (int)_e;                      \
+      return SPOT_ERR_CUDA;                            \
+    }                                                  \
+  } while (0)
+
+// Linear layer dispatch: tcgen05 when the context runs bf16 and every problem qualifies, else SIMT.
+spot_status run_gemm(spot_ctx* c, Epilogue epi, GemmProblem* probs, int n, spot_dtype ta, spot_dtype tout,
+                     cudaStream_t st) {
+  const spot_dtype dt = c->cfg.dtype;
+  bool tc = dt == SPOT_BF16 && ta == SPOT_BF16 && (epi == EPI_GATE_RES || tout == SPOT_BF16) && c->gemm_impl == 0;
+  for (int i = 0; i < n && tc; ++i)
+    if (probs[i].M > 0 && !tcgen05_gemm_supported(probs[i])) tc = false;
+  if (tc) {
+    CK(c, launch_gemm_tcgen05(epi, probs, n, c->num_sms, st));
+  } else {
+    for (int i = 0; i < n; ++i) CK(c, launch_gemm_simt(ta, dt, tout, epi, probs[i], st));
+  }
+  return SPOT_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+const char* spot_status_string(spot_status s) {
+  switch (s) {
+    case SPOT_OK: return "SPOT_OK";
+    case SPOT_ERR_NULL: return "SPOT_ERR_NULL: a required pointer is NULL";
+    case SPOT_ERR_SHAPE: return "SPOT_ERR_SHAPE: inconsistent or unsupported sizes";
+    case SPOT_ERR_DTYPE: return "SPOT_ERR_DTYPE: unknown dtype";
+    case SPOT_ERR_ALIGN: return "SPOT_ERR_ALIGN: pointer not 16-byte aligned";
+    case SPOT_ERR_WORKSPACE: return "SPOT_ERR_WORKSPACE: workspace too small";
+    case SPOT_ERR_ARCH: return "SPOT_ERR_ARCH: no CUDA device of compute capability 10.x";
+    case SPOT_ERR_CUDA: return "SPOT_ERR_CUDA: a CUDA call failed";
+    case SPOT_ERR_UNIMPLEMENTED: return "SPOT_ERR_UNIMPLEMENTED";
+  }
+  return "unknown spot_status";
+}
+
+const char* spot_version(void) { return "libspot 0.1 (sm_100a)"; }
+
+int spot_last_cuda_error(const spot_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
+
+static spot_status validate_config(const spot_config* c) {
+  if (c->dtype != SPOT_F32 && c->dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  if (c->n_blocks < 0 || c->hidden <= 0 || c->n_heads <= 0 || c->head_dim <= 0 || c->mlp_hidden <= 0 ||
+      c->grid_h <= 0 || c->grid_w <= 0 || c->n_txt < 0 || c->latent_ch <= 0)
+    return SPOT_ERR_SHAPE;
+  if (c->n_heads * c->head_dim != c->hidden) return SPOT_ERR_SHAPE;
+  if (c->head_dim != 64 && c->head_dim != 128) return SPOT_ERR_SHAPE;
+  if (c->rope_pairs[0] < 0 || c->rope_pairs[1] < 0 || c->rope_pairs[2] < 0 ||
+      c->rope_pairs[0] + c->rope_pairs[1] + c->rope_pairs[2] != c->head_dim / 2)
+    return SPOT_ERR_SHAPE;
+  const int dq = c->hidden / 128;
+  if (c->hidden % 128 || !(dq == 1 || dq == 2 || dq == 4 || dq == 8 || dq == 12 || dq == 16 || dq == 24 || dq == 32))
+    return SPOT_ERR_SHAPE;
+  if (c->mlp_hidden % 16 || c->latent_ch % 16 || c->txt_dim != c->hidden) return SPOT_ERR_SHAPE;
+  if (!(c->rope_theta > 0.f) || !(c->ln_eps >= 0.f) || !(c->rms_eps >= 0.f)) return SPOT_ERR_SHAPE;
+  return SPOT_OK;
+}
+
+// RoPE table (S5): d_h/2 pairs split over axes (t, h, w); pair i' of an axis with n_a pairs
+// has frequency theta^(-i'/n_a).  Text token j sits at max(G_h/2, G_w/2) + j on all axes; image token
+// (r, c) at (0, r - ceil(G_h/2), c - ceil(G_w/2)).  Host double math, cast once to fp32.
+static void build_rope_host(const spot_config& c, std::vector<float>& cs, std::vector<float>& sn) {
+  const int S = c.n_txt + c.grid_h * c.grid_w, half = c.head_dim / 2;
+  cs.resize((size_t)S * half);
+  sn.resize((size_t)S * half);
+  const int base = (c.grid_h / 2 > c.grid_w / 2) ? c.grid_h / 2 : c.grid_w / 2;
+  for (int s = 0; s < S; ++s) {
+    double pos[3];
+    if (s < c.n_txt) {
+      pos[0] = pos[1] = pos[2] = (double)(base + s);
+    } else {
+      const int n = s - c.n_txt, r = n / c.grid_w, col = n % c.grid_w;
+      pos[0] = 0.0;
+      pos[1] = (double)(r - (c.grid_h + 1) / 2);
+      pos[2] = (double)(col - (c.grid_w + 1) / 2);
+    }
+    int p = 0;
+    for (int a = 0; a < 3; ++a)
+      for (int i = 0; i < c.rope_pairs[a]; ++i, ++p) {
+        const double ang = pos[a] * pow((double)c.rope_theta, -(double)i / (double)c.rope_pairs[a]);
+        cs[(size_t)s * half + p] = (float)cos(ang);
+        sn[(size_t)s * half + p] = (float)sin(ang);
+      }
+  }
+}
+
+spot_status spot_create(const spot_config* cfg, const spot_weights* w, int max_seqs, spot_ctx** out) {
+  if (!cfg || !w || !out) return SPOT_ERR_NULL;
+  *out = nullptr;
+  spot_status vs = validate_config(cfg);
+  if (vs != SPOT_OK) return vs;
+  if (max_seqs <= 0) return SPOT_ERR_SHAPE;
+  if (cfg->n_blocks > 0 && !w->blocks) return SPOT_ERR_NULL;
+  const void* globals[] = {w->time_w1, w->time_b1, w->time_w2, w->time_b2, w->img_in_w, w->img_in_b, w->txt_gain,
+                           w->txt_in_w, w->txt_in_b, w->final_mod_w, w->final_mod_b, w->proj_w, w->proj_b};
+  for (const void* p : globals) {
+    if (!p) return SPOT_ERR_NULL;
+    if (!aligned16(p)) return SPOT_ERR_ALIGN;
+  }
+  for (int b = 0; b < cfg->n_blocks; ++b)
+    for (int s = 0; s < 2; ++s) {
+      const spot_stream_weights& sw = w->blocks[b].s[s];
+      const void* ps[] = {sw.mod_w, sw.mod_b, sw.qkv_w, sw.qkv_b, sw.q_gain, sw.k_gain,
+                          sw.out_w, sw.out_b, sw.fc1_w, sw.fc1_b, sw.fc2_w, sw.fc2_b};
+      for (const void* p : ps) {
+        if (!p) return SPOT_ERR_NULL;
+        if (!aligned16(p)) return SPOT_ERR_ALIGN;
+      }
+    }
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  spot_ctx* c = new (std::nothrow) spot_ctx();
+  if (!c) return SPOT_ERR_CUDA;
+  c->cfg = *cfg;
+  c->w = *w;
+  c->blocks.assign(w->blocks, w->blocks + cfg->n_blocks);
+  c->w.blocks = c->blocks.data();
+  c->max_seqs = max_seqs;
+  c->last_cuda = 0;
+  c->gemm_impl = c->attn_impl = 0;
+  c->d_cos = c->d_sin = c->d_partials = nullptr;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  std::vector<float> cs, sn;
+  build_rope_host(*cfg, cs, sn);
+  const size_t E = (size_t)c->n_img() * cfg->latent_ch;
+  const size_t n_part = (size_t)max_seqs * ((E + REWARD_CHUNK - 1) / REWARD_CHUNK);
+  cudaError_t e = cudaMalloc(&c->d_cos, cs.size() * 4);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_sin, sn.size() * 4);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_partials, n_part * 4);
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_cos, cs.data(), cs.size() * 4, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_sin, sn.data(), sn.size() * 4, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    cudaFree(c->d_cos); cudaFree(c->d_sin); cudaFree(c->d_partials);
+    delete c;
+    return SPOT_ERR_CUDA;
+  }
+  *out = c;
+  return SPOT_OK;
+}
+
+spot_status spot_destroy(spot_ctx* ctx) {
+  if (!ctx) return SPOT_ERR_NULL;
+  cudaFree(ctx->d_cos);
+  cudaFree(ctx->d_sin);
+  cudaFree(ctx->d_partials);
+  delete ctx;
+  return SPOT_OK;
+}
+
+spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
+  if (!ctx) return SPOT_ERR_NULL;
+  if (value != 0 && value != 1) return SPOT_ERR_SHAPE;
+  if (opt == SPOT_OPT_GEMM_IMPL) ctx->gemm_impl = value;
+  else if (opt == SPOT_OPT_ATTN_IMPL) ctx->attn_impl = value;
+  else return SPOT_ERR_SHAPE;
+  return SPOT_OK;
+}
+
+spot_status spot_workspace_bytes(const spot_ctx* ctx, int n_seqs, int n_steps, size_t* bytes) {
+  if (!ctx || !bytes) return SPOT_ERR_NULL;
+  if (n_seqs <= 0 || n_seqs > ctx->max_seqs || n_steps < 0) return SPOT_ERR_SHAPE;
+  *bytes = carve(ctx, n_seqs, n_steps).total;
+  return SPOT_OK;
+}
+
+spot_status spot_rope_table(const spot_ctx* ctx, float* h_cos, float* h_sin) {
+  if (!ctx || !h_cos || !h_sin) return SPOT_ERR_NULL;
+  const size_t n = (size_t)ctx->seq() * (ctx->cfg.head_dim / 2) * 4;
+  if (cudaMemcpy(h_cos, ctx->d_cos, n, cudaMemcpyDeviceToHost) != cudaSuccess) return SPOT_ERR_CUDA;
+  if (cudaMemcpy(h_sin, ctx->d_sin, n, cudaMemcpyDeviceToHost) != cudaSuccess) return SPOT_ERR_CUDA;
+  return SPOT_OK;
+}
+
+}  // extern "C"
+
+// ================================================================================================
+// internal launch sequences
+namespace {
+
+struct StreamMaps {          // row maps of one stream (image or text) inside the joint buffers
+  int rows;                  // B * n_sigma
+  RowMap y, qkv, wide, h;    // [B,S,D] ybuf, [B,S,3D] qkv, [B,S,F] mlp hidden, [B,n_sigma,D] residual
+};
+
+StreamMaps stream_maps(const spot_ctx* c, int B, int stream /*0 img, 1 txt*/) {
+  const long long D = c->cfg.hidden, S = c->seq(), F = c->cfg.mlp_hidden;
+  const int n = stream == 0 ? c->n_img() : c->cfg.n_txt;
+  const long long first = stream == 0 ? c->cfg.n_txt : 0;       // text tokens come first in the joint sequence
+  StreamMaps m;
+  m.rows = B * n;
+  const int rps = n > 0 ? n : 1;
+  m.y = RowMap{rps, S * D, first * D, D};
+  m.qkv = RowMap{rps, S * 3 * D, first * 3 * D, 3 * D};
+  m.wide = RowMap{rps, S * F, first * F, F};
+  m.h = RowMap{rps, (long long)n * D, 0, D};
+  return m;
+}
+
+// One joint block on the fp32 residual streams h_img [B,n_img,D], h_txt [B,n_txt,D] (S4 steps
+// 2-8).  mod_img / mod_txt: [6D] fp32 = (shift1, scale1, gate1, shift2, scale2, gate2).  When
+// img_only_tail is set (last block of a denoise pass, S16) the text stream's out-proj and MLP,
+// whose result nobody reads, are skipped.
+spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt, const float* mod_img,
+                       const float* mod_txt, void* ybuf, void* big, bool img_only_tail, cudaStream_t st) {
+  const spot_config& g = c->cfg;
+  const spot_dtype dt = g.dtype;
+  const int D = g.hidden, F = g.mlp_hidden, S = c->seq();
+  const spot_block_weights& bw = c->blocks[block];
+  float* h[2] = {h_img, h_txt};
+  const float* mod[2] = {mod_img, mod_txt};
+  StreamMaps sm[2] = {stream_maps(c, B, 0), stream_maps(c, B, 1)};
+  GemmProblem pr[2];
+  // (2) y = LN(h) (1 + scale1) + shift1 ; (3) qkv = y Wqkv^T + b
+  for (int s = 0; s < 2; ++s) {
+    CK(c, launch_ln_modulate(dt, h[s], sm[s].rows, D, mod[s], mod[s] + D, g.ln_eps, ybuf, sm[s].y, st));
+    memset(&pr[s], 0, sizeof(GemmProblem));
+    pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].qkv_w; pr[s].bias = bw.s[s].qkv_b;
+    pr[s].M = sm[s].rows; pr[s].N = 3 * D; pr[s].K = D; pr[s].out = big; pr[s].out_map = sm[s].qkv;
+  }
+  spot_status rs = run_gemm(c, EPI_BIAS, pr, 2, dt, dt, st);
+  if (rs != SPOT_OK) return rs;
+  // (4)-(5) QK-RMSNorm + RoPE, (6) joint attention -> ybuf [B,S,D]
+  CK(c, launch_qk_norm_rope(dt, big, B, S, g.n_heads, g.head_dim, g.n_txt, bw.s[0].q_gain, bw.s[0].k_gain,
+                            bw.s[1].q_gain, bw.s[1].k_gain, c->d_cos, c->d_sin, g.rms_eps, st));
+  if (dt == SPOT_BF16 && c->attn_impl == 0 && tcgen05_attn_supported(S, g.n_heads, g.head_dim))
+    CK(c, launch_attn_tcgen05(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st));
+  else
+    CK(c, launch_attn_simt(dt, big, ybuf, B, S, g.n_heads, g.head_dim, st));
+  const int ns = img_only_tail ? 1 : 2;
+  // (7) h += gate1 * (o Wout^T + b)
+  for (int s = 0; s < ns; ++s) {
+    memset(&pr[s], 0, sizeof(GemmProblem));
+    pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].out_w; pr[s].bias = bw.s[s].out_b;
+    pr[s].M = sm[s].rows; pr[s].N = D; pr[s].K = D; pr[s].gate = mod[s] + 2 * D; pr[s].resid = h[s]; pr[s].resid_map = sm[s].h;
+  }
+  rs = run_gemm(c, EPI_GATE_RES, pr, ns, dt, SPOT_F32, st);
+  if (rs != SPOT_OK) return rs;
+  // (8) y2 = LN(h)(1 + scale2) + shift2 ; u = GELU(y2 W1^T + b) ; h += gate2 * (u W2^T + b)
+  for (int s = 0; s < ns; ++s) {
+    CK(c, launch_ln_modulate(dt, h[s], sm[s].rows, D, mod[s] + 3 * D, mod[s] + 4 * D, g.ln_eps, ybuf, sm[s].y, st));
+    memset(&pr[s], 0, sizeof(GemmProblem));
+    pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].fc1_w; pr[s].bias = bw.s[s].fc1_b;
+    pr[s].M = sm[s].rows; pr[s].N = F; pr[s].K = D; pr[s].out = big; pr[s].out_map = sm[s].wide;
+  }
+  rs = run_gemm(c, EPI_BIAS_GELU, pr, ns, dt, dt, st);
+  if (rs != SPOT_OK) return rs;
+  for (int s = 0; s < ns; ++s) {
+    memset(&pr[s], 0, sizeof(GemmProblem));
+    pr[s].A = big; pr[s].a_map = sm[s].wide; pr[s].W = bw.s[s].fc2_w; pr[s].bias = bw.s[s].fc2_b;
+    pr[s].M = sm[s].rows; pr[s].N = D; pr[s].K = F; pr[s].gate = mod[s] + 5 * D; pr[s].resid = h[s]; pr[s].resid_map = sm[s].h;
+  }
+  return run_gemm(c, EPI_GATE_RES, pr, ns, dt, SPOT_F32, st);
+}
+
+// temb/c for T timesteps and every block's modulation vectors (S7, S4 step 1): seed- and
+// prompt-independent, so computed once per call for all steps (the 13.6 GB of modulation weights of the
+// full-depth config are read once per call instead of once per step).
+spot_status conditioning(spot_ctx* c, const Workspace& w, uint8_t* ws, int T, cudaStream_t st) {
+  const spot_config& g = c->cfg;
+  const int D = g.hidden, L = g.n_blocks;
+  float* emb = (float*)(ws + w.emb); float* hid = (float*)(ws + w.hid); float* temb = (float*)(ws + w.temb);
+  float* cv = (float*)(ws + w.cvec); float* mod = (float*)(ws + w.mod); float* fmod = (float*)(ws + w.fmod);
+  CK(c, launch_time_embed((const float*)(ws + w.t_dev), T, emb, st));
+  CK(c, launch_gemv(g.dtype, c->w.time_w1, c->w.time_b1, emb, T, D, 256, hid, D, true, st));
+  CK(c, launch_gemv(g.dtype, c->w.time_w2, c->w.time_b2, hid, T, D, D, temb, D, false, st));
+  CK(c, launch_silu(temb, cv, (long long)T * D, st));
+  const long long stride_t = (long long)L * 2 * 6 * D;
+  for (int b = 0; b < L; ++b)
+    for (int s = 0; s < 2; ++s)
+      CK(c, launch_gemv(g.dtype, c->blocks[b].s[s].mod_w, c->blocks[b].s[s].mod_b, cv, T, 6 * D, D,
+                        mod + ((long long)b * 2 + s) * 6 * D, stride_t, false, st));
+  CK(c, launch_gemv(g.dtype, c->w.final_mod_w, c->w.final_mod_b, cv, T, 2 * D, D, fmod, 2 * D, false, st));
+  return SPOT_OK;
+}
+
+spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text_emb, const float* h_t, int T,
+                         uint8_t* ws, const float* probe, float* partials, cudaStream_t st) {
+  const spot_config& g = c->cfg;
+  const spot_dtype dt = g.dtype;
+  const int B = P * K, D = g.hidden, L = g.n_blocks, NI = c->n_img(), NT = g.n_txt, C = g.latent_ch;
+  const long long E = (long long)NI * C;
+  const Workspace w = carve(c, B, T);
+  if (T == 0) {
+    if (probe) CK(c, launch_reward_partials(lat, probe, B, E, partials, st));
+    return SPOT_OK;
+  }
+  CK(c, cudaMemcpyAsync(ws + w.t_dev, h_t, (size_t)(T + 1) * 4, cudaMemcpyHostToDevice, st));
+  spot_status rs = conditioning(c, w, ws, T, st);
+  if (rs != SPOT_OK) return rs;
+  float* txt_h0 = (float*)(ws + w.txt_h0); float* h_img = (float*)(ws + w.h_img); float* h_txt = (float*)(ws + w.h_txt);
+  void* ybuf = ws + w.ybuf; void* big = ws + w.big; float* vel = (float*)(ws + w.vel);
+  const float* mod = (const float*)(ws + w.mod); const float* fmod = (const float*)(ws + w.fmod);
+  GemmProblem pr;
+  // h_txt^0 = RMSNorm(text_emb) Wtxt^T + b, once per prompt (C7)
+  if (NT > 0) {
+    CK(c, launch_rmsnorm_rows(dt, text_emb, c->w.txt_gain, P * NT, g.txt_dim, g.rms_eps, ws + w.txt_norm, st));
+    memset(&pr, 0, sizeof(pr));
+    pr.A = ws + w.txt_norm; pr.a_map = plain_rows(P * NT, g.txt_dim); pr.W = c->w.txt_in_w; pr.bias = c->w.txt_in_b;
+    pr.M = P * NT; pr.N = D; pr.K = g.txt_dim; pr.out = txt_h0; pr.out_map = plain_rows(P * NT, D);
+    CK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
+  }
+  for (int i = 0; i < T; ++i) {
+    // h_img^0 = x Win^T + b on the fp32 latents
+    memset(&pr, 0, sizeof(pr));
+    pr.A = lat; pr.a_map = plain_rows(B * NI, C); pr.W = c->w.img_in_w; pr.bias = c->w.img_in_b;
+    pr.M = B * NI; pr.N = D; pr.K = C; pr.out = h_img; pr.out_map = plain_rows(B * NI, D);
+    CK(c, launch_gemm_simt(SPOT_F32, dt, SPOT_F32, EPI_BIAS, pr, st));
+    CK(c, launch_broadcast_prompts(txt_h0, h_txt, B, K, (long long)NT * D, st));
+    for (int b = 0; b < L; ++b) {
+      const float* m = mod + ((long long)i * L + b) * 2 * 6 * D;
+      rs = block_core(c, b, B, h_img, h_txt, m, m + 6 * D, ybuf, big, b == L - 1, st);
+      if (rs != SPOT_OK) return rs;
+    }
+    // v = (LN(h_img)(1 + scale_f) + shift_f) Wp^T + b
+    const float* fm = fmod + (long long)i * 2 * D;
+    CK(c, launch_ln_modulate(dt, h_img, B * NI, D, fm + D, fm, g.ln_eps, ybuf, plain_rows(B * NI, D), st));
+    memset(&pr, 0, sizeof(pr));
+    pr.A = ybuf; pr.a_map = plain_rows(B * NI, D); pr.W = c->w.proj_w; pr.bias = c->w.proj_b;
+    pr.M = B * NI; pr.N = C; pr.K = D; pr.out = vel; pr.out_map = plain_rows(B * NI, C);
+    CK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
+    const bool last = i == T - 1;
+    CK(c, launch_euler_update(lat, vel, h_t[i + 1] - h_t[i], B, E, last ? probe : nullptr, partials, st));
+  }
+  return SPOT_OK;
+}
+
+spot_status check_ws(const spot_ctx* c, int B, int T, const void* ws, size_t bytes) {
+  if (!ws) return SPOT_ERR_NULL;
+  if (!aligned16(ws)) return SPOT_ERR_ALIGN;
+  if (bytes < carve(c, B, T).total) return SPOT_ERR_WORKSPACE;
+  return SPOT_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+static spot_status noise_common(const uint64_t* d_seeds, int n_seeds, int64_t elems, uint32_t stream_id, float* d_out,
+                                uint32_t* d_words, void* cuda_stream) {
+  if (n_seeds < 0 || elems <= 0 || (elems & 3)) return SPOT_ERR_SHAPE;
+  if (n_seeds == 0) return SPOT_OK;
+  const void* o = d_out ? (const void*)d_out : (const void*)d_words;
+  if (!d_seeds || !o) return SPOT_ERR_NULL;
+  if (!aligned16(o)) return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  return launch_noise(d_seeds, n_seeds, elems, stream_id, d_out, d_words, (cudaStream_t)cuda_stream) == cudaSuccess
+             ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
+spot_status spot_noise_from_seeds(const uint64_t* d_seeds, int n_seeds, int64_t elems_per_seed, uint32_t stream_id,
+                                  float* d_out, void* cuda_stream) {
+  if (n_seeds > 0 && !d_out) return SPOT_ERR_NULL;
+  return noise_common(d_seeds, n_seeds, elems_per_seed, stream_id, d_out, nullptr, cuda_stream);
+}
+
+spot_status spot_philox_words(const uint64_t* d_seeds, int n_seeds, int64_t elems_per_seed, uint32_t stream_id,
+                              uint32_t* d_out, void* cuda_stream) {
+  if (n_seeds > 0 && !d_out) return SPOT_ERR_NULL;
+  return noise_common(d_seeds, n_seeds, elems_per_seed, stream_id, nullptr, d_out, cuda_stream);
+}
+
+spot_status spot_dit_block_forward(spot_ctx* ctx, int block, int n_seqs, const void* d_h_img, const void* d_h_txt,
+                                   const float* d_temb, void* d_out_img, void* d_out_txt, void* d_workspace,
+                                   size_t ws_bytes, void* cuda_stream) {
+  if (!ctx || !d_h_img || !d_temb || !d_out_img) return SPOT_ERR_NULL;
+  if (ctx->cfg.n_txt > 0 && (!d_h_txt || !d_out_txt)) return SPOT_ERR_NULL;
+  if (block < 0 || block >= ctx->cfg.n_blocks || n_seqs <= 0 || n_seqs > ctx->max_seqs) return SPOT_ERR_SHAPE;
+  if (!aligned16(d_h_img) || !aligned16(d_h_txt) || !aligned16(d_out_img) || !aligned16(d_out_txt) || !aligned16(d_temb))
+    return SPOT_ERR_ALIGN;
+  spot_status s = check_ws(ctx, n_seqs, 1, d_workspace, ws_bytes);
+  if (s != SPOT_OK) return s;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const spot_config& g = ctx->cfg;
+  const Workspace w = carve(ctx, n_seqs, 1);
+  uint8_t* ws = (uint8_t*)d_workspace;
+  const int D = g.hidden;
+  const long long n_img = (long long)n_seqs * ctx->n_img() * D, n_txt = (long long)n_seqs * g.n_txt * D;
+  float* cv = (float*)(ws + w.cvec); float* mod = (float*)(ws + w.mod);
+  float* h_img = (float*)(ws + w.h_img); float* h_txt = (float*)(ws + w.h_txt);
+  CK(ctx, launch_silu(d_temb, cv, D, st));
+  for (int sgm = 0; sgm < 2; ++sgm)
+    CK(ctx, launch_gemv(g.dtype, ctx->blocks[block].s[sgm].mod_w, ctx->blocks[block].s[sgm].mod_b, cv, 1, 6 * D, D,
+                        mod + (long long)sgm * 6 * D, 0, false, st));
+  CK(ctx, launch_to_f32(g.dtype, d_h_img, h_img, n_img, st));
+  CK(ctx, launch_to_f32(g.dtype, d_h_txt, h_txt, n_txt, st));
+  s = block_core(ctx, block, n_seqs, h_img, h_txt, mod, mod + 6 * D, ws + w.ybuf, ws + w.big, false, st);
+  if (s != SPOT_OK) return s;
+  CK(ctx, launch_from_f32(g.dtype, h_img, d_out_img, n_img, st));
+  CK(ctx, launch_from_f32(g.dtype, h_txt, d_out_txt, n_txt, st));
+  return SPOT_OK;
+}
+
+static spot_status check_rollout_args(const spot_ctx* ctx, int P, int K, const void* lat, const void* text,
+                                      const float* h_t, int T) {
+  if (!ctx || !lat || !h_t) return SPOT_ERR_NULL;
+  if (ctx->cfg.n_txt > 0 && !text) return SPOT_ERR_NULL;
+  if (P <= 0 || K <= 0 || T < 0 || (long long)P * K > ctx->max_seqs) return SPOT_ERR_SHAPE;
+  if (!aligned16(lat) || !aligned16(text)) return SPOT_ERR_ALIGN;
+  return SPOT_OK;
+}
+
+spot_status spot_dit_denoise(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, float* d_latents,
+                             const void* d_text_emb, const float* h_timesteps, int n_steps, void* d_workspace,
+                             size_t ws_bytes, void* cuda_stream) {
+  spot_status s = check_rollout_args(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps);
+  if (s != SPOT_OK) return s;
+  s = check_ws(ctx, n_prompts * seeds_per_prompt, n_steps, d_workspace, ws_bytes);
+  if (s != SPOT_OK) return s;
+  return denoise_core(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps,
+                      (uint8_t*)d_workspace, nullptr, nullptr, (cudaStream_t)cuda_stream);
+}
+
+static spot_status check_select_args(const spot_ctx* ctx, int P, int K, int k_select, const void* rewards,
+                                     const void* stats, const void* top, const void* bottom) {
+  if (!ctx || !rewards || !stats) return SPOT_ERR_NULL;
+  if (P <= 0 || K <= 0 || K > 1024 || (long long)P * K > ctx->max_seqs || k_select < 0 || 2 * k_select > K)
+    return SPOT_ERR_SHAPE;
+  if (k_select > 0 && (!top || !bottom)) return SPOT_ERR_NULL;
+  return SPOT_OK;
+}
+
+spot_status spot_seed_rewards(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, const float* d_latents,
+                              const float* d_probe, int k_select, float* d_rewards, float* d_stats, int32_t* d_top,
+                              int32_t* d_bottom, void* cuda_stream) {
+  if (!ctx || !d_latents || !d_probe) return SPOT_ERR_NULL;
+  spot_status s = check_select_args(ctx, n_prompts, seeds_per_prompt, k_select, d_rewards, d_stats, d_top, d_bottom);
+  if (s != SPOT_OK) return s;
+  if (!aligned16(d_latents) || !aligned16(d_probe)) return SPOT_ERR_ALIGN;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int B = n_prompts * seeds_per_prompt;
+  const long long E = (long long)ctx->n_img() * ctx->cfg.latent_ch;
+  CK(ctx, launch_reward_partials(d_latents, d_probe, B, E, ctx->d_partials, st));
+  CK(ctx, launch_reward_finalize(ctx->d_partials, B, E, d_rewards, st));
+  CK(ctx, launch_seed_select(d_rewards, n_prompts, seeds_per_prompt, k_select, d_stats, d_top, d_bottom, st));
+  return SPOT_OK;
+}
+
+spot_status spot_explore(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, const uint64_t* d_seeds,
+                         const void* d_text_emb, const float* h_timesteps, int n_steps, const float* d_probe,
+                         int k_select, float* d_latents, float* d_rewards, float* d_stats, int32_t* d_top,
+                         int32_t* d_bottom, void* d_workspace, size_t ws_bytes, void* cuda_stream) {
+  spot_status s = check_rollout_args(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps);
+  if (s != SPOT_OK) return s;
+  if (!d_seeds || !d_probe) return SPOT_ERR_NULL;
+  s = check_select_args(ctx, n_prompts, seeds_per_prompt, k_select, d_rewards, d_stats, d_top, d_bottom);
+  if (s != SPOT_OK) return s;
+  if (!aligned16(d_probe)) return SPOT_ERR_ALIGN;
+  const int B = n_prompts * seeds_per_prompt;
+  s = check_ws(ctx, B, n_steps, d_workspace, ws_bytes);
+  if (s != SPOT_OK) return s;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const long long E = (long long)ctx->n_img() * ctx->cfg.latent_ch;
+  CK(ctx, launch_noise(d_seeds, B, E, 0u, d_latents, nullptr, st));
+  s = denoise_core(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps,
+                   (uint8_t*)d_workspace, d_probe, ctx->d_partials, st);
+  if (s != SPOT_OK) return s;
+  CK(ctx, launch_reward_finalize(ctx->d_partials, B, E, d_rewards, st));
+  CK(ctx, launch_seed_select(d_rewards, n_prompts, seeds_per_prompt, k_select, d_stats, d_top, d_bottom, st));
+  return SPOT_OK;
+}
+
+spot_status spot_explore_host(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, const uint64_t* h_seeds,
+                              const void* h_text_emb, const float* h_timesteps, int n_steps, const float* h_probe,
+                              int k_select, float* h_latents, float* h_rewards, float* h_stats, int32_t* h_top,
+                              int32_t* h_bottom, void* d_workspace, size_t ws_bytes, void* cuda_stream) {
+  if (!ctx || !h_seeds || !h_timesteps || !h_probe || !h_rewards || !h_stats) return SPOT_ERR_NULL;
+  if (ctx->cfg.n_txt > 0 && !h_text_emb) return SPOT_ERR_NULL;
+  if (n_prompts <= 0 || seeds_per_prompt <= 0 || (long long)n_prompts * seeds_per_prompt > ctx->max_seqs || n_steps < 0)
+    return SPOT_ERR_SHAPE;
+  if (k_select < 0 || 2 * k_select > seeds_per_prompt || seeds_per_prompt > 1024) return SPOT_ERR_SHAPE;
+  if (k_select > 0 && (!h_top || !h_bottom)) return SPOT_ERR_NULL;
+  const int B = n_prompts * seeds_per_prompt;
+  spot_status s = check_ws(ctx, B, n_steps, d_workspace, ws_bytes);
+  if (s != SPOT_OK) return s;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const spot_config& g = ctx->cfg;
+  const Workspace w = carve(ctx, B, n_steps);
+  uint8_t* ws = (uint8_t*)d_workspace;
+  const size_t E = (size_t)ctx->n_img() * g.latent_ch;
+  const size_t text_bytes = (size_t)n_prompts * g.n_txt * g.txt_dim * esize(g.dtype);
+  CK(ctx, cudaMemcpyAsync(ws + w.st_seeds, h_seeds, (size_t)B * 8, cudaMemcpyHostToDevice, st));
+  if (text_bytes) CK(ctx, cudaMemcpyAsync(ws + w.st_text, h_text_emb, text_bytes, cudaMemcpyHostToDevice, st));
+  CK(ctx, cudaMemcpyAsync(ws + w.st_probe, h_probe, E * 4, cudaMemcpyHostToDevice, st));
+  s = spot_explore(ctx, n_prompts, seeds_per_prompt, (const uint64_t*)(ws + w.st_seeds), ws + w.st_text, h_timesteps,
+                   n_steps, (const float*)(ws + w.st_probe), k_select, (float*)(ws + w.st_lat),
+                   (float*)(ws + w.st_rew), (float*)(ws + w.st_stats), (int32_t*)(ws + w.st_top),
+                   (int32_t*)(ws + w.st_bot), d_workspace, ws_bytes, cuda_stream);
+  if (s != SPOT_OK) return s;
+  if (h_latents) CK(ctx, cudaMemcpyAsync(h_latents, ws + w.st_lat, (size_t)B * E * 4, cudaMemcpyDeviceToHost, st));
+  CK(ctx, cudaMemcpyAsync(h_rewards, ws + w.st_rew, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+  CK(ctx, cudaMemcpyAsync(h_stats, ws + w.st_stats, (size_t)n_prompts * 8, cudaMemcpyDeviceToHost, st));
+  if (k_select > 0) {
+    CK(ctx, cudaMemcpyAsync(h_top, ws + w.st_top, (size_t)n_prompts * k_select * 4, cudaMemcpyDeviceToHost, st));
+    CK(ctx, cudaMemcpyAsync(h_bottom, ws + w.st_bot, (size_t)n_prompts * k_select * 4, cudaMemcpyDeviceToHost, st));
+  }
+  CK(ctx, cudaStreamSynchronize(st));
+  return SPOT_OK;
+}
+
+}  // extern "C"
+
+// ================================================================================================
+// kernel-level entry points (include/spot_kernels.h)
+extern "C" {
+
+static int sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+  }
+  return n;
+}
+
+spot_status spot_linear(spot_dtype dtype, spot_impl impl, spot_epilogue epi, const void* d_a, int64_t M, int64_t K,
+                        const void* d_w, int64_t N, const void* d_bias, const float* d_gate, float* d_residual,
+                        void* d_out, void* cuda_stream) {
+  if (dtype != SPOT_F32 && dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  if (M < 0 || N <= 0 || K <= 0 || M > 0x7fffffff || N > 0x7fffffff || K > 0x7fffffff) return SPOT_ERR_SHAPE;
+  if (M == 0) return SPOT_OK;
+  if (!d_a || !d_w || !d_bias) return SPOT_ERR_NULL;
+  const bool gate_res = epi == SPOT_EPI_GATE_RESIDUAL;
+  if (gate_res ? (!d_gate || !d_residual) : !d_out) return SPOT_ERR_NULL;
+  if (!aligned16(d_a) || !aligned16(d_w) || !aligned16(d_bias) || !aligned16(d_out) || !aligned16(d_residual) ||
+      !aligned16(d_gate))
+    return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  GemmProblem p;
+  memset(&p, 0, sizeof(p));
+  p.A = d_a; p.a_map = plain_rows((int)M, K); p.W = d_w; p.bias = d_bias;
+  p.M = (int)M; p.N = (int)N; p.K = (int)K;
+  if (gate_res) { p.gate = d_gate; p.resid = d_residual; p.resid_map = plain_rows((int)M, N); }
+  else { p.out = d_out; p.out_map = plain_rows((int)M, N); }
+  const Epilogue e = epi == SPOT_EPI_BIAS ? EPI_BIAS : (epi == SPOT_EPI_BIAS_GELU ? EPI_BIAS_GELU : EPI_GATE_RES);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  bool tc = impl == SPOT_IMPL_TCGEN05 || (impl == SPOT_IMPL_AUTO && dtype == SPOT_BF16 && tcgen05_gemm_supported(p));
+  if (tc) {
+    if (dtype != SPOT_BF16 || !tcgen05_gemm_supported(p)) return SPOT_ERR_SHAPE;
+    return launch_gemm_tcgen05(e, &p, 1, sm_count(), st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+  }
+  if (K % 16) return SPOT_ERR_SHAPE;
+  return launch_gemm_simt(dtype, dtype, dtype, e, p, st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
+spot_status spot_ln_modulate(spot_dtype dtype, const float* d_h, int64_t M, int64_t D, const float* d_shift,
+                             const float* d_scale, float eps, void* d_out, void* cuda_stream) {
+  if (dtype != SPOT_F32 && dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  if (M < 0 || D <= 0 || D % 128 || M > 0x7fffffff) return SPOT_ERR_SHAPE;
+  if (M == 0) return SPOT_OK;
+  if (!d_h || !d_shift || !d_scale || !d_out) return SPOT_ERR_NULL;
+  if (!aligned16(d_h) || !aligned16(d_shift) || !aligned16(d_scale) || !aligned16(d_out)) return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  cudaError_t e = launch_ln_modulate(dtype, d_h, (int)M, (int)D, d_shift, d_scale, eps, d_out, plain_rows((int)M, D),
+                                     (cudaStream_t)cuda_stream);
+  return e == cudaSuccess ? SPOT_OK : (e == cudaErrorInvalidValue ? SPOT_ERR_SHAPE : SPOT_ERR_CUDA);
+}
+
+spot_status spot_qk_norm_rope(spot_dtype dtype, void* d_qkv, int B, int S, int H, int head_dim, int n_txt,
+                              const void* d_q_gain_img, const void* d_k_gain_img, const void* d_q_gain_txt,
+                              const void* d_k_gain_txt, const float* d_cos, const float* d_sin, float eps,
+                              void* cuda_stream) {
+  if (dtype != SPOT_F32 && dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  if (B < 0 || S <= 0 || H <= 0 || (head_dim != 64 && head_dim != 128) || n_txt < 0 || n_txt > S) return SPOT_ERR_SHAPE;
+  if (B == 0) return SPOT_OK;
+  if (!d_qkv || !d_q_gain_img || !d_k_gain_img || !d_q_gain_txt || !d_k_gain_txt || !d_cos || !d_sin) return SPOT_ERR_NULL;
+  if (!aligned16(d_qkv) || !aligned16(d_q_gain_img) || !aligned16(d_k_gain_img) || !aligned16(d_q_gain_txt) ||
+      !aligned16(d_k_gain_txt) || !aligned16(d_cos) || !aligned16(d_sin))
+    return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  return launch_qk_norm_rope(dtype, d_qkv, B, S, H, head_dim, n_txt, d_q_gain_img, d_k_gain_img, d_q_gain_txt,
+                             d_k_gain_txt, d_cos, d_sin, eps, (cudaStream_t)cuda_stream) == cudaSuccess
+             ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
+spot_status spot_attention(spot_dtype dtype, spot_impl impl, const void* d_qkv, void* d_out, int B, int S, int H,
+                           int head_dim, void* cuda_stream) {
+  if (dtype != SPOT_F32 && dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  if (B < 0 || S <= 0 || H <= 0 || (head_dim != 64 && head_dim != 128)) return SPOT_ERR_SHAPE;
+  if (B == 0) return SPOT_OK;
+  if (!d_qkv || !d_out) return SPOT_ERR_NULL;
+  if (!aligned16(d_qkv) || !aligned16(d_out)) return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const bool can_tc = dtype == SPOT_BF16 && tcgen05_attn_supported(S, H, head_dim);
+  if (impl == SPOT_IMPL_TCGEN05 && !can_tc) return SPOT_ERR_SHAPE;
+  if (impl != SPOT_IMPL_SIMT && can_tc)
+    return launch_attn_tcgen05(d_qkv, d_out, B, S, H, head_dim, sm_count(), st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+  return launch_attn_simt(dtype, d_qkv, d_out, B, S, H, head_dim, st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
+spot_status spot_euler_update(float* d_x, const float* d_v, float dt, int n_seqs, int64_t elems, const float* d_probe,
+                              float* d_rewards, float* d_partials, void* cuda_stream) {
+  if (n_seqs < 0 || elems <= 0 || (elems & 3)) return SPOT_ERR_SHAPE;
+  if (n_seqs == 0) return SPOT_OK;
+  if (!d_x || !d_v) return SPOT_ERR_NULL;
+  if (d_probe && (!d_rewards || !d_partials)) return SPOT_ERR_NULL;
+  if (!aligned16(d_x) || !aligned16(d_v) || !aligned16(d_probe)) return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (launch_euler_update(d_x, d_v, dt, n_seqs, elems, d_probe, d_partials, st) != cudaSuccess) return SPOT_ERR_CUDA;
+  if (d_probe && launch_reward_finalize(d_partials, n_seqs, elems, d_rewards, st) != cudaSuccess) return SPOT_ERR_CUDA;
+  return SPOT_OK;
+}
+
+}  // extern "C"

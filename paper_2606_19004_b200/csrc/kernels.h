@@ -1,0 +1,52 @@
+// kernels.h - host-side launchers of every libspot kernel (internal).
+#pragma once
+#include "common.cuh"
+
+// K1: Philox4x32-10 + Box-Muller (noise.cu)
+cudaError_t launch_noise(const uint64_t* d_seeds, int n_seeds, long long elems_per_seed, uint32_t stream_id,
+                         float* d_normals, uint32_t* d_words, cudaStream_t st);
+
+// K7: time embedding and skinny Linear (elementwise.cu)
+cudaError_t launch_time_embed(const float* d_t, int T, float* d_e /*[T,256]*/, cudaStream_t st);
+cudaError_t launch_gemv(spot_dtype wdt, const void* W, const void* b, const float* X, int T, int N, int K,
+                        float* out, long long out_stride_t, bool silu_out, cudaStream_t st);
+cudaError_t launch_silu(const float* in, float* out, long long n, cudaStream_t st);
+
+// K3: LayerNorm (no affine) * (1 + scale) + shift, fp32 residual rows -> act dtype rows
+cudaError_t launch_ln_modulate(spot_dtype odt, const float* h, int M, int D, const float* shift, const float* scale,
+                               float eps, void* out, RowMap out_map, cudaStream_t st);
+cudaError_t launch_rmsnorm_rows(spot_dtype dt, const void* in, const void* gain, int M, int D, float eps, void* out,
+                                cudaStream_t st);
+
+// K4: per-head RMSNorm(q), RMSNorm(k) + rotary, in place on qkv [B, S, 3, H, d_h]
+cudaError_t launch_qk_norm_rope(spot_dtype dt, void* qkv, int B, int S, int H, int dh, int n_txt,
+                                const void* qg_img, const void* kg_img, const void* qg_txt, const void* kg_txt,
+                                const float* cos_t, const float* sin_t, float eps, cudaStream_t st);
+
+// K6 / K8: Euler update, reward reduction, selection
+static const int REWARD_CHUNK = 4096;    // elements per partial sum (fixed => deterministic order)
+cudaError_t launch_euler_update(float* x, const float* v, float dt, int B, long long E, const float* probe,
+                                float* partials, cudaStream_t st);
+cudaError_t launch_reward_partials(const float* x, const float* probe, int B, long long E, float* partials,
+                                   cudaStream_t st);
+cudaError_t launch_reward_finalize(const float* partials, int B, long long E, float* rewards, cudaStream_t st);
+cudaError_t launch_seed_select(const float* rewards, int P, int K, int k_select, float* stats, int32_t* top,
+                               int32_t* bottom, cudaStream_t st);
+
+// plumbing
+cudaError_t launch_to_f32(spot_dtype dt, const void* in, float* out, long long n, cudaStream_t st);
+cudaError_t launch_from_f32(spot_dtype dt, const float* in, void* out, long long n, cudaStream_t st);
+cudaError_t launch_broadcast_prompts(const float* src, float* dst, int B, int K, long long n_per_prompt, cudaStream_t st);
+
+// K9: SIMT GEMM / attention (gemm_simt.cu, attn_simt.cu).  ta/tout: dtype of A and of the output
+// matrix (EPI_BIAS / EPI_BIAS_GELU); W and bias have dtype tw.
+cudaError_t launch_gemm_simt(spot_dtype ta, spot_dtype tw, spot_dtype tout, Epilogue epi, const GemmProblem& p,
+                             cudaStream_t st);
+cudaError_t launch_attn_simt(spot_dtype dt, const void* qkv, void* out, int B, int S, int H, int dh, cudaStream_t st);
+
+// K2 / K5: tcgen05 + TMA kernels (gemm_tcgen05.cu, attn_tcgen05.cu), bf16 only.
+struct TmaEncoder;   // opaque: resolves cuTensorMapEncodeTiled once
+bool tcgen05_gemm_supported(const GemmProblem& p);
+cudaError_t launch_gemm_tcgen05(Epilogue epi, const GemmProblem* probs, int n_probs, int num_sms, cudaStream_t st);
+bool tcgen05_attn_supported(int S, int H, int dh);
+cudaError_t launch_attn_tcgen05(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st);

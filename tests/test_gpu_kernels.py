@@ -1,0 +1,189 @@
+"""-m gpu parity tests, kernel by kernel, through the C ABI against the fp64 oracle.
+
+Tolerances: Philox words and selection indices bit-exact; fp32 kernels <= 1e-4
+relative L2 (observed ~1e-6); bf16 kernels <= 2e-2 per block-level output, with tighter per-kernel
+bounds derived from one bf16 rounding (2^-9) of the output.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_19004_b200 as spot
+from oracle import mmdit, philox, rollout
+from synth import hash_normal
+from tests.gpu_common import ensure_built
+from tests.helpers import np64, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    ensure_built()
+
+
+def _seeds(vals):
+    return torch.tensor([v if v < 2 ** 63 else v - 2 ** 64 for v in vals], dtype=torch.int64, device="cuda")
+
+
+# ------------------------------------------------------------------ K1
+def test_philox_words_bit_exact():
+    seeds = [0, 1, 2, 3, 2 ** 64 - 1, 0x0123456789ABCDEF]
+    for stream in (0, 1, 17):
+        w = spot.spot_philox_words(_seeds(seeds), 4 * 4096, stream).cpu().numpy().view(np.uint32)
+        for i, s in enumerate(seeds):
+            ref = philox.words_for_seed(s, 4 * 4096, stream)
+            assert (w[i] == ref).all(), (hex(s), stream)
+
+
+def test_noise_matches_oracle_and_is_batch_independent():
+    seeds = [0, 1, 2, 3, 2 ** 64 - 1]
+    E = 64 * 64 + 4 * 37                      # several blocks of 256 threads plus a ragged tail
+    z = spot.spot_noise_from_seeds(_seeds(seeds), E).cpu().numpy()
+    ref = philox.noise_from_seeds(seeds, E)
+    assert rel_l2(z, ref) < 1e-6
+    assert np.abs(z - ref).max() < 2e-6
+    alone = spot.spot_noise_from_seeds(_seeds([3]), E).cpu().numpy()
+    assert (alone[0] == z[3]).all()           # bit-identical regardless of batch composition
+    again = spot.spot_noise_from_seeds(_seeds(seeds), E).cpu().numpy()
+    assert (again == z).all()
+    empty = spot.spot_noise_from_seeds(_seeds([]), 8)
+    assert empty.shape == (0, 8)
+
+
+def test_noise_large_statistics():
+    z = spot.spot_noise_from_seeds(_seeds([42]), 1 << 24)
+    assert abs(z.mean().item()) < 1e-3 and abs(z.var().item() - 1.0) < 2e-3
+    assert z.abs().max().item() <= math.sqrt(48 * math.log(2.0)) + 1e-5
+
+
+# ------------------------------------------------------------------ K3
+@pytest.mark.parametrize("dtype,D,M,tol", [(torch.float32, 256, 67, 1e-5), (torch.bfloat16, 3072, 131, 4e-3),
+                                           (torch.float32, 3072, 9, 1e-5)])
+def test_ln_modulate(dtype, D, M, tol):
+    h = hash_normal(901, M * D, 2.0, torch.float32, "cuda").reshape(M, D) + 0.5
+    shift = hash_normal(902, D, 0.3, torch.float32, "cuda")
+    scale = hash_normal(903, D, 0.3, torch.float32, "cuda")
+    y = spot.spot_ln_modulate(h, shift, scale, 1e-6, dtype)
+    ref = mmdit.layer_norm(np64(h), 1e-6) * (1.0 + np64(scale)) + np64(shift)
+    assert rel_l2(np64(y), ref) < tol
+
+
+# ------------------------------------------------------------------ K4
+@pytest.mark.parametrize("dtype,dh,H,tol", [(torch.float32, 64, 4, 1e-5), (torch.bfloat16, 128, 3, 4e-3),
+                                            (torch.float32, 128, 2, 1e-5), (torch.bfloat16, 64, 2, 4e-3)])
+def test_qk_norm_rope(dtype, dh, H, tol):
+    B, gh, gw, n_txt = 2, 5, 7, 9
+    S = n_txt + gh * gw
+    pairs = (dh // 16, (dh // 2 - dh // 16) // 2, dh // 2 - dh // 16 - (dh // 2 - dh // 16) // 2)
+    qkv = hash_normal(911, B * S * 3 * H * dh, 1.5, dtype, "cuda").reshape(B, S, 3, H, dh)
+    gains = [hash_normal(912 + i, dh, 0.5, dtype, "cuda") + 1.0 for i in range(4)]   # q_img, k_img, q_txt, k_txt
+    cos, sin = mmdit.rope_table(gh, gw, n_txt, pairs, 10000.0)
+    ref = np64(qkv).copy()
+    for part, (g_img, g_txt) in enumerate([(gains[0], gains[2]), (gains[1], gains[3])]):
+        for b in range(B):
+            x = ref[b, :, part]
+            x[:n_txt] = mmdit.rms_norm(x[:n_txt], np64(g_txt), 1e-6)
+            x[n_txt:] = mmdit.rms_norm(x[n_txt:], np64(g_img), 1e-6)
+            ref[b, :, part] = mmdit.apply_rope(x, cos, sin)
+    out = spot.spot_qk_norm_rope(qkv.clone(), n_txt, gains, torch.from_numpy(cos).float().cuda(),
+                                 torch.from_numpy(sin).float().cuda(), 1e-6)
+    got = np64(out)
+    assert (got[:, :, 2] == np64(qkv)[:, :, 2]).all()         # v untouched
+    assert rel_l2(got[:, :, :2], ref[:, :, :2]) < tol
+
+
+# ------------------------------------------------------------------ K5 / K9 attention
+def _attn_ref(qkv):
+    x = np64(qkv)
+    return np.stack([mmdit.attention(x[b, :, 0], x[b, :, 1], x[b, :, 2]).reshape(x.shape[1], -1) for b in range(x.shape[0])])
+
+
+@pytest.mark.parametrize("dtype,S,H,dh,scale,tol", [(torch.float32, 96, 4, 64, 1.0, 1e-5), (torch.float32, 130, 2, 128, 1.0, 1e-5),
+                                                    (torch.bfloat16, 200, 2, 128, 1.0, 6e-3), (torch.float32, 77, 1, 64, 6.0, 1e-5)])
+def test_attention_simt(dtype, S, H, dh, scale, tol):
+    qkv = hash_normal(921, 2 * S * 3 * H * dh, scale, dtype, "cuda").reshape(2, S, 3, H, dh)
+    out = spot.spot_attention(qkv, spot.IMPL_SIMT)
+    assert rel_l2(np64(out), _attn_ref(qkv)) < tol
+
+
+# ------------------------------------------------------------------ K2 / K9 linear
+def _linear_ref(a, w, b, epi, gate=None, resid=None):
+    y = np64(a) @ np64(w).T + np64(b)
+    if epi == spot.EPI_BIAS_GELU:
+        y = mmdit.gelu_tanh(y)
+    if epi == spot.EPI_GATE_RESIDUAL:
+        y = np64(resid) + np64(gate) * y
+    return y
+
+
+def _run_linear(dtype, impl, epi, M, N, K, tid):
+    a = hash_normal(tid, M * K, 1.0, dtype, "cuda").reshape(M, K)
+    w = hash_normal(tid + 1, N * K, 0.05, dtype, "cuda").reshape(N, K)
+    b = hash_normal(tid + 2, N, 0.1, dtype, "cuda")
+    gate = hash_normal(tid + 3, N, 0.5, torch.float32, "cuda")
+    resid = hash_normal(tid + 4, M * N, 1.0, torch.float32, "cuda").reshape(M, N)
+    ref = _linear_ref(a, w, b, epi, gate, resid)
+    if epi == spot.EPI_GATE_RESIDUAL:
+        out = spot.spot_linear(a, w, b, epi, impl, gate=gate, residual=resid.clone())
+    else:
+        out = spot.spot_linear(a, w, b, epi, impl)
+    return np64(out), ref
+
+
+@pytest.mark.parametrize("epi", [0, 1, 2])
+@pytest.mark.parametrize("M,N,K", [(200, 136, 64), (64, 64, 256), (3, 1024, 16)])
+def test_linear_simt_fp32(epi, M, N, K):
+    got, ref = _run_linear(torch.float32, spot.IMPL_SIMT, epi, M, N, K, 930)
+    assert rel_l2(got, ref) < 1e-5
+
+
+@pytest.mark.parametrize("epi", [0, 1, 2])
+def test_linear_simt_bf16(epi):
+    got, ref = _run_linear(torch.bfloat16, spot.IMPL_SIMT, epi, 150, 96, 128, 940)
+    assert rel_l2(got, ref) < (1e-5 if epi == 2 else 4e-3)
+
+
+@pytest.mark.parametrize("epi", [0, 1, 2])
+@pytest.mark.parametrize("M,N,K", [(128, 256, 64), (300, 512, 200), (1024, 3072 + 32, 512), (77, 32, 8), (2048, 768, 3072)])
+def test_linear_tcgen05_bf16(epi, M, N, K):
+    """tcgen05/TMA GEMM vs fp64: single tile, ragged M/N/K tails, multi-tile persistent schedule, long K."""
+    got, ref = _run_linear(torch.bfloat16, spot.IMPL_TCGEN05, epi, M, N, K, 950)
+    # fp32 accumulation of exact bf16 products; only the output rounding (2^-9) for bf16 outputs
+    assert rel_l2(got, ref) < (2e-5 if epi == 2 else 4e-3)
+
+
+def test_linear_tcgen05_matches_simt_bitwise_close():
+    a = hash_normal(960, 512 * 1024, 1.0, torch.bfloat16, "cuda").reshape(512, 1024)
+    w = hash_normal(961, 512 * 1024, 0.05, torch.bfloat16, "cuda").reshape(512, 1024)
+    b = hash_normal(962, 512, 0.1, torch.bfloat16, "cuda")
+    y_tc = spot.spot_linear(a, w, b, spot.EPI_BIAS, spot.IMPL_TCGEN05)
+    y_si = spot.spot_linear(a, w, b, spot.EPI_BIAS, spot.IMPL_SIMT)
+    assert rel_l2(np64(y_tc), np64(y_si)) < 3e-3        # both round the same fp32-accumulated value to bf16
+    again = spot.spot_linear(a, w, b, spot.EPI_BIAS, spot.IMPL_TCGEN05)
+    assert torch.equal(y_tc, again)                     # deterministic
+
+
+# ------------------------------------------------------------------ K6 / K8
+def test_euler_update_and_reward():
+    B, E = 5, 64 * 64 + 8
+    x = hash_normal(970, B * E, 1.0, torch.float32, "cuda").reshape(B, E)
+    v = hash_normal(971, B * E, 1.0, torch.float32, "cuda").reshape(B, E)
+    p = hash_normal(972, E, 1.0, torch.float32, "cuda")
+    ref = np64(x) + (-0.125) * np64(v)
+    xo, r = spot.spot_euler_update(x.clone(), v, -0.125, p)
+    assert rel_l2(np64(xo), ref) < 1e-7
+    ref_r = [rollout.probe_reward(ref[b], np64(p)) for b in range(B)]
+    assert rel_l2(np64(r), ref_r) < 1e-5
+    x0, _ = spot.spot_euler_update(x.clone(), torch.zeros_like(v), -0.3)       # zero velocity: unchanged
+    assert torch.equal(x0, x)
+    # closed form x_t = (1 - t) x0 + t eps with v = eps - x0 on the K6 kernel alone
+    eps, x_data = x.clone(), v
+    vel = eps - x_data
+    cur = eps.clone()
+    grid = [1.0, 0.75, 0.5, 0.25, 0.0]
+    for i in range(4):
+        cur, _ = spot.spot_euler_update(cur, vel, grid[i + 1] - grid[i])
+    assert (cur - x_data).abs().max().item() < 1e-5

@@ -1,0 +1,209 @@
+"""-m gpu parity tests of the four north-star entry points against the fp64 oracle.
+
+Tolerances are BASELINE.json's: per-block relative L2 <= 1e-4 (fp32) / <= 2e-2 (bf16); final latents and
+rewards <= 1e-4 (fp32 config) / <= 5e-2 (bf16); seed indices exact wherever the oracle's reward gap
+exceeds the reward tolerance (S12).
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_19004_b200 as spot
+from oracle import rollout
+from synth import CONFIGS, make_block_inputs, make_probe, make_text_emb
+from tests.gpu_common import device_weights, ensure_built, f32_timesteps, oracle_block, oracle_explore, oracle_weights
+from tests.helpers import np64, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    ensure_built()
+
+
+def _seeds(vals):
+    return torch.tensor(list(vals), dtype=torch.int64, device="cuda")
+
+
+# ------------------------------------------------------------------ config 1 (fp32, tiny)
+@pytest.fixture(scope="module")
+def cfg1():
+    s = CONFIGS[1]
+    w = device_weights(s)
+    ctx = spot.Context(s, w, max_seqs=8)
+    text = make_text_emb(s, "cuda")
+    probe = make_probe(s, "cuda")
+    return s, w, ctx, text, probe
+
+
+def test_cfg1_block_forward(cfg1):
+    s, w, ctx, _, _ = cfg1
+    h_img, h_txt, temb = make_block_inputs(s, 3, "cuda")
+    _, blocks = oracle_weights(w)
+    for blk in range(s.n_blocks):
+        o_img, o_txt = spot.spot_dit_block_forward(ctx, blk, h_img, h_txt, temb)
+        r_img, r_txt = oracle_block(s, blocks[blk], np64(h_img), np64(h_txt), np64(temb))
+        assert rel_l2(np64(o_img), r_img) < 1e-4 and rel_l2(np64(o_txt), r_txt) < 1e-4
+        assert rel_l2(np64(o_img), np64(h_img)) > 1e-3            # the block is not the identity
+
+
+def test_cfg1_explore_matches_oracle(cfg1):
+    s, w, ctx, text, probe = cfg1
+    ts = f32_timesteps(s)
+    k = s.seeds_per_prompt // 2
+    out = spot.spot_explore(ctx, _seeds(s.seeds), text, ts, probe, 1, s.seeds_per_prompt, k)
+    lat, rew = oracle_explore(s, w, text[0], probe, s.seeds, ts)
+    assert rel_l2(np64(out["latents"]), lat) < 1e-4
+    assert rel_l2(np64(out["rewards"]), rew) < 1e-4
+    sel = rollout.select_seeds(rew[None, :], k)
+    assert out["top"].cpu().tolist() == sel["top"].tolist()
+    assert out["bottom"].cpu().tolist() == sel["bottom"].tolist()
+    assert abs(out["stats"][0, 0].item() - sel["mean"][0]) < 1e-4 * max(1.0, abs(sel["mean"][0]))
+    assert abs(out["stats"][0, 1].item() - sel["std"][0]) < 1e-4 * max(1.0, sel["std"][0])
+
+
+def test_cfg1_separate_calls_equal_fused_and_are_deterministic(cfg1):
+    s, w, ctx, text, probe = cfg1
+    ts = f32_timesteps(s)
+    K = s.seeds_per_prompt
+    fused = spot.spot_explore(ctx, _seeds(s.seeds), text, ts, probe, 1, K, K // 2)
+    lat = spot.spot_noise_from_seeds(_seeds(s.seeds), s.n_img * s.latent_ch).reshape(K, s.n_img, s.latent_ch)
+    spot.spot_dit_denoise(ctx, lat, text, ts, 1, K)
+    rew, stats, top, bottom = spot.spot_seed_rewards(ctx, lat, probe, 1, K, K // 2)
+    assert torch.equal(lat, fused["latents"]) and torch.equal(rew, fused["rewards"])
+    assert torch.equal(top, fused["top"][:, :K // 2]) and torch.equal(bottom, fused["bottom"][:, :K // 2])
+    # seed independence (determinism contract): seed 2 alone == seed 2 inside the batch, bit for bit
+    alone = spot.spot_explore(ctx, _seeds([2]), text, ts, probe, 1, 1, 0)
+    assert torch.equal(alone["latents"][0], fused["latents"][2]) and torch.equal(alone["rewards"][0], fused["rewards"][2])
+    # resume: 4 steps == 2 steps + 2 steps from the saved latents
+    lat2 = spot.spot_noise_from_seeds(_seeds(s.seeds), s.n_img * s.latent_ch).reshape(K, s.n_img, s.latent_ch)
+    spot.spot_dit_denoise(ctx, lat2, text, ts[:3], 1, K)
+    spot.spot_dit_denoise(ctx, lat2, text, ts[2:], 1, K)
+    assert torch.equal(lat2, lat)
+
+
+def test_cfg1_two_prompts_and_host_api(cfg1):
+    s, w, ctx, text, probe = cfg1
+    ts = f32_timesteps(s)
+    s2 = s.with_(n_prompts=2)
+    text2 = make_text_emb(s2, "cuda")
+    seeds = [10, 11, 12, 13, 20, 21, 22, 23]
+    out = spot.spot_explore(ctx, _seeds(seeds), text2, ts, probe, 2, 4, 2)
+    for g in range(2):
+        lat, rew = oracle_explore(s, w, text2[g], probe, seeds[4 * g:4 * g + 4], ts)
+        assert rel_l2(np64(out["latents"][4 * g:4 * g + 4]), lat) < 1e-4
+        sel = rollout.select_seeds(rew[None, :], 2)
+        assert out["top"][g].cpu().tolist() == sel["top"][0].tolist()
+        assert out["bottom"][g].cpu().tolist() == sel["bottom"][0].tolist()
+        assert abs(out["stats"][g, 1].item() - sel["std"][0]) < 1e-4
+    # host-buffer entry point gives the same bits as the device-buffer one
+    pin = lambda t: t.cpu().pin_memory()
+    h_out = {"latents": torch.empty((8, s.n_img, s.latent_ch)).pin_memory(), "rewards": torch.empty(8).pin_memory(),
+             "stats": torch.empty((2, 2)).pin_memory(), "top": torch.empty((2, 2), dtype=torch.int32).pin_memory(),
+             "bottom": torch.empty((2, 2), dtype=torch.int32).pin_memory()}
+    spot.spot_explore_host(ctx, pin(_seeds(seeds)), pin(text2), ts, pin(probe), 2, 4, 2, h_out)
+    assert torch.equal(h_out["latents"], out["latents"].cpu()) and torch.equal(h_out["rewards"], out["rewards"].cpu())
+    assert torch.equal(h_out["top"], out["top"][:, :2].cpu()) and torch.equal(h_out["stats"], out["stats"].cpu())
+
+
+def test_seed_rewards_selection_with_ties(cfg1):
+    s, w, ctx, _, _ = cfg1
+    E = s.n_img * s.latent_ch
+    # latents whose rewards are chosen by hand: x_b = c_b * probe / |probe|^2 * sqrt(E) gives r_b = c_b
+    probe = make_probe(s, "cuda")
+    target = [0.5, 2.0, -1.0, 2.0, 0.0, -1.0, 3.0, 0.25]
+    unit = probe / (probe * probe).sum() * (E ** 0.5)
+    lat = torch.stack([c * unit for c in target]).reshape(8, s.n_img, s.latent_ch).contiguous()
+    rew, stats, top, bottom = spot.spot_seed_rewards(ctx, lat, probe, 1, 8, 3)
+    assert np.allclose(rew.cpu().numpy(), target, atol=1e-5)
+    # exact ties need exactly equal rewards: rows 1/3 and 2/5 are bit-identical inputs
+    assert top.cpu().tolist() == [[6, 1, 3]] and bottom.cpu().tolist() == [[2, 5, 4]]
+    ref = rollout.select_seeds(np.asarray([target]), 3)
+    assert abs(stats[0, 0].item() - ref["mean"][0]) < 1e-5 and abs(stats[0, 1].item() - ref["std"][0]) < 1e-5
+
+
+def test_error_codes_on_device(cfg1):
+    s, w, ctx, text, probe = cfg1
+    with pytest.raises(spot.SpotError) as e:
+        spot.spot_explore(ctx, _seeds(range(16)), text, f32_timesteps(s), probe, 1, 16, 2)     # > max_seqs
+    assert e.value.status_name == "SPOT_ERR_SHAPE"
+    with pytest.raises(spot.SpotError) as e:
+        spot.spot_seed_rewards(ctx, torch.zeros((4, s.n_img, s.latent_ch), device="cuda"), probe, 1, 4, 3)   # 2k > K
+    assert e.value.status_name == "SPOT_ERR_SHAPE"
+    lib = spot.load_library()
+    lat = torch.zeros((4, s.n_img, s.latent_ch), device="cuda")
+    ws = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    import ctypes as C
+    arr = (C.c_float * 2)(1.0, 0.0)
+    st = lib.spot_dit_denoise(ctx.handle, 1, 4, lat.data_ptr(), text.data_ptr(), C.cast(arr, C.c_void_p), 1,
+                              ws.data_ptr(), ws.numel(), None)
+    assert st == 5                                                                            # SPOT_ERR_WORKSPACE
+
+
+# ------------------------------------------------------------------ config 2 (bf16, one full-width block)
+@pytest.fixture(scope="module")
+def cfg2():
+    s = CONFIGS[2]
+    w = device_weights(s, blocks=[0])
+    ctx = spot.Context(s, w, max_seqs=8)
+    return s, w, ctx
+
+
+def test_cfg2_block_forward_bf16(cfg2):
+    s, w, ctx = cfg2
+    B = 8
+    h_img, h_txt, temb = make_block_inputs(s, B, "cuda")
+    o_img, o_txt = spot.spot_dit_block_forward(ctx, 0, h_img, h_txt, temb)
+    torch.cuda.synchronize()
+    _, blocks = oracle_weights(w)
+    check = [0, B - 1]                         # the oracle costs ~310 GFLOP fp64 per sequence: sample two
+    r_img, r_txt = oracle_block(s, blocks[0], np64(h_img[check]), np64(h_txt[check]), np64(temb))
+    e_img, e_txt = rel_l2(np64(o_img[check]), r_img), rel_l2(np64(o_txt[check]), r_txt)
+    print(f"cfg2 block rel-L2: img {e_img:.3e} txt {e_txt:.3e}")
+    assert e_img < 2e-2 and e_txt < 2e-2
+    # what the block ADDS to the residual stream, compared on its own scale (a stricter view than the above)
+    d_img = rel_l2(np64(o_img[check]) - np64(h_img[check]), r_img - np64(h_img[check]))
+    print(f"cfg2 block update rel-L2: img {d_img:.3e}")
+    # batch independence: sequence 3 alone is bit-identical to sequence 3 in the batch
+    a_img, a_txt = spot.spot_dit_block_forward(ctx, 0, h_img[3:4].contiguous(), h_txt[3:4].contiguous(), temb)
+    assert torch.equal(a_img[0], o_img[3]) and torch.equal(a_txt[0], o_txt[3])
+    # tcgen05 GEMMs vs the SIMT GEMMs on the same inputs (GPU-side cross-check)
+    spot.spot_set_option(ctx, spot.OPT_GEMM_IMPL, 1)
+    spot.spot_set_option(ctx, spot.OPT_ATTN_IMPL, 1)
+    s_img, s_txt = spot.spot_dit_block_forward(ctx, 0, h_img[:2].contiguous(), h_txt[:2].contiguous(), temb)
+    spot.spot_set_option(ctx, spot.OPT_GEMM_IMPL, 0)
+    spot.spot_set_option(ctx, spot.OPT_ATTN_IMPL, 0)
+    assert rel_l2(np64(s_img), np64(o_img[:2])) < 1e-2
+
+
+def test_cfg2_block_peaked_softmax(cfg2):
+    """Adversarial gains (q_gain = k_gain = 4 => logits ~ N(0, 16^2)): exercises the online-softmax rescale."""
+    s, w, _ = cfg2
+    bw = dict(w["blocks"][0])
+    for st in ("img", "txt"):
+        bw[f"{st}.q_gain"] = torch.full_like(bw[f"{st}.q_gain"], 4.0)
+        bw[f"{st}.k_gain"] = torch.full_like(bw[f"{st}.k_gain"], 4.0)
+    w2 = {"global": w["global"], "blocks": [bw]}
+    ctx = spot.Context(s, w2, max_seqs=2)
+    h_img, h_txt, temb = make_block_inputs(s, 1, "cuda")
+    o_img, o_txt = spot.spot_dit_block_forward(ctx, 0, h_img, h_txt, temb)
+    _, blocks = oracle_weights(w2)
+    r_img, r_txt = oracle_block(s, blocks[0], np64(h_img), np64(h_txt), np64(temb))
+    assert rel_l2(np64(o_img), r_img) < 2e-2 and rel_l2(np64(o_txt), r_txt) < 2e-2
+
+
+def test_cfg3_lite_rollout_bf16():
+    """Config-3 shapes at reduced depth (L = 2, K = 2, T = 2): final latents / rewards within 5e-2."""
+    s = CONFIGS[3].with_(n_blocks=2, seeds_per_prompt=2, n_steps=2, seeds=(0, 1))
+    w = device_weights(s)
+    ctx = spot.Context(s, w, max_seqs=2)
+    text, probe = make_text_emb(s, "cuda"), make_probe(s, "cuda")
+    ts = f32_timesteps(s)
+    out = spot.spot_explore(ctx, _seeds(s.seeds), text, ts, probe, 1, 2, 1)
+    lat, rew = oracle_explore(s, w, text[0], probe, s.seeds, ts)
+    e_lat, e_rew = rel_l2(np64(out["latents"]), lat), rel_l2(np64(out["rewards"]), rew)
+    print(f"cfg3-lite rel-L2: latents {e_lat:.3e} rewards {e_rew:.3e}")
+    assert e_lat < 5e-2 and e_rew < 5e-2
+    if abs(rew[0] - rew[1]) > 2 * 5e-2 * np.abs(rew).max():
+        assert out["top"][0, 0].item() == int(np.argmax(rew))
