@@ -93,7 +93,8 @@ typedef struct spot_ctx spot_ctx;
 /* Options for spot_set_option. */
 typedef enum {
   SPOT_OPT_GEMM_IMPL = 0,   /* 0 = auto (tcgen05 for bf16), 1 = force the SIMT FFMA GEMM */
-  SPOT_OPT_ATTN_IMPL = 1    /* 0 = auto (tcgen05 for bf16, d_h = 128), 1 = force the SIMT attention */
+  SPOT_OPT_ATTN_IMPL = 1,   /* 0 = auto (tcgen05 for bf16, d_h = 128), 1 = force the SIMT attention */
+  SPOT_OPT_TIMING = 2       /* 1 = bracket every tcgen05 GEMM launch with CUDA events on the launch stream */
 } spot_option;
 
 /* Validates cfg and w, builds the RoPE table (S5) and returns a context.  max_seqs bounds
@@ -104,6 +105,11 @@ spot_status spot_set_option(spot_ctx *ctx, spot_option opt, int value);
 /* Bytes of device workspace needed by spot_dit_block_forward / spot_dit_denoise / spot_explore*
  * for n_seqs sequences and up to n_steps Euler steps (n_prompts <= n_seqs is assumed). */
 spot_status spot_workspace_bytes(const spot_ctx *ctx, int n_seqs, int n_steps, size_t *bytes);
+/* Counters since the last reset: kernels launched through ctx, tcgen05 GEMM launches, how many of those
+ * were event-timed (SPOT_OPT_TIMING) and their summed device time in ms.  The caller must have
+ * synchronised the stream(s) first.  Any output pointer may be NULL. */
+spot_status spot_get_counters(spot_ctx *ctx, uint64_t *launches, uint64_t *gemm_launches, uint64_t *gemm_timed,
+                              double *gemm_ms, int reset);
 const char *spot_status_string(spot_status s);
 int spot_last_cuda_error(const spot_ctx *ctx);          /* cudaError_t of the last failed CUDA call */
 const char *spot_version(void);

@@ -19,7 +19,7 @@ _lib: Optional[C.CDLL] = None
 SPOT_F32, SPOT_BF16 = 0, 1
 EPI_BIAS, EPI_BIAS_GELU, EPI_GATE_RESIDUAL = 0, 1, 2
 IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05 = 0, 1, 2
-OPT_GEMM_IMPL, OPT_ATTN_IMPL = 0, 1
+OPT_GEMM_IMPL, OPT_ATTN_IMPL, OPT_TIMING = 0, 1, 2
 STATUS_NAMES = ["SPOT_OK", "SPOT_ERR_NULL", "SPOT_ERR_SHAPE", "SPOT_ERR_DTYPE", "SPOT_ERR_ALIGN",
                 "SPOT_ERR_WORKSPACE", "SPOT_ERR_ARCH", "SPOT_ERR_CUDA", "SPOT_ERR_UNIMPLEMENTED"]
 
@@ -78,6 +78,8 @@ def load_library() -> C.CDLL:
         "spot_set_option": [vp, i32, i32],
         "spot_workspace_bytes": [vp, i32, i32, C.POINTER(sz)],
         "spot_last_cuda_error": [vp],
+        "spot_get_counters": [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64),
+                              C.POINTER(C.c_double), i32],
         "spot_noise_from_seeds": [vp, i32, i64, u32, vp, vp],
         "spot_philox_words": [vp, i32, i64, u32, vp, vp],
         "spot_dit_block_forward": [vp, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp],
@@ -184,6 +186,13 @@ def spot_version() -> str:
 
 def spot_set_option(ctx: Context, opt: int, value: int) -> None:
     _check(load_library().spot_set_option(ctx.handle, opt, value), "spot_set_option", ctx)
+
+
+def spot_get_counters(ctx: Context, reset: bool = False) -> dict:
+    a, b, c, d = C.c_uint64(), C.c_uint64(), C.c_uint64(), C.c_double()
+    _check(load_library().spot_get_counters(ctx.handle, C.byref(a), C.byref(b), C.byref(c), C.byref(d), int(reset)),
+           "spot_get_counters", ctx)
+    return {"launches": int(a.value), "gemm_launches": int(b.value), "gemm_timed": int(c.value), "gemm_ms": float(d.value)}
 
 
 def spot_workspace_bytes(ctx: Context, n_seqs: int, n_steps: int) -> int:

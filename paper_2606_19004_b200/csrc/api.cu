@@ -22,6 +22,11 @@ struct spot_ctx {
   float* d_cos;                  // [S, d_h/2]
   float* d_sin;
   float* d_partials;             // [max_seqs, reward chunks]
+  unsigned long long n_launches; // kernels launched through this context
+  int timing;                    // 1: bracket every tcgen05 GEMM launch with CUDA events
+  std::vector<cudaEvent_t> ev;   // event pool (pairs)
+  size_t ev_used;
+  unsigned long long gemm_launches;
   int n_img() const { return cfg.grid_h * cfg.grid_w; }
   int seq() const { return cfg.n_txt + n_img(); }
 };
@@ -47,6 +52,8 @@ int device_state() {
   }
   return state;
 }
+
+constexpr size_t kMaxTimingEvents = 1 << 16;
 
 struct Workspace {
   // all offsets in bytes from the workspace base
@@ -99,6 +106,13 @@ Workspace carve(const spot_ctx* c, int B, int T) {
     }                                                  \
   } while (0)
 
+// LK = CK for a kernel launcher: also counts the launch (reported by spot_get_counters).
+#define LK(ctx, expr)       \
+  do {                      \
+    ++(ctx)->n_launches;    \
+    CK(ctx, expr);          \
+  } while (0)
+
 // Linear layer dispatch: tcgen05 when the context runs bf16 and every problem qualifies, else SIMT.
 spot_status run_gemm(spot_ctx* c, Epilogue epi, GemmProblem* probs, int n, spot_dtype ta, spot_dtype tout,
                      cudaStream_t st) {
@@ -107,9 +121,23 @@ spot_status run_gemm(spot_ctx* c, Epilogue epi, GemmProblem* probs, int n, spot_
   for (int i = 0; i < n && tc; ++i)
     if (probs[i].M > 0 && !tcgen05_gemm_supported(probs[i])) tc = false;
   if (tc) {
-    CK(c, launch_gemm_tcgen05(epi, probs, n, c->num_sms, st));
+    const bool timed = c->timing && c->ev_used + 2 <= kMaxTimingEvents;
+    if (timed) {
+      while (c->ev.size() < c->ev_used + 2) {
+        cudaEvent_t e;
+        CK(c, cudaEventCreate(&e));
+        c->ev.push_back(e);
+      }
+      CK(c, cudaEventRecord(c->ev[c->ev_used], st));
+    }
+    LK(c, launch_gemm_tcgen05(epi, probs, n, c->num_sms, st));
+    ++c->gemm_launches;
+    if (timed) {
+      CK(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
+      c->ev_used += 2;
+    }
   } else {
-    for (int i = 0; i < n; ++i) CK(c, launch_gemm_simt(ta, dt, tout, epi, probs[i], st));
+    for (int i = 0; i < n; ++i) LK(c, launch_gemm_simt(ta, dt, tout, epi, probs[i], st));
   }
   return SPOT_OK;
 }
@@ -217,6 +245,9 @@ spot_status spot_create(const spot_config* cfg, const spot_weights* w, int max_s
   c->max_seqs = max_seqs;
   c->last_cuda = 0;
   c->gemm_impl = c->attn_impl = 0;
+  c->n_launches = c->gemm_launches = 0;
+  c->timing = 0;
+  c->ev_used = 0;
   c->d_cos = c->d_sin = c->d_partials = nullptr;
   int dev = 0;
   cudaGetDevice(&dev);
@@ -244,6 +275,7 @@ spot_status spot_destroy(spot_ctx* ctx) {
   cudaFree(ctx->d_cos);
   cudaFree(ctx->d_sin);
   cudaFree(ctx->d_partials);
+  for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   delete ctx;
   return SPOT_OK;
 }
@@ -253,7 +285,26 @@ spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
   if (value != 0 && value != 1) return SPOT_ERR_SHAPE;
   if (opt == SPOT_OPT_GEMM_IMPL) ctx->gemm_impl = value;
   else if (opt == SPOT_OPT_ATTN_IMPL) ctx->attn_impl = value;
+  else if (opt == SPOT_OPT_TIMING) ctx->timing = value;
   else return SPOT_ERR_SHAPE;
+  return SPOT_OK;
+}
+
+spot_status spot_get_counters(spot_ctx* ctx, uint64_t* launches, uint64_t* gemm_launches, uint64_t* gemm_timed,
+                              double* gemm_ms, int reset) {
+  if (!ctx) return SPOT_ERR_NULL;
+  double ms = 0.0;
+  for (size_t i = 0; i + 1 < ctx->ev_used; i += 2) {
+    float t = 0.f;
+    cudaError_t e = cudaEventElapsedTime(&t, ctx->ev[i], ctx->ev[i + 1]);
+    if (e != cudaSuccess) { ctx->last_cuda = (int)e; return SPOT_ERR_CUDA; }
+    ms += t;
+  }
+  if (launches) *launches = ctx->n_launches;
+  if (gemm_launches) *gemm_launches = ctx->gemm_launches;
+  if (gemm_timed) *gemm_timed = ctx->ev_used / 2;
+  if (gemm_ms) *gemm_ms = ms;
+  if (reset) { ctx->n_launches = ctx->gemm_launches = 0; ctx->ev_used = 0; }
   return SPOT_OK;
 }
 
@@ -313,7 +364,7 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
   GemmProblem pr[2];
   // (2) y = LN(h) (1 + scale1) + shift1 ; (3) qkv = y Wqkv^T + b
   for (int s = 0; s < 2; ++s) {
-    CK(c, launch_ln_modulate(dt, h[s], sm[s].rows, D, mod[s], mod[s] + D, g.ln_eps, ybuf, sm[s].y, st));
+    LK(c, launch_ln_modulate(dt, h[s], sm[s].rows, D, mod[s], mod[s] + D, g.ln_eps, ybuf, sm[s].y, st));
     memset(&pr[s], 0, sizeof(GemmProblem));
     pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].qkv_w; pr[s].bias = bw.s[s].qkv_b;
     pr[s].M = sm[s].rows; pr[s].N = 3 * D; pr[s].K = D; pr[s].out = big; pr[s].out_map = sm[s].qkv;
@@ -321,12 +372,12 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
   spot_status rs = run_gemm(c, EPI_BIAS, pr, 2, dt, dt, st);
   if (rs != SPOT_OK) return rs;
   // (4)-(5) QK-RMSNorm + RoPE, (6) joint attention -> ybuf [B,S,D]
-  CK(c, launch_qk_norm_rope(dt, big, B, S, g.n_heads, g.head_dim, g.n_txt, bw.s[0].q_gain, bw.s[0].k_gain,
+  LK(c, launch_qk_norm_rope(dt, big, B, S, g.n_heads, g.head_dim, g.n_txt, bw.s[0].q_gain, bw.s[0].k_gain,
                             bw.s[1].q_gain, bw.s[1].k_gain, c->d_cos, c->d_sin, g.rms_eps, st));
   if (dt == SPOT_BF16 && c->attn_impl == 0 && tcgen05_attn_supported(S, g.n_heads, g.head_dim))
-    CK(c, launch_attn_tcgen05(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st));
+    LK(c, launch_attn_tcgen05(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st));
   else
-    CK(c, launch_attn_simt(dt, big, ybuf, B, S, g.n_heads, g.head_dim, st));
+    LK(c, launch_attn_simt(dt, big, ybuf, B, S, g.n_heads, g.head_dim, st));
   const int ns = img_only_tail ? 1 : 2;
   // (7) h += gate1 * (o Wout^T + b)
   for (int s = 0; s < ns; ++s) {
@@ -338,7 +389,7 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
   if (rs != SPOT_OK) return rs;
   // (8) y2 = LN(h)(1 + scale2) + shift2 ; u = GELU(y2 W1^T + b) ; h += gate2 * (u W2^T + b)
   for (int s = 0; s < ns; ++s) {
-    CK(c, launch_ln_modulate(dt, h[s], sm[s].rows, D, mod[s] + 3 * D, mod[s] + 4 * D, g.ln_eps, ybuf, sm[s].y, st));
+    LK(c, launch_ln_modulate(dt, h[s], sm[s].rows, D, mod[s] + 3 * D, mod[s] + 4 * D, g.ln_eps, ybuf, sm[s].y, st));
     memset(&pr[s], 0, sizeof(GemmProblem));
     pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].fc1_w; pr[s].bias = bw.s[s].fc1_b;
     pr[s].M = sm[s].rows; pr[s].N = F; pr[s].K = D; pr[s].out = big; pr[s].out_map = sm[s].wide;
@@ -361,16 +412,16 @@ spot_status conditioning(spot_ctx* c, const Workspace& w, uint8_t* ws, int T, cu
   const int D = g.hidden, L = g.n_blocks;
   float* emb = (float*)(ws + w.emb); float* hid = (float*)(ws + w.hid); float* temb = (float*)(ws + w.temb);
   float* cv = (float*)(ws + w.cvec); float* mod = (float*)(ws + w.mod); float* fmod = (float*)(ws + w.fmod);
-  CK(c, launch_time_embed((const float*)(ws + w.t_dev), T, emb, st));
-  CK(c, launch_gemv(g.dtype, c->w.time_w1, c->w.time_b1, emb, T, D, 256, hid, D, true, st));
-  CK(c, launch_gemv(g.dtype, c->w.time_w2, c->w.time_b2, hid, T, D, D, temb, D, false, st));
-  CK(c, launch_silu(temb, cv, (long long)T * D, st));
+  LK(c, launch_time_embed((const float*)(ws + w.t_dev), T, emb, st));
+  LK(c, launch_gemv(g.dtype, c->w.time_w1, c->w.time_b1, emb, T, D, 256, hid, D, true, st));
+  LK(c, launch_gemv(g.dtype, c->w.time_w2, c->w.time_b2, hid, T, D, D, temb, D, false, st));
+  LK(c, launch_silu(temb, cv, (long long)T * D, st));
   const long long stride_t = (long long)L * 2 * 6 * D;
   for (int b = 0; b < L; ++b)
     for (int s = 0; s < 2; ++s)
-      CK(c, launch_gemv(g.dtype, c->blocks[b].s[s].mod_w, c->blocks[b].s[s].mod_b, cv, T, 6 * D, D,
+      LK(c, launch_gemv(g.dtype, c->blocks[b].s[s].mod_w, c->blocks[b].s[s].mod_b, cv, T, 6 * D, D,
                         mod + ((long long)b * 2 + s) * 6 * D, stride_t, false, st));
-  CK(c, launch_gemv(g.dtype, c->w.final_mod_w, c->w.final_mod_b, cv, T, 2 * D, D, fmod, 2 * D, false, st));
+  LK(c, launch_gemv(g.dtype, c->w.final_mod_w, c->w.final_mod_b, cv, T, 2 * D, D, fmod, 2 * D, false, st));
   return SPOT_OK;
 }
 
@@ -382,7 +433,7 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
   const long long E = (long long)NI * C;
   const Workspace w = carve(c, B, T);
   if (T == 0) {
-    if (probe) CK(c, launch_reward_partials(lat, probe, B, E, partials, st));
+    if (probe) LK(c, launch_reward_partials(lat, probe, B, E, partials, st));
     return SPOT_OK;
   }
   CK(c, cudaMemcpyAsync(ws + w.t_dev, h_t, (size_t)(T + 1) * 4, cudaMemcpyHostToDevice, st));
@@ -394,19 +445,19 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
   GemmProblem pr;
   // h_txt^0 = RMSNorm(text_emb) Wtxt^T + b, once per prompt (C7)
   if (NT > 0) {
-    CK(c, launch_rmsnorm_rows(dt, text_emb, c->w.txt_gain, P * NT, g.txt_dim, g.rms_eps, ws + w.txt_norm, st));
+    LK(c, launch_rmsnorm_rows(dt, text_emb, c->w.txt_gain, P * NT, g.txt_dim, g.rms_eps, ws + w.txt_norm, st));
     memset(&pr, 0, sizeof(pr));
     pr.A = ws + w.txt_norm; pr.a_map = plain_rows(P * NT, g.txt_dim); pr.W = c->w.txt_in_w; pr.bias = c->w.txt_in_b;
     pr.M = P * NT; pr.N = D; pr.K = g.txt_dim; pr.out = txt_h0; pr.out_map = plain_rows(P * NT, D);
-    CK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
+    LK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
   }
   for (int i = 0; i < T; ++i) {
     // h_img^0 = x Win^T + b on the fp32 latents
     memset(&pr, 0, sizeof(pr));
     pr.A = lat; pr.a_map = plain_rows(B * NI, C); pr.W = c->w.img_in_w; pr.bias = c->w.img_in_b;
     pr.M = B * NI; pr.N = D; pr.K = C; pr.out = h_img; pr.out_map = plain_rows(B * NI, D);
-    CK(c, launch_gemm_simt(SPOT_F32, dt, SPOT_F32, EPI_BIAS, pr, st));
-    CK(c, launch_broadcast_prompts(txt_h0, h_txt, B, K, (long long)NT * D, st));
+    LK(c, launch_gemm_simt(SPOT_F32, dt, SPOT_F32, EPI_BIAS, pr, st));
+    LK(c, launch_broadcast_prompts(txt_h0, h_txt, B, K, (long long)NT * D, st));
     for (int b = 0; b < L; ++b) {
       const float* m = mod + ((long long)i * L + b) * 2 * 6 * D;
       rs = block_core(c, b, B, h_img, h_txt, m, m + 6 * D, ybuf, big, b == L - 1, st);
@@ -414,13 +465,13 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
     }
     // v = (LN(h_img)(1 + scale_f) + shift_f) Wp^T + b
     const float* fm = fmod + (long long)i * 2 * D;
-    CK(c, launch_ln_modulate(dt, h_img, B * NI, D, fm + D, fm, g.ln_eps, ybuf, plain_rows(B * NI, D), st));
+    LK(c, launch_ln_modulate(dt, h_img, B * NI, D, fm + D, fm, g.ln_eps, ybuf, plain_rows(B * NI, D), st));
     memset(&pr, 0, sizeof(pr));
     pr.A = ybuf; pr.a_map = plain_rows(B * NI, D); pr.W = c->w.proj_w; pr.bias = c->w.proj_b;
     pr.M = B * NI; pr.N = C; pr.K = D; pr.out = vel; pr.out_map = plain_rows(B * NI, C);
-    CK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
+    LK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
     const bool last = i == T - 1;
-    CK(c, launch_euler_update(lat, vel, h_t[i + 1] - h_t[i], B, E, last ? probe : nullptr, partials, st));
+    LK(c, launch_euler_update(lat, vel, h_t[i + 1] - h_t[i], B, E, last ? probe : nullptr, partials, st));
   }
   return SPOT_OK;
 }
@@ -479,16 +530,16 @@ spot_status spot_dit_block_forward(spot_ctx* ctx, int block, int n_seqs, const v
   const long long n_img = (long long)n_seqs * ctx->n_img() * D, n_txt = (long long)n_seqs * g.n_txt * D;
   float* cv = (float*)(ws + w.cvec); float* mod = (float*)(ws + w.mod);
   float* h_img = (float*)(ws + w.h_img); float* h_txt = (float*)(ws + w.h_txt);
-  CK(ctx, launch_silu(d_temb, cv, D, st));
+  LK(ctx, launch_silu(d_temb, cv, D, st));
   for (int sgm = 0; sgm < 2; ++sgm)
-    CK(ctx, launch_gemv(g.dtype, ctx->blocks[block].s[sgm].mod_w, ctx->blocks[block].s[sgm].mod_b, cv, 1, 6 * D, D,
+    LK(ctx, launch_gemv(g.dtype, ctx->blocks[block].s[sgm].mod_w, ctx->blocks[block].s[sgm].mod_b, cv, 1, 6 * D, D,
                         mod + (long long)sgm * 6 * D, 0, false, st));
-  CK(ctx, launch_to_f32(g.dtype, d_h_img, h_img, n_img, st));
-  CK(ctx, launch_to_f32(g.dtype, d_h_txt, h_txt, n_txt, st));
+  LK(ctx, launch_to_f32(g.dtype, d_h_img, h_img, n_img, st));
+  LK(ctx, launch_to_f32(g.dtype, d_h_txt, h_txt, n_txt, st));
   s = block_core(ctx, block, n_seqs, h_img, h_txt, mod, mod + 6 * D, ws + w.ybuf, ws + w.big, false, st);
   if (s != SPOT_OK) return s;
-  CK(ctx, launch_from_f32(g.dtype, h_img, d_out_img, n_img, st));
-  CK(ctx, launch_from_f32(g.dtype, h_txt, d_out_txt, n_txt, st));
+  LK(ctx, launch_from_f32(g.dtype, h_img, d_out_img, n_img, st));
+  LK(ctx, launch_from_f32(g.dtype, h_txt, d_out_txt, n_txt, st));
   return SPOT_OK;
 }
 
@@ -531,9 +582,9 @@ spot_status spot_seed_rewards(spot_ctx* ctx, int n_prompts, int seeds_per_prompt
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int B = n_prompts * seeds_per_prompt;
   const long long E = (long long)ctx->n_img() * ctx->cfg.latent_ch;
-  CK(ctx, launch_reward_partials(d_latents, d_probe, B, E, ctx->d_partials, st));
-  CK(ctx, launch_reward_finalize(ctx->d_partials, B, E, d_rewards, st));
-  CK(ctx, launch_seed_select(d_rewards, n_prompts, seeds_per_prompt, k_select, d_stats, d_top, d_bottom, st));
+  LK(ctx, launch_reward_partials(d_latents, d_probe, B, E, ctx->d_partials, st));
+  LK(ctx, launch_reward_finalize(ctx->d_partials, B, E, d_rewards, st));
+  LK(ctx, launch_seed_select(d_rewards, n_prompts, seeds_per_prompt, k_select, d_stats, d_top, d_bottom, st));
   return SPOT_OK;
 }
 
@@ -552,12 +603,12 @@ spot_status spot_explore(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, con
   if (s != SPOT_OK) return s;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const long long E = (long long)ctx->n_img() * ctx->cfg.latent_ch;
-  CK(ctx, launch_noise(d_seeds, B, E, 0u, d_latents, nullptr, st));
+  LK(ctx, launch_noise(d_seeds, B, E, 0u, d_latents, nullptr, st));
   s = denoise_core(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps,
                    (uint8_t*)d_workspace, d_probe, ctx->d_partials, st);
   if (s != SPOT_OK) return s;
-  CK(ctx, launch_reward_finalize(ctx->d_partials, B, E, d_rewards, st));
-  CK(ctx, launch_seed_select(d_rewards, n_prompts, seeds_per_prompt, k_select, d_stats, d_top, d_bottom, st));
+  LK(ctx, launch_reward_finalize(ctx->d_partials, B, E, d_rewards, st));
+  LK(ctx, launch_seed_select(d_rewards, n_prompts, seeds_per_prompt, k_select, d_stats, d_top, d_bottom, st));
   return SPOT_OK;
 }
 

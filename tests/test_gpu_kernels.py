@@ -187,3 +187,22 @@ def test_euler_update_and_reward():
     for i in range(4):
         cur, _ = spot.spot_euler_update(cur, vel, grid[i + 1] - grid[i])
     assert (cur - x_data).abs().max().item() < 1e-5
+
+
+# ------------------------------------------------------------------ K5 tcgen05 attention
+@pytest.mark.parametrize("B,S,H,scale", [(1, 128, 1, 1.0), (2, 256, 2, 1.0), (1, 200, 2, 1.0), (2, 1280, 3, 1.0),
+                                         (1, 333, 1, 6.0), (1, 1280, 2, 5.0)])
+def test_attention_tcgen05(B, S, H, scale):
+    """TMA + tcgen05 flash attention vs the fp64 oracle: one tile, several tiles, ragged last query/key tile,
+    and peaked softmax (logits ~ N(0, (scale^2 * sqrt(128))^2)) that forces the lazy-rescale path."""
+    dh = 128
+    qkv = hash_normal(981, B * S * 3 * H * dh, scale, torch.bfloat16, "cuda").reshape(B, S, 3, H, dh)
+    out = spot.spot_attention(qkv, spot.IMPL_TCGEN05)
+    ref = _attn_ref(qkv)
+    err = rel_l2(np64(out), ref)
+    print(f"attention tcgen05 B={B} S={S} H={H} scale={scale}: rel-L2 {err:.3e}")
+    assert err < 8e-3
+    again = spot.spot_attention(qkv, spot.IMPL_TCGEN05)
+    assert torch.equal(out, again)
+    simt = spot.spot_attention(qkv, spot.IMPL_SIMT)
+    assert rel_l2(np64(out), np64(simt)) < 8e-3
