@@ -1,0 +1,301 @@
+#!/usr/bin/env python
+"""bench.py - seed-exploration rollout throughput on B200 (contract: see DESIGN.md "Measurement").
+
+A "step" is ONE whole pass of the hot path over one batch: seeds -> Philox/Box-Muller latents -> T Euler steps
+of the 60-block MMDiT -> probe rewards -> top/bottom-k selection (spot_explore).  Default workload = config 3
+of BASELINE.json (512x512, 60 blocks, 1 prompt x 16 seeds, 10 Euler steps, bf16), the configuration the
+metric's ">= 50 % of dense BF16 peak" target is quoted on.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg4|cfg5] [--impl reference]
+
+N > 1 is launched by torch.distributed.run (one rank per GPU); ranks hold replicated weights and disjoint
+seed groups (weak scaling, no data-path collective; the K fp32 rewards are all-gathered once per step).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from synth import CONFIGS, make_probe, make_text_emb, make_weights  # noqa: E402
+
+METRIC = "image-tokens*steps/s"
+WORKLOADS = {"cfg3": 3, "cfg4": 4, "cfg5": 5}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"],
+                "bf16_tflops_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx, self.rows, self.proc = gpu_index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.idx), "-lms", "200"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        sm, mx, reasons, power = [], [], set(), []
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2])); power.append(float(r[3]))
+            except (ValueError, IndexError):
+                continue
+            for name, col in (("hw_slowdown", 5), ("hw_thermal_slowdown", 6), ("sw_thermal_slowdown", 7), ("sw_power_cap", 8)):
+                if len(r) > col and r[col].lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(shape, w_host, text_host, n_blocks_sample: int):
+    """The oracle as it stands on a bounded sample: 1 seed, 1 Euler step, `n_blocks_sample` of the L blocks at
+    full width (work is exactly linear in seeds, steps and blocks).  Returns seconds."""
+    from oracle import mmdit, philox
+    from tests.helpers import np64
+    g = {k: np64(v) for k, v in w_host["global"].items()}
+    blocks = [{k: np64(v) for k, v in b.items()} for b in w_host["blocks"][:n_blocks_sample]]
+    te = np64(text_host)[0]
+    t0 = time.perf_counter()
+    cos, sin = mmdit.rope_table(shape.grid_h, shape.grid_w, shape.n_txt, shape.rope_pairs, shape.rope_theta)
+    h0 = mmdit.text_input(te, g)
+    x0 = philox.noise_from_seeds([0], shape.n_img * shape.latent_ch)[0].reshape(shape.n_img, shape.latent_ch)
+    v = mmdit.dit_velocity(x0, 1.0, h0, g, blocks, n_heads=shape.n_heads, cos=cos, sin=sin)
+    _ = x0 + (-0.1) * v
+    return time.perf_counter() - t0
+
+
+def cpu_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+        n = [i["num_threads"] for i in threadpool_info() if i.get("user_api") == "blas"]
+        if n:
+            return max(n)
+    except Exception:
+        pass
+    return os.cpu_count() or 1
+
+
+def run_reference(args, shape):
+    """--impl reference: the fp64 oracle timed on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    nb = 2
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    w = make_weights(shape, device=dev, blocks=range(nb))
+    w_host = {"global": {k: v.cpu() for k, v in w["global"].items()}, "blocks": [{k: v.cpu() for k, v in b.items()} for b in w["blocks"]]}
+    text = make_text_emb(shape, dev, prompts=[0]).cpu()
+    del w
+    times = []
+    for i in range(args.warmup + args.steps):
+        dt = oracle_sample(shape, w_host, text, nb)
+        if i >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * sum(times) / len(times)
+    value = shape.n_img * (nb / shape.n_blocks) / (ms / 1e3)
+    cores = cpu_threads()
+    sample = f"1 seed x 1 Euler step x {nb} of {shape.n_blocks} blocks at full width per step (work is linear in seeds, steps, blocks)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": shape.name, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="spot", choices=["spot", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    shape = CONFIGS[WORKLOADS[args.workload]]
+    if args.impl == "reference":
+        return run_reference(args, shape)
+
+    import paper_2606_19004_b200 as spot
+    from paper_2606_19004_b200 import build as spot_build
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: the product path has no CPU fallback"
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if rank == 0:
+        spot_build.build()
+    if dist is not None:
+        dist.barrier()
+    spot.load_library()
+    peaks = load_peaks()
+
+    P, K, T = shape.n_prompts, shape.seeds_per_prompt, shape.n_steps
+    B = P * K
+    t0 = time.time()
+    weights = make_weights(shape, device="cuda")
+    text = make_text_emb(shape, "cuda")
+    probe = make_probe(shape, "cuda")
+    torch.cuda.synchronize()
+    gen_s = time.time() - t0
+    ctx = spot.Context(shape, weights, max_seqs=B)
+    ts = [float(np.float32(t)) for t in shape.timesteps]
+    k_sel = K // 2
+    # each rank explores its own seed group (weak scaling): seeds offset by rank * B
+    seeds = torch.tensor([int(s) + rank * B for s in shape.seeds], dtype=torch.int64, device="cuda")
+    out = None
+
+    def step():
+        nonlocal out
+        out = spot.spot_explore(ctx, seeds, text, ts, probe, P, K, k_sel, out)
+        if dist is not None:
+            gathered = torch.empty(world * B, dtype=torch.float32, device="cuda")
+            dist.all_gather_into_tensor(gathered, out["rewards"])
+
+    def sync_all():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    sync_all()
+    spot.spot_get_counters(ctx, reset=True)
+    spot.spot_set_option(ctx, spot.OPT_TIMING, 1)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sync_all()
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    sync_all()
+    clocks = sampler.stop()
+    ms_total = ev0.elapsed_time(ev1)
+    counters = spot.spot_get_counters(ctx, reset=True)
+    spot.spot_set_option(ctx, spot.OPT_TIMING, 0)
+    if dist is not None:
+        tt = torch.tensor([ms_total], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = tt.item()
+    ms_step = ms_total / args.steps
+    units_per_step = world * B * shape.n_img * T                     # image tokens x Euler steps, all ranks
+    value = units_per_step / (ms_step / 1e3)
+    flops_step = shape.flops_per_rollout()
+    tflops = flops_step / (ms_step / 1e3) / 1e12                     # per GPU
+
+    # roofline of the dominant kernel (tcgen05 GEMM): algorithmic GEMM FLOPs / event-timed GEMM device time
+    S, D, F, L = shape.seq, shape.hidden, shape.mlp_hidden, shape.n_blocks
+    lin_per_seq_block = 2 * D * (3 * D + D + 2 * F)                   # per token
+    gemm_flops_step = T * B * (L * S * lin_per_seq_block - shape.n_txt * 2 * D * (D + 2 * F))   # last block: no text tail
+    timed_frac = counters["gemm_timed"] / max(1, counters["gemm_launches"])
+    gemm_ms = counters["gemm_ms"]
+    gemm_tflops = (gemm_flops_step * args.steps * timed_frac) / (gemm_ms / 1e3) / 1e12 if gemm_ms > 0 else None
+    roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_kernel", "achieved": gemm_tflops,
+                "peak": peaks["bf16_tflops_sustained"], "peak_kind": f"{peaks['source']} sustained bf16 (kernel timed inside a long step)",
+                "unit": "TFLOP/s", "frac": (gemm_tflops / peaks["bf16_tflops_sustained"]) if gemm_tflops else None,
+                "traffic": None, "launches_timed": counters["gemm_timed"],
+                "avg_launch_ms": gemm_ms / max(1, counters["gemm_timed"]), "share_of_step": gemm_ms / ms_total / max(timed_frac, 1e-9)}
+
+    # e2e: the host-buffer C-ABI call, host<->device copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda t: t.cpu().pin_memory()
+        h_seeds, h_text, h_probe = pin(seeds), pin(text), pin(probe)
+        h_out = {"latents": torch.empty((B, shape.n_img, shape.latent_ch)).pin_memory(), "rewards": torch.empty(B).pin_memory(),
+                 "stats": torch.empty((P, 2)).pin_memory(), "top": torch.empty((P, k_sel), dtype=torch.int32).pin_memory(),
+                 "bottom": torch.empty((P, k_sel), dtype=torch.int32).pin_memory()}
+        spot.spot_explore_host(ctx, h_seeds, h_text, ts, h_probe, P, K, k_sel, h_out)
+        sync_all()
+        w0 = time.perf_counter()
+        ev0.record()
+        for _ in range(args.steps):
+            spot.spot_explore_host(ctx, h_seeds, h_text, ts, h_probe, P, K, k_sel, h_out)
+        ev1.record()
+        sync_all()
+        e_ms = ev0.elapsed_time(ev1) / args.steps
+        wall_ms = (time.perf_counter() - w0) * 1e3 / args.steps
+        e_ms = max(e_ms, wall_ms)                                      # the host call synchronises: wall clock bounds it
+        if dist is not None:
+            tt = torch.tensor([e_ms], device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            e_ms = tt.item()
+        h2d = h_seeds.numel() * 8 + h_text.numel() * h_text.element_size() + h_probe.numel() * 4
+        d2h = sum(t.numel() * t.element_size() for t in h_out.values())
+        e2e = {"value": units_per_step / (e_ms / 1e3), "unit": METRIC, "ms_per_step": e_ms,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+        assert torch.equal(h_out["rewards"], out["rewards"].cpu()), "host and device entry points disagree"
+
+    cpu_baseline = None
+    if rank == 0 and not args.no_cpu_baseline:
+        nb = 2
+        w_host = {"global": {k: v.cpu() for k, v in weights["global"].items()},
+                  "blocks": [{k: v.cpu() for k, v in b.items()} for b in weights["blocks"][:nb]]}
+        dt = min(oracle_sample(shape, w_host, text[:1].cpu(), nb) for _ in range(2))
+        cpu_baseline = {"value": shape.n_img * (nb / L) / dt, "unit": METRIC, "cores": cpu_threads(), "kind": "oracle",
+                        "seconds": dt, "host_cores": os.cpu_count(),
+                        "sample": f"1 seed x 1 Euler step x {nb} of {L} blocks at full width, best of 2 "
+                                  "(work is linear in seeds, steps, blocks)"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+                "data": "synthetic",
+                "config": {"workload": shape.name, "n_prompts": P, "seeds_per_prompt": K, "euler_steps": T, "blocks": L,
+                           "hidden": D, "image_tokens": shape.n_img, "text_tokens": shape.n_txt,
+                           "l2": "inputs (40.8 GB of weights streamed every Euler step) are larger than L2",
+                           "parallelism": f"replicas x{world}, disjoint seed groups"},
+                "seeds_per_s": world * B / (ms_step / 1e3), "tflops_per_gpu": tflops,
+                "frac_of_bf16_peak": {"burst": tflops / peaks["bf16_tflops"], "sustained": tflops / peaks["bf16_tflops_sustained"],
+                                      "nominal_2250": tflops / 2250.0, "peaks": peaks["source"]},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": counters["launches"], "roofline": roofline,
+                "cpu_baseline": cpu_baseline, "weight_gen_s": gen_s}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
