@@ -32,6 +32,9 @@ if ROOT not in sys.path:
 from synth import CONFIGS, make_probe, make_text_emb, make_weights  # noqa: E402
 
 METRIC = "image-tokens*steps/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of gemm_tcgen05_kernel, averaged over its four uses in a
+# block (QKV 0.995 GB, out-proj 0.655 GB, fc1 1.346 GB, fc2 2.384 GB) - profiles/r1_ncu_full_gemm_attn.txt (config 3)
+GEMM_DRAM_TRAFFIC_PER_LAUNCH = {"cfg3": 1.345e9}
 WORKLOADS = {"cfg3": 3, "cfg4": 4, "cfg5": 5}
 
 
@@ -235,8 +238,9 @@ def main():
     roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_kernel", "achieved": gemm_tflops,
                 "peak": peaks["bf16_tflops_sustained"], "peak_kind": f"{peaks['source']} sustained bf16 (kernel timed inside a long step)",
                 "unit": "TFLOP/s", "frac": (gemm_tflops / peaks["bf16_tflops_sustained"]) if gemm_tflops else None,
-                "traffic": None, "launches_timed": counters["gemm_timed"],
-                "avg_launch_ms": gemm_ms / max(1, counters["gemm_timed"]), "share_of_step": gemm_ms / ms_total / max(timed_frac, 1e-9)}
+                "traffic": GEMM_DRAM_TRAFFIC_PER_LAUNCH.get(args.workload), "launches_timed": counters["gemm_timed"],
+                "avg_launch_ms": gemm_ms / max(1, counters["gemm_timed"]), "share_of_step": gemm_ms / ms_total / max(timed_frac, 1e-9),
+                "flops_per_launch": gemm_flops_step / max(1, counters["gemm_launches"] / args.steps)}
 
     # e2e: the host-buffer C-ABI call, host<->device copies inside the timed region
     e2e = None

@@ -1,0 +1,93 @@
+"""Writes tests/golden/cfg3_seed0.json + cfg3_seed0_latent.npy: the fp64 ORACLE's result for one sampled
+seed of config 3 at FULL size (60 blocks, hidden 3072, 1024 + 256 tokens, 10 Euler steps), the launch
+configuration bench.py times.  Calls only oracle/ and the input generators in synth/ (CPU); never the CUDA
+path.  Cost: ~40 min to generate the 20.4 G weights on 8 cores + ~15 min of fp64 BLAS (186 TFLOP).
+
+    python tests/golden/make_cfg3_golden.py [--blocks L] [--steps T] [--seed S] [--out NAME]
+
+The GPU test (tests/test_gpu_fullsize.py) regenerates the same weights on the device, checks their
+per-block checksums against the ones stored here, runs the 16-seed batch and compares seed S.
+"""
+import argparse
+import json
+import os
+import sys
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+
+from oracle import mmdit, philox, rollout  # noqa: E402
+from synth import CONFIGS, make_probe, make_text_emb, tensor_checksum  # noqa: E402
+from synth.manifest import make_block_weights, make_global_weights  # noqa: E402
+
+
+def np64(t):
+    return t.to(torch.float64).numpy()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--blocks", type=int, default=None)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--out", default="cfg3_seed0")
+    a = ap.parse_args()
+    s = CONFIGS[3]
+    if a.blocks is not None:
+        s = s.with_(n_blocks=a.blocks)
+    if a.steps is not None:
+        s = s.with_(n_steps=a.steps)
+    here = os.path.dirname(os.path.abspath(__file__))
+    t0 = time.time()
+    gw = make_global_weights(s)
+    blocks, sums = [], []
+    for b in range(s.n_blocks):
+        bw = make_block_weights(s, b)
+        sums.append({k: tensor_checksum(v) for k, v in sorted(bw.items())})
+        blocks.append(bw)                                  # kept as bf16 (40.8 GB at full depth)
+        print(f"block {b} generated ({time.time() - t0:.0f} s)", flush=True)
+    gsum = {k: tensor_checksum(v) for k, v in sorted(gw.items())}
+    text = make_text_emb(s)
+    probe = make_probe(s)
+    ts = [float(np.float32(t)) for t in s.timesteps]
+    g = {k: np64(v) for k, v in gw.items()}
+    cos, sin = mmdit.rope_table(s.grid_h, s.grid_w, s.n_txt, s.rope_pairs, s.rope_theta)
+    h0 = mmdit.text_input(np64(text)[0], g, s.rms_eps)
+    x0 = philox.noise_from_seeds([a.seed], s.n_img * s.latent_ch)[0].reshape(s.n_img, s.latent_ch)
+    x0 = x0.astype(np.float32).astype(np.float64)          # the CUDA path stores the initial latent in fp32
+    t1 = time.time()
+
+    class LazyBlocks:                                      # widen one block at a time to fp64 (2.7 GB transient)
+        def __iter__(self):
+            for bw in blocks:
+                yield {k: np64(v) for k, v in bw.items()}
+
+    hist = []
+
+    def vel(x, t):
+        v = mmdit.dit_velocity(x, t, h0, g, LazyBlocks(), n_heads=s.n_heads, cos=cos, sin=sin, ln_eps=s.ln_eps, rms_eps=s.rms_eps)
+        print(f"  velocity at t={t:.3f} done ({time.time() - t1:.0f} s)", flush=True)
+        return v
+
+    xT = rollout.euler_denoise(x0, ts, vel, hist)
+    reward = rollout.probe_reward(xT, np64(probe))
+    np.save(os.path.join(here, a.out + "_latent.npy"), xT.astype(np.float32))
+    meta = {"written_by": "tests/golden/make_cfg3_golden.py (oracle/ + synth/ only)", "config": s.name, "n_blocks": s.n_blocks,
+            "n_steps": s.n_steps, "seed": a.seed, "timesteps": ts, "reward": reward,
+            "latent_l2": float(np.linalg.norm(xT)), "x0_l2": float(np.linalg.norm(x0)),
+            "per_step_l2": [float(np.linalg.norm(h)) for h in hist],
+            "per_step_head": [[float(v) for v in h.reshape(-1)[:16]] for h in hist],
+            "global_checksums": gsum, "block_checksums": sums, "text_checksum": tensor_checksum(text),
+            "probe_checksum": tensor_checksum(probe), "oracle_seconds": time.time() - t1, "weightgen_seconds": t1 - t0,
+            "host_cores": os.cpu_count()}
+    with open(os.path.join(here, a.out + ".json"), "w") as f:
+        json.dump(meta, f, indent=1)
+    print("done", reward, time.time() - t0)
+
+
+if __name__ == "__main__":
+    main()
