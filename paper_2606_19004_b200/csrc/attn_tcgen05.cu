@@ -1,17 +1,21 @@
 // attn_tcgen05.cu - K5: flash-style joint text+image attention O = softmax(Q K^T / sqrt(d_h)) V over all S
 // keys, no mask (north_star (d); S4 step 6, S6), bf16, d_h = 128.
 //
-// One CTA = one 128-row query tile of one (sequence, head); it streams the S keys in tiles of 128:
-//   warp 0      TMA producer: Q once, then K_j / V_j tiles (2-stage rings), all from ONE 3-D tensor map over
-//               qkv [B, S, 3*H*d_h] (box 64 x 128 x 1, 128-byte swizzle; rows past S are zero-filled)
-//   warp 1      TMEM allocator + MMA issuer: S_j = Q K_j^T (tcgen05.mma M128 N128 K16 x 8, K-major operands)
-//               into one of two TMEM score buffers, and O += P_j V_j (V as MN-major B operand) into a TMEM
-//               accumulator; S_{j+1} is issued before P_j V_j so the tensor pipe works during softmax_j
-//   warps 2-5   softmax: thread = one query row; tcgen05.ld of the 128 scores, row max, exp2 with the scale
-//               folded into one FFMA, row sum, bf16 P written to shared memory in the swizzled K-major layout
-//               the MMA reads.  Online softmax with LAZY rescaling: the running reference maximum is only
-//               raised (and O in TMEM corrected by tcgen05.ld/st) when a row's maximum grows by more than 8
-//               (log2 units), decided per warp with a vote; P stays <= 2^8, the final O / l is exact.
+// One CTA = TWO 128-row query tiles (A, B) of one (sequence, head), processed in ping-pong so that the
+// softmax of one tile overlaps the tensor-core work of the other.  Keys are streamed in tiles of 128:
+//   warp 0      TMA producer: Q_A, Q_B once, then K_j / V_j tiles (2-stage rings), all from ONE 3-D tensor map
+//               over qkv [B, S, 3*H*d_h] (box 64 x 128 x 1, 128-byte swizzle; rows past S are zero-filled)
+//   warp 1      TMEM allocator + MMA issuer (one thread):
+//                 S_t = Q_t K_j^T   tcgen05.mma M128 N128 K16 x 8, both operands K-major in shared memory
+//                 O_t += P_t V_j    A operand = P_t read from TENSOR MEMORY, B = V_j as MN-major shared memory
+//               issue order per key tile: PV_A(j), S_A(j+1), PV_B(j), S_B(j+1)
+//   warps 2-5   softmax warpgroup of tile A, warps 6-9 of tile B: thread = one query row; two tcgen05.ld passes over the 128
+//               scores (row max, then exp), exp2 with the scale folded into one FFMA, row sum, P packed to bf16 and written
+//               back with tcgen05.st over the columns S_t occupied (P never touches shared memory).
+//               Online softmax with LAZY rescaling: the reference maximum is raised (and O_t in TMEM corrected)
+//               only when a row's maximum grows by more than 2^8, decided per warp by a vote; the final O / l is
+//               exact because P and l always use the same reference.
+// TMEM columns: [0,128) S_A/P_A, [128,256) S_B/P_B, [256,384) O_A, [384,512) O_B.
 // Tensor-pipe bound (+ MUFU ex2): 4 S^2 d_h FLOP per (sequence, head).
 #include <string.h>
 
@@ -20,19 +24,34 @@
 
 namespace {
 
-constexpr int DH = 128, BQ = 128, BKV = 128, KV_STAGES = 2;
+constexpr int DH = 128, BQ = 128, BKV = 128, KV_STAGES = 2, QT = 2;
 constexpr uint32_t SUB_BYTES = 128 * 64 * 2;          // one [128 x 64] bf16 sub-tile, 128-byte rows
 constexpr uint32_t TILE_BYTES = 2 * SUB_BYTES;        // [128 x 128]
-constexpr uint32_t OFF_Q = 0, OFF_K = TILE_BYTES, OFF_V = OFF_K + KV_STAGES * TILE_BYTES,
-                   OFF_P = OFF_V + KV_STAGES * TILE_BYTES, OFF_BAR = OFF_P + TILE_BYTES;
+constexpr uint32_t OFF_Q = 0, OFF_K = QT * TILE_BYTES, OFF_V = OFF_K + KV_STAGES * TILE_BYTES,
+                   OFF_BAR = OFF_V + KV_STAGES * TILE_BYTES;
 constexpr uint32_t ATT_SMEM = OFF_BAR + 256 + 1024;
-constexpr int ATT_THREADS = 192;
+constexpr int ATT_THREADS = 64 + QT * 128;    // warps 0-1: TMA, MMA; warps 2-5 / 6-9: softmax warpgroups
 constexpr float RESCALE_THRESHOLD = 8.0f;
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+
+// D[tmem] (+)= A[tmem] * B[smem desc]
+__device__ __forceinline__ void mma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
+                                           uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}\n" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+
+__device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&v);
 }
 
 __global__ void __launch_bounds__(ATT_THREADS, 1)
@@ -47,13 +66,14 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict
   auto k_empty = [&](int s) { return bar + 8u * (3 + s); };
   auto v_full = [&](int s) { return bar + 8u * (5 + s); };
   auto v_empty = [&](int s) { return bar + 8u * (7 + s); };
-  auto s_full = [&](int s) { return bar + 8u * (9 + s); };
-  auto s_empty = [&](int s) { return bar + 8u * (11 + s); };
-  const uint32_t p_full = bar + 8u * 13, pv_done = bar + 8u * 14, tmem_slot = bar + 8u * 15;
+  auto s_full = [&](int t) { return bar + 8u * (9 + t); };
+  auto p_full = [&](int t) { return bar + 8u * (11 + t); };
+  auto pv_done = [&](int t) { return bar + 8u * (13 + t); };
+  const uint32_t tmem_slot = bar + 8u * 15;
   volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(base_ptr + OFF_BAR + 8 * 15);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int q0 = blockIdx.x * BQ, head = blockIdx.y, seq = blockIdx.z;
+  const int q0 = blockIdx.x * (QT * BQ), head = blockIdx.y, seq = blockIdx.z;
   const int n_kv = (S + BKV - 1) / BKV;
   const int col_q = head * DH, col_k = (H + head) * DH, col_v = (2 * H + head) * DH;
 
@@ -64,9 +84,8 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict
       for (int s = 0; s < 2; ++s) {
         ptx::mbar_init(k_full(s), 1); ptx::mbar_init(k_empty(s), 1);
         ptx::mbar_init(v_full(s), 1); ptx::mbar_init(v_empty(s), 1);
-        ptx::mbar_init(s_full(s), 1); ptx::mbar_init(s_empty(s), 4);
+        ptx::mbar_init(s_full(s), 1); ptx::mbar_init(p_full(s), 4); ptx::mbar_init(pv_done(s), 1);
       }
-      ptx::mbar_init(p_full, 4); ptx::mbar_init(pv_done, 1);
       ptx::fence_barrier_init();
     }
     __syncwarp();
@@ -77,14 +96,16 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict
   __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  const uint32_t tmem_s0 = tmem_base, tmem_o = tmem_base + 256;       // S buffers at columns 0 and 128
 
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (lane == 0) {
-      ptx::mbar_arrive_expect_tx(q_full, TILE_BYTES);
-      ptx::tma_load_3d(base + OFF_Q, &tm_qkv, q_full, col_q, q0, seq);
-      ptx::tma_load_3d(base + OFF_Q + SUB_BYTES, &tm_qkv, q_full, col_q + 64, q0, seq);
+      ptx::mbar_arrive_expect_tx(q_full, QT * TILE_BYTES);
+#pragma unroll
+      for (int t = 0; t < QT; ++t) {
+        ptx::tma_load_3d(base + OFF_Q + t * TILE_BYTES, &tm_qkv, q_full, col_q, q0 + t * BQ, seq);
+        ptx::tma_load_3d(base + OFF_Q + t * TILE_BYTES + SUB_BYTES, &tm_qkv, q_full, col_q + 64, q0 + t * BQ, seq);
+      }
       for (int j = 0; j < n_kv; ++j) {
         const int st = j & 1;
         const uint32_t ph = (uint32_t)(j >> 1) & 1u;
@@ -101,142 +122,134 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (lane == 0) {
-      constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(BQ, BKV, 0, 0);   // A = Q (K-major), B = K (K-major)
-      constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(BQ, DH, 0, 1);    // A = P (K-major), B = V (MN-major)
-      auto issue_qk = [&](int j) {
+      constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(BQ, BKV, 0, 0);   // A = Q (K-major smem), B = K (K-major smem)
+      constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(BQ, DH, 0, 1);    // A = P (TMEM), B = V (MN-major smem)
+      auto issue_qk = [&](int t, int j) {
         const int st = j & 1;
-        ptx::mbar_wait(k_full(st), (uint32_t)(j >> 1) & 1u);
-        ptx::mbar_wait(s_empty(st), ((uint32_t)(j >> 1) & 1u) ^ 1u);
-        ptx::tc_fence_after();
-        const uint32_t qa = base + OFF_Q, ka = base + OFF_K + st * TILE_BYTES;
+        const uint32_t qa = base + OFF_Q + t * TILE_BYTES, ka = base + OFF_K + st * TILE_BYTES;
 #pragma unroll
         for (int k = 0; k < DH / 16; ++k) {
           const uint32_t off = (k >> 2) * SUB_BYTES + (k & 3) * 32;
-          ptx::mma_f16_ss(tmem_s0 + st * BKV, ptx::make_smem_desc(qa + off, 16, 1024),
+          ptx::mma_f16_ss(tmem_base + t * BKV, ptx::make_smem_desc(qa + off, 16, 1024),
                           ptx::make_smem_desc(ka + off, 16, 1024), idesc_qk, k ? 1u : 0u);
         }
-        ptx::mma_commit(k_empty(st));
-        ptx::mma_commit(s_full(st));
+        ptx::mma_commit(s_full(t));
+        if (t == QT - 1) ptx::mma_commit(k_empty(st));
       };
       ptx::mbar_wait(q_full, 0);
-      issue_qk(0);
+      ptx::mbar_wait(k_full(0), 0);
+      ptx::tc_fence_after();
+      issue_qk(0, 0);
+      issue_qk(1, 0);
       for (int j = 0; j < n_kv; ++j) {
-        if (j + 1 < n_kv) issue_qk(j + 1);
         const int st = j & 1;
         ptx::mbar_wait(v_full(st), (uint32_t)(j >> 1) & 1u);
-        ptx::mbar_wait(p_full, (uint32_t)j & 1u);
-        ptx::tc_fence_after();
-        const uint32_t pa = base + OFF_P, va = base + OFF_V + st * TILE_BYTES;
 #pragma unroll
-        for (int k = 0; k < BKV / 16; ++k) {
-          const uint64_t da = ptx::make_smem_desc(pa + (k >> 2) * SUB_BYTES + (k & 3) * 32, 16, 1024);
-          const uint64_t db = ptx::make_smem_desc(va + k * 2048, SUB_BYTES, 1024);   // 16 keys = 2 x 1024-byte groups
-          ptx::mma_f16_ss(tmem_o, da, db, idesc_pv, (j | k) ? 1u : 0u);
+        for (int t = 0; t < QT; ++t) {
+          ptx::mbar_wait(p_full(t), (uint32_t)j & 1u);
+          ptx::tc_fence_after();
+          const uint32_t va = base + OFF_V + st * TILE_BYTES;
+#pragma unroll
+          for (int k = 0; k < BKV / 16; ++k)        // 16 keys = 8 packed TMEM columns of P, 2 x 1024-byte groups of V
+            mma_f16_ts(tmem_base + 256 + t * DH, tmem_base + t * BKV + k * 8,
+                       ptx::make_smem_desc(va + k * 2048, SUB_BYTES, 1024), idesc_pv, (j | k) ? 1u : 0u);
+          ptx::mma_commit(pv_done(t));
+          if (t == QT - 1) ptx::mma_commit(v_empty(st));
+          if (j + 1 < n_kv) {
+            if (t == 0) { ptx::mbar_wait(k_full((j + 1) & 1), (uint32_t)((j + 1) >> 1) & 1u); ptx::tc_fence_after(); }
+            issue_qk(t, j + 1);
+          }
         }
-        ptx::mma_commit(v_empty(st));
-        ptx::mma_commit(pv_done);
       }
     }
   } else {
-    // ===================== softmax / correction / epilogue (128 threads, one query row each) ===========
-    const int quarter = warp & 3;
+    // ===================== softmax / correction / epilogue: 2 warpgroups x 128 rows =====================
+    const int t = (warp - 2) >> 2;                      // query tile of this warpgroup
+    const int quarter = warp & 3;                       // TMEM lane quarter this warp may access
     const int row = quarter * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
+    const uint32_t tmem_s = tmem_base + t * BKV + lane_addr, tmem_o = tmem_base + 256 + t * DH + lane_addr;
     float m_ref = -INFINITY, l = 0.f;
-    uint8_t* p_row = base_ptr + OFF_P + row * 128;
     for (int j = 0; j < n_kv; ++j) {
-      const int st = j & 1;
-      ptx::mbar_wait(s_full(st), (uint32_t)(j >> 1) & 1u);
+      ptx::mbar_wait(s_full(t), (uint32_t)j & 1u);     // also implies PV_t(j-1) has completed (in-order pipe)
       ptx::tc_fence_after();
-      uint32_t sv[4][32];
-#pragma unroll
-      for (int c = 0; c < 4; ++c) ptx::tmem_ld_32x32(tmem_s0 + st * BKV + c * 32 + lane_addr, sv[c]);
-      ptx::tmem_ld_wait();
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(s_empty(st));
-      const int valid = S - j * BKV;                       // keys of this tile that exist (>= 128 except the last)
+      const int valid = S - j * BKV;                   // keys of this tile that exist (>= 128 except the last)
+      // pass 1 over TMEM: row maximum (two passes keep the live registers at 64 scores instead of 128)
       float mx = -INFINITY;
 #pragma unroll
-      for (int c = 0; c < 4; ++c)
+      for (int c = 0; c < 4; ++c) {
+        uint32_t sv[32];
+        ptx::tmem_ld_32x32(tmem_s + c * 32, sv);
+        ptx::tmem_ld_wait();
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          float s = __uint_as_float(sv[c][i]);
-          if (valid < BKV && c * 32 + i >= valid) { s = -INFINITY; sv[c][i] = __float_as_uint(s); }
-          mx = fmaxf(mx, s);
-        }
-      // lazy rescale, decided per warp
+        for (int i = 0; i < 32; ++i)
+          if (valid >= BKV || c * 32 + i < valid) mx = fmaxf(mx, __uint_as_float(sv[i]));
+      }
       const bool need = (mx - m_ref) * scale_log2 > RESCALE_THRESHOLD;     // true on the first tile (m_ref = -inf)
       if (__any_sync(0xffffffffu, need)) {
         const float m_new = fmaxf(m_ref, mx);
         if (j > 0) {
           const float alpha = ex2_approx((m_ref - m_new) * scale_log2);
           l *= alpha;
-          ptx::mbar_wait(pv_done, (uint32_t)(j - 1) & 1u);                 // O must be quiescent
-          ptx::tc_fence_after();
 #pragma unroll
           for (int c = 0; c < 4; ++c) {
             uint32_t ov[32];
-            ptx::tmem_ld_32x32(tmem_o + c * 32 + lane_addr, ov);
+            ptx::tmem_ld_32x32(tmem_o + c * 32, ov);
             ptx::tmem_ld_wait();
 #pragma unroll
             for (int i = 0; i < 32; ++i) ov[i] = __float_as_uint(__uint_as_float(ov[i]) * alpha);
-            ptx::tmem_st_32x32(tmem_o + c * 32 + lane_addr, ov);
+            ptx::tmem_st_32x32(tmem_o + c * 32, ov);
           }
-          ptx::tmem_st_wait();
         }
         m_ref = m_new;
       }
       const float mc = m_ref * scale_log2;
-      if (j > 0) ptx::mbar_wait(pv_done, (uint32_t)(j - 1) & 1u);          // P buffer free again
       float sum = 0.f;
+      // pass 2: 64 keys at a time -> exp2 -> 32 packed bf16x2 columns written over the consumed score columns
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
+      for (int hlf = 0; hlf < 2; ++hlf) {
+        uint32_t sv[2][32];
+        ptx::tmem_ld_32x32(tmem_s + hlf * 64, sv[0]);
+        ptx::tmem_ld_32x32(tmem_s + hlf * 64 + 32, sv[1]);
+        ptx::tmem_ld_wait();
+        uint32_t pk[32];
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {                                      // 8 keys = one 16-byte chunk
-          float p[8];
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            p[i] = ex2_approx(fmaf(__uint_as_float(sv[c][g * 8 + i]), scale_log2, -mc));
-            sum += p[i];
-          }
-          uint4 pk;
-          __nv_bfloat162 b0 = __floats2bfloat162_rn(p[0], p[1]), b1 = __floats2bfloat162_rn(p[2], p[3]);
-          __nv_bfloat162 b2 = __floats2bfloat162_rn(p[4], p[5]), b3 = __floats2bfloat162_rn(p[6], p[7]);
-          pk.x = *reinterpret_cast<uint32_t*>(&b0); pk.y = *reinterpret_cast<uint32_t*>(&b1);
-          pk.z = *reinterpret_cast<uint32_t*>(&b2); pk.w = *reinterpret_cast<uint32_t*>(&b3);
-          const int key_chunk = c * 4 + g;                                  // 0..15 : keys key_chunk*8 ..
-          const int sub = key_chunk >> 3, ch = key_chunk & 7;
-          *reinterpret_cast<uint4*>(p_row + sub * SUB_BYTES + ((ch ^ (row & 7)) << 4)) = pk;
+        for (int i = 0; i < 32; ++i) {
+          const int c = i >> 4, e = (i & 15) * 2, key = hlf * 64 + 2 * i;
+          float p0 = ex2_approx(fmaf(__uint_as_float(sv[c][e]), scale_log2, -mc));
+          float p1 = ex2_approx(fmaf(__uint_as_float(sv[c][e + 1]), scale_log2, -mc));
+          if (valid < BKV) { if (key >= valid) p0 = 0.f; if (key + 1 >= valid) p1 = 0.f; }
+          sum += p0 + p1;
+          pk[i] = pack_bf16(p0, p1);
         }
+        ptx::tmem_st_32x32(tmem_s + hlf * 32, pk);
       }
       l += sum;
-      ptx::fence_proxy_async_smem();
+      ptx::tmem_st_wait();
       ptx::tc_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(p_full);
+      if (lane == 0) ptx::mbar_arrive(p_full(t));
     }
     // epilogue: O / l -> bf16
-    ptx::mbar_wait(pv_done, (uint32_t)(n_kv - 1) & 1u);
+    ptx::mbar_wait(pv_done(t), (uint32_t)(n_kv - 1) & 1u);
     ptx::tc_fence_after();
     const float inv = 1.f / l;
-    const bool row_ok = q0 + row < S;
-    bf16* orow = out + ((long long)seq * S + q0 + row) * (long long)(H * DH) + head * DH;
+    const int qrow = q0 + t * BQ + row;
+    const bool row_ok = qrow < S;
+    bf16* orow = out + ((long long)seq * S + qrow) * (long long)(H * DH) + head * DH;
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
       uint32_t ov[32];
-      ptx::tmem_ld_32x32(tmem_o + c * 32 + lane_addr, ov);
+      ptx::tmem_ld_32x32(tmem_o + c * 32, ov);
       ptx::tmem_ld_wait();
       if (row_ok) {
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
           uint4 pk;
-          __nv_bfloat162 b0 = __floats2bfloat162_rn(__uint_as_float(ov[g * 8]) * inv, __uint_as_float(ov[g * 8 + 1]) * inv);
-          __nv_bfloat162 b1 = __floats2bfloat162_rn(__uint_as_float(ov[g * 8 + 2]) * inv, __uint_as_float(ov[g * 8 + 3]) * inv);
-          __nv_bfloat162 b2 = __floats2bfloat162_rn(__uint_as_float(ov[g * 8 + 4]) * inv, __uint_as_float(ov[g * 8 + 5]) * inv);
-          __nv_bfloat162 b3 = __floats2bfloat162_rn(__uint_as_float(ov[g * 8 + 6]) * inv, __uint_as_float(ov[g * 8 + 7]) * inv);
-          pk.x = *reinterpret_cast<uint32_t*>(&b0); pk.y = *reinterpret_cast<uint32_t*>(&b1);
-          pk.z = *reinterpret_cast<uint32_t*>(&b2); pk.w = *reinterpret_cast<uint32_t*>(&b3);
+          pk.x = pack_bf16(__uint_as_float(ov[g * 8]) * inv, __uint_as_float(ov[g * 8 + 1]) * inv);
+          pk.y = pack_bf16(__uint_as_float(ov[g * 8 + 2]) * inv, __uint_as_float(ov[g * 8 + 3]) * inv);
+          pk.z = pack_bf16(__uint_as_float(ov[g * 8 + 4]) * inv, __uint_as_float(ov[g * 8 + 5]) * inv);
+          pk.w = pack_bf16(__uint_as_float(ov[g * 8 + 6]) * inv, __uint_as_float(ov[g * 8 + 7]) * inv);
           *reinterpret_cast<uint4*>(orow + c * 32 + g * 8) = pk;
         }
       }
@@ -269,7 +282,7 @@ cudaError_t launch_attn_tcgen05(const void* qkv, void* out, int B, int S, int H,
     SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ATT_SMEM));
     attr_set = true;
   }
-  dim3 grid((S + BQ - 1) / BQ, H, B);
+  dim3 grid((S + QT * BQ - 1) / (QT * BQ), H, B);
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)DH);
   attn_tcgen05_kernel<<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, (bf16*)out, S, H, scale_log2);
   return cudaGetLastError();
