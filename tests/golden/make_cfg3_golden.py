@@ -4,6 +4,7 @@ configuration bench.py times.  Calls only oracle/ and the input generators in sy
 path.  Cost: ~40 min to generate the 20.4 G weights on 8 cores + ~15 min of fp64 BLAS (186 TFLOP).
 
     python tests/golden/make_cfg3_golden.py [--blocks L] [--steps T] [--seed S] [--out NAME]
+    python tests/golden/make_cfg3_golden.py --config 5 --prompt 7 --seed 229 --out cfg5_p7     (config 5, prompt 7)
 
 The GPU test (tests/test_gpu_fullsize.py) regenerates the same weights on the device, checks their
 per-block checksums against the ones stored here, runs the 16-seed batch and compares seed S.
@@ -35,8 +36,10 @@ def main():
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--out", default="cfg3_seed0")
+    ap.add_argument("--config", type=int, default=3, choices=[3, 5])
+    ap.add_argument("--prompt", type=int, default=0)
     a = ap.parse_args()
-    s = CONFIGS[3]
+    s = CONFIGS[a.config]
     if a.blocks is not None:
         s = s.with_(n_blocks=a.blocks)
     if a.steps is not None:
@@ -51,7 +54,7 @@ def main():
         blocks.append(bw)                                  # kept as bf16 (40.8 GB at full depth)
         print(f"block {b} generated ({time.time() - t0:.0f} s)", flush=True)
     gsum = {k: tensor_checksum(v) for k, v in sorted(gw.items())}
-    text = make_text_emb(s)
+    text = make_text_emb(s, prompts=[a.prompt])
     probe = make_probe(s)
     ts = [float(np.float32(t)) for t in s.timesteps]
     g = {k: np64(v) for k, v in gw.items()}
@@ -77,7 +80,7 @@ def main():
     reward = rollout.probe_reward(xT, np64(probe))
     np.save(os.path.join(here, a.out + "_latent.npy"), xT.astype(np.float32))
     meta = {"written_by": "tests/golden/make_cfg3_golden.py (oracle/ + synth/ only)", "config": s.name, "n_blocks": s.n_blocks,
-            "n_steps": s.n_steps, "seed": a.seed, "timesteps": ts, "reward": reward,
+            "n_steps": s.n_steps, "seed": a.seed, "prompt": a.prompt, "timesteps": ts, "reward": reward,
             "latent_l2": float(np.linalg.norm(xT)), "x0_l2": float(np.linalg.norm(x0)),
             "per_step_l2": [float(np.linalg.norm(h)) for h in hist],
             "per_step_head": [[float(v) for v in h.reshape(-1)[:16]] for h in hist],
