@@ -140,8 +140,93 @@ def run_reference(args, shape):
     print(json.dumps(line))
 
 
+def run_kernels(args, shape):
+    """--kernels: each kernel of the path alone at the workload's shapes, L2 flushed between iterations, one
+    CUDA-event pair per launch; prints one JSON line with achieved GB/s (HBM-bound kernels, algorithmic bytes of
+    DESIGN.md section 5) or TFLOP/s (tensor-bound kernels) against the measured burst peaks."""
+    import paper_2606_19004_b200 as spot
+    from paper_2606_19004_b200 import build as spot_build
+    from synth import hash_normal
+    spot_build.build()
+    spot.load_library()
+    peaks = load_peaks()
+    torch.cuda.set_device(0)
+    B, S, D, F, H, dh = shape.n_seqs, shape.seq, shape.hidden, shape.mlp_hidden, shape.n_heads, shape.head_dim
+    M = B * S
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    bf = torch.bfloat16
+
+    def rnd(tid, shp, dtype, scale=1.0):
+        n = int(np.prod(shp))
+        return hash_normal(900 + tid, n, scale, dtype, "cuda").reshape(shp)
+
+    def timed(fn, iters):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(iters):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return statistics.median(ts)
+
+    res = {}
+
+    def hbm(name, fn, nbytes, iters=10):
+        ms = timed(fn, iters)
+        gbs = nbytes / ms / 1e6
+        res[name] = {"bound": "hbm", "ms": ms, "algorithmic_bytes": nbytes, "achieved": gbs, "unit": "GB/s",
+                     "peak": peaks["hbm_gbs"], "frac": gbs / peaks["hbm_gbs"]}
+
+    def tensor(name, fn, flops, iters=10):
+        ms = timed(fn, iters)
+        tf = flops / ms / 1e9
+        res[name] = {"bound": "tensor", "ms": ms, "flops": flops, "achieved": tf, "unit": "TFLOP/s",
+                     "peak": peaks["bf16_tflops"], "frac": tf / peaks["bf16_tflops"]}
+
+    # K1 Philox + Box-Muller: 2^28 normals (16 seeds x 2^24), 4 B/element written
+    seeds = torch.arange(16, dtype=torch.int64, device="cuda")
+    nz = torch.empty((16, 1 << 24), dtype=torch.float32, device="cuda")
+    hbm("K1_noise", lambda: spot.spot_noise_from_seeds(seeds, 1 << 24, 0, nz), 4.0 * 16 * (1 << 24))
+    del nz
+    # K3 LN + modulate: fp32 residual rows in, bf16 out
+    h = rnd(1, (M, D), torch.float32)
+    sh, sc = rnd(2, (D,), torch.float32, 0.1), rnd(3, (D,), torch.float32, 0.1)
+    hbm("K3_ln_modulate", lambda: spot.spot_ln_modulate(h, sh, sc, 1e-6, bf), M * D * (4.0 + 2.0))
+    # K4 QK-RMSNorm + RoPE in place on q and k
+    qkv = rnd(4, (B, S, 3, H, dh), bf)
+    gains = [torch.ones(dh, dtype=bf, device="cuda") for _ in range(4)]
+    cs, sn = rnd(5, (S, dh // 2), torch.float32), rnd(6, (S, dh // 2), torch.float32)
+    hbm("K4_qk_norm_rope", lambda: spot.spot_qk_norm_rope(qkv, shape.n_txt, gains, cs, sn, 1e-6), 2.0 * 2 * B * S * H * dh * 2)
+    # K5 attention
+    tensor("K5_attention", lambda: spot.spot_attention(qkv, spot.IMPL_TCGEN05), 4.0 * S * S * dh * H * B)
+    del qkv
+    # K6 Euler update (+ reward): 2^26 elements so that the working set exceeds L2
+    Bx, E = 1024, shape.n_img * shape.latent_ch if shape.n_img * shape.latent_ch <= 65536 else 65536
+    x, v, pr = rnd(7, (Bx, E), torch.float32), rnd(8, (Bx, E), torch.float32), rnd(9, (E,), torch.float32)
+    hbm("K6_euler_update", lambda: spot.spot_euler_update(x, v, -0.1), 12.0 * Bx * E)
+    hbm("K6_euler_update_reward", lambda: spot.spot_euler_update(x, v, -0.1, pr), 12.0 * Bx * E + 4.0 * E)
+    del x, v
+    # K2 the four GEMMs of a block (image + text rows together, one weight set)
+    for name, (N, K, epi) in {"K2_gemm_qkv": (3 * D, D, spot.EPI_BIAS), "K2_gemm_out": (D, D, spot.EPI_GATE_RESIDUAL),
+                              "K2_gemm_fc1": (F, D, spot.EPI_BIAS_GELU), "K2_gemm_fc2": (D, F, spot.EPI_GATE_RESIDUAL)}.items():
+        a, w, b = rnd(10, (M, K), bf), rnd(11, (N, K), bf, 0.02), rnd(12, (N,), bf, 0.02)
+        gate, resid = rnd(13, (N,), torch.float32, 0.1), torch.zeros((M, N), dtype=torch.float32, device="cuda")
+        out = torch.empty((M, N), dtype=bf, device="cuda")
+        tensor(name, lambda: spot.spot_linear(a, w, b, epi, spot.IMPL_TCGEN05, gate=gate, residual=resid, out=out), 2.0 * M * N * K)
+        del a, w, out, resid
+    print(json.dumps({"mode": "kernels", "workload": shape.name, "rows": M, "l2": "512 MiB written between iterations",
+                      "peaks": peaks, "kernels": res}))
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--kernels", action="store_true", help="time every kernel alone against its roofline")
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
@@ -153,6 +238,8 @@ def main():
     shape = CONFIGS[WORKLOADS[args.workload]]
     if args.impl == "reference":
         return run_reference(args, shape)
+    if args.kernels:
+        return run_kernels(args, shape)
 
     import paper_2606_19004_b200 as spot
     from paper_2606_19004_b200 import build as spot_build
@@ -184,16 +271,18 @@ def main():
     ctx = spot.Context(shape, weights, max_seqs=B)
     ts = [float(np.float32(t)) for t in shape.timesteps]
     k_sel = K // 2
-    # each rank explores its own seed group (weak scaling): seeds offset by rank * B
-    seeds = torch.tensor([int(s) + rank * B for s in shape.seeds], dtype=torch.int64, device="cuda")
+    # weak scaling: the job explores world * B sequences; rank r owns the contiguous shard [r*B, (r+1)*B)
+    from paper_2606_19004_b200 import sharding
+    lo, hi = sharding.shard_range(world * B, rank, world)
+    assert hi - lo == B
+    seeds = torch.tensor([int(shape.seeds[i % B]) + (i // B) * B for i in range(lo, hi)], dtype=torch.int64, device="cuda")
     out = None
 
     def step():
         nonlocal out
         out = spot.spot_explore(ctx, seeds, text, ts, probe, P, K, k_sel, out)
         if dist is not None:
-            gathered = torch.empty(world * B, dtype=torch.float32, device="cuda")
-            dist.all_gather_into_tensor(gathered, out["rewards"])
+            sharding.gather_rewards(out["rewards"], world * B)      # the path's only exchange: world*B fp32 rewards
 
     def sync_all():
         if dist is not None:
