@@ -234,6 +234,7 @@ def main():
     ap.add_argument("--impl", default="spot", choices=["spot", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--gemm-impl", type=int, default=0, help="0 auto, 2 one-CTA tcgen05, 3 CTA-pair tcgen05 (A/B testing)")
     args = ap.parse_args()
     shape = CONFIGS[WORKLOADS[args.workload]]
     if args.impl == "reference":
@@ -269,6 +270,8 @@ def main():
     torch.cuda.synchronize()
     gen_s = time.time() - t0
     ctx = spot.Context(shape, weights, max_seqs=B)
+    if args.gemm_impl:
+        spot.spot_set_option(ctx, spot.OPT_GEMM_IMPL, args.gemm_impl)
     ts = [float(np.float32(t)) for t in shape.timesteps]
     k_sel = K // 2
     # weak scaling: the job explores world * B sequences; rank r owns the contiguous shard [r*B, (r+1)*B)

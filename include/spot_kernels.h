@@ -15,7 +15,12 @@ extern "C" {
 #endif
 
 typedef enum { SPOT_EPI_BIAS = 0, SPOT_EPI_BIAS_GELU = 1, SPOT_EPI_GATE_RESIDUAL = 2 } spot_epilogue;
-typedef enum { SPOT_IMPL_AUTO = 0, SPOT_IMPL_SIMT = 1, SPOT_IMPL_TCGEN05 = 2 } spot_impl;
+typedef enum {
+  SPOT_IMPL_AUTO = 0,
+  SPOT_IMPL_SIMT = 1,
+  SPOT_IMPL_TCGEN05 = 2,       /* one CTA per 128 x 256 tile (cta_group::1) */
+  SPOT_IMPL_TCGEN05_2CTA = 3   /* CTA pair per 256 x 256 tile (cta_group::2); GEMM only */
+} spot_impl;
 
 /* Linear layer y = x W^T + b with a fused epilogue (north_star (b); S4 steps 3, 7, 8).
  *   d_a [M, K], d_w [N, K], d_bias [N] of `dtype`.

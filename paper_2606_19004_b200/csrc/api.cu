@@ -117,7 +117,7 @@ Workspace carve(const spot_ctx* c, int B, int T) {
 spot_status run_gemm(spot_ctx* c, Epilogue epi, GemmProblem* probs, int n, spot_dtype ta, spot_dtype tout,
                      cudaStream_t st) {
   const spot_dtype dt = c->cfg.dtype;
-  bool tc = dt == SPOT_BF16 && ta == SPOT_BF16 && (epi == EPI_GATE_RES || tout == SPOT_BF16) && c->gemm_impl == 0;
+  bool tc = dt == SPOT_BF16 && ta == SPOT_BF16 && (epi == EPI_GATE_RES || tout == SPOT_BF16) && c->gemm_impl != 1;
   for (int i = 0; i < n && tc; ++i)
     if (probs[i].M > 0 && !tcgen05_gemm_supported(probs[i])) tc = false;
   if (tc) {
@@ -130,7 +130,8 @@ spot_status run_gemm(spot_ctx* c, Epilogue epi, GemmProblem* probs, int n, spot_
       }
       CK(c, cudaEventRecord(c->ev[c->ev_used], st));
     }
-    LK(c, launch_gemm_tcgen05(epi, probs, n, c->num_sms, st));
+    if (c->gemm_impl != 2) LK(c, launch_gemm_tcgen05_2cta(epi, probs, n, c->num_sms, st));   // auto = CTA pairs
+    else LK(c, launch_gemm_tcgen05(epi, probs, n, c->num_sms, st));
     ++c->gemm_launches;
     if (timed) {
       CK(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
@@ -282,6 +283,11 @@ spot_status spot_destroy(spot_ctx* ctx) {
 
 spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
   if (!ctx) return SPOT_ERR_NULL;
+  if (opt == SPOT_OPT_GEMM_IMPL) {
+    if (value < 0 || value > 3) return SPOT_ERR_SHAPE;
+    ctx->gemm_impl = value;
+    return SPOT_OK;
+  }
   if (value != 0 && value != 1) return SPOT_ERR_SHAPE;
   if (opt == SPOT_OPT_GEMM_IMPL) ctx->gemm_impl = value;
   else if (opt == SPOT_OPT_ATTN_IMPL) ctx->attn_impl = value;
@@ -687,10 +693,13 @@ spot_status spot_linear(spot_dtype dtype, spot_impl impl, spot_epilogue epi, con
   else { p.out = d_out; p.out_map = plain_rows((int)M, N); }
   const Epilogue e = epi == SPOT_EPI_BIAS ? EPI_BIAS : (epi == SPOT_EPI_BIAS_GELU ? EPI_BIAS_GELU : EPI_GATE_RES);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  bool tc = impl == SPOT_IMPL_TCGEN05 || (impl == SPOT_IMPL_AUTO && dtype == SPOT_BF16 && tcgen05_gemm_supported(p));
+  bool tc = impl == SPOT_IMPL_TCGEN05 || impl == SPOT_IMPL_TCGEN05_2CTA ||
+            (impl == SPOT_IMPL_AUTO && dtype == SPOT_BF16 && tcgen05_gemm_supported(p));
   if (tc) {
     if (dtype != SPOT_BF16 || !tcgen05_gemm_supported(p)) return SPOT_ERR_SHAPE;
-    return launch_gemm_tcgen05(e, &p, 1, sm_count(), st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+    cudaError_t ce = impl != SPOT_IMPL_TCGEN05 ? launch_gemm_tcgen05_2cta(e, &p, 1, sm_count(), st)
+                                                    : launch_gemm_tcgen05(e, &p, 1, sm_count(), st);
+    return ce == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
   }
   if (K % 16) return SPOT_ERR_SHAPE;
   return launch_gemm_simt(dtype, dtype, dtype, e, p, st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;

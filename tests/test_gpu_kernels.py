@@ -146,11 +146,13 @@ def test_linear_simt_bf16(epi):
     assert rel_l2(got, ref) < (1e-5 if epi == 2 else 4e-3)
 
 
+@pytest.mark.parametrize("impl", [2, 3])
 @pytest.mark.parametrize("epi", [0, 1, 2])
 @pytest.mark.parametrize("M,N,K", [(128, 256, 64), (300, 512, 200), (1024, 3072 + 32, 512), (77, 32, 8), (2048, 768, 3072)])
-def test_linear_tcgen05_bf16(epi, M, N, K):
-    """tcgen05/TMA GEMM vs fp64: single tile, ragged M/N/K tails, multi-tile persistent schedule, long K."""
-    got, ref = _run_linear(torch.bfloat16, spot.IMPL_TCGEN05, epi, M, N, K, 950)
+def test_linear_tcgen05_bf16(epi, M, N, K, impl):
+    """tcgen05/TMA GEMM (impl 2: one CTA per tile, impl 3: CTA pair, cta_group::2) vs fp64: single tile, ragged
+    M/N/K tails, multi-tile persistent schedule, long K."""
+    got, ref = _run_linear(torch.bfloat16, impl, epi, M, N, K, 950)
     # fp32 accumulation of exact bf16 products; only the output rounding (2^-9) for bf16 outputs
     assert rel_l2(got, ref) < (2e-5 if epi == 2 else 4e-3)
 
