@@ -351,3 +351,72 @@ def spot_rope_table(ctx: Context):
     sin = torch.empty_like(cos)
     _check(load_library().spot_rope_table(ctx.handle, _ptr(cos), _ptr(sin)), "spot_rope_table", ctx)
     return cos, sin
+
+
+# ---- host bandit planner (include/spot_planner.h) -------------------------------------------------------
+class SpotAction(C.Structure):
+    _fields_ = [("d", C.c_int32), ("s", C.c_int32)]
+
+
+def _planner_sigs(lib):
+    if getattr(lib, "_planner_ready", False):
+        return lib
+    vp, i32, dbl = C.c_void_p, C.c_int, C.c_double
+    lib.spot_planner_create.argtypes = [C.POINTER(C.c_int32), i32, C.POINTER(C.c_int32), i32, i32, dbl, dbl, i32, C.POINTER(vp)]
+    lib.spot_planner_destroy.argtypes = [vp]
+    lib.spot_planner_eligible.argtypes = [vp, dbl, dbl, C.POINTER(SpotAction), i32, C.POINTER(i32)]
+    lib.spot_planner_select.argtypes = [vp, dbl, dbl, C.POINTER(SpotAction), C.POINTER(dbl)]
+    lib.spot_planner_feedback.argtypes = [C.POINTER(C.c_float), i32, C.POINTER(C.c_float), i32, C.POINTER(dbl)]
+    lib.spot_planner_update.argtypes = [vp, SpotAction, dbl]
+    lib.spot_planner_stats.argtypes = [vp, SpotAction, C.POINTER(dbl), C.POINTER(i32), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    for n in ("create", "destroy", "eligible", "select", "feedback", "update", "stats"):
+        getattr(lib, "spot_planner_" + n).restype = C.c_int
+    lib._planner_ready = True
+    return lib
+
+
+class Planner:
+    """spot_planner: UCB exploration planner (host code in libspot.so; argument marshalling only here)."""
+
+    def __init__(self, d_values, s_values, n_prompts: int, t_step: float, beta: float = 0.5, window: int = 8):
+        lib = _planner_sigs(load_library())
+        d = (C.c_int32 * len(d_values))(*d_values)
+        s = (C.c_int32 * len(s_values))(*s_values)
+        h = C.c_void_p()
+        _check(lib.spot_planner_create(d, len(d_values), s, len(s_values), n_prompts, t_step, beta, window, C.byref(h)),
+               "spot_planner_create")
+        self.handle, self._n = h, len(d_values) * len(s_values)
+
+    def __del__(self):
+        if getattr(self, "handle", None):
+            load_library().spot_planner_destroy(self.handle)
+            self.handle = None
+
+    def spot_planner_eligible(self, t_train: float, n_spot: float):
+        out = (SpotAction * self._n)()
+        n = C.c_int()
+        _check(load_library().spot_planner_eligible(self.handle, t_train, n_spot, out, self._n, C.byref(n)), "spot_planner_eligible")
+        return [(out[i].d, out[i].s) for i in range(n.value)]
+
+    def spot_planner_select(self, t_train: float, n_spot: float):
+        a, u = SpotAction(), C.c_double()
+        _check(load_library().spot_planner_select(self.handle, t_train, n_spot, C.byref(a), C.byref(u)), "spot_planner_select")
+        return (a.d, a.s), u.value
+
+    def spot_planner_update(self, action, r: float) -> None:
+        _check(load_library().spot_planner_update(self.handle, SpotAction(*action), r), "spot_planner_update")
+
+    def spot_planner_stats(self, action):
+        m, n, ni, nt = C.c_double(), C.c_int(), C.c_int64(), C.c_int64()
+        _check(load_library().spot_planner_stats(self.handle, SpotAction(*action), C.byref(m), C.byref(n), C.byref(ni), C.byref(nt)),
+               "spot_planner_stats")
+        return {"mean": m.value, "n_i": n.value, "N_i": ni.value, "N": nt.value}
+
+
+def spot_planner_feedback(sigma_cov, sigma_unc) -> float:
+    lib = _planner_sigs(load_library())
+    a = (C.c_float * max(1, len(sigma_cov)))(*sigma_cov)
+    b = (C.c_float * max(1, len(sigma_unc)))(*sigma_unc)
+    r = C.c_double()
+    _check(lib.spot_planner_feedback(a, len(sigma_cov), b, len(sigma_unc), C.byref(r)), "spot_planner_feedback")
+    return r.value

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libspot.so")
-SOURCES = ["api.cu", "noise.cu", "elementwise.cu", "gemm_simt.cu", "attn_simt.cu", "gemm_tcgen05.cu", "gemm_tcgen05_2cta.cu", "attn_tcgen05.cu"]
+SOURCES = ["api.cu", "noise.cu", "elementwise.cu", "gemm_simt.cu", "attn_simt.cu", "gemm_tcgen05.cu", "gemm_tcgen05_2cta.cu", "attn_tcgen05.cu", "planner.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 
@@ -25,7 +25,7 @@ def _nvcc() -> str:
 
 def _digest() -> str:
     h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
-    incs = [os.path.join(HERE, "..", "include", f) for f in ("spot.h", "spot_kernels.h")]
+    incs = [os.path.join(HERE, "..", "include", f) for f in ("spot.h", "spot_kernels.h", "spot_planner.h")]
     for p in sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC)) + incs:
         with open(p, "rb") as f:
             h.update(f.read())
@@ -42,7 +42,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     flags = list(NVCC_FLAGS)
 
     def compile_one(src):
-        obj = os.path.join(OBJ, src.replace(".cu", ".o"))
+        obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
         cmd = [nvcc, *flags, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
