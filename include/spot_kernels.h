@@ -19,7 +19,8 @@ typedef enum {
   SPOT_IMPL_AUTO = 0,
   SPOT_IMPL_SIMT = 1,
   SPOT_IMPL_TCGEN05 = 2,       /* one CTA per 128 x 256 tile (cta_group::1) */
-  SPOT_IMPL_TCGEN05_2CTA = 3   /* CTA pair per 256 x 256 tile (cta_group::2); GEMM only */
+  SPOT_IMPL_TCGEN05_2CTA = 3,  /* CTA pair per 256 x 256 tile (cta_group::2), per-thread global epilogue; GEMM only */
+  SPOT_IMPL_TCGEN05_TMA = 4    /* CTA pair + shared-memory staged TMA store / reduce-add epilogue (what AUTO picks); GEMM only */
 } spot_impl;
 
 /* Linear layer y = x W^T + b with a fused epilogue (north_star (b); S4 steps 3, 7, 8).
@@ -32,6 +33,15 @@ typedef enum {
 spot_status spot_linear(spot_dtype dtype, spot_impl impl, spot_epilogue epi, const void *d_a, int64_t M, int64_t K,
                         const void *d_w, int64_t N, const void *d_bias, const float *d_gate, float *d_residual,
                         void *d_out, void *cuda_stream);
+
+/* The QKV projection with K4 fused into its epilogue (north_star (b) + (c); S4 steps 3-5), one stream:
+ *   d_out [n_seqs * rows_per_seq, 3 * hidden] bf16 = [ RoPE(RMSNorm(q) * q_gain) | RoPE(RMSNorm(k) * k_gain) | v ],
+ *   [q | k | v] = d_a [n_seqs * rows_per_seq, K] d_w[3 * hidden, K]^T + d_bias, heads of 128 columns; row r of a
+ *   sequence is rotated by row pos_off + r of d_cos / d_sin [S, 64] fp32 (S >= pos_off + rows_per_seq).
+ * bf16 only; hidden % 128 == 0, K % 8 == 0; gains [128] bf16.  Errors as spot_linear. */
+spot_status spot_qkv_rope_linear(const void *d_a, int n_seqs, int rows_per_seq, int64_t K, const void *d_w, int64_t hidden,
+                                 const void *d_bias, const void *d_q_gain, const void *d_k_gain, const float *d_cos,
+                                 const float *d_sin, int pos_off, float eps, void *d_out, void *cuda_stream);
 
 /* y = LayerNorm(h) * (1 + scale) + shift over the last axis, biased variance, no affine (S4
  * step 2).  d_h [M, D] fp32 (residual stream), d_shift/d_scale [D] fp32, d_out [M, D] of `dtype`.

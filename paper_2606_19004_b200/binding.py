@@ -18,7 +18,7 @@ _lib: Optional[C.CDLL] = None
 
 SPOT_F32, SPOT_BF16 = 0, 1
 EPI_BIAS, EPI_BIAS_GELU, EPI_GATE_RESIDUAL = 0, 1, 2
-IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_2CTA = 0, 1, 2, 3
+IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_2CTA, IMPL_TCGEN05_TMA = 0, 1, 2, 3, 4
 OPT_GEMM_IMPL, OPT_ATTN_IMPL, OPT_TIMING = 0, 1, 2
 STATUS_NAMES = ["SPOT_OK", "SPOT_ERR_NULL", "SPOT_ERR_SHAPE", "SPOT_ERR_DTYPE", "SPOT_ERR_ALIGN",
                 "SPOT_ERR_WORKSPACE", "SPOT_ERR_ARCH", "SPOT_ERR_CUDA", "SPOT_ERR_UNIMPLEMENTED"]
@@ -88,6 +88,7 @@ def load_library() -> C.CDLL:
         "spot_explore": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_explore_host": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_linear": [i32, i32, i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp],
+        "spot_qkv_rope_linear": [vp, i32, i32, i64, vp, i64, vp, vp, vp, vp, vp, i32, f32, vp, vp],
         "spot_ln_modulate": [i32, vp, i64, i64, vp, vp, f32, vp, vp],
         "spot_qk_norm_rope": [i32, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, f32, vp],
         "spot_attention": [i32, i32, vp, vp, i32, i32, i32, i32, vp],
@@ -306,6 +307,17 @@ def spot_linear(a: torch.Tensor, w: torch.Tensor, bias: torch.Tensor, epi: int =
     _check(load_library().spot_linear(_dt(w.dtype), impl, epi, _ptr(a), M, K, _ptr(w), N, _ptr(bias), _ptr(gate),
                                       _ptr(residual), _ptr(out), _stream()), "spot_linear")
     return residual if epi == EPI_GATE_RESIDUAL else out
+
+
+def spot_qkv_rope_linear(a: torch.Tensor, w: torch.Tensor, bias: torch.Tensor, q_gain: torch.Tensor, k_gain: torch.Tensor,
+                         cos: torch.Tensor, sin: torch.Tensor, pos_off: int, eps: float) -> torch.Tensor:
+    """a [n_seqs, rows_per_seq, K] bf16 -> [n_seqs, rows_per_seq, 3 * hidden] bf16 (QKV projection with K4 fused)."""
+    n_seqs, rps, K = a.shape
+    hidden = w.shape[0] // 3
+    out = torch.empty((n_seqs, rps, 3 * hidden), dtype=a.dtype, device=a.device)
+    _check(load_library().spot_qkv_rope_linear(_ptr(a), n_seqs, rps, K, _ptr(w), hidden, _ptr(bias), _ptr(q_gain), _ptr(k_gain),
+                                               _ptr(cos), _ptr(sin), pos_off, eps, _ptr(out), _stream()), "spot_qkv_rope_linear")
+    return out
 
 
 def spot_ln_modulate(h: torch.Tensor, shift: torch.Tensor, scale: torch.Tensor, eps: float, dtype: torch.dtype) -> torch.Tensor:

@@ -130,8 +130,9 @@ spot_status run_gemm(spot_ctx* c, Epilogue epi, GemmProblem* probs, int n, spot_
       }
       CK(c, cudaEventRecord(c->ev[c->ev_used], st));
     }
-    if (c->gemm_impl != 2) LK(c, launch_gemm_tcgen05_2cta(epi, probs, n, c->num_sms, st));   // auto = CTA pairs
-    else LK(c, launch_gemm_tcgen05(epi, probs, n, c->num_sms, st));
+    if (c->gemm_impl == 2) LK(c, launch_gemm_tcgen05(epi, probs, n, c->num_sms, st));
+    else if (c->gemm_impl == 3) LK(c, launch_gemm_tcgen05_2cta(epi, probs, n, c->num_sms, st));
+    else LK(c, launch_gemm_tcgen05_v3(epi, probs, n, c->num_sms, st));   // auto = CTA pairs + TMA-store epilogue
     ++c->gemm_launches;
     if (timed) {
       CK(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
@@ -284,7 +285,7 @@ spot_status spot_destroy(spot_ctx* ctx) {
 spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
   if (!ctx) return SPOT_ERR_NULL;
   if (opt == SPOT_OPT_GEMM_IMPL) {
-    if (value < 0 || value > 3) return SPOT_ERR_SHAPE;
+    if (value < 0 || value > 4) return SPOT_ERR_SHAPE;
     ctx->gemm_impl = value;
     return SPOT_OK;
   }
@@ -375,11 +376,19 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
     pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].qkv_w; pr[s].bias = bw.s[s].qkv_b;
     pr[s].M = sm[s].rows; pr[s].N = 3 * D; pr[s].K = D; pr[s].out = big; pr[s].out_map = sm[s].qkv;
   }
-  spot_status rs = run_gemm(c, EPI_BIAS, pr, 2, dt, dt, st);
+  // (4)-(5) QK-RMSNorm + RoPE: fused into the epilogue of the QKV projection (v3 kernel, d_h = 128), else K4
+  bool fuse_qk = dt == SPOT_BF16 && c->gemm_impl == 0 && g.head_dim == 128;
+  for (int s = 0; s < 2; ++s) {
+    pr[s].q_gain = bw.s[s].q_gain; pr[s].k_gain = bw.s[s].k_gain; pr[s].cos_t = c->d_cos; pr[s].sin_t = c->d_sin;
+    pr[s].pos_off = s == 0 ? g.n_txt : 0; pr[s].rms_eps = g.rms_eps;
+    if (pr[s].M > 0 && !(tcgen05_gemm_supported(pr[s]) && tcgen05_v3_qkv_rope_supported(pr[s]))) fuse_qk = false;
+  }
+  spot_status rs = run_gemm(c, fuse_qk ? EPI_QKV_ROPE : EPI_BIAS, pr, 2, dt, dt, st);
   if (rs != SPOT_OK) return rs;
-  // (4)-(5) QK-RMSNorm + RoPE, (6) joint attention -> ybuf [B,S,D]
-  LK(c, launch_qk_norm_rope(dt, big, B, S, g.n_heads, g.head_dim, g.n_txt, bw.s[0].q_gain, bw.s[0].k_gain,
-                            bw.s[1].q_gain, bw.s[1].k_gain, c->d_cos, c->d_sin, g.rms_eps, st));
+  if (!fuse_qk)
+    LK(c, launch_qk_norm_rope(dt, big, B, S, g.n_heads, g.head_dim, g.n_txt, bw.s[0].q_gain, bw.s[0].k_gain,
+                              bw.s[1].q_gain, bw.s[1].k_gain, c->d_cos, c->d_sin, g.rms_eps, st));
+  // (6) joint attention -> ybuf [B,S,D]
   if (dt == SPOT_BF16 && c->attn_impl == 0 && tcgen05_attn_supported(S, g.n_heads, g.head_dim))
     LK(c, launch_attn_tcgen05(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st));
   else
@@ -693,16 +702,41 @@ spot_status spot_linear(spot_dtype dtype, spot_impl impl, spot_epilogue epi, con
   else { p.out = d_out; p.out_map = plain_rows((int)M, N); }
   const Epilogue e = epi == SPOT_EPI_BIAS ? EPI_BIAS : (epi == SPOT_EPI_BIAS_GELU ? EPI_BIAS_GELU : EPI_GATE_RES);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  bool tc = impl == SPOT_IMPL_TCGEN05 || impl == SPOT_IMPL_TCGEN05_2CTA ||
+  bool tc = impl == SPOT_IMPL_TCGEN05 || impl == SPOT_IMPL_TCGEN05_2CTA || impl == SPOT_IMPL_TCGEN05_TMA ||
             (impl == SPOT_IMPL_AUTO && dtype == SPOT_BF16 && tcgen05_gemm_supported(p));
   if (tc) {
     if (dtype != SPOT_BF16 || !tcgen05_gemm_supported(p)) return SPOT_ERR_SHAPE;
-    cudaError_t ce = impl != SPOT_IMPL_TCGEN05 ? launch_gemm_tcgen05_2cta(e, &p, 1, sm_count(), st)
-                                                    : launch_gemm_tcgen05(e, &p, 1, sm_count(), st);
+    cudaError_t ce = impl == SPOT_IMPL_TCGEN05 ? launch_gemm_tcgen05(e, &p, 1, sm_count(), st)
+                     : impl == SPOT_IMPL_TCGEN05_2CTA ? launch_gemm_tcgen05_2cta(e, &p, 1, sm_count(), st)
+                                                      : launch_gemm_tcgen05_v3(e, &p, 1, sm_count(), st);
     return ce == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
   }
   if (K % 16) return SPOT_ERR_SHAPE;
   return launch_gemm_simt(dtype, dtype, dtype, e, p, st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
+spot_status spot_qkv_rope_linear(const void* d_a, int n_seqs, int rows_per_seq, int64_t K, const void* d_w, int64_t hidden,
+                                 const void* d_bias, const void* d_q_gain, const void* d_k_gain, const float* d_cos,
+                                 const float* d_sin, int pos_off, float eps, void* d_out, void* cuda_stream) {
+  if (n_seqs < 0 || rows_per_seq <= 0 || K <= 0 || hidden <= 0 || hidden % 128 || pos_off < 0 || K > 0x7fffffff ||
+      3 * hidden > 0x7fffffff || (long long)n_seqs * rows_per_seq > 0x7fffffff)
+    return SPOT_ERR_SHAPE;
+  if (n_seqs == 0) return SPOT_OK;
+  if (!d_a || !d_w || !d_bias || !d_q_gain || !d_k_gain || !d_cos || !d_sin || !d_out) return SPOT_ERR_NULL;
+  if (!aligned16(d_a) || !aligned16(d_w) || !aligned16(d_bias) || !aligned16(d_q_gain) || !aligned16(d_k_gain) ||
+      !aligned16(d_cos) || !aligned16(d_sin) || !aligned16(d_out))
+    return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  GemmProblem p;
+  memset(&p, 0, sizeof(p));
+  const int M = n_seqs * rows_per_seq;
+  const long long N = 3 * hidden;
+  p.A = d_a; p.a_map = RowMap{rows_per_seq, (long long)rows_per_seq * K, 0, K}; p.W = d_w; p.bias = d_bias;
+  p.M = M; p.N = (int)N; p.K = (int)K; p.out = d_out; p.out_map = RowMap{rows_per_seq, (long long)rows_per_seq * N, 0, N};
+  p.q_gain = d_q_gain; p.k_gain = d_k_gain; p.cos_t = d_cos; p.sin_t = d_sin; p.pos_off = pos_off; p.rms_eps = eps;
+  if (!tcgen05_gemm_supported(p) || !tcgen05_v3_qkv_rope_supported(p)) return SPOT_ERR_SHAPE;
+  return launch_gemm_tcgen05_v3(EPI_QKV_ROPE, &p, 1, sm_count(), (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK
+                                                                                                           : SPOT_ERR_CUDA;
 }
 
 spot_status spot_ln_modulate(spot_dtype dtype, const float* d_h, int64_t M, int64_t D, const float* d_shift,

@@ -23,7 +23,9 @@ struct RowMap {
 };
 static inline RowMap plain_rows(int M, long long ld) { RowMap r{M > 0 ? M : 1, 0, 0, ld}; return r; }
 
-enum Epilogue { EPI_BIAS = 0, EPI_BIAS_GELU = 1, EPI_GATE_RES = 2 };
+// EPI_QKV_ROPE: the QKV projection with K4 fused: +bias, then per-head RMSNorm * gain and the rotary
+// rotation on the q and k heads (v heads: +bias only), bf16 out (tcgen05 v3 kernel only, head_dim 128)
+enum Epilogue { EPI_BIAS = 0, EPI_BIAS_GELU = 1, EPI_GATE_RES = 2, EPI_QKV_ROPE = 3 };
 
 // One GEMM problem C = epi(A W^T + bias); A rows addressed through a_map (K contiguous), W [N, K].
 struct GemmProblem {
@@ -37,6 +39,14 @@ struct GemmProblem {
   const float* gate;    // EPI_GATE_RES: [N] fp32
   float* resid;         // EPI_GATE_RES: fp32 residual stream, updated in place
   RowMap resid_map;
+  // EPI_QKV_ROPE only: N = 3 * hidden, columns [q | k | v], heads of 128; row r of a sequence sits at joint
+  // position pos_off + r of the rotary table cos_t / sin_t [S, 64] fp32; gains [128] in the element type of W
+  const void* q_gain;
+  const void* k_gain;
+  const float* cos_t;
+  const float* sin_t;
+  int pos_off;
+  float rms_eps;
 };
 
 __device__ __forceinline__ float to_f32(float v) { return v; }

@@ -1,0 +1,432 @@
+// gemm_tcgen05_v3.cu - K2, CTA-pair GEMM with a TMA-store epilogue (the default since round 1b).
+// Mainloop as gemm_tcgen05_2cta.cu: a cluster of two CTAs works on one 256 x 256 output tile with
+// tcgen05.mma.cta_group::2 (M 256, N 256, K 16), a 6-stage TMA ring of 128-byte-swizzled K-major tiles and two
+// 256-column TMEM accumulators, so the epilogue of tile i overlaps the mainloop of tile i + 1.
+//
+// What is new is the epilogue (warps 4-7 of each CTA, one TMEM lane quarter = 32 rows each):
+//   * results leave the SM through shared memory and TMA instead of per-thread global accesses: each warp packs
+//     32 rows x 128 bytes into its own swizzled staging buffer (two buffers per warp, so the TMA engine drains
+//     one while the warp fills the other) and one lane issues cp.async.bulk.tensor (store) - full 128-byte
+//     lines, rows past the end of a sequence clipped by the tensor map;
+//   * EPI_GATE_RES  h += gate * (y + bias): the tile of gate * (y + bias) is sent with cp.reduce.async.bulk.tensor
+//     .add.f32, so the fp32 residual stream is never loaded by the SM (the add happens in the memory system; every
+//     element belongs to exactly one tile, so the result does not depend on scheduling);
+//   * EPI_BIAS_GELU uses tanh.approx.f32 (one MUFU op; abs. error < 2^-10, below the bf16 rounding of the output);
+//   * EPI_QKV_ROPE  fuses K4 (north_star (c)) into the QKV projection: a 256-column tile is two whole heads and a
+//     thread owns one token row of the accumulator, so the per-head RMS is thread-local: pass 1 over TMEM sums the
+//     squares of (acc + bias), pass 2 scales by rsqrt(mean + eps) * gain, rotates pairs (2i, 2i+1) by the table
+//     angle of the token's joint position and stores bf16.  v heads take the plain bias path.
+#include <stdlib.h>
+#include <string.h>
+
+#include "kernels.h"
+#include "tcgen05.cuh"
+
+namespace {
+
+constexpr int BLOCK_M = 128 /*per CTA*/, PAIR_M = 256, BLOCK_N = 256, HALF_N = 128, BLOCK_K = 64, UMMA_K = 16;
+constexpr int STAGES = 6, GROUP_M = 8;
+constexpr uint32_t A_BYTES = BLOCK_M * BLOCK_K * 2, B_BYTES = HALF_N * BLOCK_K * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr uint32_t STG_BYTES = 32 * 128;                         // one staging buffer: 32 rows x 128 bytes
+constexpr uint32_t OFF_STG = STAGES * STAGE_BYTES;               // 4 warps x 2 buffers
+constexpr uint32_t OFF_BAR = OFF_STG + 4 * 2 * STG_BYTES;
+constexpr uint32_t SMEM_BYTES = OFF_BAR + 256 /*barriers*/ + 1024 /*align slack*/;
+constexpr int NUM_THREADS = 256;
+static_assert(SMEM_BYTES <= 232448, "shared memory budget");
+
+struct V3Problem {
+  int m_tiles, n_tiles, tiles_per_seq, rps, N, k_blocks, tile_start;   // m_tiles counts 256-row pair tiles
+  const bf16* bias;
+  const float* gate;
+  // EPI_QKV_ROPE
+  const bf16* q_gain;
+  const bf16* k_gain;
+  const float* cos_t;
+  const float* sin_t;
+  int pos_off, hidden;
+  float rms_eps;
+};
+struct V3Params {
+  V3Problem p[2];
+  int n_probs, total_tiles;
+};
+struct TileCoord { int prob, mt, nt; };
+
+__device__ __forceinline__ TileCoord decode_tile(const V3Params& P, int t) {
+  TileCoord c;
+  c.prob = (P.n_probs > 1 && t >= P.p[1].tile_start) ? 1 : 0;
+  const V3Problem& q = P.p[c.prob];
+  t -= q.tile_start;
+  const int per_group = GROUP_M * q.n_tiles;
+  const int g = t / per_group, first_m = g * GROUP_M;
+  const int gm = min(GROUP_M, q.m_tiles - first_m);
+  const int r = t - g * per_group;
+  c.mt = first_m + r % gm;
+  c.nt = r / gm;
+  return c;
+}
+
+__device__ __forceinline__ float tanh_approx(float x) {
+  float y;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float gelu_tanh_fast(float x) {
+  const float k0 = 0.7978845608028654f, k1 = 0.7978845608028654f * 0.044715f;
+  const float x2 = x * x;
+  const float inner = x * fmaf(k1, x2, k0);
+  const float hx = 0.5f * x;
+  return fmaf(hx, tanh_approx(inner), hx);
+}
+__device__ __forceinline__ uint32_t pack2(float a, float b) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+// acc (fp32 bits from TMEM) + bias for 32 consecutive columns starting at bias pointer bp (16-byte aligned)
+__device__ __forceinline__ void add_bias32(const uint32_t (&v)[32], const bf16* bp, float (&y)[32]) {
+  const uint4* p4 = reinterpret_cast<const uint4*>(bp);
+#pragma unroll
+  for (int g = 0; g < 4; ++g) {
+    uint4 braw = __ldg(p4 + g);
+    const bf16* bb = reinterpret_cast<const bf16*>(&braw);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) y[g * 8 + j] = __uint_as_float(v[g * 8 + j]) + __bfloat162float(bb[j]);
+  }
+}
+// 32 fp32 values -> 64 bytes of bf16 = 16-byte chunks c0 .. c0+3 of this thread's 128-byte staging row
+__device__ __forceinline__ void stage_bf16_32(uint32_t row_addr, int sw, int c0, const float (&y)[32]) {
+#pragma unroll
+  for (int g = 0; g < 4; ++g)
+    st_shared_v4(row_addr + (uint32_t)(((c0 + g) ^ sw) << 4), pack2(y[8 * g], y[8 * g + 1]), pack2(y[8 * g + 2], y[8 * g + 3]),
+                 pack2(y[8 * g + 4], y[8 * g + 5]), pack2(y[8 * g + 6], y[8 * g + 7]));
+}
+
+template <int EPI>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
+gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmW0,
+                       const __grid_constant__ CUtensorMap tmO0, const __grid_constant__ CUtensorMap tmA1,
+                       const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmO1,
+                       const V3Params P) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + OFF_BAR;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + 2 + a); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
+  volatile uint32_t* tmem_slot_ptr =
+      reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = ptx::cluster_ctarank();            // 0 = leader of the pair
+  const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmA0); ptx::prefetch_tmap(&tmW0); ptx::prefetch_tmap(&tmO0);
+    if (P.n_probs > 1) { ptx::prefetch_tmap(&tmA1); ptx::prefetch_tmap(&tmW1); ptx::prefetch_tmap(&tmO1); }
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    for (int a = 0; a < 2; ++a) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 8); }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 2) { ptx::tmem_alloc_2cta(tmem_slot, 512); ptx::tmem_relinquish_2cta(); }
+  ptx::tc_fence_before();
+  ptx::cluster_sync();                                      // barriers of both CTAs initialised, TMEM allocated
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  if (warp == 0) {
+    // ===================== TMA producer (both CTAs) =====================
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int t = pair; t < P.total_tiles; t += n_pairs) {
+        const TileCoord c = decode_tile(P, t);
+        const V3Problem& q = P.p[c.prob];
+        const CUtensorMap* mA = c.prob ? &tmA1 : &tmA0;
+        const CUtensorMap* mW = c.prob ? &tmW1 : &tmW0;
+        const int seq = c.mt / q.tiles_per_seq;
+        const int r0 = (c.mt - seq * q.tiles_per_seq) * PAIR_M + (int)rank * BLOCK_M;
+        const int n0 = c.nt * BLOCK_N + (int)rank * HALF_N;
+        for (int kb = 0; kb < q.k_blocks; ++kb) {
+          ptx::mbar_wait(empty_bar(stage), phase ^ 1);
+          const uint32_t leader_full = ptx::map_to_cta(full_bar(stage), 0);
+          const uint32_t sa = smem_base + stage * STAGE_BYTES;
+          ptx::tma_load_3d_2cta(sa, mA, leader_full, kb * BLOCK_K, r0, seq);
+          ptx::tma_load_2d_2cta(sa + A_BYTES, mW, leader_full, kb * BLOCK_K, n0);
+          // only the leader arms its barrier, for the bytes of BOTH CTAs (see gemm_tcgen05_2cta.cu)
+          if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (leader CTA only) =====================
+    if (rank == 0 && lane == 0) {
+      constexpr uint32_t idesc = ptx::make_idesc_bf16(PAIR_M, BLOCK_N, 0, 0);
+      int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t acc_phase = 0;
+      for (int t = pair; t < P.total_tiles; t += n_pairs) {
+        const TileCoord c = decode_tile(P, t);
+        const int k_blocks = P.p[c.prob].k_blocks;
+        ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + acc * BLOCK_N;
+        for (int kb = 0; kb < k_blocks; ++kb) {
+          ptx::mbar_wait(full_bar(stage), phase);
+          ptx::tc_fence_after();
+          const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
+#pragma unroll
+          for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+            const uint64_t da = ptx::make_smem_desc(sa + k * UMMA_K * 2, 16, 1024);
+            const uint64_t db = ptx::make_smem_desc(sb + k * UMMA_K * 2, 16, 1024);
+            ptx::mma_f16_ss_2cta(d_tmem, da, db, idesc, (kb | k) ? 1u : 0u);
+          }
+          ptx::mma_commit_2cta(empty_bar(stage));
+          if (kb == k_blocks - 1) ptx::mma_commit_2cta(tfull_bar(acc));
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+        if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue (both CTAs, own 128 TMEM lanes) =====================
+    const int q4 = warp & 3;
+    const uint32_t stg0 = smem_base + OFF_STG + (uint32_t)q4 * 2 * STG_BYTES;
+    const uint32_t row_off = (uint32_t)lane * 128u;
+    const int sw = lane & 7;
+    int buf = 0;
+    int acc = 0; uint32_t acc_phase = 0;
+    for (int t = pair; t < P.total_tiles; t += n_pairs) {
+      const TileCoord c = decode_tile(P, t);
+      const V3Problem& q = P.p[c.prob];
+      const CUtensorMap* mO = c.prob ? &tmO1 : &tmO0;
+      const int seq = c.mt / q.tiles_per_seq;
+      const int row0 = (c.mt - seq * q.tiles_per_seq) * PAIR_M + (int)rank * BLOCK_M + q4 * 32;   // first row of this warp
+      const bool warp_ok = row0 < q.rps;                    // whole warp past the end of the sequence: nothing to store
+      ptx::mbar_wait(tfull_bar(acc), acc_phase);
+      ptx::tc_fence_after();
+      const uint32_t taddr0 = tmem_base + acc * BLOCK_N + ((uint32_t)(q4 * 32) << 16);
+      const int ncol0 = c.nt * BLOCK_N;
+
+      // hand a filled staging buffer to the TMA engine
+      auto send = [&](int n0) {
+        ptx::fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          if (warp_ok) {
+            if (EPI == EPI_GATE_RES) ptx::tma_reduce_add_3d(mO, stg0 + buf * STG_BYTES, n0, row0, seq);
+            else ptx::tma_store_3d(mO, stg0 + buf * STG_BYTES, n0, row0, seq);
+          }
+          ptx::bulk_commit();
+        }
+        buf ^= 1;
+      };
+      // wait until the TMA engine has read the buffer filled two sends ago
+      auto acquire = [&]() {
+        if (lane == 0) ptx::bulk_wait_read<1>();
+        __syncwarp();
+        return stg0 + buf * STG_BYTES + row_off;
+      };
+
+      if (EPI == EPI_GATE_RES) {
+#pragma unroll 1
+        for (int ch = 0; ch < BLOCK_N / 32; ++ch) {
+          const int n0 = ncol0 + ch * 32;
+          if (n0 >= q.N) break;
+          uint32_t v[32];
+          ptx::tmem_ld_32x32(taddr0 + ch * 32, v);
+          const uint32_t ra = acquire();
+          ptx::tmem_ld_wait();
+          float y[32];
+          add_bias32(v, q.bias + n0, y);
+          const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
+#pragma unroll
+          for (int g = 0; g < 8; ++g) {
+            const float4 gt = __ldg(gp + g);
+            st_shared_v4(ra + (uint32_t)((g ^ sw) << 4), __float_as_uint(gt.x * y[4 * g]), __float_as_uint(gt.y * y[4 * g + 1]),
+                         __float_as_uint(gt.z * y[4 * g + 2]), __float_as_uint(gt.w * y[4 * g + 3]));
+          }
+          send(n0);
+        }
+      } else {
+        const int row = row0 + lane;                          // row inside the sequence (may be past its end)
+#pragma unroll 1
+        for (int hh = 0; hh < BLOCK_N / 128; ++hh) {          // a 128-column half tile = one head of the QKV output
+          const int hcol0 = ncol0 + hh * 128;
+          if (hcol0 >= q.N) break;
+          float rinv = 0.f;
+          const bf16* gain = nullptr;
+          const float* cs = nullptr;
+          const float* sn = nullptr;
+          if (EPI == EPI_QKV_ROPE) {
+            const int which = hcol0 / q.hidden;               // 0 = q, 1 = k, 2 = v
+            if (which < 2) {
+              gain = which ? q.k_gain : q.q_gain;
+              const long long pos = q.pos_off + (row < q.rps ? row : 0);
+              cs = q.cos_t + pos * 64;
+              sn = q.sin_t + pos * 64;
+              float ss = 0.f;                                 // pass 1: sum of squares of (acc + bias) over the head
+#pragma unroll 1
+              for (int c4 = 0; c4 < 4; ++c4) {
+                uint32_t v[32];
+                ptx::tmem_ld_32x32(taddr0 + hh * 128 + c4 * 32, v);
+                ptx::tmem_ld_wait();
+                float y[32];
+                add_bias32(v, q.bias + hcol0 + c4 * 32, y);
+#pragma unroll
+                for (int j = 0; j < 32; ++j) ss = fmaf(y[j], y[j], ss);
+              }
+              rinv = rsqrtf(ss * (1.f / 128.f) + q.rms_eps);
+            }
+          }
+#pragma unroll 1
+          for (int c2 = 0; c2 < 2; ++c2) {                    // 64 columns = 128 bytes of bf16 per row
+            const int n0 = hcol0 + c2 * 64;
+            if (n0 >= q.N) break;
+            const bool second = n0 + 32 < q.N;
+            uint32_t v0[32], v1[32];
+            ptx::tmem_ld_32x32(taddr0 + hh * 128 + c2 * 64, v0);
+            ptx::tmem_ld_32x32(taddr0 + hh * 128 + c2 * 64 + 32, v1);
+            const uint32_t ra = acquire();
+            ptx::tmem_ld_wait();
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+              float y[32];
+              if (hf == 0) add_bias32(v0, q.bias + n0, y);
+              else if (second) add_bias32(v1, q.bias + n0 + 32, y);
+              else {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) y[j] = 0.f;
+              }
+              if (EPI == EPI_BIAS_GELU) {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) y[j] = gelu_tanh_fast(y[j]);
+              }
+              if (EPI == EPI_QKV_ROPE && gain != nullptr) {
+                const int hc = c2 * 64 + hf * 32;             // first column of this group inside the head
+                const uint4* g4 = reinterpret_cast<const uint4*>(gain + hc);
+                const float4* c4p = reinterpret_cast<const float4*>(cs + hc / 2);
+                const float4* s4p = reinterpret_cast<const float4*>(sn + hc / 2);
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {                 // 8 columns = 4 rotation pairs
+                  uint4 graw = __ldg(g4 + g);
+                  const bf16* gg = reinterpret_cast<const bf16*>(&graw);
+                  const float4 cv = __ldg(c4p + g), sv = __ldg(s4p + g);
+                  const float cc[4] = {cv.x, cv.y, cv.z, cv.w}, sd[4] = {sv.x, sv.y, sv.z, sv.w};
+#pragma unroll
+                  for (int pr = 0; pr < 4; ++pr) {
+                    const float a = y[8 * g + 2 * pr] * rinv * __bfloat162float(gg[2 * pr]);
+                    const float b = y[8 * g + 2 * pr + 1] * rinv * __bfloat162float(gg[2 * pr + 1]);
+                    y[8 * g + 2 * pr] = a * cc[pr] - b * sd[pr];
+                    y[8 * g + 2 * pr + 1] = a * sd[pr] + b * cc[pr];
+                  }
+                }
+              }
+              stage_bf16_32(ra, sw, hf * 4, y);
+            }
+            send(n0);
+          }
+        }
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive_cluster(ptx::map_to_cta(tempty_bar(acc), 0));
+      if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+    }
+    if (lane == 0) ptx::bulk_wait<0>();                     // all stores of this warp have completed
+  }
+
+  ptx::tc_fence_before();
+  ptx::cluster_sync();                                      // nobody of the pair still uses TMEM or remote barriers
+  if (warp == 2) { ptx::tc_fence_after(); ptx::tmem_dealloc_2cta(tmem_base, 512); }
+}
+
+}  // namespace
+
+bool tcgen05_v3_qkv_rope_supported(const GemmProblem& g) {
+  return g.N % 3 == 0 && (g.N / 3) % 128 == 0 && g.q_gain && g.k_gain && g.cos_t && g.sin_t && g.pos_off >= 0 &&
+         reinterpret_cast<uintptr_t>(g.q_gain) % 16 == 0 && reinterpret_cast<uintptr_t>(g.k_gain) % 16 == 0 &&
+         reinterpret_cast<uintptr_t>(g.cos_t) % 16 == 0 && reinterpret_cast<uintptr_t>(g.sin_t) % 16 == 0;
+}
+
+cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n_probs, int num_sms, cudaStream_t st) {
+  if (n_probs < 1 || n_probs > 2) return cudaErrorInvalidValue;
+  V3Params P;
+  memset(&P, 0, sizeof(P));
+  CUtensorMap tm[6];
+  memset(tm, 0, sizeof(tm));
+  int tiles = 0, np = 0;
+  for (int i = 0; i < n_probs; ++i) {
+    const GemmProblem& g = probs[i];
+    if (g.M <= 0) continue;
+    if (!tcgen05_gemm_supported(g)) return cudaErrorInvalidValue;
+    if ((epi == EPI_GATE_RES) != (g.resid != nullptr)) return cudaErrorInvalidValue;
+    if (epi != EPI_GATE_RES && !g.out) return cudaErrorInvalidValue;
+    if (epi == EPI_QKV_ROPE && !tcgen05_v3_qkv_rope_supported(g)) return cudaErrorInvalidValue;
+    V3Problem& q = P.p[np];
+    const int rps = g.a_map.rows_per_seq, nseq = g.M / rps;
+    q.rps = rps;
+    q.tiles_per_seq = (rps + PAIR_M - 1) / PAIR_M;
+    q.m_tiles = nseq * q.tiles_per_seq;
+    q.n_tiles = (g.N + BLOCK_N - 1) / BLOCK_N;
+    q.N = g.N;
+    q.k_blocks = (g.K + BLOCK_K - 1) / BLOCK_K;
+    q.tile_start = tiles;
+    q.bias = (const bf16*)g.bias;
+    q.gate = g.gate;
+    q.q_gain = (const bf16*)g.q_gain; q.k_gain = (const bf16*)g.k_gain;
+    q.cos_t = g.cos_t; q.sin_t = g.sin_t; q.pos_off = g.pos_off; q.hidden = g.N / 3; q.rms_eps = g.rms_eps;
+    tiles += q.m_tiles * q.n_tiles;
+    const uint64_t adims[3] = {(uint64_t)g.K, (uint64_t)rps, (uint64_t)nseq};
+    const uint64_t astr[2] = {(uint64_t)g.a_map.ld * 2,
+                              (uint64_t)(nseq > 1 ? g.a_map.seq_stride : g.a_map.ld * (long long)rps) * 2};
+    const uint32_t abox[3] = {BLOCK_K, BLOCK_M, 1};
+    SPOT_CUDA_TRY(spot_make_tmap_bf16(&tm[3 * np], (const bf16*)g.A + g.a_map.offset, 3, adims, astr, abox));
+    const uint64_t wdims[2] = {(uint64_t)g.K, (uint64_t)g.N};
+    const uint64_t wstr[1] = {(uint64_t)g.K * 2};
+    const uint32_t wbox[2] = {BLOCK_K, HALF_N};
+    SPOT_CUDA_TRY(spot_make_tmap_bf16(&tm[3 * np + 1], g.W, 2, wdims, wstr, wbox));
+    const uint64_t odims[3] = {(uint64_t)g.N, (uint64_t)rps, (uint64_t)nseq};
+    if (epi == EPI_GATE_RES) {
+      const RowMap& m = g.resid_map;
+      const uint64_t ostr[2] = {(uint64_t)m.ld * 4, (uint64_t)(nseq > 1 ? m.seq_stride : m.ld * (long long)rps) * 4};
+      const uint32_t obox[3] = {32, 32, 1};
+      SPOT_CUDA_TRY(spot_make_tmap_f32(&tm[3 * np + 2], g.resid + m.offset, 3, odims, ostr, obox));
+    } else {
+      const RowMap& m = g.out_map;
+      const uint64_t ostr[2] = {(uint64_t)m.ld * 2, (uint64_t)(nseq > 1 ? m.seq_stride : m.ld * (long long)rps) * 2};
+      const uint32_t obox[3] = {64, 32, 1};
+      SPOT_CUDA_TRY(spot_make_tmap_bf16(&tm[3 * np + 2], (bf16*)g.out + m.offset, 3, odims, ostr, obox));
+    }
+    ++np;
+  }
+  if (np == 0) return cudaSuccess;
+  if (np == 1) { tm[3] = tm[0]; tm[4] = tm[1]; tm[5] = tm[2]; }
+  P.n_probs = np;
+  P.total_tiles = tiles;
+  int pairs = num_sms / 2;
+  if (tiles < pairs) pairs = tiles;
+  const int grid = 2 * pairs;
+#define V3_LAUNCH(E)                                                                                              \
+  do {                                                                                                            \
+    static bool attr_set = false;                                                                                 \
+    if (!attr_set) {                                                                                              \
+      SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_v3_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                         (int)SMEM_BYTES));                                                       \
+      attr_set = true;                                                                                            \
+    }                                                                                                             \
+    gemm_tcgen05_v3_kernel<E><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], tm[4], tm[5], P); \
+  } while (0)
+  switch (epi) {
+    case EPI_BIAS: V3_LAUNCH(EPI_BIAS); break;
+    case EPI_BIAS_GELU: V3_LAUNCH(EPI_BIAS_GELU); break;
+    case EPI_GATE_RES: V3_LAUNCH(EPI_GATE_RES); break;
+    case EPI_QKV_ROPE: V3_LAUNCH(EPI_QKV_ROPE); break;
+  }
+#undef V3_LAUNCH
+  return cudaGetLastError();
+}

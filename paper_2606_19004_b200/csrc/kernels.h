@@ -49,5 +49,8 @@ struct TmaEncoder;   // opaque: resolves cuTensorMapEncodeTiled once
 bool tcgen05_gemm_supported(const GemmProblem& p);
 cudaError_t launch_gemm_tcgen05(Epilogue epi, const GemmProblem* probs, int n_probs, int num_sms, cudaStream_t st);
 cudaError_t launch_gemm_tcgen05_2cta(Epilogue epi, const GemmProblem* probs, int n_probs, int num_sms, cudaStream_t st);
+// v3: CTA pairs + TMA-store epilogue (+ EPI_QKV_ROPE, the QKV projection with K4 fused)
+cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n_probs, int num_sms, cudaStream_t st);
+bool tcgen05_v3_qkv_rope_supported(const GemmProblem& p);
 bool tcgen05_attn_supported(int S, int H, int dh);
 cudaError_t launch_attn_tcgen05(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st);

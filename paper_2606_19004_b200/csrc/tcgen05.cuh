@@ -164,6 +164,31 @@ spot_encode_tiled_fn spot_get_encode_tiled();
 // bf16 tensor, `rank` dims (innermost first), byte strides for dims 1..rank-1, 128-byte swizzle.
 cudaError_t spot_make_tmap_bf16(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
                                 const uint64_t* strides_bytes, const uint32_t* box);
+// same for an fp32 tensor (TMA store / reduce-add of the residual stream)
+cudaError_t spot_make_tmap_f32(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
+                               const uint64_t* strides_bytes, const uint32_t* box);
+
+// ---- TMA stores (shared -> global through a tensor map), bulk async-groups ---------------------------------
+namespace ptx {
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(
+                   reinterpret_cast<uint64_t>(m)),
+               "r"(src), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+// global[tile] += shared[tile] (fp32 add performed by the memory system; each element is touched by one tile only)
+__device__ __forceinline__ void tma_reduce_add_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(
+                   reinterpret_cast<uint64_t>(m)),
+               "r"(src), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
+}  // namespace ptx
 
 // ---- 2-CTA (cta_group::2) variants: a CTA pair of one cluster shares one M = 256 MMA ------------------------
 namespace ptx {

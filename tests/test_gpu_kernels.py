@@ -146,12 +146,12 @@ def test_linear_simt_bf16(epi):
     assert rel_l2(got, ref) < (1e-5 if epi == 2 else 4e-3)
 
 
-@pytest.mark.parametrize("impl", [2, 3])
+@pytest.mark.parametrize("impl", [2, 3, 4])
 @pytest.mark.parametrize("epi", [0, 1, 2])
 @pytest.mark.parametrize("M,N,K", [(128, 256, 64), (300, 512, 200), (1024, 3072 + 32, 512), (77, 32, 8), (2048, 768, 3072)])
 def test_linear_tcgen05_bf16(epi, M, N, K, impl):
-    """tcgen05/TMA GEMM (impl 2: one CTA per tile, impl 3: CTA pair, cta_group::2) vs fp64: single tile, ragged
-    M/N/K tails, multi-tile persistent schedule, long K."""
+    """tcgen05/TMA GEMM (impl 2: one CTA per tile, impl 3: CTA pair, cta_group::2, impl 4: CTA pair with the
+    TMA-store / reduce-add epilogue) vs fp64: single tile, ragged M/N/K tails, multi-tile persistent schedule, long K."""
     got, ref = _run_linear(torch.bfloat16, impl, epi, M, N, K, 950)
     # fp32 accumulation of exact bf16 products; only the output rounding (2^-9) for bf16 outputs
     assert rel_l2(got, ref) < (2e-5 if epi == 2 else 4e-3)
@@ -166,6 +166,58 @@ def test_linear_tcgen05_matches_simt_bitwise_close():
     assert rel_l2(np64(y_tc), np64(y_si)) < 3e-3        # both round the same fp32-accumulated value to bf16
     again = spot.spot_linear(a, w, b, spot.EPI_BIAS, spot.IMPL_TCGEN05)
     assert torch.equal(y_tc, again)                     # deterministic
+
+
+def test_linear_tma_epilogue_is_deterministic_and_leaves_neighbours_alone():
+    """impl 4: the reduce-add epilogue touches every element of the residual exactly once (bit-identical run to run),
+    and a store into a column slice of a wider buffer does not write outside the slice (tensor-map clipping)."""
+    M, N, K = 300, 160, 128
+    a = hash_normal(963, M * K, 1.0, torch.bfloat16, "cuda").reshape(M, K)
+    w = hash_normal(964, N * K, 0.05, torch.bfloat16, "cuda").reshape(N, K)
+    b = hash_normal(965, N, 0.1, torch.bfloat16, "cuda")
+    gate = hash_normal(966, N, 0.5, torch.float32, "cuda")
+    resid = hash_normal(967, M * N, 1.0, torch.float32, "cuda").reshape(M, N)
+    r1 = spot.spot_linear(a, w, b, spot.EPI_GATE_RESIDUAL, spot.IMPL_TCGEN05_TMA, gate=gate, residual=resid.clone())
+    r2 = spot.spot_linear(a, w, b, spot.EPI_GATE_RESIDUAL, spot.IMPL_TCGEN05_TMA, gate=gate, residual=resid.clone())
+    assert torch.equal(r1, r2)
+    y1 = spot.spot_linear(a, w, b, spot.EPI_BIAS, spot.IMPL_TCGEN05_TMA)
+    y3 = spot.spot_linear(a, w, b, spot.EPI_BIAS, spot.IMPL_TCGEN05_2CTA)
+    assert torch.equal(y1, y3)                           # same accumulation order, same rounding: bit-identical
+    g1 = spot.spot_linear(a, w, b, spot.EPI_BIAS_GELU, spot.IMPL_TCGEN05_TMA)
+    g3 = spot.spot_linear(a, w, b, spot.EPI_BIAS_GELU, spot.IMPL_TCGEN05_2CTA)
+    assert rel_l2(np64(g1), np64(g3)) < 3e-3             # tanh.approx vs tanhf, both rounded to bf16
+
+
+@pytest.mark.parametrize("n_seqs,rps,H,K,pos_off,gscale", [(2, 200, 2, 256, 9, 1.0), (1, 384, 4, 128, 0, 1.0), (3, 77, 1, 64, 5, 4.0),
+                                                        (2, 1024, 6, 768, 256, 1.0)])
+def test_qkv_rope_linear_fused(n_seqs, rps, H, K, pos_off, gscale):
+    """The QKV projection with K4 fused into its epilogue (EPI_QKV_ROPE) vs the oracle's Linear -> RMSNorm -> RoPE,
+    ragged row tiles, hidden not a multiple of the 256-column tile (H odd), positions offset into the table."""
+    dh, hidden = 128, H * 128
+    S = pos_off + rps + 3
+    a = hash_normal(990, n_seqs * rps * K, 1.0, torch.bfloat16, "cuda").reshape(n_seqs, rps, K)
+    w = hash_normal(991, 3 * hidden * K, 0.05, torch.bfloat16, "cuda").reshape(3 * hidden, K)
+    b = hash_normal(992, 3 * hidden, 0.1, torch.bfloat16, "cuda")
+    qg = (hash_normal(993, dh, 0.3, torch.bfloat16, "cuda") + 1.0) * gscale
+    kg = (hash_normal(994, dh, 0.3, torch.bfloat16, "cuda") + 1.0) * gscale
+    ang = hash_normal(995, S * 64, 2.0, torch.float32, "cuda").reshape(S, 64)
+    cos, sin = torch.cos(ang), torch.sin(ang)
+    out = spot.spot_qkv_rope_linear(a, w, b, qg, kg, cos, sin, pos_off, 1e-6)
+    y = (np64(a).reshape(-1, K) @ np64(w).T + np64(b)).reshape(n_seqs, rps, 3, H, dh)
+    c64, s64 = np64(cos)[pos_off:pos_off + rps], np64(sin)[pos_off:pos_off + rps]
+    ref = y.copy()
+    for part, gn in ((0, qg), (1, kg)):
+        for i in range(n_seqs):
+            ref[i, :, part] = mmdit.apply_rope(mmdit.rms_norm(y[i, :, part], np64(gn), 1e-6), c64, s64)
+    got = np64(out).reshape(n_seqs, rps, 3, H, dh)
+    for part in range(3):
+        err = rel_l2(got[:, :, part], ref[:, :, part])
+        assert err < 4e-3, (part, err)
+    # against the unfused pair of kernels: the fused path skips one bf16 rounding, so close but not identical
+    lin = spot.spot_linear(a.reshape(-1, K), w, b, spot.EPI_BIAS, spot.IMPL_TCGEN05_TMA).reshape(n_seqs, rps, 3, H, dh)
+    assert torch.equal(lin[:, :, 2], out.reshape(n_seqs, rps, 3, H, dh)[:, :, 2])   # v columns take the plain bias path
+    again = spot.spot_qkv_rope_linear(a, w, b, qg, kg, cos, sin, pos_off, 1e-6)
+    assert torch.equal(out, again)
 
 
 # ------------------------------------------------------------------ K6 / K8
