@@ -218,8 +218,13 @@ def run_kernels(args, shape):
         a, w, b = rnd(10, (M, K), bf), rnd(11, (N, K), bf, 0.02), rnd(12, (N,), bf, 0.02)
         gate, resid = rnd(13, (N,), torch.float32, 0.1), torch.zeros((M, N), dtype=torch.float32, device="cuda")
         out = torch.empty((M, N), dtype=bf, device="cuda")
-        tensor(name, lambda: spot.spot_linear(a, w, b, epi, spot.IMPL_TCGEN05, gate=gate, residual=resid, out=out), 2.0 * M * N * K)
+        tensor(name, lambda: spot.spot_linear(a, w, b, epi, spot.IMPL_AUTO, gate=gate, residual=resid, out=out), 2.0 * M * N * K)
         del a, w, out, resid
+    # K2 + K4 fused: the QKV projection whose epilogue applies QK-RMSNorm + RoPE (what the rollout launches)
+    a, w, b = rnd(10, (B, S, D), bf), rnd(11, (3 * D, D), bf, 0.02), rnd(12, (3 * D,), bf, 0.02)
+    tensor("K2_gemm_qkv_rope_fused", lambda: spot.spot_qkv_rope_linear(a, w, b, gains[0], gains[1], cs, sn, 0, 1e-6),
+           2.0 * M * 3 * D * D)
+    del a, w
     print(json.dumps({"mode": "kernels", "workload": shape.name, "rows": M, "l2": "512 MiB written between iterations",
                       "peaks": peaks, "kernels": res}))
 
