@@ -32,9 +32,9 @@ if ROOT not in sys.path:
 from synth import CONFIGS, make_probe, make_text_emb, make_weights  # noqa: E402
 
 METRIC = "image-tokens*steps/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of gemm_tcgen05_kernel, averaged over its four uses in a
-# block (QKV 0.995 GB, out-proj 0.655 GB, fc1 1.346 GB, fc2 2.384 GB) - profiles/r1_ncu_full_gemm_attn.txt (config 3)
-GEMM_DRAM_TRAFFIC_PER_LAUNCH = {"cfg3": 1.345e9}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of gemm_tcgen05_v3_kernel, averaged over its four uses in a
+# block (QKV+RoPE 1.055 GB, out-proj 0.645 GB, fc1 1.395 GB, fc2 2.652 GB) - profiles/r1_ncu_full_gemm_v3.txt (config 3)
+GEMM_DRAM_TRAFFIC_PER_LAUNCH = {"cfg3": 1.437e9}
 WORKLOADS = {"cfg3": 3, "cfg4": 4, "cfg5": 5}
 
 
@@ -239,7 +239,12 @@ def main():
     ap.add_argument("--impl", default="spot", choices=["spot", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--gemm-impl", type=int, default=0, help="0 auto, 2 one-CTA tcgen05, 3 CTA-pair tcgen05 (A/B testing)")
+    ap.add_argument("--gemm-impl", type=int, default=0,
+                    help="0 auto (CTA pair + TMA-store epilogue, K4 fused), 2 one-CTA tcgen05, 3 CTA pair with per-thread "
+                         "epilogue, 4 as 0 with K4 as its own kernel (A/B testing)")
+    ap.add_argument("--cache-threshold", type=float, default=None,
+                    help="run the cached-step variant (spot_explore_cached, PAPER.md:155-157) with this threshold; the line "
+                         "adds the effective denoising steps; no e2e leg")
     args = ap.parse_args()
     shape = CONFIGS[WORKLOADS[args.workload]]
     if args.impl == "reference":
@@ -286,9 +291,16 @@ def main():
     seeds = torch.tensor([int(shape.seeds[i % B]) + (i // B) * B for i in range(lo, hi)], dtype=torch.int64, device="cuda")
     out = None
 
+    cached = args.cache_threshold is not None
+    if cached:
+        args.no_e2e = True
+
     def step():
         nonlocal out
-        out = spot.spot_explore(ctx, seeds, text, ts, probe, P, K, k_sel, out)
+        if cached:
+            out = spot.spot_explore_cached(ctx, seeds, text, ts, probe, P, K, k_sel, args.cache_threshold, None, out)
+        else:
+            out = spot.spot_explore(ctx, seeds, text, ts, probe, P, K, k_sel, out)
         if dist is not None:
             sharding.gather_rewards(out["rewards"], world * B)      # the path's only exchange: world*B fp32 rewards
 
@@ -322,17 +334,18 @@ def main():
     ms_step = ms_total / args.steps
     units_per_step = world * B * shape.n_img * T                     # image tokens x Euler steps, all ranks
     value = units_per_step / (ms_step / 1e3)
-    flops_step = shape.flops_per_rollout()
+    eff_frac = float(out["computed"].sum().item()) / (B * T) if cached else 1.0     # share of (sequence, step) pairs computed
+    flops_step = shape.flops_per_rollout() * eff_frac
     tflops = flops_step / (ms_step / 1e3) / 1e12                     # per GPU
 
     # roofline of the dominant kernel (tcgen05 GEMM): algorithmic GEMM FLOPs / event-timed GEMM device time
     S, D, F, L = shape.seq, shape.hidden, shape.mlp_hidden, shape.n_blocks
     lin_per_seq_block = 2 * D * (3 * D + D + 2 * F)                   # per token
-    gemm_flops_step = T * B * (L * S * lin_per_seq_block - shape.n_txt * 2 * D * (D + 2 * F))   # last block: no text tail
+    gemm_flops_step = eff_frac * T * B * (L * S * lin_per_seq_block - shape.n_txt * 2 * D * (D + 2 * F))   # last block: no text tail
     timed_frac = counters["gemm_timed"] / max(1, counters["gemm_launches"])
     gemm_ms = counters["gemm_ms"]
     gemm_tflops = (gemm_flops_step * args.steps * timed_frac) / (gemm_ms / 1e3) / 1e12 if gemm_ms > 0 else None
-    roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_kernel", "achieved": gemm_tflops,
+    roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_v3_kernel", "achieved": gemm_tflops,
                 "peak": peaks["bf16_tflops_sustained"], "peak_kind": f"{peaks['source']} sustained bf16 (kernel timed inside a long step)",
                 "unit": "TFLOP/s", "frac": (gemm_tflops / peaks["bf16_tflops_sustained"]) if gemm_tflops else None,
                 "traffic": GEMM_DRAM_TRAFFIC_PER_LAUNCH.get(args.workload), "launches_timed": counters["gemm_timed"],
@@ -392,6 +405,11 @@ def main():
                                       "nominal_2250": tflops / 2250.0, "peaks": peaks["source"]},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": counters["launches"], "roofline": roofline,
                 "cpu_baseline": cpu_baseline, "weight_gen_s": gen_s}
+        if cached:
+            eff = out["computed"].sum(1).tolist()
+            line["cache"] = {"threshold": args.cache_threshold, "scheduled_steps": T, "effective_steps_mean": sum(eff) / len(eff),
+                             "effective_steps_per_sequence": eff, "note": "value counts SCHEDULED steps (PAPER.md:157: cached "
+                             "steps reuse the previous transformer residual); tflops_per_gpu counts computed steps only"}
         print(json.dumps(line))
     if dist is not None:
         dist.barrier()

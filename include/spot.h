@@ -177,6 +177,37 @@ spot_status spot_explore_host(spot_ctx *ctx, int n_prompts, int seeds_per_prompt
                               int32_t *h_top, int32_t *h_bottom,
                               void *d_workspace, size_t ws_bytes, void *cuda_stream);
 
+/* ---- Cached-step exploration: the paper's "effective denoising steps" axis s -------------------------------
+ * PAPER.md:155 "We therefore control effective denoising steps via a caching strategy rather than truncation";
+ * PAPER.md:157 "caches and reuses intermediate transformer outputs across adjacent denoising steps when their
+ * residual difference falls below a threshold.  Each Teacache threshold corresponds to an average number of
+ * effective denoising steps s".  DESIGN.md section 10 (readings T1-T5) states the rule: per sequence and Euler step i,
+ *   m_i = LN(img_in(x_i)) (1 + scale1) + shift1 (block 0, image stream);  steps 0 and T-1 always compute (acc <- 0);
+ *   otherwise rel = mean|m_i - m_{i-1}| / mean|m_{i-1}|, acc += poly(rel); acc < threshold: SKIP the L blocks and
+ *   use h_img^0 + R (R = h_img^L - h_img^0 of the last computed step); else compute and acc <- 0.
+ * poly(r) = sum_j coeffs[j] r^j; n_coeffs == 0 selects the identity poly(r) = r.  Sequences decide independently
+ * (a request is one prompt x one seed), the computing ones are compacted into a dense batch for the block kernels.
+ * These calls copy the list of computing sequences to the host and synchronise the stream ONCE PER EULER STEP.
+ * h_computed (HOST, [P*K, n_steps] bytes, may be NULL) receives 1 where the blocks ran; its row sums are the
+ * effective steps per sequence.  h_rel (HOST, [P*K, n_steps] fp32, may be NULL) receives rel (0 at step 0).
+ * Requires P*K <= 1024, threshold >= 0, n_coeffs <= 8; workspace from spot_workspace_bytes_cached. */
+typedef struct {
+  float threshold;
+  int32_t n_coeffs;
+  float coeffs[8];   /* ascending powers */
+} spot_cache_config;
+spot_status spot_workspace_bytes_cached(const spot_ctx *ctx, int n_seqs, int n_steps, size_t *bytes);
+spot_status spot_dit_denoise_cached(spot_ctx *ctx, int n_prompts, int seeds_per_prompt, float *d_latents,
+                                    const void *d_text_emb, const float *h_timesteps, int n_steps,
+                                    const spot_cache_config *cache, uint8_t *h_computed, float *h_rel,
+                                    void *d_workspace, size_t ws_bytes, void *cuda_stream);
+/* spot_explore with cached steps (noise -> cached denoise -> rewards -> selection). */
+spot_status spot_explore_cached(spot_ctx *ctx, int n_prompts, int seeds_per_prompt, const uint64_t *d_seeds,
+                                const void *d_text_emb, const float *h_timesteps, int n_steps, const float *d_probe,
+                                int k_select, const spot_cache_config *cache, float *d_latents, float *d_rewards,
+                                float *d_stats, int32_t *d_top, int32_t *d_bottom, uint8_t *h_computed, float *h_rel,
+                                void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -86,6 +86,10 @@ def load_library() -> C.CDLL:
         "spot_dit_denoise": [vp, i32, i32, vp, vp, vp, i32, vp, sz, vp],
         "spot_seed_rewards": [vp, i32, i32, vp, vp, i32, vp, vp, vp, vp, vp],
         "spot_explore": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
+        "spot_workspace_bytes_cached": [vp, i32, i32, C.POINTER(sz)],
+        "spot_dit_denoise_cached": [vp, i32, i32, vp, vp, vp, i32, C.POINTER(SpotCacheConfig), vp, vp, vp, sz, vp],
+        "spot_explore_cached": [vp, i32, i32, vp, vp, vp, i32, vp, i32, C.POINTER(SpotCacheConfig), vp, vp, vp, vp, vp, vp, vp,
+                                vp, sz, vp],
         "spot_explore_host": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_linear": [i32, i32, i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp],
         "spot_qkv_rope_linear": [vp, i32, i32, i64, vp, i64, vp, vp, vp, vp, vp, i32, f32, vp, vp],
@@ -132,6 +136,19 @@ def _check(status: int, where: str, ctx: Optional["Context"] = None) -> None:
         raise SpotError(status, where, ce)
 
 
+class SpotCacheConfig(C.Structure):
+    _fields_ = [("threshold", C.c_float), ("n_coeffs", C.c_int32), ("coeffs", C.c_float * 8)]
+
+
+def _cache_cfg(threshold: float, coeffs: Optional[Sequence[float]]) -> SpotCacheConfig:
+    cc = SpotCacheConfig(threshold=float(threshold), n_coeffs=0)
+    if coeffs is not None:
+        cc.n_coeffs = len(coeffs)
+        for j, v in enumerate(list(coeffs)[:8]):      # the library rejects n_coeffs > 8
+            cc.coeffs[j] = float(v)
+    return cc
+
+
 class Context:
     """spot_ctx: validated config + borrowed weights (keeps the torch tensors alive)."""
 
@@ -173,8 +190,8 @@ class Context:
         except Exception:
             pass
 
-    def workspace(self, n_seqs: int, n_steps: int) -> torch.Tensor:
-        n = spot_workspace_bytes(self, n_seqs, n_steps)
+    def workspace(self, n_seqs: int, n_steps: int, cached: bool = False) -> torch.Tensor:
+        n = spot_workspace_bytes(self, n_seqs, n_steps, cached)
         if self._ws is None or self._ws.numel() < n:
             self._ws = None
             self._ws = torch.empty(n, dtype=torch.uint8, device="cuda")
@@ -196,9 +213,10 @@ def spot_get_counters(ctx: Context, reset: bool = False) -> dict:
     return {"launches": int(a.value), "gemm_launches": int(b.value), "gemm_timed": int(c.value), "gemm_ms": float(d.value)}
 
 
-def spot_workspace_bytes(ctx: Context, n_seqs: int, n_steps: int) -> int:
+def spot_workspace_bytes(ctx: Context, n_seqs: int, n_steps: int, cached: bool = False) -> int:
     out = C.c_size_t()
-    _check(load_library().spot_workspace_bytes(ctx.handle, n_seqs, n_steps, C.byref(out)), "spot_workspace_bytes", ctx)
+    fn = load_library().spot_workspace_bytes_cached if cached else load_library().spot_workspace_bytes
+    _check(fn(ctx.handle, n_seqs, n_steps, C.byref(out)), "spot_workspace_bytes", ctx)
     return int(out.value)
 
 
@@ -281,6 +299,49 @@ def spot_explore(ctx: Context, seeds: torch.Tensor, text_emb: torch.Tensor, time
                                        _ptr(out["rewards"]), _ptr(out["stats"]), _ptr(out["top"]), _ptr(out["bottom"]),
                                        _ptr(ws), ws.numel(), _stream()), "spot_explore", ctx)
     return out
+
+
+def spot_explore_cached(ctx: Context, seeds: torch.Tensor, text_emb: torch.Tensor, timesteps: Sequence[float],
+                        probe: torch.Tensor, n_prompts: int, seeds_per_prompt: int, k_select: int, threshold: float,
+                        coeffs: Optional[Sequence[float]] = None, out: Optional[dict] = None) -> dict:
+    """Cached-step exploration.  Adds out["computed"] [B, T] uint8 (host) and out["rel"] [B, T] fp32
+    (host); out["computed"].sum(1) = effective denoising steps per sequence.  Synchronises once per Euler step."""
+    dev = seeds.device
+    B = n_prompts * seeds_per_prompt
+    s = ctx.shape
+    if out is None:
+        out = {"latents": torch.empty((B, s.n_img, s.latent_ch), dtype=torch.float32, device=dev),
+               "rewards": torch.empty(B, dtype=torch.float32, device=dev),
+               "stats": torch.empty((n_prompts, 2), dtype=torch.float32, device=dev),
+               "top": torch.empty((n_prompts, max(k_select, 1)), dtype=torch.int32, device=dev),
+               "bottom": torch.empty((n_prompts, max(k_select, 1)), dtype=torch.int32, device=dev)}
+    arr, T = _timesteps(timesteps)
+    out["computed"] = torch.zeros((B, T), dtype=torch.uint8)
+    out["rel"] = torch.zeros((B, T), dtype=torch.float32)
+    ws = ctx.workspace(B, T, cached=True)
+    cc = _cache_cfg(threshold, coeffs)
+    _check(load_library().spot_explore_cached(ctx.handle, n_prompts, seeds_per_prompt, _ptr(seeds), _ptr(text_emb),
+                                              C.cast(arr, C.c_void_p), T, _ptr(probe), k_select, C.byref(cc),
+                                              _ptr(out["latents"]), _ptr(out["rewards"]), _ptr(out["stats"]), _ptr(out["top"]),
+                                              _ptr(out["bottom"]), _ptr(out["computed"]), _ptr(out["rel"]), _ptr(ws), ws.numel(),
+                                              _stream()), "spot_explore_cached", ctx)
+    return out
+
+
+def spot_dit_denoise_cached(ctx: Context, latents: torch.Tensor, text_emb: torch.Tensor, timesteps: Sequence[float],
+                            n_prompts: int, seeds_per_prompt: int, threshold: float,
+                            coeffs: Optional[Sequence[float]] = None):
+    """In place on latents; returns (latents, computed [B, T] uint8 host, rel [B, T] fp32 host)."""
+    B = n_prompts * seeds_per_prompt
+    arr, T = _timesteps(timesteps)
+    computed = torch.zeros((B, T), dtype=torch.uint8)
+    rel = torch.zeros((B, T), dtype=torch.float32)
+    ws = ctx.workspace(B, T, cached=True)
+    cc = _cache_cfg(threshold, coeffs)
+    _check(load_library().spot_dit_denoise_cached(ctx.handle, n_prompts, seeds_per_prompt, _ptr(latents), _ptr(text_emb),
+                                                  C.cast(arr, C.c_void_p), T, C.byref(cc), _ptr(computed), _ptr(rel), _ptr(ws),
+                                                  ws.numel(), _stream()), "spot_dit_denoise_cached", ctx)
+    return latents, computed, rel
 
 
 def spot_explore_host(ctx: Context, h_seeds: torch.Tensor, h_text_emb: torch.Tensor, timesteps: Sequence[float],

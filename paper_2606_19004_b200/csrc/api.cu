@@ -59,9 +59,11 @@ struct Workspace {
   // all offsets in bytes from the workspace base
   size_t t_dev, emb, hid, temb, cvec, mod, fmod, txt_norm, txt_h0, h_img, h_txt, ybuf, big, vel, stage, total;
   size_t st_seeds, st_text, st_probe, st_lat, st_rew, st_stats, st_top, st_bot;
+  // cached-step variant only (carve(..., cached = true)): uncompacted h_img^0, previous modulated input, cached residual
+  size_t tc_h0, tc_mprev, tc_resid, tc_rowpart, tc_acc, tc_coeffs, tc_idx, tc_pos, tc_nact, tc_comp, tc_rel;
 };
 
-Workspace carve(const spot_ctx* c, int B, int T) {
+Workspace carve(const spot_ctx* c, int B, int T, bool cached = false) {
   const spot_config& g = c->cfg;
   const size_t D = g.hidden, S = c->seq(), NI = c->n_img(), NT = g.n_txt, L = g.n_blocks, es = esize(g.dtype);
   const size_t E = NI * g.latent_ch;
@@ -93,6 +95,21 @@ Workspace carve(const spot_ctx* c, int B, int T) {
   w.st_stats = take((size_t)B * 2 * 4);
   w.st_top = take((size_t)B * 4);
   w.st_bot = take((size_t)B * 4);
+  w.tc_h0 = w.tc_mprev = w.tc_resid = w.tc_rowpart = w.tc_acc = w.tc_coeffs = w.tc_idx = w.tc_pos = w.tc_nact = w.tc_comp =
+      w.tc_rel = 0;
+  if (cached) {
+    w.tc_h0 = take((size_t)B * NI * D * 4);
+    w.tc_mprev = take((size_t)B * NI * D * 4);
+    w.tc_resid = take((size_t)B * NI * D * 4);
+    w.tc_rowpart = take((size_t)B * NI * 8);
+    w.tc_acc = take((size_t)B * 8);
+    w.tc_coeffs = take(8 * 8);
+    w.tc_idx = take((size_t)B * 4 + 4);      // active_idx[B] followed by n_active (copied to the host together)
+    w.tc_nact = w.tc_idx + (size_t)B * 4;
+    w.tc_pos = take((size_t)B * 4);
+    w.tc_comp = take((size_t)B * 4);
+    w.tc_rel = take((size_t)B * 4);
+  }
   w.total = o;
   return w;
 }
@@ -491,10 +508,95 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
   return SPOT_OK;
 }
 
-spot_status check_ws(const spot_ctx* c, int B, int T, const void* ws, size_t bytes) {
+// Cached-step exploration: as denoise_core, but every step first measures
+// rel-L1 of the block-0 modulated image input per sequence, decides per sequence whether to run the L blocks, runs
+// them on the compacted batch of computing sequences and reuses the cached residual for the others.  One small
+// device->host copy (the list of computing sequences) and one stream synchronisation per Euler step.
+spot_status denoise_cached_core(spot_ctx* c, int P, int K, float* lat, const void* text_emb, const float* h_t, int T,
+                                const spot_cache_config* cc, uint8_t* h_computed, float* h_rel, uint8_t* ws,
+                                const float* probe, float* partials, cudaStream_t st) {
+  const spot_config& g = c->cfg;
+  const spot_dtype dt = g.dtype;
+  const int B = P * K, D = g.hidden, L = g.n_blocks, NI = c->n_img(), NT = g.n_txt, C = g.latent_ch;
+  const long long E = (long long)NI * C, per_img = (long long)NI * D, per_txt = (long long)NT * D;
+  const Workspace w = carve(c, B, T, true);
+  if (T == 0) {
+    if (probe) LK(c, launch_reward_partials(lat, probe, B, E, partials, st));
+    return SPOT_OK;
+  }
+  double coeffs[8] = {0.0, 1.0, 0, 0, 0, 0, 0, 0};
+  int n_coeffs = 2;
+  if (cc->n_coeffs > 0) {
+    n_coeffs = cc->n_coeffs;
+    for (int j = 0; j < n_coeffs; ++j) coeffs[j] = (double)cc->coeffs[j];
+  }
+  CK(c, cudaMemcpyAsync(ws + w.tc_coeffs, coeffs, sizeof(coeffs), cudaMemcpyHostToDevice, st));
+  CK(c, cudaMemsetAsync(ws + w.tc_acc, 0, (size_t)B * 8, st));
+  CK(c, cudaMemcpyAsync(ws + w.t_dev, h_t, (size_t)(T + 1) * 4, cudaMemcpyHostToDevice, st));
+  spot_status rs = conditioning(c, w, ws, T, st);
+  if (rs != SPOT_OK) return rs;
+  float* txt_h0 = (float*)(ws + w.txt_h0); float* hc = (float*)(ws + w.h_img); float* h_txt = (float*)(ws + w.h_txt);
+  float* h0 = (float*)(ws + w.tc_h0); float* m_prev = (float*)(ws + w.tc_mprev); float* resid = (float*)(ws + w.tc_resid);
+  float* row_part = (float*)(ws + w.tc_rowpart); double* acc = (double*)(ws + w.tc_acc);
+  int* d_idx = (int*)(ws + w.tc_idx); int* d_pos = (int*)(ws + w.tc_pos); int* d_nact = (int*)(ws + w.tc_nact);
+  int* d_comp = (int*)(ws + w.tc_comp); float* d_rel = (float*)(ws + w.tc_rel);
+  void* ybuf = ws + w.ybuf; void* big = ws + w.big; float* vel = (float*)(ws + w.vel);
+  const float* mod = (const float*)(ws + w.mod); const float* fmod = (const float*)(ws + w.fmod);
+  std::vector<int> h_idx((size_t)B + 1), h_comp((size_t)B);
+  std::vector<float> h_relv((size_t)B);
+  GemmProblem pr;
+  if (NT > 0) {
+    LK(c, launch_rmsnorm_rows(dt, text_emb, c->w.txt_gain, P * NT, g.txt_dim, g.rms_eps, ws + w.txt_norm, st));
+    memset(&pr, 0, sizeof(pr));
+    pr.A = ws + w.txt_norm; pr.a_map = plain_rows(P * NT, g.txt_dim); pr.W = c->w.txt_in_w; pr.bias = c->w.txt_in_b;
+    pr.M = P * NT; pr.N = D; pr.K = g.txt_dim; pr.out = txt_h0; pr.out_map = plain_rows(P * NT, D);
+    LK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
+  }
+  for (int i = 0; i < T; ++i) {
+    // h0 = img_in(x) for every sequence; metric on m = LN(h0)(1 + scale1) + shift1 of block 0's image stream
+    memset(&pr, 0, sizeof(pr));
+    pr.A = lat; pr.a_map = plain_rows(B * NI, C); pr.W = c->w.img_in_w; pr.bias = c->w.img_in_b;
+    pr.M = B * NI; pr.N = D; pr.K = C; pr.out = h0; pr.out_map = plain_rows(B * NI, D);
+    LK(c, launch_gemm_simt(SPOT_F32, dt, SPOT_F32, EPI_BIAS, pr, st));
+    const float* m0 = mod + (long long)i * L * 2 * 6 * D;          // block 0, image stream: (shift1, scale1, ...)
+    const bool first = i == 0, force = i == 0 || i == T - 1;
+    if (L > 0) LK(c, launch_tc_metric(h0, m_prev, m0, m0 + D, (long long)B * NI, D, g.ln_eps, first, row_part, st));
+    LK(c, launch_tc_decide(row_part, B, NI, first || L == 0, force, (double)cc->threshold, n_coeffs,
+                           (const double*)(ws + w.tc_coeffs), acc, d_idx, d_pos, d_nact, d_comp, d_rel, st));
+    CK(c, cudaMemcpyAsync(h_idx.data(), d_idx, ((size_t)B + 1) * 4, cudaMemcpyDeviceToHost, st));
+    if (h_computed) CK(c, cudaMemcpyAsync(h_comp.data(), d_comp, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+    if (h_rel) CK(c, cudaMemcpyAsync(h_relv.data(), d_rel, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+    CK(c, cudaStreamSynchronize(st));
+    const int n_act = h_idx[(size_t)B];
+    if (h_computed) for (int b = 0; b < B; ++b) h_computed[(size_t)b * T + i] = (uint8_t)h_comp[(size_t)b];
+    if (h_rel) for (int b = 0; b < B; ++b) h_rel[(size_t)b * T + i] = h_relv[(size_t)b];
+    if (n_act < 0 || n_act > B) return SPOT_ERR_CUDA;
+    if (n_act > 0) {
+      LK(c, launch_tc_gather(h0, hc, d_idx, 1, n_act, per_img, st));
+      if (NT > 0) LK(c, launch_tc_gather(txt_h0, h_txt, d_idx, K, n_act, per_txt, st));
+      for (int b = 0; b < L; ++b) {
+        const float* m = mod + ((long long)i * L + b) * 2 * 6 * D;
+        rs = block_core(c, b, n_act, hc, h_txt, m, m + 6 * D, ybuf, big, b == L - 1, st);
+        if (rs != SPOT_OK) return rs;
+      }
+    }
+    LK(c, launch_tc_combine(h0, resid, hc, d_pos, B, per_img, st));
+    const float* fm = fmod + (long long)i * 2 * D;
+    LK(c, launch_ln_modulate(dt, h0, B * NI, D, fm + D, fm, g.ln_eps, ybuf, plain_rows(B * NI, D), st));
+    memset(&pr, 0, sizeof(pr));
+    pr.A = ybuf; pr.a_map = plain_rows(B * NI, D); pr.W = c->w.proj_w; pr.bias = c->w.proj_b;
+    pr.M = B * NI; pr.N = C; pr.K = D; pr.out = vel; pr.out_map = plain_rows(B * NI, C);
+    LK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
+    const bool last = i == T - 1;
+    LK(c, launch_euler_update(lat, vel, h_t[i + 1] - h_t[i], B, E, last ? probe : nullptr, partials, st));
+  }
+  return SPOT_OK;
+}
+
+spot_status check_ws(const spot_ctx* c, int B, int T, const void* ws, size_t bytes, bool cached = false) {
   if (!ws) return SPOT_ERR_NULL;
   if (!aligned16(ws)) return SPOT_ERR_ALIGN;
-  if (bytes < carve(c, B, T).total) return SPOT_ERR_WORKSPACE;
+  if (bytes < carve(c, B, T, cached).total) return SPOT_ERR_WORKSPACE;
   return SPOT_OK;
 }
 
@@ -621,6 +723,60 @@ spot_status spot_explore(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, con
   LK(ctx, launch_noise(d_seeds, B, E, 0u, d_latents, nullptr, st));
   s = denoise_core(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps,
                    (uint8_t*)d_workspace, d_probe, ctx->d_partials, st);
+  if (s != SPOT_OK) return s;
+  LK(ctx, launch_reward_finalize(ctx->d_partials, B, E, d_rewards, st));
+  LK(ctx, launch_seed_select(d_rewards, n_prompts, seeds_per_prompt, k_select, d_stats, d_top, d_bottom, st));
+  return SPOT_OK;
+}
+
+static spot_status check_cache_cfg(const spot_cache_config* cc, int B) {
+  if (!cc) return SPOT_ERR_NULL;
+  if (cc->n_coeffs < 0 || cc->n_coeffs > 8 || !(cc->threshold >= 0.f) || B > 1024) return SPOT_ERR_SHAPE;
+  return SPOT_OK;
+}
+
+spot_status spot_workspace_bytes_cached(const spot_ctx* ctx, int n_seqs, int n_steps, size_t* bytes) {
+  if (!ctx || !bytes) return SPOT_ERR_NULL;
+  if (n_seqs <= 0 || n_seqs > ctx->max_seqs || n_steps < 0) return SPOT_ERR_SHAPE;
+  *bytes = carve(ctx, n_seqs, n_steps, true).total;
+  return SPOT_OK;
+}
+
+spot_status spot_dit_denoise_cached(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, float* d_latents,
+                                    const void* d_text_emb, const float* h_timesteps, int n_steps,
+                                    const spot_cache_config* cache, uint8_t* h_computed, float* h_rel, void* d_workspace,
+                                    size_t ws_bytes, void* cuda_stream) {
+  spot_status s = check_rollout_args(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps);
+  if (s != SPOT_OK) return s;
+  s = check_cache_cfg(cache, n_prompts * seeds_per_prompt);
+  if (s != SPOT_OK) return s;
+  s = check_ws(ctx, n_prompts * seeds_per_prompt, n_steps, d_workspace, ws_bytes, true);
+  if (s != SPOT_OK) return s;
+  return denoise_cached_core(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps, cache,
+                             h_computed, h_rel, (uint8_t*)d_workspace, nullptr, nullptr, (cudaStream_t)cuda_stream);
+}
+
+spot_status spot_explore_cached(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, const uint64_t* d_seeds,
+                                const void* d_text_emb, const float* h_timesteps, int n_steps, const float* d_probe,
+                                int k_select, const spot_cache_config* cache, float* d_latents, float* d_rewards,
+                                float* d_stats, int32_t* d_top, int32_t* d_bottom, uint8_t* h_computed, float* h_rel,
+                                void* d_workspace, size_t ws_bytes, void* cuda_stream) {
+  spot_status s = check_rollout_args(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps);
+  if (s != SPOT_OK) return s;
+  if (!d_seeds || !d_probe) return SPOT_ERR_NULL;
+  s = check_select_args(ctx, n_prompts, seeds_per_prompt, k_select, d_rewards, d_stats, d_top, d_bottom);
+  if (s != SPOT_OK) return s;
+  if (!aligned16(d_probe)) return SPOT_ERR_ALIGN;
+  const int B = n_prompts * seeds_per_prompt;
+  s = check_cache_cfg(cache, B);
+  if (s != SPOT_OK) return s;
+  s = check_ws(ctx, B, n_steps, d_workspace, ws_bytes, true);
+  if (s != SPOT_OK) return s;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const long long E = (long long)ctx->n_img() * ctx->cfg.latent_ch;
+  LK(ctx, launch_noise(d_seeds, B, E, 0u, d_latents, nullptr, st));
+  s = denoise_cached_core(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps, cache, h_computed,
+                          h_rel, (uint8_t*)d_workspace, d_probe, ctx->d_partials, st);
   if (s != SPOT_OK) return s;
   LK(ctx, launch_reward_finalize(ctx->d_partials, B, E, d_rewards, st));
   LK(ctx, launch_seed_select(d_rewards, n_prompts, seeds_per_prompt, k_select, d_stats, d_top, d_bottom, st));

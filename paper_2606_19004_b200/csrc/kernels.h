@@ -33,6 +33,17 @@ cudaError_t launch_reward_finalize(const float* partials, int B, long long E, fl
 cudaError_t launch_seed_select(const float* rewards, int P, int K, int k_select, float* stats, int32_t* top,
                                int32_t* bottom, cudaStream_t st);
 
+// cached-step exploration (teacache.cu)
+cudaError_t launch_tc_metric(const float* h0, float* m_prev, const float* shift, const float* scale, long long rows, int D,
+                             float eps, bool first, float* row_part, cudaStream_t st);
+cudaError_t launch_tc_decide(const float* row_part, int B, int rows_per_seq, bool first, bool force, double threshold,
+                             int n_coeffs, const double* d_coeffs, double* acc, int* active_idx, int* pos, int* n_active,
+                             int* computed, float* rel, cudaStream_t st);
+cudaError_t launch_tc_gather(const float* src, float* dst, const int* idx, int div, int n, long long n_per_seq,
+                             cudaStream_t st);
+cudaError_t launch_tc_combine(float* h0, float* resid, const float* hc, const int* pos, int B, long long n_per_seq,
+                              cudaStream_t st);
+
 // plumbing
 cudaError_t launch_to_f32(spot_dtype dt, const void* in, float* out, long long n, cudaStream_t st);
 cudaError_t launch_from_f32(spot_dtype dt, const float* in, void* out, long long n, cudaStream_t st);
