@@ -309,6 +309,9 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    full_rewards = None
+    if cached:                                   # the full rollout's rewards, for the rank correlation of PAPER.md:340
+        full_rewards = spot.spot_explore(ctx, seeds, text, ts, probe, P, K, k_sel)["rewards"].clone()
     for _ in range(args.warmup):
         step()
     sync_all()
@@ -407,8 +410,12 @@ def main():
                 "cpu_baseline": cpu_baseline, "weight_gen_s": gen_s}
         if cached:
             eff = out["computed"].sum(1).tolist()
+            rk = lambda v: torch.argsort(torch.argsort(v)).double()
+            corr = [float(torch.corrcoef(torch.stack([rk(out["rewards"][g * K:(g + 1) * K]), rk(full_rewards[g * K:(g + 1) * K])]))[0, 1])
+                    for g in range(P)]
             line["cache"] = {"threshold": args.cache_threshold, "scheduled_steps": T, "effective_steps_mean": sum(eff) / len(eff),
-                             "effective_steps_per_sequence": eff, "note": "value counts SCHEDULED steps (PAPER.md:157: cached "
+                             "effective_steps_per_sequence": eff, "reward_rank_correlation_vs_full_rollout_per_prompt": corr,
+                             "note": "value counts SCHEDULED steps (PAPER.md:157: cached "
                              "steps reuse the previous transformer residual); tflops_per_gpu counts computed steps only"}
         print(json.dumps(line))
     if dist is not None:
