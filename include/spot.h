@@ -208,6 +208,21 @@ spot_status spot_explore_cached(spot_ctx *ctx, int n_prompts, int seeds_per_prom
                                 float *d_stats, int32_t *d_top, int32_t *d_bottom, uint8_t *h_computed, float *h_rel,
                                 void *d_workspace, size_t ws_bytes, void *cuda_stream);
 
+/* ---- Stochastic sampler: the full-quality rollout that follows exploration ---------------------------------
+ * PAPER.md:145 step 5 (the selected seeds are rolled out with DiT(n+1) for training), :227 "The algorithm backbone is
+ * FlowGRPO", Table 2 (:477-482) "SDE window".  DESIGN.md section 11 (readings D1-D4): steps window_lo <= i < window_hi
+ * of the grid take the marginal-preserving reverse-SDE step of the rectified flow
+ *     mean = x (1 + sigma^2/(2 t_i) dt) + v (1 + sigma^2 (1 - t_i)/(2 t_i)) dt,   x_next = mean + sigma sqrt(-dt) xi,
+ *     sigma = noise_level * sqrt(t/(1-t))  (t = t_i, or t_{i+1} when t_i == 1),  dt = t_{i+1} - t_i < 0,
+ * with xi ~ N(0, I) from Philox stream 256 + i of the sequence's seed (same generator as (1)); all other steps are the
+ * Euler steps of (3).  d_logp [P*K, n_steps] fp32 receives log N(x_next; mean, sigma^2 (-dt) I) averaged over the
+ * elements of the latent (0 for deterministic steps) - the per-step log-probability GRPO consumes.
+ * Requires 1 >= t_0 > t_1 > ... > t_T >= 0, noise_level >= 0, 0 <= window_lo <= window_hi.  Workspace as (3). */
+spot_status spot_dit_denoise_sde(spot_ctx *ctx, int n_prompts, int seeds_per_prompt, const uint64_t *d_seeds,
+                                 float *d_latents, const void *d_text_emb, const float *h_timesteps, int n_steps,
+                                 float noise_level, int window_lo, int window_hi, float *d_logp,
+                                 void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -67,6 +67,13 @@ spot_status spot_attention(spot_dtype dtype, spot_impl impl, const void *d_qkv, 
 spot_status spot_euler_update(float *d_x, const float *d_v, float dt, int n_seqs, int64_t elems, const float *d_probe,
                               float *d_rewards, float *d_partials, void *cuda_stream);
 
+/* One stochastic sampler step on [n_seqs, elems] fp32 (spot.h spot_dit_denoise_sde): x <- mean +
+ * sigma sqrt(-dt) xi with xi from Philox stream 256 + step of d_seeds[b]; d_logp[b] = the step's log-probability.
+ * noise_level == 0 degenerates to the Euler update (d_logp = 0).  d_partials: [n_seqs, ceil(elems / 4096)] fp32 scratch. */
+spot_status spot_sde_update(float *d_x, const float *d_v, const uint64_t *d_seeds, int step, float t_i, float t_next,
+                            float noise_level, int n_seqs, int64_t elems, float *d_logp, float *d_partials,
+                            void *cuda_stream);
+
 /* The RoPE table the context built at spot_create (S5): copies cos and sin [S, d_h/2] fp32 to HOST. */
 spot_status spot_rope_table(const spot_ctx *ctx, float *h_cos, float *h_sin);
 

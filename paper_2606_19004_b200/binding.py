@@ -90,6 +90,8 @@ def load_library() -> C.CDLL:
         "spot_dit_denoise_cached": [vp, i32, i32, vp, vp, vp, i32, C.POINTER(SpotCacheConfig), vp, vp, vp, sz, vp],
         "spot_explore_cached": [vp, i32, i32, vp, vp, vp, i32, vp, i32, C.POINTER(SpotCacheConfig), vp, vp, vp, vp, vp, vp, vp,
                                 vp, sz, vp],
+        "spot_dit_denoise_sde": [vp, i32, i32, vp, vp, vp, vp, i32, f32, i32, i32, vp, vp, sz, vp],
+        "spot_sde_update": [vp, vp, vp, i32, f32, f32, f32, i32, i64, vp, vp, vp],
         "spot_explore_host": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_linear": [i32, i32, i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp],
         "spot_qkv_rope_linear": [vp, i32, i32, i64, vp, i64, vp, vp, vp, vp, vp, i32, f32, vp, vp],
@@ -342,6 +344,32 @@ def spot_dit_denoise_cached(ctx: Context, latents: torch.Tensor, text_emb: torch
                                                   C.cast(arr, C.c_void_p), T, C.byref(cc), _ptr(computed), _ptr(rel), _ptr(ws),
                                                   ws.numel(), _stream()), "spot_dit_denoise_cached", ctx)
     return latents, computed, rel
+
+
+def spot_dit_denoise_sde(ctx: Context, seeds: torch.Tensor, latents: torch.Tensor, text_emb: torch.Tensor,
+                         timesteps: Sequence[float], n_prompts: int, seeds_per_prompt: int, noise_level: float,
+                         window: Sequence[int]):
+    """In place on latents; returns (latents, logp [B, T] fp32 device).  PAPER.md:227, Table 2 "SDE window"."""
+    B = n_prompts * seeds_per_prompt
+    arr, T = _timesteps(timesteps)
+    logp = torch.empty((B, T), dtype=torch.float32, device=latents.device)
+    ws = ctx.workspace(B, T)
+    _check(load_library().spot_dit_denoise_sde(ctx.handle, n_prompts, seeds_per_prompt, _ptr(seeds), _ptr(latents), _ptr(text_emb),
+                                               C.cast(arr, C.c_void_p), T, float(noise_level), int(window[0]), int(window[1]),
+                                               _ptr(logp), _ptr(ws), ws.numel(), _stream()), "spot_dit_denoise_sde", ctx)
+    return latents, logp
+
+
+def spot_sde_update(x: torch.Tensor, v: torch.Tensor, seeds: torch.Tensor, step: int, t_i: float, t_next: float,
+                    noise_level: float):
+    """One stochastic step in place on x [B, ...]; returns (x, logp [B])."""
+    B = x.shape[0]
+    E = x.numel() // B
+    logp = torch.empty(B, dtype=torch.float32, device=x.device)
+    partials = torch.empty((B, (E + 4095) // 4096), dtype=torch.float32, device=x.device)
+    _check(load_library().spot_sde_update(_ptr(x), _ptr(v), _ptr(seeds), step, t_i, t_next, noise_level, B, E, _ptr(logp),
+                                          _ptr(partials), _stream()), "spot_sde_update")
+    return x, logp
 
 
 def spot_explore_host(ctx: Context, h_seeds: torch.Tensor, h_text_emb: torch.Tensor, timesteps: Sequence[float],

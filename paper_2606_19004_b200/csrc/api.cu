@@ -22,6 +22,7 @@ struct spot_ctx {
   float* d_cos;                  // [S, d_h/2]
   float* d_sin;
   float* d_partials;             // [max_seqs, reward chunks]
+  float* d_partials2;            // [max_seqs, reward chunks]: sum xi^2 of the stochastic step
   unsigned long long n_launches; // kernels launched through this context
   int timing;                    // 1: bracket every tcgen05 GEMM launch with CUDA events
   std::vector<cudaEvent_t> ev;   // event pool (pairs)
@@ -267,7 +268,7 @@ spot_status spot_create(const spot_config* cfg, const spot_weights* w, int max_s
   c->n_launches = c->gemm_launches = 0;
   c->timing = 0;
   c->ev_used = 0;
-  c->d_cos = c->d_sin = c->d_partials = nullptr;
+  c->d_cos = c->d_sin = c->d_partials = c->d_partials2 = nullptr;
   int dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
@@ -278,10 +279,11 @@ spot_status spot_create(const spot_config* cfg, const spot_weights* w, int max_s
   cudaError_t e = cudaMalloc(&c->d_cos, cs.size() * 4);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_sin, sn.size() * 4);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_partials, n_part * 4);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_partials2, n_part * 4);
   if (e == cudaSuccess) e = cudaMemcpy(c->d_cos, cs.data(), cs.size() * 4, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(c->d_sin, sn.data(), sn.size() * 4, cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
-    cudaFree(c->d_cos); cudaFree(c->d_sin); cudaFree(c->d_partials);
+    cudaFree(c->d_cos); cudaFree(c->d_sin); cudaFree(c->d_partials); cudaFree(c->d_partials2);
     delete c;
     return SPOT_ERR_CUDA;
   }
@@ -294,6 +296,7 @@ spot_status spot_destroy(spot_ctx* ctx) {
   cudaFree(ctx->d_cos);
   cudaFree(ctx->d_sin);
   cudaFree(ctx->d_partials);
+  cudaFree(ctx->d_partials2);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   delete ctx;
   return SPOT_OK;
@@ -457,8 +460,30 @@ spot_status conditioning(spot_ctx* c, const Workspace& w, uint8_t* ws, int T, cu
   return SPOT_OK;
 }
 
+// Stochastic steps: steps lo <= i < hi of the grid use the SDE update with noise level a.
+struct SdeRun {
+  const uint64_t* seeds;   // device, [B]
+  float noise_level;
+  int lo, hi;
+  float* logp;             // device, [B, T] (zero for deterministic steps)
+};
+constexpr uint32_t kSdeStreamBase = 256;
+
+// cx, cv, cn of the step t_i -> t_next (readings D1-D2); returns false when sigma == 0 (a deterministic step)
+bool sde_coeffs(float t_i, float t_next, float noise_level, double* cx, double* cv, double* cn) {
+  const double t = (double)t_i, tn = (double)t_next, dt = tn - t;
+  const double ts = t < 1.0 ? t : tn;
+  const double sig = (double)noise_level * sqrt(ts / (1.0 - ts));
+  if (!(sig > 0.0) || !(dt < 0.0)) return false;
+  *cx = 1.0 + sig * sig / (2.0 * t) * dt;
+  *cv = (1.0 + sig * sig * (1.0 - t) / (2.0 * t)) * dt;
+  *cn = sig * sqrt(-dt);
+  return true;
+}
+
 spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text_emb, const float* h_t, int T,
-                         uint8_t* ws, const float* probe, float* partials, cudaStream_t st) {
+                         uint8_t* ws, const float* probe, float* partials, cudaStream_t st,
+                         const SdeRun* sde = nullptr) {
   const spot_config& g = c->cfg;
   const spot_dtype dt = g.dtype;
   const int B = P * K, D = g.hidden, L = g.n_blocks, NI = c->n_img(), NT = g.n_txt, C = g.latent_ch;
@@ -503,7 +528,12 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
     pr.M = B * NI; pr.N = C; pr.K = D; pr.out = vel; pr.out_map = plain_rows(B * NI, C);
     LK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
     const bool last = i == T - 1;
-    LK(c, launch_euler_update(lat, vel, h_t[i + 1] - h_t[i], B, E, last ? probe : nullptr, partials, st));
+    double cx, cv, cn;
+    if (sde && i >= sde->lo && i < sde->hi && sde_coeffs(h_t[i], h_t[i + 1], sde->noise_level, &cx, &cv, &cn))
+      LK(c, launch_sde_update(lat, vel, sde->seeds, kSdeStreamBase + (uint32_t)i, cx, cv, cn, B, E, last ? probe : nullptr,
+                              c->d_partials2, partials, sde->logp + i, T, st));
+    else
+      LK(c, launch_euler_update(lat, vel, h_t[i + 1] - h_t[i], B, E, last ? probe : nullptr, partials, st));
   }
   return SPOT_OK;
 }
@@ -783,6 +813,27 @@ spot_status spot_explore_cached(spot_ctx* ctx, int n_prompts, int seeds_per_prom
   return SPOT_OK;
 }
 
+spot_status spot_dit_denoise_sde(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, const uint64_t* d_seeds,
+                                 float* d_latents, const void* d_text_emb, const float* h_timesteps, int n_steps,
+                                 float noise_level, int window_lo, int window_hi, float* d_logp, void* d_workspace,
+                                 size_t ws_bytes, void* cuda_stream) {
+  spot_status s = check_rollout_args(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps);
+  if (s != SPOT_OK) return s;
+  if (!d_seeds || !d_logp) return SPOT_ERR_NULL;
+  if (!(noise_level >= 0.f) || window_lo < 0 || window_hi < window_lo) return SPOT_ERR_SHAPE;
+  for (int i = 0; i < n_steps; ++i)
+    if (!(h_timesteps[i] > 0.f && h_timesteps[i] <= 1.f && h_timesteps[i + 1] < h_timesteps[i] && h_timesteps[i + 1] >= 0.f))
+      return SPOT_ERR_SHAPE;                                 // the schedule sigma = a sqrt(t/(1-t)) needs 1 >= t_i > t_{i+1} >= 0
+  const int B = n_prompts * seeds_per_prompt;
+  s = check_ws(ctx, B, n_steps, d_workspace, ws_bytes);
+  if (s != SPOT_OK) return s;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (n_steps > 0) CK(ctx, cudaMemsetAsync(d_logp, 0, (size_t)B * n_steps * 4, st));
+  SdeRun run{d_seeds, noise_level, window_lo, window_hi, d_logp};
+  return denoise_core(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps, (uint8_t*)d_workspace,
+                      nullptr, nullptr, st, &run);
+}
+
 spot_status spot_explore_host(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, const uint64_t* h_seeds,
                               const void* h_text_emb, const float* h_timesteps, int n_steps, const float* h_probe,
                               int k_select, float* h_latents, float* h_rewards, float* h_stats, int32_t* h_top,
@@ -953,6 +1004,26 @@ spot_status spot_euler_update(float* d_x, const float* d_v, float dt, int n_seqs
   if (launch_euler_update(d_x, d_v, dt, n_seqs, elems, d_probe, d_partials, st) != cudaSuccess) return SPOT_ERR_CUDA;
   if (d_probe && launch_reward_finalize(d_partials, n_seqs, elems, d_rewards, st) != cudaSuccess) return SPOT_ERR_CUDA;
   return SPOT_OK;
+}
+
+spot_status spot_sde_update(float* d_x, const float* d_v, const uint64_t* d_seeds, int step, float t_i, float t_next,
+                            float noise_level, int n_seqs, int64_t elems, float* d_logp, float* d_partials,
+                            void* cuda_stream) {
+  if (n_seqs < 0 || elems <= 0 || (elems & 3) || step < 0) return SPOT_ERR_SHAPE;
+  if (n_seqs == 0) return SPOT_OK;
+  if (!d_x || !d_v || !d_seeds || !d_logp || !d_partials) return SPOT_ERR_NULL;
+  if (!aligned16(d_x) || !aligned16(d_v)) return SPOT_ERR_ALIGN;
+  if (!(t_i > 0.f && t_i <= 1.f && t_next < t_i && t_next >= 0.f) || !(noise_level >= 0.f)) return SPOT_ERR_SHAPE;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  double cx, cv, cn;
+  if (!sde_coeffs(t_i, t_next, noise_level, &cx, &cv, &cn)) {
+    if (cudaMemsetAsync(d_logp, 0, (size_t)n_seqs * 4, st) != cudaSuccess) return SPOT_ERR_CUDA;
+    return launch_euler_update(d_x, d_v, t_next - t_i, n_seqs, elems, nullptr, nullptr, st) == cudaSuccess ? SPOT_OK
+                                                                                                       : SPOT_ERR_CUDA;
+  }
+  return launch_sde_update(d_x, d_v, d_seeds, kSdeStreamBase + (uint32_t)step, cx, cv, cn, n_seqs, elems, nullptr, d_partials,
+                           nullptr, d_logp, 1, st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
 }
 
 }  // extern "C"

@@ -33,6 +33,13 @@ cudaError_t launch_reward_finalize(const float* partials, int B, long long E, fl
 cudaError_t launch_seed_select(const float* rewards, int P, int K, int k_select, float* stats, int32_t* top,
                                int32_t* bottom, cudaStream_t st);
 
+// stochastic sampler step (sde.cu; Table 2 "SDE window"): x <- cx x + cv v + cn xi, xi from Philox
+// stream `stream_id` of seeds[b]; logp[b * logp_stride] = log N(x_next; mean, cn^2) averaged over elements; when
+// probe != nullptr also the reward partials of the updated x (as launch_euler_update)
+cudaError_t launch_sde_update(float* x, const float* v, const uint64_t* seeds, uint32_t stream_id, double cx, double cv,
+                              double cn, int B, long long E, const float* probe, float* lp_partials, float* rw_partials,
+                              float* logp, long long logp_stride, cudaStream_t st);
+
 // cached-step exploration (teacache.cu)
 cudaError_t launch_tc_metric(const float* h0, float* m_prev, const float* shift, const float* scale, long long rows, int D,
                              float eps, bool first, float* row_part, cudaStream_t st);
