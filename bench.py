@@ -205,6 +205,7 @@ def run_kernels(args, shape):
     hbm("K4_qk_norm_rope", lambda: spot.spot_qk_norm_rope(qkv, shape.n_txt, gains, cs, sn, 1e-6), 2.0 * 2 * B * S * H * dh * 2)
     # K5 attention
     tensor("K5_attention", lambda: spot.spot_attention(qkv, spot.IMPL_TCGEN05), 4.0 * S * S * dh * H * B)
+    tensor("K5_attention_prev_two_pass", lambda: spot.spot_attention(qkv, spot.IMPL_TCGEN05_2CTA), 4.0 * S * S * dh * H * B)
     del qkv
     # K6 Euler update (+ reward): 2^26 elements so that the working set exceeds L2
     Bx, E = 1024, shape.n_img * shape.latent_ch if shape.n_img * shape.latent_ch <= 65536 else 65536

@@ -95,7 +95,7 @@ typedef enum {
   SPOT_OPT_GEMM_IMPL = 0,   /* 0 = auto (bf16: CTA-pair tcgen05 with TMA-store epilogue, QK-norm+RoPE fused into the QKV projection),
                              * 1 = SIMT FFMA GEMM, 2 = 1-CTA tcgen05, 3 = CTA-pair tcgen05 with per-thread epilogue,
                              * 4 = as 0 but K4 (QK-norm+RoPE) as its own kernel */
-  SPOT_OPT_ATTN_IMPL = 1,   /* 0 = auto (tcgen05 for bf16, d_h = 128), 1 = force the SIMT attention */
+  SPOT_OPT_ATTN_IMPL = 1,   /* 0 = auto (tcgen05 for bf16, d_h = 128: one-pass kernel, 64-key tiles), 1 = SIMT attention, 2 = previous two-pass tcgen05 kernel */
   SPOT_OPT_TIMING = 2       /* 1 = bracket every tcgen05 GEMM launch with CUDA events on the launch stream */
 } spot_option;
 

@@ -58,7 +58,8 @@ spot_status spot_qk_norm_rope(spot_dtype dtype, void *d_qkv, int B, int S, int H
 
 /* O = softmax(Q K^T / sqrt(d_h)) V over all S keys per (sequence, head), no mask (north_star (d); DESIGN.md
  * S4 step 6).  d_qkv [B, S, 3, H, d_h] -> d_out [B, S, H * d_h], both `dtype`.  SPOT_IMPL_TCGEN05 requires
- * bf16, d_h = 128. */
+ * bf16, d_h = 128 (one-pass kernel, 64-key tiles); for this call SPOT_IMPL_TCGEN05_2CTA selects the previous two-pass
+ * tcgen05 kernel (128-key tiles), kept for A/B timing. */
 spot_status spot_attention(spot_dtype dtype, spot_impl impl, const void *d_qkv, void *d_out, int B, int S, int H,
                            int head_dim, void *cuda_stream);
 

@@ -309,9 +309,13 @@ spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
     ctx->gemm_impl = value;
     return SPOT_OK;
   }
+  if (opt == SPOT_OPT_ATTN_IMPL) {
+    if (value < 0 || value > 2) return SPOT_ERR_SHAPE;
+    ctx->attn_impl = value;
+    return SPOT_OK;
+  }
   if (value != 0 && value != 1) return SPOT_ERR_SHAPE;
   if (opt == SPOT_OPT_GEMM_IMPL) ctx->gemm_impl = value;
-  else if (opt == SPOT_OPT_ATTN_IMPL) ctx->attn_impl = value;
   else if (opt == SPOT_OPT_TIMING) ctx->timing = value;
   else return SPOT_ERR_SHAPE;
   return SPOT_OK;
@@ -409,8 +413,10 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
     LK(c, launch_qk_norm_rope(dt, big, B, S, g.n_heads, g.head_dim, g.n_txt, bw.s[0].q_gain, bw.s[0].k_gain,
                               bw.s[1].q_gain, bw.s[1].k_gain, c->d_cos, c->d_sin, g.rms_eps, st));
   // (6) joint attention -> ybuf [B,S,D]
-  if (dt == SPOT_BF16 && c->attn_impl == 0 && tcgen05_attn_supported(S, g.n_heads, g.head_dim))
-    LK(c, launch_attn_tcgen05(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st));
+  if (dt == SPOT_BF16 && c->attn_impl != 1 && tcgen05_attn_supported(S, g.n_heads, g.head_dim)) {
+    if (c->attn_impl == 2) LK(c, launch_attn_tcgen05(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st));
+    else LK(c, launch_attn_tcgen05_v3(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st));
+  }
   else
     LK(c, launch_attn_simt(dt, big, ybuf, B, S, g.n_heads, g.head_dim, st));
   const int ns = img_only_tail ? 1 : 2;
@@ -987,8 +993,10 @@ spot_status spot_attention(spot_dtype dtype, spot_impl impl, const void* d_qkv, 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const bool can_tc = dtype == SPOT_BF16 && tcgen05_attn_supported(S, H, head_dim);
   if (impl == SPOT_IMPL_TCGEN05 && !can_tc) return SPOT_ERR_SHAPE;
-  if (impl != SPOT_IMPL_SIMT && can_tc)
+  if (impl == SPOT_IMPL_TCGEN05_2CTA && can_tc)   // for attention this value selects the previous (two-pass, 128-key tile) kernel
     return launch_attn_tcgen05(d_qkv, d_out, B, S, H, head_dim, sm_count(), st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+  if (impl != SPOT_IMPL_SIMT && can_tc)
+    return launch_attn_tcgen05_v3(d_qkv, d_out, B, S, H, head_dim, sm_count(), st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
   return launch_attn_simt(dtype, d_qkv, d_out, B, S, H, head_dim, st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
 }
 

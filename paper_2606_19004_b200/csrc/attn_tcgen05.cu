@@ -99,7 +99,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict
 
   if (warp == 0) {
     // ===================== TMA producer =====================
-    if (lane == 0) {
+    // (elect.sync, not `lane == 0`: the compiler then issues UTMALDG / UTCHMMA straight from uniform registers instead
+    //  of wrapping each one in a per-lane ELECT / BRA.U.ANY loop - see "warp-uniform issue" in tcgen05.cuh)
+    if (ptx::elect_one()) {
       ptx::mbar_arrive_expect_tx(q_full, QT * TILE_BYTES);
 #pragma unroll
       for (int t = 0; t < QT; ++t) {
@@ -121,7 +123,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
+    if (ptx::elect_one()) {
       constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(BQ, BKV, 0, 0);   // A = Q (K-major smem), B = K (K-major smem)
       constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(BQ, DH, 0, 1);    // A = P (TMEM), B = V (MN-major smem)
       auto issue_qk = [&](int t, int j) {

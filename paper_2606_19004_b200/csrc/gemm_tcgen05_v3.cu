@@ -121,8 +121,8 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
   volatile uint32_t* tmem_slot_ptr =
       reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = ptx::cluster_ctarank();            // 0 = leader of the pair
+  const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;   // warp index uniform FOR THE COMPILER (tcgen05.cuh)
+  const uint32_t rank = __shfl_sync(0xffffffffu, ptx::cluster_ctarank(), 0);   // 0 = leader of the pair (uniform for the compiler)
   const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
 
   if (warp == 0 && lane == 0) {
@@ -138,11 +138,13 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
   ptx::tc_fence_before();
   ptx::cluster_sync();                                      // barriers of both CTAs initialised, TMEM allocated
   ptx::tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot_ptr;
+  const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot_ptr, 0);
 
   if (warp == 0) {
     // ===================== TMA producer (both CTAs) =====================
-    if (lane == 0) {
+    // elect.sync (not `lane == 0`): the compiler then knows the region is single-threaded and issues UTMALDG /
+    // UTCHMMA straight from uniform registers (see "warp-uniform issue" in tcgen05.cuh)
+    if (ptx::elect_one()) {
       int stage = 0; uint32_t phase = 0;
       for (int t = pair; t < P.total_tiles; t += n_pairs) {
         const TileCoord c = decode_tile(P, t);
@@ -158,18 +160,21 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
           const uint32_t sa = smem_base + stage * STAGE_BYTES;
           ptx::tma_load_3d_2cta(sa, mA, leader_full, kb * BLOCK_K, r0, seq);
           ptx::tma_load_2d_2cta(sa + A_BYTES, mW, leader_full, kb * BLOCK_K, n0);
-          // only the leader arms its barrier, for the bytes of BOTH CTAs (see gemm_tcgen05_2cta.cu)
+          // only the leader CTA arms its barrier, for the bytes of BOTH CTAs (see gemm_tcgen05_2cta.cu)
           if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer (leader CTA only) =====================
-    if (rank == 0 && lane == 0) {
+    // ===================== MMA issuer (leader CTA only, one elected thread) =====================
+    // (the non-leader CTA runs the same code over zero tiles: a branch on `rank` around the elected region makes the
+    //  compiler fall back to per-lane ELECT / BRA.U.ANY loops around every UTCHMMA)
+    if (ptx::elect_one()) {
+      const int my_tiles = rank == 0 ? P.total_tiles : 0;
       constexpr uint32_t idesc = ptx::make_idesc_bf16(PAIR_M, BLOCK_N, 0, 0);
       int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t acc_phase = 0;
-      for (int t = pair; t < P.total_tiles; t += n_pairs) {
+      for (int t = pair; t < my_tiles; t += n_pairs) {
         const TileCoord c = decode_tile(P, t);
         const int k_blocks = P.p[c.prob].k_blocks;
         ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1);
@@ -216,7 +221,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
       auto send = [&](int n0) {
         ptx::fence_proxy_async_smem();
         __syncwarp();
-        if (lane == 0) {
+        if (ptx::elect_one()) {                           // deterministic: the same lane every time (it owns the bulk groups)
           if (warp_ok) {
             if (EPI == EPI_GATE_RES) ptx::tma_reduce_add_3d(mO, stg0 + buf * STG_BYTES, n0, row0, seq);
             else ptx::tma_store_3d(mO, stg0 + buf * STG_BYTES, n0, row0, seq);
@@ -227,7 +232,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
       };
       // wait until the TMA engine has read the buffer filled two sends ago
       auto acquire = [&]() {
-        if (lane == 0) ptx::bulk_wait_read<1>();
+        ptx::bulk_wait_read<1>();                         // the elected lane waits for its groups; trivially true elsewhere
         __syncwarp();
         return stg0 + buf * STG_BYTES + row_off;
       };
@@ -337,7 +342,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
       if (lane == 0) ptx::mbar_arrive_cluster(ptx::map_to_cta(tempty_bar(acc), 0));
       if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
-    if (lane == 0) ptx::bulk_wait<0>();                     // all stores of this warp have completed
+    ptx::bulk_wait<0>();                                    // all stores of this warp have completed
   }
 
   ptx::tc_fence_before();

@@ -72,3 +72,5 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
 bool tcgen05_v3_qkv_rope_supported(const GemmProblem& p);
 bool tcgen05_attn_supported(int S, int H, int dh);
 cudaError_t launch_attn_tcgen05(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st);
+// v3: 64-key tiles, one pass over the scores, double-buffered S per query tile (the default)
+cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st);
