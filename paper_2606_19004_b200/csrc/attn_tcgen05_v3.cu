@@ -13,6 +13,11 @@
 //   * S_t = Q_t K_j^T: tcgen05.mma M128 N64 K16 x 8 (both operands K-major shared memory); O_t += P_t V_j: M128 N128
 //     K16 x 4 with P read from tensor memory (bf16, written over the consumed score columns) and V as MN-major B.
 //   * online softmax with lazy rescaling as v2 (threshold 2^8, per-warp vote, O corrected in TMEM only then).
+//   * PERSISTENT: one CTA per SM walks the list of work items (sequence, head, pair of query tiles).  A CTA's fixed
+//     cost (launch, TMEM allocation, first loads, pipeline fill, O read-out) measured 8.2 us against 1.5-2.3 us per 128
+//     keys, i.e. a quarter of the run time at S = 1280; now TMEM is allocated once, the producer runs ahead into the
+//     next item's Q / K / V, the next item's first Q K^T overlap the read-out of O, and only the first P V of an item
+//     waits for that read-out (o_free).
 // TMEM columns: [0,64) S_A0, [64,128) S_A1, [128,192) S_B0, [192,256) S_B1, [256,384) O_A, [384,512) O_B.
 // Tensor-pipe + MUFU bound: 4 S^2 d_h FLOP and S^2 ex2 per (sequence, head).
 #include <string.h>
@@ -51,13 +56,14 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 }
 
 __global__ void __launch_bounds__(ATT_THREADS, 1)
-attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict__ out, int S, int H, float scale_log2) {
+attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict__ out, int S, int H, int n_items,
+                       float scale_log2) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw_addr = ptx::smem_u32(smem_raw);
   const uint32_t base = (raw_addr + 1023u) & ~1023u;
   uint8_t* base_ptr = smem_raw + (base - raw_addr);
   const uint32_t bar = base + OFF_BAR;
-  const uint32_t q_full = bar;
+  const uint32_t q_full = bar, q_empty = bar + 8u * 31;
   auto k_full = [&](int s) { return bar + 8u * (1 + s); };
   auto k_empty = [&](int s) { return bar + 8u * (5 + s); };
   auto v_full = [&](int s) { return bar + 8u * (9 + s); };
@@ -65,19 +71,20 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
   auto s_full = [&](int t, int b) { return bar + 8u * (17 + 2 * t + b); };
   auto p_full = [&](int t, int b) { return bar + 8u * (21 + 2 * t + b); };
   auto pv_done = [&](int t) { return bar + 8u * (25 + t); };
-  auto o_final = [&](int t) { return bar + 8u * (27 + t); };      // all P V of query tile t have completed
-  const uint32_t tmem_slot = bar + 8u * 29;
-  volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(base_ptr + OFF_BAR + 8 * 29);
+  auto o_final = [&](int t) { return bar + 8u * (27 + t); };      // all P V of query tile t of this item have completed
+  auto o_free = [&](int t) { return bar + 8u * (29 + t); };       // the epilogue has read O_t: the next item may overwrite it
+  const uint32_t tmem_slot = bar + 8u * 32;
+  volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(base_ptr + OFF_BAR + 8 * 32);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int q0 = blockIdx.x * (QT * BQ), head = blockIdx.y, seq = blockIdx.z;
   const int n_kv = (S + BKV - 1) / BKV;
-  const int col_q = head * DH, col_k = (H + head) * DH, col_v = (2 * H + head) * DH;
+  const int n_qt = (S + QT * BQ - 1) / (QT * BQ);           // work item = (sequence, head, pair of query tiles)
 
   if (warp == 0 && lane == 0) ptx::prefetch_tmap(&tm_qkv);
   if (warp == 1) {
     if (lane == 0) {
       ptx::mbar_init(q_full, 1);
+      ptx::mbar_init(q_empty, 1);
       for (int s = 0; s < KV_STAGES; ++s) {
         ptx::mbar_init(k_full(s), 1); ptx::mbar_init(k_empty(s), 1);
         ptx::mbar_init(v_full(s), 1); ptx::mbar_init(v_empty(s), 1);
@@ -86,6 +93,7 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
         for (int b = 0; b < 2; ++b) { ptx::mbar_init(s_full(t, b), 1); ptx::mbar_init(p_full(t, b), 4); }
         ptx::mbar_init(pv_done(t), 1);
         ptx::mbar_init(o_final(t), 1);
+        ptx::mbar_init(o_free(t), 4);
       }
       ptx::fence_barrier_init();
     }
@@ -98,31 +106,40 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
   ptx::tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
+  // Every role walks the same list of items (w = blockIdx.x, blockIdx.x + gridDim.x, ...) and counts key tiles with
+  // one running index g = it * n_kv + j across items: ring stage g % 4, S/P buffer g & 1, barrier parities from g.
   if (warp == 0) {
     // ===================== TMA producer =====================
     // (elect.sync, not `lane == 0`: the compiler then issues UTMALDG / UTCHMMA straight from uniform registers instead
     //  of wrapping each one in a per-lane ELECT / BRA.U.ANY loop - see "warp-uniform issue" in tcgen05.cuh)
     if (ptx::elect_one()) {
-      ptx::mbar_arrive_expect_tx(q_full, QT * Q_TILE);
+      int it = 0;
+      for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++it) {
+        const int x = w % n_qt, head = (w / n_qt) % H, seq = w / (n_qt * H);
+        const int q0 = x * (QT * BQ);
+        const int col_q = head * DH, col_k = (H + head) * DH, col_v = (2 * H + head) * DH;
+        ptx::mbar_wait(q_empty, (uint32_t)(it & 1) ^ 1u);    // the last Q K^T of the previous item has read Q
+        ptx::mbar_arrive_expect_tx(q_full, QT * Q_TILE);
 #pragma unroll
-      for (int t = 0; t < QT; ++t)
+        for (int t = 0; t < QT; ++t)
 #pragma unroll
-        for (int hf = 0; hf < 2; ++hf)                    // d_h halves (64 columns = 128 bytes)
+          for (int hf = 0; hf < 2; ++hf)                    // d_h halves (64 columns = 128 bytes)
 #pragma unroll
-          for (int rh = 0; rh < 2; ++rh)                  // row halves (box = 64 rows)
-            ptx::tma_load_3d(base + OFF_Q + t * Q_TILE + hf * Q_SUB + rh * KV_SUB, &tm_qkv, q_full, col_q + hf * 64,
-                             q0 + t * BQ + rh * 64, seq);
-      for (int j = 0; j < n_kv; ++j) {
-        const int st = j % KV_STAGES;
-        const uint32_t ph = (uint32_t)(j / KV_STAGES) & 1u;
-        ptx::mbar_wait(k_empty(st), ph ^ 1);
-        ptx::mbar_arrive_expect_tx(k_full(st), KV_TILE);
-        ptx::tma_load_3d(base + OFF_K + st * KV_TILE, &tm_qkv, k_full(st), col_k, j * BKV, seq);
-        ptx::tma_load_3d(base + OFF_K + st * KV_TILE + KV_SUB, &tm_qkv, k_full(st), col_k + 64, j * BKV, seq);
-        ptx::mbar_wait(v_empty(st), ph ^ 1);
-        ptx::mbar_arrive_expect_tx(v_full(st), KV_TILE);
-        ptx::tma_load_3d(base + OFF_V + st * KV_TILE, &tm_qkv, v_full(st), col_v, j * BKV, seq);
-        ptx::tma_load_3d(base + OFF_V + st * KV_TILE + KV_SUB, &tm_qkv, v_full(st), col_v + 64, j * BKV, seq);
+            for (int rh = 0; rh < 2; ++rh)                  // row halves (box = 64 rows)
+              ptx::tma_load_3d(base + OFF_Q + t * Q_TILE + hf * Q_SUB + rh * KV_SUB, &tm_qkv, q_full, col_q + hf * 64,
+                               q0 + t * BQ + rh * 64, seq);
+        for (int j = 0; j < n_kv; ++j) {
+          const int g = it * n_kv + j, st = g % KV_STAGES;
+          const uint32_t ph = (uint32_t)(g / KV_STAGES) & 1u;
+          ptx::mbar_wait(k_empty(st), ph ^ 1);
+          ptx::mbar_arrive_expect_tx(k_full(st), KV_TILE);
+          ptx::tma_load_3d(base + OFF_K + st * KV_TILE, &tm_qkv, k_full(st), col_k, j * BKV, seq);
+          ptx::tma_load_3d(base + OFF_K + st * KV_TILE + KV_SUB, &tm_qkv, k_full(st), col_k + 64, j * BKV, seq);
+          ptx::mbar_wait(v_empty(st), ph ^ 1);
+          ptx::mbar_arrive_expect_tx(v_full(st), KV_TILE);
+          ptx::tma_load_3d(base + OFF_V + st * KV_TILE, &tm_qkv, v_full(st), col_v, j * BKV, seq);
+          ptx::tma_load_3d(base + OFF_V + st * KV_TILE + KV_SUB, &tm_qkv, v_full(st), col_v + 64, j * BKV, seq);
+        }
       }
     }
   } else if (warp == 1) {
@@ -130,43 +147,52 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
     if (ptx::elect_one()) {
       constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(BQ, BKV, 0, 0);   // A = Q (K-major smem), B = K_j (K-major smem)
       constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(BQ, DH, 0, 1);    // A = P (TMEM), B = V_j (MN-major smem)
-      auto issue_qk = [&](int t, int j) {                                  // S_t(j) -> buffer j & 1
-        const int st = j % KV_STAGES;
+      auto issue_qk = [&](int t, int g) {                                  // S_t(g) -> buffer g & 1
+        const int st = g % KV_STAGES;
         const uint32_t qa = base + OFF_Q + t * Q_TILE, ka = base + OFF_K + st * KV_TILE;
-        const uint32_t d = tmem_base + (uint32_t)(t * 128 + (j & 1) * 64);
+        const uint32_t d = tmem_base + (uint32_t)(t * 128 + (g & 1) * 64);
 #pragma unroll
         for (int k = 0; k < DH / 16; ++k)
           ptx::mma_f16_ss(d, ptx::make_smem_desc(qa + (k >> 2) * Q_SUB + (k & 3) * 32, 16, 1024),
                           ptx::make_smem_desc(ka + (k >> 2) * KV_SUB + (k & 3) * 32, 16, 1024), idesc_qk, k ? 1u : 0u);
-        ptx::mma_commit(s_full(t, j & 1));
+        ptx::mma_commit(s_full(t, g & 1));
         if (t == QT - 1) ptx::mma_commit(k_empty(st));
       };
-      ptx::mbar_wait(q_full, 0);
-      for (int j = 0; j < 2 && j < n_kv; ++j) {
-        ptx::mbar_wait(k_full(j % KV_STAGES), 0);
-        ptx::tc_fence_after();
-        issue_qk(0, j);
-        issue_qk(1, j);
-      }
-      for (int j = 0; j < n_kv; ++j) {
-        const int st = j % KV_STAGES;
-        ptx::mbar_wait(v_full(st), (uint32_t)(j / KV_STAGES) & 1u);
-#pragma unroll
-        for (int t = 0; t < QT; ++t) {
-          ptx::mbar_wait(p_full(t, j & 1), (uint32_t)(j >> 1) & 1u);
+      int it = 0;
+      for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++it) {
+        const int g0 = it * n_kv;
+        ptx::mbar_wait(q_full, (uint32_t)(it & 1));
+        for (int j = 0; j < 2 && j < n_kv; ++j) {           // the S buffers are free: every P of the previous item was
+          const int g = g0 + j;                             // consumed by a P V issued before (in-order tensor pipe)
+          ptx::mbar_wait(k_full(g % KV_STAGES), (uint32_t)(g / KV_STAGES) & 1u);
           ptx::tc_fence_after();
-          const uint32_t va = base + OFF_V + st * KV_TILE;
-          const uint32_t p_tmem = tmem_base + (uint32_t)(t * 128 + (j & 1) * 64);
+          issue_qk(0, g);
+          issue_qk(1, g);
+          if (j == n_kv - 1) ptx::mma_commit(q_empty);
+        }
+        for (int j = 0; j < n_kv; ++j) {
+          const int g = g0 + j, st = g % KV_STAGES;
+          ptx::mbar_wait(v_full(st), (uint32_t)(g / KV_STAGES) & 1u);
 #pragma unroll
-          for (int k = 0; k < BKV / 16; ++k)        // 16 keys = 8 packed TMEM columns of P, 16 rows (2048 bytes) of V
-            mma_f16_ts(tmem_base + 256 + t * DH, p_tmem + k * 8, ptx::make_smem_desc(va + k * 2048, KV_SUB, 1024), idesc_pv,
-                       (j | k) ? 1u : 0u);
-          ptx::mma_commit(pv_done(t));
-          if (j == n_kv - 1) ptx::mma_commit(o_final(t));
-          if (t == QT - 1) ptx::mma_commit(v_empty(st));
-          if (j + 2 < n_kv) {
-            if (t == 0) { ptx::mbar_wait(k_full((j + 2) % KV_STAGES), (uint32_t)((j + 2) / KV_STAGES) & 1u); ptx::tc_fence_after(); }
-            issue_qk(t, j + 2);                     // overwrites the buffer P_t(j) sat in: ordered behind PV_t(j) in the pipe
+          for (int t = 0; t < QT; ++t) {
+            ptx::mbar_wait(p_full(t, g & 1), (uint32_t)(g >> 1) & 1u);
+            if (j == 0) ptx::mbar_wait(o_free(t), (uint32_t)(it & 1) ^ 1u);   // the previous item's epilogue has read O_t
+            ptx::tc_fence_after();
+            const uint32_t va = base + OFF_V + st * KV_TILE;
+            const uint32_t p_tmem = tmem_base + (uint32_t)(t * 128 + (g & 1) * 64);
+#pragma unroll
+            for (int k = 0; k < BKV / 16; ++k)      // 16 keys = 8 packed TMEM columns of P, 16 rows (2048 bytes) of V
+              mma_f16_ts(tmem_base + 256 + t * DH, p_tmem + k * 8, ptx::make_smem_desc(va + k * 2048, KV_SUB, 1024), idesc_pv,
+                         (j | k) ? 1u : 0u);
+            ptx::mma_commit(pv_done(t));
+            if (j == n_kv - 1) ptx::mma_commit(o_final(t));
+            if (t == QT - 1) ptx::mma_commit(v_empty(st));
+            if (j + 2 < n_kv) {
+              const int g2 = g + 2;
+              if (t == 0) { ptx::mbar_wait(k_full(g2 % KV_STAGES), (uint32_t)(g2 / KV_STAGES) & 1u); ptx::tc_fence_after(); }
+              issue_qk(t, g2);                      // overwrites the buffer P_t(g) sat in: ordered behind PV_t(g) in the pipe
+              if (t == QT - 1 && j + 2 == n_kv - 1) ptx::mma_commit(q_empty);   // last Q K^T of the item: Q may be replaced
+            }
           }
         }
       }
@@ -178,83 +204,93 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
     const int row = quarter * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     const uint32_t tmem_s = tmem_base + t * 128 + lane_addr, tmem_o = tmem_base + 256 + t * DH + lane_addr;
-    float m_ref = -INFINITY, l = 0.f;
-    for (int j = 0; j < n_kv; ++j) {
-      const int b = j & 1;
-      ptx::mbar_wait(s_full(t, b), (uint32_t)(j >> 1) & 1u);
-      ptx::tc_fence_after();
-      const int valid = S - j * BKV;                   // keys of this tile that exist (>= 64 except the last)
-      uint32_t sv[2][32];
-      ptx::tmem_ld_32x32(tmem_s + b * 64, sv[0]);
-      ptx::tmem_ld_32x32(tmem_s + b * 64 + 32, sv[1]);
-      ptx::tmem_ld_wait();
-      float mx = -INFINITY;
+    int it = 0;
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++it) {
+      const int x = w % n_qt, head = (w / n_qt) % H, seq = w / (n_qt * H);
+      const int q0 = x * (QT * BQ);
+      float m_ref = -INFINITY, l = 0.f;
+      for (int j = 0; j < n_kv; ++j) {
+        const int g = it * n_kv + j, b = g & 1;
+        ptx::mbar_wait(s_full(t, b), (uint32_t)(g >> 1) & 1u);
+        ptx::tc_fence_after();
+        const int valid = S - j * BKV;                   // keys of this tile that exist (>= 64 except the last)
+        uint32_t sv[2][32];
+        ptx::tmem_ld_32x32(tmem_s + b * 64, sv[0]);
+        ptx::tmem_ld_32x32(tmem_s + b * 64 + 32, sv[1]);
+        ptx::tmem_ld_wait();
+        float mx = -INFINITY;
 #pragma unroll
-      for (int c = 0; c < 2; ++c)
+        for (int c = 0; c < 2; ++c)
 #pragma unroll
-        for (int i = 0; i < 32; ++i)
-          if (valid >= BKV || c * 32 + i < valid) mx = fmaxf(mx, __uint_as_float(sv[c][i]));
-      const bool need = (mx - m_ref) * scale_log2 > RESCALE_THRESHOLD;     // true on the first tile (m_ref = -inf)
-      if (__any_sync(0xffffffffu, need)) {
-        const float m_new = fmaxf(m_ref, mx);
-        if (j > 0) {
-          ptx::mbar_wait(pv_done(t), (uint32_t)(j - 1) & 1u);             // O_t holds P V of tiles 0 .. j-1
-          ptx::tc_fence_after();
-          const float alpha = ex2_approx((m_ref - m_new) * scale_log2);
-          l *= alpha;
+          for (int i = 0; i < 32; ++i)
+            if (valid >= BKV || c * 32 + i < valid) mx = fmaxf(mx, __uint_as_float(sv[c][i]));
+        const bool need = (mx - m_ref) * scale_log2 > RESCALE_THRESHOLD;     // true on the first tile (m_ref = -inf)
+        if (__any_sync(0xffffffffu, need)) {
+          const float m_new = fmaxf(m_ref, mx);
+          if (j > 0) {
+            ptx::mbar_wait(pv_done(t), (uint32_t)(g - 1) & 1u);             // O_t holds P V of tiles 0 .. j-1 of this item
+            ptx::tc_fence_after();
+            const float alpha = ex2_approx((m_ref - m_new) * scale_log2);
+            l *= alpha;
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            uint32_t ov[32];
-            ptx::tmem_ld_32x32(tmem_o + c * 32, ov);
-            ptx::tmem_ld_wait();
+            for (int c = 0; c < 4; ++c) {
+              uint32_t ov[32];
+              ptx::tmem_ld_32x32(tmem_o + c * 32, ov);
+              ptx::tmem_ld_wait();
 #pragma unroll
-            for (int i = 0; i < 32; ++i) ov[i] = __float_as_uint(__uint_as_float(ov[i]) * alpha);
-            ptx::tmem_st_32x32(tmem_o + c * 32, ov);
+              for (int i = 0; i < 32; ++i) ov[i] = __float_as_uint(__uint_as_float(ov[i]) * alpha);
+              ptx::tmem_st_32x32(tmem_o + c * 32, ov);
+            }
           }
+          m_ref = m_new;
         }
-        m_ref = m_new;
+        const float mc = m_ref * scale_log2;
+        float sum = 0.f;
+        uint32_t pk[32];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+          const int c = i >> 4, e = (i & 15) * 2, key = 2 * i;
+          float p0 = ex2_approx(fmaf(__uint_as_float(sv[c][e]), scale_log2, -mc));
+          float p1 = ex2_approx(fmaf(__uint_as_float(sv[c][e + 1]), scale_log2, -mc));
+          if (valid < BKV) { if (key >= valid) p0 = 0.f; if (key + 1 >= valid) p1 = 0.f; }
+          sum += p0 + p1;
+          pk[i] = pack_bf16(p0, p1);
+        }
+        ptx::tmem_st_32x32(tmem_s + b * 64, pk);
+        l += sum;
+        ptx::tmem_st_wait();
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(p_full(t, b));
       }
-      const float mc = m_ref * scale_log2;
-      float sum = 0.f;
-      uint32_t pk[32];
+      // epilogue: O / l -> bf16.  (pv_done's parity is only unambiguous one phase back - the softmax of tile g runs at
+      // most one P V ahead of it - so the end of the item's LAST P V has its own barrier.)
+      ptx::mbar_wait(o_final(t), (uint32_t)(it & 1));
+      ptx::tc_fence_after();
+      const float inv = 1.f / l;
+      const int qrow = q0 + t * BQ + row;
+      const bool row_ok = qrow < S;
+      bf16* orow = out + ((long long)seq * S + qrow) * (long long)(H * DH) + head * DH;
 #pragma unroll
-      for (int i = 0; i < 32; ++i) {
-        const int c = i >> 4, e = (i & 15) * 2, key = 2 * i;
-        float p0 = ex2_approx(fmaf(__uint_as_float(sv[c][e]), scale_log2, -mc));
-        float p1 = ex2_approx(fmaf(__uint_as_float(sv[c][e + 1]), scale_log2, -mc));
-        if (valid < BKV) { if (key >= valid) p0 = 0.f; if (key + 1 >= valid) p1 = 0.f; }
-        sum += p0 + p1;
-        pk[i] = pack_bf16(p0, p1);
-      }
-      ptx::tmem_st_32x32(tmem_s + b * 64, pk);
-      l += sum;
-      ptx::tmem_st_wait();
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(p_full(t, b));
-    }
-    // epilogue: O / l -> bf16.  (pv_done's parity is only unambiguous one phase back - the softmax of tile j runs at
-    // most one P V ahead of it - so the end of the LAST P V has its own barrier.)
-    ptx::mbar_wait(o_final(t), 0);
-    ptx::tc_fence_after();
-    const float inv = 1.f / l;
-    const int qrow = q0 + t * BQ + row;
-    const bool row_ok = qrow < S;
-    bf16* orow = out + ((long long)seq * S + qrow) * (long long)(H * DH) + head * DH;
+      for (int c = 0; c < 4; ++c) {
+        uint32_t ov[32];
+        ptx::tmem_ld_32x32(tmem_o + c * 32, ov);
+        ptx::tmem_ld_wait();
+        if (c == 3) {                                     // O_t is in registers: the next item's first P V may overwrite it
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(o_free(t));
+        }
+        if (row_ok) {
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      uint32_t ov[32];
-      ptx::tmem_ld_32x32(tmem_o + c * 32, ov);
-      ptx::tmem_ld_wait();
-      if (row_ok) {
-#pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          uint4 pkt;
-          pkt.x = pack_bf16(__uint_as_float(ov[g * 8]) * inv, __uint_as_float(ov[g * 8 + 1]) * inv);
-          pkt.y = pack_bf16(__uint_as_float(ov[g * 8 + 2]) * inv, __uint_as_float(ov[g * 8 + 3]) * inv);
-          pkt.z = pack_bf16(__uint_as_float(ov[g * 8 + 4]) * inv, __uint_as_float(ov[g * 8 + 5]) * inv);
-          pkt.w = pack_bf16(__uint_as_float(ov[g * 8 + 6]) * inv, __uint_as_float(ov[g * 8 + 7]) * inv);
-          *reinterpret_cast<uint4*>(orow + c * 32 + g * 8) = pkt;
+          for (int g4 = 0; g4 < 4; ++g4) {
+            uint4 pkt;
+            pkt.x = pack_bf16(__uint_as_float(ov[g4 * 8]) * inv, __uint_as_float(ov[g4 * 8 + 1]) * inv);
+            pkt.y = pack_bf16(__uint_as_float(ov[g4 * 8 + 2]) * inv, __uint_as_float(ov[g4 * 8 + 3]) * inv);
+            pkt.z = pack_bf16(__uint_as_float(ov[g4 * 8 + 4]) * inv, __uint_as_float(ov[g4 * 8 + 5]) * inv);
+            pkt.w = pack_bf16(__uint_as_float(ov[g4 * 8 + 6]) * inv, __uint_as_float(ov[g4 * 8 + 7]) * inv);
+            *reinterpret_cast<uint4*>(orow + c * 32 + g4 * 8) = pkt;
+          }
         }
       }
     }
@@ -268,7 +304,6 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
 }  // namespace
 
 cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st) {
-  (void)num_sms;
   if (dh != DH) return cudaErrorInvalidValue;
   if (B <= 0) return cudaSuccess;
   CUtensorMap tm;
@@ -282,8 +317,10 @@ cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int
     SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_tcgen05_v3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ATT_SMEM));
     attr_set = true;
   }
-  dim3 grid((S + QT * BQ - 1) / (QT * BQ), H, B);
+  const long long items = (long long)((S + QT * BQ - 1) / (QT * BQ)) * H * B;
+  if (items > 0x7fffffffLL / 128) return cudaErrorInvalidValue;
+  const int grid = (int)(items < num_sms ? items : num_sms);       // persistent: one CTA per SM walks the item list
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)DH);
-  attn_tcgen05_v3_kernel<<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, (bf16*)out, S, H, scale_log2);
+  attn_tcgen05_v3_kernel<<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, (bf16*)out, S, H, (int)items, scale_log2);
   return cudaGetLastError();
 }
