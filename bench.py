@@ -33,8 +33,8 @@ from synth import CONFIGS, make_probe, make_text_emb, make_weights  # noqa: E402
 
 METRIC = "image-tokens*steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of gemm_tcgen05_v3_kernel, averaged over its four uses in a
-# block (QKV+RoPE 1.055 GB, out-proj 0.645 GB, fc1 1.395 GB, fc2 2.652 GB) - profiles/r1_ncu_full_gemm_v3.txt (config 3)
-GEMM_DRAM_TRAFFIC_PER_LAUNCH = {"cfg3": 1.437e9}
+# block (QKV+RoPE 1.071 GB, out-proj 0.646 GB, fc1 1.451 GB, fc2 2.680 GB) - profiles/r1_ncu_full_gemm_v3.txt (config 3)
+GEMM_DRAM_TRAFFIC_PER_LAUNCH = {"cfg3": 1.462e9}
 WORKLOADS = {"cfg3": 3, "cfg4": 4, "cfg5": 5}
 
 

@@ -394,8 +394,10 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
   StreamMaps sm[2] = {stream_maps(c, B, 0), stream_maps(c, B, 1)};
   GemmProblem pr[2];
   // (2) y = LN(h) (1 + scale1) + shift1 ; (3) qkv = y Wqkv^T + b
+  LnProblem lp[2];
+  for (int s = 0; s < 2; ++s) lp[s] = LnProblem{h[s], sm[s].rows, mod[s], mod[s] + D, ybuf, sm[s].y};
+  LK(c, launch_ln_modulate2(dt, lp, 2, D, g.ln_eps, st));   // image and text rows in one launch
   for (int s = 0; s < 2; ++s) {
-    LK(c, launch_ln_modulate(dt, h[s], sm[s].rows, D, mod[s], mod[s] + D, g.ln_eps, ybuf, sm[s].y, st));
     memset(&pr[s], 0, sizeof(GemmProblem));
     pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].qkv_w; pr[s].bias = bw.s[s].qkv_b;
     pr[s].M = sm[s].rows; pr[s].N = 3 * D; pr[s].K = D; pr[s].out = big; pr[s].out_map = sm[s].qkv;
@@ -429,8 +431,9 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
   rs = run_gemm(c, EPI_GATE_RES, pr, ns, dt, SPOT_F32, st);
   if (rs != SPOT_OK) return rs;
   // (8) y2 = LN(h)(1 + scale2) + shift2 ; u = GELU(y2 W1^T + b) ; h += gate2 * (u W2^T + b)
+  for (int s = 0; s < ns; ++s) lp[s] = LnProblem{h[s], sm[s].rows, mod[s] + 3 * D, mod[s] + 4 * D, ybuf, sm[s].y};
+  LK(c, launch_ln_modulate2(dt, lp, ns, D, g.ln_eps, st));
   for (int s = 0; s < ns; ++s) {
-    LK(c, launch_ln_modulate(dt, h[s], sm[s].rows, D, mod[s] + 3 * D, mod[s] + 4 * D, g.ln_eps, ybuf, sm[s].y, st));
     memset(&pr[s], 0, sizeof(GemmProblem));
     pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].fc1_w; pr[s].bias = bw.s[s].fc1_b;
     pr[s].M = sm[s].rows; pr[s].N = F; pr[s].K = D; pr[s].out = big; pr[s].out_map = sm[s].wide;

@@ -1,6 +1,8 @@
 // elementwise.cu - the HBM-bound kernels: K3 ln_modulate, K4 qk_norm_rope, K6 euler_update(+reward),
 // K7 time embedding / skinny Linear, K8 seed selection, and small plumbing kernels.
 // Readings S4-S12 of DESIGN.md; paper passages are cited at each kernel.
+#include <string.h>
+
 #include "kernels.h"
 
 namespace {
@@ -75,13 +77,20 @@ __global__ void silu_kernel(const float* __restrict__ in, float* __restrict__ ou
 // modulated" in north_star (b)).  One warp per row; the row (fp32 residual stream) is read once into
 // registers (NV float4 per lane), mean and variance are two exact passes over registers, the
 // output is written once in the activation dtype.  Algorithmic bytes: 4 D read + sizeof(T) D write.
+// Up to two problems (the image and the text stream of a block) share one launch: rows [0, M0) belong to p[0].
 template <typename TO, int NV>
-__global__ void __launch_bounds__(256) ln_modulate_kernel(const float* __restrict__ h, int M, int D,
-                                                          const float* __restrict__ shift,
-                                                          const float* __restrict__ scale, float eps,
-                                                          TO* __restrict__ out, RowMap omap) {
-  const int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (row >= M) return;
+__global__ void __launch_bounds__(256) ln_modulate_kernel(const LnProblem p0, const LnProblem p1, int D, float eps) {
+  int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  const bool second = row >= p0.M;
+  if (second) row -= p0.M;
+  const LnProblem& P = second ? p1 : p0;
+  if (row >= P.M) return;
+  const float* __restrict__ h = P.h;
+  const float* __restrict__ shift = P.shift;
+  const float* __restrict__ scale = P.scale;
+  TO* __restrict__ out = reinterpret_cast<TO*>(P.out);
+  const RowMap omap = P.out_map;
   const float4* src = reinterpret_cast<const float4*>(h + (long long)row * D);
   float4 v[NV];
   float s = 0.f;
@@ -339,12 +348,11 @@ cudaError_t launch_silu(const float* in, float* out, long long n, cudaStream_t s
 }
 
 template <typename TO>
-static cudaError_t ln_dispatch(const float* h, int M, int D, const float* shift, const float* scale, float eps,
-                               TO* out, RowMap omap, cudaStream_t st) {
-  const int grid = (M + 7) / 8;
+static cudaError_t ln_dispatch(const LnProblem& p0, const LnProblem& p1, int D, float eps, cudaStream_t st) {
+  const int grid = (p0.M + p1.M + 7) / 8;
 #define LN_CASE(nv)                                                                                     \
   case nv:                                                                                              \
-    ln_modulate_kernel<TO, nv><<<grid, 256, 0, st>>>(h, M, D, shift, scale, eps, out, omap);            \
+    ln_modulate_kernel<TO, nv><<<grid, 256, 0, st>>>(p0, p1, D, eps);                                   \
     break;
   switch (D / 128) {
     LN_CASE(1) LN_CASE(2) LN_CASE(4) LN_CASE(8) LN_CASE(12) LN_CASE(16) LN_CASE(24) LN_CASE(32)
@@ -354,12 +362,22 @@ static cudaError_t ln_dispatch(const float* h, int M, int D, const float* shift,
   return cudaGetLastError();
 }
 
+cudaError_t launch_ln_modulate2(spot_dtype odt, const LnProblem* probs, int n_probs, int D, float eps, cudaStream_t st) {
+  if (n_probs < 1 || n_probs > 2 || D % 128) return cudaErrorInvalidValue;
+  LnProblem p0 = probs[0], p1;
+  memset(&p1, 0, sizeof(p1));
+  if (n_probs == 2) p1 = probs[1];
+  if (p0.M < 0 || p1.M < 0) return cudaErrorInvalidValue;
+  if (p0.M == 0) { p0 = p1; p1.M = 0; }
+  if (p0.M == 0) return cudaSuccess;
+  return odt == SPOT_F32 ? ln_dispatch<float>(p0, p1, D, eps, st) : ln_dispatch<bf16>(p0, p1, D, eps, st);
+}
+
 cudaError_t launch_ln_modulate(spot_dtype odt, const float* h, int M, int D, const float* shift, const float* scale,
                                float eps, void* out, RowMap out_map, cudaStream_t st) {
   if (M <= 0) return cudaSuccess;
-  if (D % 128) return cudaErrorInvalidValue;
-  return odt == SPOT_F32 ? ln_dispatch<float>(h, M, D, shift, scale, eps, (float*)out, out_map, st)
-                         : ln_dispatch<bf16>(h, M, D, shift, scale, eps, (bf16*)out, out_map, st);
+  LnProblem p{h, M, shift, scale, out, out_map};
+  return launch_ln_modulate2(odt, &p, 1, D, eps, st);
 }
 
 cudaError_t launch_rmsnorm_rows(spot_dtype dt, const void* in, const void* gain, int M, int D, float eps, void* out,

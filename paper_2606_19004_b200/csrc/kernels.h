@@ -15,6 +15,16 @@ cudaError_t launch_silu(const float* in, float* out, long long n, cudaStream_t s
 // K3: LayerNorm (no affine) * (1 + scale) + shift, fp32 residual rows -> act dtype rows
 cudaError_t launch_ln_modulate(spot_dtype odt, const float* h, int M, int D, const float* shift, const float* scale,
                                float eps, void* out, RowMap out_map, cudaStream_t st);
+struct LnProblem {          // one stream of launch_ln_modulate2
+  const float* h;           // [M, D] fp32 rows
+  int M;
+  const float* shift;       // [D]
+  const float* scale;       // [D]
+  void* out;                // activation dtype, rows addressed through out_map
+  RowMap out_map;
+};
+// the same for up to two problems (image and text stream of a block) in ONE launch
+cudaError_t launch_ln_modulate2(spot_dtype odt, const LnProblem* probs, int n_probs, int D, float eps, cudaStream_t st);
 cudaError_t launch_rmsnorm_rows(spot_dtype dt, const void* in, const void* gain, int M, int D, float eps, void* out,
                                 cudaStream_t st);
 
