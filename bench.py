@@ -201,7 +201,8 @@ def run_kernels(args, shape):
     # K4 QK-RMSNorm + RoPE in place on q and k
     qkv = rnd(4, (B, S, 3, H, dh), bf)
     gains = [torch.ones(dh, dtype=bf, device="cuda") for _ in range(4)]
-    cs, sn = rnd(5, (S, dh // 2), torch.float32), rnd(6, (S, dh // 2), torch.float32)
+    ang = rnd(5, (S, dh // 2), torch.float32, 3.0)             # a rotation table (cos, sin of arbitrary angles): norm-preserving
+    cs, sn = torch.cos(ang).contiguous(), torch.sin(ang).contiguous()
     hbm("K4_qk_norm_rope", lambda: spot.spot_qk_norm_rope(qkv, shape.n_txt, gains, cs, sn, 1e-6), 2.0 * 2 * B * S * H * dh * 2)
     # K5 attention
     tensor("K5_attention", lambda: spot.spot_attention(qkv, spot.IMPL_TCGEN05), 4.0 * S * S * dh * H * B)

@@ -25,7 +25,7 @@
 namespace {
 
 constexpr int BLOCK_M = 128 /*per CTA*/, PAIR_M = 256, BLOCK_N = 256, HALF_N = 128, BLOCK_K = 64, UMMA_K = 16;
-constexpr int STAGES = 6, GROUP_M = 8;
+constexpr int STAGES = 6;
 constexpr uint32_t A_BYTES = BLOCK_M * BLOCK_K * 2, B_BYTES = HALF_N * BLOCK_K * 2, STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr uint32_t STG_BYTES = 32 * 128;                         // one staging buffer: 32 rows x 128 bytes
 constexpr uint32_t OFF_STG = STAGES * STAGE_BYTES;               // 4 warps x 2 buffers
@@ -36,6 +36,7 @@ static_assert(SMEM_BYTES <= 232448, "shared memory budget");
 
 struct V3Problem {
   int m_tiles, n_tiles, tiles_per_seq, rps, N, k_blocks, tile_start;   // m_tiles counts 256-row pair tiles
+  int group_m;              // rasterisation: tiles run n-major inside groups of group_m M-tiles (L2 residency)
   const bf16* bias;
   const float* gate;
   // EPI_QKV_ROPE
@@ -57,9 +58,9 @@ __device__ __forceinline__ TileCoord decode_tile(const V3Params& P, int t) {
   c.prob = (P.n_probs > 1 && t >= P.p[1].tile_start) ? 1 : 0;
   const V3Problem& q = P.p[c.prob];
   t -= q.tile_start;
-  const int per_group = GROUP_M * q.n_tiles;
-  const int g = t / per_group, first_m = g * GROUP_M;
-  const int gm = min(GROUP_M, q.m_tiles - first_m);
+  const int per_group = q.group_m * q.n_tiles;
+  const int g = t / per_group, first_m = g * q.group_m;
+  const int gm = min(q.group_m, q.m_tiles - first_m);
   const int r = t - g * per_group;
   c.mt = first_m + r % gm;
   c.nt = r / gm;
@@ -381,6 +382,22 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
     q.N = g.N;
     q.k_blocks = (g.K + BLOCK_K - 1) / BLOCK_K;
     q.tile_start = tiles;
+    {
+      // Rasterisation: tiles of one group sweep all N for group_m M-tiles, so a wave of 74 pair tiles touches
+      // ~group_m A panels and 74 / group_m W panels.  Measured at config 3 (M = 20480; TFLOP/s alone, group 2 / 8 / 16):
+      // QKV (N 9216, K 3072) 1594 / 1622 / 1658, fc1 (N 12288) 1506 / 1575 / 1627, out-proj (N 3072) 1627 / 1606 / 1585,
+      // fc2 (N 3072, K 12288) 1521 / 1505 / 1493: wide outputs want tall groups (W is re-used from L2 across 16 M-tiles),
+      // narrow outputs want short ones.  SPOT_GEMM_GROUP_M overrides (A/B timing only).
+      static int forced = -1;
+      if (forced < 0) { const char* e = getenv("SPOT_GEMM_GROUP_M"); forced = e ? atoi(e) : 0; }
+      int gm = 2;
+      if (q.n_tiles >= 24) {
+        gm = (int)(25.0e6 / (2.0 * PAIR_M * (double)g.K));         // A panel of a group ~25 MB
+        if (gm > 16) gm = 16;
+        if (gm < 2) gm = 2;
+      }
+      q.group_m = forced > 0 ? forced : gm;
+    }
     q.bias = (const bf16*)g.bias;
     q.gate = g.gate;
     q.q_gain = (const bf16*)g.q_gain; q.k_gain = (const bf16*)g.k_gain;
