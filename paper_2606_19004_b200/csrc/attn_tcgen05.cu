@@ -100,7 +100,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict
   if (warp == 0) {
     // ===================== TMA producer =====================
     // (elect.sync, not `lane == 0`: the compiler then issues UTMALDG / UTCHMMA straight from uniform registers instead
-    //  of wrapping each one in a per-lane ELECT / BRA.U.ANY loop - see "warp-uniform issue" in tcgen05.cuh)
+    //  of wrapping each one in a per-lane ELECT / BRA.U.ANY loop - see "single-thread issue paths" in tcgen05.cuh)
     if (ptx::elect_one()) {
       ptx::mbar_arrive_expect_tx(q_full, QT * TILE_BYTES);
 #pragma unroll

@@ -111,7 +111,7 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
   if (warp == 0) {
     // ===================== TMA producer =====================
     // (elect.sync, not `lane == 0`: the compiler then issues UTMALDG / UTCHMMA straight from uniform registers instead
-    //  of wrapping each one in a per-lane ELECT / BRA.U.ANY loop - see "warp-uniform issue" in tcgen05.cuh)
+    //  of wrapping each one in a per-lane ELECT / BRA.U.ANY loop - see "single-thread issue paths" in tcgen05.cuh)
     if (ptx::elect_one()) {
       int it = 0;
       for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++it) {

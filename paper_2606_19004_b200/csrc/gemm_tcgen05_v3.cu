@@ -144,7 +144,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
   if (warp == 0) {
     // ===================== TMA producer (both CTAs) =====================
     // elect.sync (not `lane == 0`): the compiler then knows the region is single-threaded and issues UTMALDG /
-    // UTCHMMA straight from uniform registers (see "warp-uniform issue" in tcgen05.cuh)
+    // UTCHMMA straight from uniform registers (see "single-thread issue paths" in tcgen05.cuh)
     if (ptx::elect_one()) {
       int stage = 0; uint32_t phase = 0;
       for (int t = pair; t < P.total_tiles; t += n_pairs) {

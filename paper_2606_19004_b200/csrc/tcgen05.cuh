@@ -252,95 +252,19 @@ __device__ __forceinline__ void mma_commit_2cta(uint32_t bar) {
 
 }  // namespace ptx
 
-// ---- warp-uniform issue ------------------------------------------------------------------------------------------
+// ---- single-thread issue paths -----------------------------------------------------------------------------------
 // tcgen05.mma / tcgen05.commit / TMA instructions take their operands from UNIFORM registers.  Issued from a
-// divergent branch (`if (lane == 0)`) the compiler cannot prove the operands uniform and wraps every one of them in
-// an ELECT / R2UR / BRA.U.ANY loop (~20 SASS instructions per MMA): the single issuing thread then becomes the
-// bottleneck of the kernel (measured: 430 instructions per 64-key step of the attention kernel, 130 per K block of
-// the GEMM).  The `_if` variants below are called by ALL lanes of a converged warp with warp-uniform operands and a
-// `leader` flag (elect_one() once per warp); only the instruction itself is predicated, so it compiles to one
-// UTCHMMA / UTCBAR / UTMALDG.  The warp index must be made uniform for the compiler: uniform_warp_idx().
+// `if (lane == 0)` branch the compiler cannot tell that one thread is active and wraps every one of them in an
+// ELECT / R2UR / BRA.U.ANY loop (~20 SASS instructions per MMA): the issuing thread then becomes the bottleneck of the
+// kernel (measured: 430 instructions per 64-key step of the attention kernel, 130 per K block of the GEMM, tensor pipe
+// capped near 90 %).  Guarding the region with elect.sync instead - `if (ptx::elect_one()) { ... }`, entered by a
+// converged warp - makes it provably single-threaded and every UTCHMMA / UTCBAR / UTMALDG is emitted bare.  Two traps:
+// a branch on a value the compiler cannot prove uniform (e.g. %cluster_ctarank read through asm volatile) AROUND the
+// elected region brings the loops back - fold such conditions into loop bounds; and elect.sync elects the same lane
+// every time for the same membermask, which the per-thread bulk async-groups of the TMA-store epilogue rely on.
 namespace ptx {
 
+// warp index as a value the compiler knows to be warp-uniform
 __device__ __forceinline__ int uniform_warp_idx() { return __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0); }
-
-__device__ __forceinline__ void mbar_arrive_expect_tx_if(uint32_t leader, uint32_t bar, uint32_t bytes) {
-  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %2, 0;\n\t@q mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n\t}\n" ::"r"(bar),
-               "r"(bytes), "r"(leader)
-               : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_if(uint32_t leader, uint32_t bar) {
-  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %1, 0;\n\t@q mbarrier.arrive.shared::cta.b64 _, [%0];\n\t}\n" ::"r"(bar), "r"(leader) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_cluster_if(uint32_t leader, uint32_t cluster_addr) {
-  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %1, 0;\n\t@q mbarrier.arrive.shared::cluster.b64 _, [%0];\n\t}\n" ::"r"(cluster_addr), "r"(leader) : "memory");
-}
-__device__ __forceinline__ void tma_load_3d_if(uint32_t leader, uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1, int c2) {
-  asm volatile(
-      "{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %6, 0;\n\t"
-      "@q cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];\n\t}\n" ::"r"(dst),
-      "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(leader)
-      : "memory");
-}
-__device__ __forceinline__ void tma_load_3d_2cta_if(uint32_t leader, uint32_t dst, const CUtensorMap* m, uint32_t leader_bar, int c0, int c1, int c2) {
-  asm volatile(
-      "{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %6, 0;\n\t"
-      "@q cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];\n\t}\n" ::"r"(dst),
-      "l"(reinterpret_cast<uint64_t>(m)), "r"(leader_bar), "r"(c0), "r"(c1), "r"(c2), "r"(leader)
-      : "memory");
-}
-__device__ __forceinline__ void tma_load_2d_2cta_if(uint32_t leader, uint32_t dst, const CUtensorMap* m, uint32_t leader_bar, int c0, int c1) {
-  asm volatile(
-      "{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %5, 0;\n\t"
-      "@q cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];\n\t}\n" ::"r"(dst),
-      "l"(reinterpret_cast<uint64_t>(m)), "r"(leader_bar), "r"(c0), "r"(c1), "r"(leader)
-      : "memory");
-}
-__device__ __forceinline__ void tma_store_3d_if(uint32_t leader, const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
-  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %5, 0;\n\t"
-               "@q cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];\n\t}\n" ::"l"(
-                   reinterpret_cast<uint64_t>(m)),
-               "r"(src), "r"(c0), "r"(c1), "r"(c2), "r"(leader)
-               : "memory");
-}
-__device__ __forceinline__ void tma_reduce_add_3d_if(uint32_t leader, const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
-  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %5, 0;\n\t"
-               "@q cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];\n\t}\n" ::"l"(
-                   reinterpret_cast<uint64_t>(m)),
-               "r"(src), "r"(c0), "r"(c1), "r"(c2), "r"(leader)
-               : "memory");
-}
-__device__ __forceinline__ void mma_f16_ss_if(uint32_t leader, uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p, q;\n\tsetp.ne.b32 p, %4, 0;\n\tsetp.ne.b32 q, %5, 0;\n\t"
-      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(d_tmem),
-      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(leader)
-      : "memory");
-}
-__device__ __forceinline__ void mma_f16_ts_if(uint32_t leader, uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p, q;\n\tsetp.ne.b32 p, %4, 0;\n\tsetp.ne.b32 q, %5, 0;\n\t"
-      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}\n" ::"r"(d_tmem),
-      "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(leader)
-      : "memory");
-}
-__device__ __forceinline__ void mma_f16_ss_2cta_if(uint32_t leader, uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p, q;\n\tsetp.ne.b32 p, %4, 0;\n\tsetp.ne.b32 q, %5, 0;\n\t"
-      "@q tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(d_tmem),
-      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(leader)
-      : "memory");
-}
-__device__ __forceinline__ void mma_commit_if(uint32_t leader, uint32_t bar) {
-  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %1, 0;\n\t"
-               "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}\n" ::"r"(bar), "r"(leader)
-               : "memory");
-}
-__device__ __forceinline__ void mma_commit_2cta_if(uint32_t leader, uint32_t bar) {
-  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %2, 0;\n\t"
-               "@q tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;\n\t}\n" ::"r"(bar),
-               "h"((uint16_t)3), "r"(leader)
-               : "memory");
-}
 
 }  // namespace ptx
