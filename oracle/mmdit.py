@@ -129,8 +129,12 @@ def modulation(c: Array, w: Array, b: Array, mode: str = "blas") -> List[Array]:
 
 def block_forward(h_img: Array, h_txt: Array, c: Array, bw: Dict[str, Array], *, n_heads: int,
                   cos: Array, sin: Array, ln_eps: float = 1e-6, rms_eps: float = 1e-6,
-                  mode: str = "blas", trace: Dict[str, Array] | None = None) -> Tuple[Array, Array]:
-    """One joint block for one sequence (C5 steps 1-8).  h_img [N_img, D], h_txt [N_txt, D], c = SiLU(temb) [D]."""
+                  mode: str = "blas", trace: Dict[str, Array] | None = None, lin=None) -> Tuple[Array, Array]:
+    """One joint block for one sequence (C5 steps 1-8).  h_img [N_img, D], h_txt [N_txt, D], c = SiLU(temb) [D].
+    `lin(x, name)`, if given, replaces y = x W^T + b for the four block Linears name = "<stream>.qkv|out|fc1|fc2"
+    (used by oracle/fp8.py to state the low-precision variant; None = the plain Linear above)."""
+    if lin is None:
+        lin = lambda x, name: linear(x, bw[f"{name}_w"], bw[f"{name}_b"], mode)
     n_txt = h_txt.shape[0]
     D = h_img.shape[1]
     dh = D // n_heads
@@ -140,7 +144,7 @@ def block_forward(h_img: Array, h_txt: Array, c: Array, bw: Dict[str, Array], *,
         mod[s] = modulation(c, bw[f"{s}.mod_w"], bw[f"{s}.mod_b"], mode)
         shift1, scale1 = mod[s][0], mod[s][1]
         y = layer_norm(h[s], ln_eps) * (1.0 + scale1) + shift1
-        qkv = linear(y, bw[f"{s}.qkv_w"], bw[f"{s}.qkv_b"], mode)
+        qkv = lin(y, f"{s}.qkv")
         n = qkv.shape[0]
         q[s] = rms_norm(qkv[:, 0 * D:1 * D].reshape(n, n_heads, dh), bw[f"{s}.q_gain"], rms_eps)
         k[s] = rms_norm(qkv[:, 1 * D:2 * D].reshape(n, n_heads, dh), bw[f"{s}.k_gain"], rms_eps)
@@ -157,10 +161,10 @@ def block_forward(h_img: Array, h_txt: Array, c: Array, bw: Dict[str, Array], *,
     out = {}
     for s in ("txt", "img"):
         _, _, gate1, shift2, scale2, gate2 = mod[s]
-        x = h[s] + gate1 * linear(o_s[s], bw[f"{s}.out_w"], bw[f"{s}.out_b"], mode)
+        x = h[s] + gate1 * lin(o_s[s], f"{s}.out")
         y2 = layer_norm(x, ln_eps) * (1.0 + scale2) + shift2
-        u = gelu_tanh(linear(y2, bw[f"{s}.fc1_w"], bw[f"{s}.fc1_b"], mode))
-        out[s] = x + gate2 * linear(u, bw[f"{s}.fc2_w"], bw[f"{s}.fc2_b"], mode)
+        u = gelu_tanh(lin(y2, f"{s}.fc1"))
+        out[s] = x + gate2 * lin(u, f"{s}.fc2")
         if trace is not None:
             trace[f"{s}.h_attn"], trace[f"{s}.u"] = x, u
     return out["img"], out["txt"]
@@ -173,14 +177,16 @@ def text_input(text_emb: Array, g: Dict[str, Array], rms_eps: float = 1e-6, mode
 
 def dit_velocity(x: Array, t: float, h_txt0: Array, g: Dict[str, Array], blocks: List[Dict[str, Array]], *,
                  n_heads: int, cos: Array, sin: Array, ln_eps: float = 1e-6, rms_eps: float = 1e-6,
-                 mode: str = "blas", trace: List[Array] | None = None) -> Array:
-    """v = DiT(x, t, text) for one sequence.  x [N_img, C] -> v [N_img, C] (C7)."""
+                 mode: str = "blas", trace: List[Array] | None = None, block_lin=None) -> Array:
+    """v = DiT(x, t, text) for one sequence.  x [N_img, C] -> v [N_img, C] (C7).
+    `block_lin(block_index)` -> the `lin` hook of block_forward for that block (None = plain Linears)."""
     _, c = time_conditioning(t, g, mode)
     h_img = linear(x, g["img_in_w"], g["img_in_b"], mode)
     h_txt = h_txt0
-    for bw in blocks:
+    for bi, bw in enumerate(blocks):
         h_img, h_txt = block_forward(h_img, h_txt, c, bw, n_heads=n_heads, cos=cos, sin=sin,
-                                     ln_eps=ln_eps, rms_eps=rms_eps, mode=mode)
+                                     ln_eps=ln_eps, rms_eps=rms_eps, mode=mode,
+                                     lin=None if block_lin is None else block_lin(bi))
         if trace is not None:
             trace.append(h_img)
     m_f = linear(c[None, :], g["final_mod_w"], g["final_mod_b"], mode)[0]
