@@ -227,6 +227,17 @@ def run_kernels(args, shape):
     tensor("K2_gemm_qkv_rope_fused", lambda: spot.spot_qkv_rope_linear(a, w, b, gains[0], gains[1], cs, sn, 0, 1e-6),
            2.0 * M * 3 * D * D)
     del a, w
+    # K2 on E4M3 operands (the low-precision exploration variant); peak = measured bf16 burst x 2
+    for name, (N, K, epi) in {"K2_fp8_gemm_out": (D, D, spot.EPI_GATE_RESIDUAL), "K2_fp8_gemm_fc1": (F, D, spot.EPI_BIAS_GELU),
+                              "K2_fp8_gemm_fc2": (D, F, spot.EPI_GATE_RESIDUAL)}.items():
+        a8 = spot.spot_quantize_e4m3(rnd(10, (M, K), bf))
+        wq, ws = spot.spot_quantize_weight_rows(rnd(11, (N, K), bf, 0.02))
+        b = rnd(12, (N,), bf, 0.02)
+        gate, resid = rnd(13, (N,), torch.float32, 0.1), torch.zeros((M, N), dtype=torch.float32, device="cuda")
+        tensor(name, lambda: spot.spot_linear_fp8(a8, wq, ws, b, epi, gate=gate, residual=resid), 2.0 * M * N * K)
+        res[name]["peak"] = 2.0 * peaks["bf16_tflops"]
+        res[name]["frac"] = res[name]["achieved"] / res[name]["peak"]
+        del a8, wq, resid
     print(json.dumps({"mode": "kernels", "workload": shape.name, "rows": M, "l2": "512 MiB written between iterations",
                       "peaks": peaks, "kernels": res}))
 
@@ -244,6 +255,9 @@ def main():
     ap.add_argument("--gemm-impl", type=int, default=0,
                     help="0 auto (CTA pair + TMA-store epilogue, K4 fused), 2 one-CTA tcgen05, 3 CTA pair with per-thread "
                          "epilogue, 4 as 0 with K4 as its own kernel (A/B testing)")
+    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp8"],
+                    help="fp8 = the low-precision exploration variant (E4M3 block Linears, DESIGN.md section 13): NOT the "
+                         "headline configuration; the line says dtype fp8 and adds the reward rank correlation with bf16")
     ap.add_argument("--cache-threshold", type=float, default=None,
                     help="run the cached-step variant (spot_explore_cached, PAPER.md:155-157) with this threshold; the line "
                          "adds the effective denoising steps; no e2e leg")
@@ -294,7 +308,8 @@ def main():
     out = None
 
     cached = args.cache_threshold is not None
-    if cached:
+    fp8 = args.precision == "fp8"
+    if cached or fp8:
         args.no_e2e = True
 
     def step():
@@ -312,8 +327,10 @@ def main():
         torch.cuda.synchronize()
 
     full_rewards = None
-    if cached:                                   # the full rollout's rewards, for the rank correlation of PAPER.md:340
+    if cached or fp8:                            # the full bf16 rollout's rewards, for the rank correlation of PAPER.md:340
         full_rewards = spot.spot_explore(ctx, seeds, text, ts, probe, P, K, k_sel)["rewards"].clone()
+    if fp8:
+        ctx.enable_fp8(True)
     for _ in range(args.warmup):
         step()
     sync_all()
@@ -350,9 +367,11 @@ def main():
     timed_frac = counters["gemm_timed"] / max(1, counters["gemm_launches"])
     gemm_ms = counters["gemm_ms"]
     gemm_tflops = (gemm_flops_step * args.steps * timed_frac) / (gemm_ms / 1e3) / 1e12 if gemm_ms > 0 else None
+    gemm_peak = peaks["bf16_tflops_sustained"] * (2.0 if fp8 else 1.0)
+    peak_kind = f"{peaks['source']} sustained bf16 (kernel timed inside a long step)" + (" x 2 (nominal fp8 : bf16 ratio)" if fp8 else "")
     roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_v3_kernel", "achieved": gemm_tflops,
-                "peak": peaks["bf16_tflops_sustained"], "peak_kind": f"{peaks['source']} sustained bf16 (kernel timed inside a long step)",
-                "unit": "TFLOP/s", "frac": (gemm_tflops / peaks["bf16_tflops_sustained"]) if gemm_tflops else None,
+                "peak": gemm_peak, "peak_kind": peak_kind,
+                "unit": "TFLOP/s", "frac": (gemm_tflops / gemm_peak) if gemm_tflops else None,
                 "traffic": GEMM_DRAM_TRAFFIC_PER_LAUNCH.get(args.workload), "launches_timed": counters["gemm_timed"],
                 "avg_launch_ms": gemm_ms / max(1, counters["gemm_timed"]), "share_of_step": gemm_ms / ms_total / max(timed_frac, 1e-9),
                 "flops_per_launch": gemm_flops_step / max(1, counters["gemm_launches"] / args.steps)}
@@ -399,7 +418,8 @@ def main():
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "fp8_e4m3 block Linears (bf16 attention, fp32 residual): exploration variant, not the headline" if fp8 else "bf16",
                 "data": "synthetic",
                 "config": {"workload": shape.name, "n_prompts": P, "seeds_per_prompt": K, "euler_steps": T, "blocks": L,
                            "hidden": D, "image_tokens": shape.n_img, "text_tokens": shape.n_txt,
@@ -410,9 +430,15 @@ def main():
                                       "nominal_2250": tflops / 2250.0, "peaks": peaks["source"]},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": counters["launches"], "roofline": roofline,
                 "cpu_baseline": cpu_baseline, "weight_gen_s": gen_s}
+        rk = lambda v: torch.argsort(torch.argsort(v)).double()
+        if fp8:
+            line["fp8"] = {"reward_rank_correlation_vs_bf16_per_prompt":
+                           [float(torch.corrcoef(torch.stack([rk(out["rewards"][g * K:(g + 1) * K]), rk(full_rewards[g * K:(g + 1) * K])]))[0, 1])
+                            for g in range(P)],
+                           "reward_rel_l2_vs_bf16": float((out["rewards"] - full_rewards).norm() / full_rewards.norm()),
+                           "note": "tflops_per_gpu counts the same algorithmic FLOPs as the bf16 line"}
         if cached:
             eff = out["computed"].sum(1).tolist()
-            rk = lambda v: torch.argsort(torch.argsort(v)).double()
             corr = [float(torch.corrcoef(torch.stack([rk(out["rewards"][g * K:(g + 1) * K]), rk(full_rewards[g * K:(g + 1) * K])]))[0, 1])
                     for g in range(P)]
             line["cache"] = {"threshold": args.cache_threshold, "scheduled_steps": T, "effective_steps_mean": sum(eff) / len(eff),

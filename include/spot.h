@@ -51,7 +51,9 @@ typedef enum {
   SPOT_ERR_UNIMPLEMENTED = 8
 } spot_status;
 
-typedef enum { SPOT_F32 = 0, SPOT_BF16 = 1 } spot_dtype;
+/* SPOT_E4M3 is a STORAGE type of activations / quantised weights in the FP8 exploration variant and
+ * of the kernel-level calls that say so; spot_config.dtype must be SPOT_F32 or SPOT_BF16. */
+typedef enum { SPOT_F32 = 0, SPOT_BF16 = 1, SPOT_E4M3 = 2 } spot_dtype;
 
 /* Model/workload shape (plain data, copied at spot_create).  n_img = grid_h * grid_w image tokens,
  * joint sequence S = n_txt + n_img with the text tokens FIRST.  hidden == n_heads * head_dim;
@@ -96,7 +98,8 @@ typedef enum {
                              * 1 = SIMT FFMA GEMM, 2 = 1-CTA tcgen05, 3 = CTA-pair tcgen05 with per-thread epilogue,
                              * 4 = as 0 but K4 (QK-norm+RoPE) as its own kernel */
   SPOT_OPT_ATTN_IMPL = 1,   /* 0 = auto (tcgen05 for bf16, d_h = 128: one-pass kernel, 64-key tiles), 1 = SIMT attention, 2 = previous two-pass tcgen05 kernel */
-  SPOT_OPT_TIMING = 2       /* 1 = bracket every tcgen05 GEMM launch with CUDA events on the launch stream */
+  SPOT_OPT_TIMING = 2,      /* 1 = bracket every tcgen05 GEMM launch with CUDA events on the launch stream */
+  SPOT_OPT_FP8 = 3          /* 1 = the four Linears of every block run on E4M3 operands (after spot_fp8_prepare) */
 } spot_option;
 
 /* Validates cfg and w, builds the RoPE table (S5) and returns a context.  max_seqs bounds
@@ -222,6 +225,22 @@ spot_status spot_dit_denoise_sde(spot_ctx *ctx, int n_prompts, int seeds_per_pro
                                  float *d_latents, const void *d_text_emb, const float *h_timesteps, int n_steps,
                                  float noise_level, int window_lo, int window_hi, float *d_logp,
                                  void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
+/* ---- Low-precision exploration variant: FP8 (E4M3) block Linears ----------------------------------------------
+ * PAPER.md:67 (s2.2): "first running a cheap exploratory rollout e.g., with reduced denoising steps or a quantized
+ * model, to identify high-contrast seeds, then performing full-quality rollout only on the selected seeds";
+ * PAPER.md:340 judges a cheaper exploration by the rank correlation of its rewards with the full rollout's.
+ * DESIGN.md section 13 (readings Q1-Q4): only the QKV, out-proj, fc1 and fc2 Linears of each block change:
+ *   weights      Wq = e4m3(W / s_n), s_n = max_k |W_nk| / 448 per output channel (made once by spot_fp8_prepare),
+ *   activations  e4m3(x) with unit scale (written by the producing kernel: LN-modulate, attention, fc1 epilogue),
+ *   y_n = s_n * sum_k xq_k Wq_nk + b_n, fp32 accumulation on kind::f8f6f4 tensor-core instructions;
+ * attention (bf16 q, k, v), norms, modulation, the fp32 residual stream, the input / final layers and the sampler are
+ * unchanged.  spot_fp8_bytes: size of the caller-owned buffer for the quantised weights and scales (about half of the
+ * bf16 block weights); spot_fp8_prepare: fills it (asynchronous on the stream; the buffer must outlive the context's
+ * FP8 use); spot_set_option(ctx, SPOT_OPT_FP8, 1) then switches every later block / denoise / explore call.
+ * bf16 configs with head_dim 128 only (SPOT_ERR_DTYPE / SPOT_ERR_SHAPE otherwise). */
+spot_status spot_fp8_bytes(const spot_ctx *ctx, size_t *bytes);
+spot_status spot_fp8_prepare(spot_ctx *ctx, void *d_buffer, size_t bytes, void *cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -45,7 +45,7 @@ spot_status spot_qkv_rope_linear(const void *d_a, int n_seqs, int rows_per_seq, 
 
 /* y = LayerNorm(h) * (1 + scale) + shift over the last axis, biased variance, no affine (S4
  * step 2).  d_h [M, D] fp32 (residual stream), d_shift/d_scale [D] fp32, d_out [M, D] of `dtype`.
- * D must be 128 * {1,2,4,8,12,16,24,32}. */
+ * D must be 128 * {1,2,4,8,12,16,24,32}.  dtype SPOT_E4M3 writes E4M3 bytes (unit scale, saturating). */
 spot_status spot_ln_modulate(spot_dtype dtype, const float *d_h, int64_t M, int64_t D, const float *d_shift,
                              const float *d_scale, float eps, void *d_out, void *cuda_stream);
 
@@ -73,6 +73,18 @@ spot_status spot_euler_update(float *d_x, const float *d_v, float dt, int n_seqs
  * noise_level == 0 degenerates to the Euler update (d_logp = 0).  d_partials: [n_seqs, ceil(elems / 4096)] fp32 scratch. */
 spot_status spot_sde_update(float *d_x, const float *d_v, const uint64_t *d_seeds, int step, float t_i, float t_next,
                             float noise_level, int n_seqs, int64_t elems, float *d_logp, float *d_partials,
+                            void *cuda_stream);
+
+/* FP8 (E4M3) building blocks of the low-precision exploration variant (spot.h).
+ * spot_quantize_weight_rows: d_w_bf16 [N, K] bf16 -> d_wq [N, K] E4M3 bytes and d_scale [N] fp32 (s_n = max|W_n| / 448).
+ * spot_quantize_e4m3: elementwise e4m3(x) with unit scale (round to nearest even, saturating at +-448), n elements.
+ * spot_linear_fp8: as spot_linear with d_a [M, K] and d_wq [N, K] E4M3 bytes, y = d_w_scale[n] * acc + bias (bias bf16);
+ *   SPOT_EPI_BIAS / SPOT_EPI_BIAS_GELU write d_out [M, N] as E4M3 bytes, SPOT_EPI_GATE_RESIDUAL updates the fp32
+ *   residual.  K % 16 == 0, N % 32 == 0. */
+spot_status spot_quantize_weight_rows(const void *d_w_bf16, int64_t N, int64_t K, void *d_wq, float *d_scale, void *cuda_stream);
+spot_status spot_quantize_e4m3(spot_dtype dtype, const void *d_in, int64_t n, void *d_out, void *cuda_stream);
+spot_status spot_linear_fp8(spot_epilogue epi, const void *d_a, int64_t M, int64_t K, const void *d_wq, int64_t N,
+                            const float *d_w_scale, const void *d_bias, const float *d_gate, float *d_residual, void *d_out,
                             void *cuda_stream);
 
 /* The RoPE table the context built at spot_create (S5): copies cos and sin [S, d_h/2] fp32 to HOST. */

@@ -19,7 +19,8 @@ _lib: Optional[C.CDLL] = None
 SPOT_F32, SPOT_BF16 = 0, 1
 EPI_BIAS, EPI_BIAS_GELU, EPI_GATE_RESIDUAL = 0, 1, 2
 IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_2CTA, IMPL_TCGEN05_TMA = 0, 1, 2, 3, 4
-OPT_GEMM_IMPL, OPT_ATTN_IMPL, OPT_TIMING = 0, 1, 2
+OPT_GEMM_IMPL, OPT_ATTN_IMPL, OPT_TIMING, OPT_FP8 = 0, 1, 2, 3
+SPOT_E4M3 = 2     # storage type of the FP8 variant's activations / quantised weights (torch.float8_e4m3fn)
 STATUS_NAMES = ["SPOT_OK", "SPOT_ERR_NULL", "SPOT_ERR_SHAPE", "SPOT_ERR_DTYPE", "SPOT_ERR_ALIGN",
                 "SPOT_ERR_WORKSPACE", "SPOT_ERR_ARCH", "SPOT_ERR_CUDA", "SPOT_ERR_UNIMPLEMENTED"]
 
@@ -92,6 +93,11 @@ def load_library() -> C.CDLL:
                                 vp, sz, vp],
         "spot_dit_denoise_sde": [vp, i32, i32, vp, vp, vp, vp, i32, f32, i32, i32, vp, vp, sz, vp],
         "spot_sde_update": [vp, vp, vp, i32, f32, f32, f32, i32, i64, vp, vp, vp],
+        "spot_fp8_bytes": [vp, C.POINTER(sz)],
+        "spot_fp8_prepare": [vp, vp, sz, vp],
+        "spot_quantize_weight_rows": [vp, i64, i64, vp, vp, vp],
+        "spot_quantize_e4m3": [i32, vp, i64, vp, vp],
+        "spot_linear_fp8": [i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp, vp],
         "spot_explore_host": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_linear": [i32, i32, i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp],
         "spot_qkv_rope_linear": [vp, i32, i32, i64, vp, i64, vp, vp, vp, vp, vp, i32, f32, vp, vp],
@@ -129,6 +135,8 @@ def _dt(dtype: torch.dtype) -> int:
         return SPOT_F32
     if dtype == torch.bfloat16:
         return SPOT_BF16
+    if dtype == torch.float8_e4m3fn:
+        return SPOT_E4M3
     raise TypeError(f"unsupported dtype {dtype}")
 
 
@@ -191,6 +199,17 @@ class Context:
             self.close()
         except Exception:
             pass
+
+    def enable_fp8(self, on: bool = True) -> None:
+        """Low-precision exploration variant: quantise the block Linears once (E4M3 weights +
+        per-output-channel scales in a buffer this object keeps alive) and switch the context's block Linears."""
+        lib = load_library()
+        if on and getattr(self, "_fp8_buf", None) is None:
+            n = C.c_size_t()
+            _check(lib.spot_fp8_bytes(self.handle, C.byref(n)), "spot_fp8_bytes", self)
+            self._fp8_buf = torch.empty(int(n.value), dtype=torch.uint8, device="cuda")
+            _check(lib.spot_fp8_prepare(self.handle, _ptr(self._fp8_buf), self._fp8_buf.numel(), _stream()), "spot_fp8_prepare", self)
+        _check(lib.spot_set_option(self.handle, OPT_FP8, 1 if on else 0), "spot_set_option", self)
 
     def workspace(self, n_seqs: int, n_steps: int, cached: bool = False) -> torch.Tensor:
         n = spot_workspace_bytes(self, n_seqs, n_steps, cached)
@@ -407,6 +426,33 @@ def spot_qkv_rope_linear(a: torch.Tensor, w: torch.Tensor, bias: torch.Tensor, q
     _check(load_library().spot_qkv_rope_linear(_ptr(a), n_seqs, rps, K, _ptr(w), hidden, _ptr(bias), _ptr(q_gain), _ptr(k_gain),
                                                _ptr(cos), _ptr(sin), pos_off, eps, _ptr(out), _stream()), "spot_qkv_rope_linear")
     return out
+
+
+def spot_quantize_weight_rows(w: torch.Tensor):
+    """bf16 [N, K] -> (E4M3 [N, K], fp32 scale [N]) with s_n = max|W_n| / 448 (DESIGN.md section 13 reading Q2)."""
+    N, K = w.shape
+    wq = torch.empty((N, K), dtype=torch.float8_e4m3fn, device=w.device)
+    scale = torch.empty(N, dtype=torch.float32, device=w.device)
+    _check(load_library().spot_quantize_weight_rows(_ptr(w), N, K, _ptr(wq), _ptr(scale), _stream()), "spot_quantize_weight_rows")
+    return wq, scale
+
+
+def spot_quantize_e4m3(x: torch.Tensor) -> torch.Tensor:
+    """Unit-scale, saturating, round-to-nearest-even cast to E4M3 (reading Q3)."""
+    out = torch.empty(x.shape, dtype=torch.float8_e4m3fn, device=x.device)
+    _check(load_library().spot_quantize_e4m3(_dt(x.dtype), _ptr(x), x.numel(), _ptr(out), _stream()), "spot_quantize_e4m3")
+    return out
+
+
+def spot_linear_fp8(a: torch.Tensor, wq: torch.Tensor, w_scale: torch.Tensor, bias: torch.Tensor, epi: int = EPI_BIAS,
+                    gate: Optional[torch.Tensor] = None, residual: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """a [M, K] and wq [N, K] E4M3; EPI_BIAS / EPI_BIAS_GELU return E4M3 [M, N], EPI_GATE_RESIDUAL updates `residual` (fp32)."""
+    M, K = a.shape
+    N = wq.shape[0]
+    out = None if epi == EPI_GATE_RESIDUAL else torch.empty((M, N), dtype=torch.float8_e4m3fn, device=a.device)
+    _check(load_library().spot_linear_fp8(epi, _ptr(a), M, K, _ptr(wq), N, _ptr(w_scale), _ptr(bias), _ptr(gate), _ptr(residual),
+                                          _ptr(out), _stream()), "spot_linear_fp8")
+    return residual if epi == EPI_GATE_RESIDUAL else out
 
 
 def spot_ln_modulate(h: torch.Tensor, shift: torch.Tensor, scale: torch.Tensor, eps: float, dtype: torch.dtype) -> torch.Tensor:

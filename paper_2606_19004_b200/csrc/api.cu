@@ -28,6 +28,11 @@ struct spot_ctx {
   std::vector<cudaEvent_t> ev;   // event pool (pairs)
   size_t ev_used;
   unsigned long long gemm_launches;
+  // FP8 exploration variant: quantised copies of the four block Linears, in a caller-owned buffer
+  struct Fp8Linear { const uint8_t* w; const float* scale; };
+  struct Fp8Block { Fp8Linear lin[2][4]; };   // [stream][qkv, out, fc1, fc2]
+  std::vector<Fp8Block> fp8_blocks;
+  int fp8;                       // 1: block Linears run on E4M3 operands (SPOT_OPT_FP8; needs spot_fp8_prepare)
   int n_img() const { return cfg.grid_h * cfg.grid_w; }
   int seq() const { return cfg.n_txt + n_img(); }
 };
@@ -157,6 +162,8 @@ spot_status run_gemm(spot_ctx* c, Epilogue epi, GemmProblem* probs, int n, spot_
       c->ev_used += 2;
     }
   } else {
+    for (int i = 0; i < n; ++i)
+      if (probs[i].fp8) return SPOT_ERR_SHAPE;            // E4M3 operands exist on the tcgen05 path only
     for (int i = 0; i < n; ++i) LK(c, launch_gemm_simt(ta, dt, tout, epi, probs[i], st));
   }
   return SPOT_OK;
@@ -267,6 +274,7 @@ spot_status spot_create(const spot_config* cfg, const spot_weights* w, int max_s
   c->gemm_impl = c->attn_impl = 0;
   c->n_launches = c->gemm_launches = 0;
   c->timing = 0;
+  c->fp8 = 0;
   c->ev_used = 0;
   c->d_cos = c->d_sin = c->d_partials = c->d_partials2 = nullptr;
   int dev = 0;
@@ -315,6 +323,12 @@ spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
     return SPOT_OK;
   }
   if (value != 0 && value != 1) return SPOT_ERR_SHAPE;
+  if (opt == SPOT_OPT_FP8) {
+    if (value && (ctx->fp8_blocks.size() != ctx->blocks.size() || ctx->cfg.dtype != SPOT_BF16 || ctx->cfg.head_dim != 128))
+      return SPOT_ERR_SHAPE;                     // spot_fp8_prepare first; bf16 configs with d_h = 128 only
+    ctx->fp8 = value;
+    return SPOT_OK;
+  }
   if (opt == SPOT_OPT_GEMM_IMPL) ctx->gemm_impl = value;
   else if (opt == SPOT_OPT_TIMING) ctx->timing = value;
   else return SPOT_ERR_SHAPE;
@@ -394,13 +408,23 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
   StreamMaps sm[2] = {stream_maps(c, B, 0), stream_maps(c, B, 1)};
   GemmProblem pr[2];
   // (2) y = LN(h) (1 + scale1) + shift1 ; (3) qkv = y Wqkv^T + b
+  // FP8 variant: the activations feeding the four Linears are stored as E4M3 (same row maps: element = byte), the
+  // weights come from the quantised copies, accumulators are dequantised per output channel in the epilogue
+  const bool f8 = c->fp8 != 0 && dt == SPOT_BF16 && c->gemm_impl == 0 && g.head_dim == 128;
+  const spot_dtype adt = f8 ? SPOT_E4M3 : dt;            // storage type of LN output, attention output, MLP hidden
+  const spot_ctx::Fp8Block* fb = f8 ? &c->fp8_blocks[block] : nullptr;
+  auto use_fp8 = [&](GemmProblem& p, int s, int which) {
+    if (!f8) return;
+    p.fp8 = 1; p.W = fb->lin[s][which].w; p.w_scale = fb->lin[s][which].scale;
+  };
   LnProblem lp[2];
   for (int s = 0; s < 2; ++s) lp[s] = LnProblem{h[s], sm[s].rows, mod[s], mod[s] + D, ybuf, sm[s].y};
-  LK(c, launch_ln_modulate2(dt, lp, 2, D, g.ln_eps, st));   // image and text rows in one launch
+  LK(c, launch_ln_modulate2(adt, lp, 2, D, g.ln_eps, st));   // image and text rows in one launch
   for (int s = 0; s < 2; ++s) {
     memset(&pr[s], 0, sizeof(GemmProblem));
     pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].qkv_w; pr[s].bias = bw.s[s].qkv_b;
     pr[s].M = sm[s].rows; pr[s].N = 3 * D; pr[s].K = D; pr[s].out = big; pr[s].out_map = sm[s].qkv;
+    use_fp8(pr[s], s, 0);
   }
   // (4)-(5) QK-RMSNorm + RoPE: fused into the epilogue of the QKV projection (v3 kernel, d_h = 128), else K4
   bool fuse_qk = dt == SPOT_BF16 && c->gemm_impl == 0 && g.head_dim == 128;
@@ -409,6 +433,7 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
     pr[s].pos_off = s == 0 ? g.n_txt : 0; pr[s].rms_eps = g.rms_eps;
     if (pr[s].M > 0 && !(tcgen05_gemm_supported(pr[s]) && tcgen05_v3_qkv_rope_supported(pr[s]))) fuse_qk = false;
   }
+  if (f8 && !fuse_qk) return SPOT_ERR_SHAPE;             // the FP8 QKV projection exists only with the fused bf16 q/k/v epilogue
   spot_status rs = run_gemm(c, fuse_qk ? EPI_QKV_ROPE : EPI_BIAS, pr, 2, dt, dt, st);
   if (rs != SPOT_OK) return rs;
   if (!fuse_qk)
@@ -417,7 +442,7 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
   // (6) joint attention -> ybuf [B,S,D]
   if (dt == SPOT_BF16 && c->attn_impl != 1 && tcgen05_attn_supported(S, g.n_heads, g.head_dim)) {
     if (c->attn_impl == 2) LK(c, launch_attn_tcgen05(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st));
-    else LK(c, launch_attn_tcgen05_v3(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st));
+    else LK(c, launch_attn_tcgen05_v3(big, ybuf, B, S, g.n_heads, g.head_dim, c->num_sms, st, f8));
   }
   else
     LK(c, launch_attn_simt(dt, big, ybuf, B, S, g.n_heads, g.head_dim, st));
@@ -427,16 +452,18 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
     memset(&pr[s], 0, sizeof(GemmProblem));
     pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].out_w; pr[s].bias = bw.s[s].out_b;
     pr[s].M = sm[s].rows; pr[s].N = D; pr[s].K = D; pr[s].gate = mod[s] + 2 * D; pr[s].resid = h[s]; pr[s].resid_map = sm[s].h;
+    use_fp8(pr[s], s, 1);
   }
   rs = run_gemm(c, EPI_GATE_RES, pr, ns, dt, SPOT_F32, st);
   if (rs != SPOT_OK) return rs;
   // (8) y2 = LN(h)(1 + scale2) + shift2 ; u = GELU(y2 W1^T + b) ; h += gate2 * (u W2^T + b)
   for (int s = 0; s < ns; ++s) lp[s] = LnProblem{h[s], sm[s].rows, mod[s] + 3 * D, mod[s] + 4 * D, ybuf, sm[s].y};
-  LK(c, launch_ln_modulate2(dt, lp, ns, D, g.ln_eps, st));
+  LK(c, launch_ln_modulate2(adt, lp, ns, D, g.ln_eps, st));
   for (int s = 0; s < ns; ++s) {
     memset(&pr[s], 0, sizeof(GemmProblem));
     pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].fc1_w; pr[s].bias = bw.s[s].fc1_b;
     pr[s].M = sm[s].rows; pr[s].N = F; pr[s].K = D; pr[s].out = big; pr[s].out_map = sm[s].wide;
+    use_fp8(pr[s], s, 2);
   }
   rs = run_gemm(c, EPI_BIAS_GELU, pr, ns, dt, dt, st);
   if (rs != SPOT_OK) return rs;
@@ -444,6 +471,7 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
     memset(&pr[s], 0, sizeof(GemmProblem));
     pr[s].A = big; pr[s].a_map = sm[s].wide; pr[s].W = bw.s[s].fc2_w; pr[s].bias = bw.s[s].fc2_b;
     pr[s].M = sm[s].rows; pr[s].N = D; pr[s].K = F; pr[s].gate = mod[s] + 5 * D; pr[s].resid = h[s]; pr[s].resid_map = sm[s].h;
+    use_fp8(pr[s], s, 3);
   }
   return run_gemm(c, EPI_GATE_RES, pr, ns, dt, SPOT_F32, st);
 }
@@ -843,6 +871,60 @@ spot_status spot_dit_denoise_sde(spot_ctx* ctx, int n_prompts, int seeds_per_pro
                       nullptr, nullptr, st, &run);
 }
 
+// ---- FP8 exploration variant ----------------------------------------------------------------
+// [N, K] of Linear `which` = (qkv, out, fc1, fc2)
+static void fp8_shape(const spot_config& g, int which, long long* N, long long* K) {
+  const long long D = g.hidden, F = g.mlp_hidden;
+  switch (which) {
+    case 0: *N = 3 * D; *K = D; break;
+    case 1: *N = D; *K = D; break;
+    case 2: *N = F; *K = D; break;
+    default: *N = D; *K = F; break;
+  }
+}
+
+spot_status spot_fp8_bytes(const spot_ctx* ctx, size_t* bytes) {
+  if (!ctx || !bytes) return SPOT_ERR_NULL;
+  if (ctx->cfg.dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  size_t per_stream = 0;
+  for (int w = 0; w < 4; ++w) {
+    long long N, K;
+    fp8_shape(ctx->cfg, w, &N, &K);
+    per_stream += align_up((size_t)N * K) + align_up((size_t)N * 4);
+  }
+  *bytes = per_stream * 2 * (size_t)ctx->cfg.n_blocks;
+  return SPOT_OK;
+}
+
+spot_status spot_fp8_prepare(spot_ctx* ctx, void* d_buffer, size_t bytes, void* cuda_stream) {
+  if (!ctx || !d_buffer) return SPOT_ERR_NULL;
+  if (ctx->cfg.dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  if (ctx->cfg.hidden % 16 || ctx->cfg.mlp_hidden % 16) return SPOT_ERR_SHAPE;
+  if (!aligned16(d_buffer)) return SPOT_ERR_ALIGN;
+  size_t need = 0;
+  spot_status s = spot_fp8_bytes(ctx, &need);
+  if (s != SPOT_OK) return s;
+  if (bytes < need) return SPOT_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  uint8_t* p = (uint8_t*)d_buffer;
+  ctx->fp8 = 0;
+  ctx->fp8_blocks.assign(ctx->blocks.size(), spot_ctx::Fp8Block());
+  for (size_t b = 0; b < ctx->blocks.size(); ++b)
+    for (int sgm = 0; sgm < 2; ++sgm) {
+      const spot_stream_weights& sw = ctx->blocks[b].s[sgm];
+      const void* src[4] = {sw.qkv_w, sw.out_w, sw.fc1_w, sw.fc2_w};
+      for (int w = 0; w < 4; ++w) {
+        long long N, K;
+        fp8_shape(ctx->cfg, w, &N, &K);
+        uint8_t* wq = p; p += align_up((size_t)N * K);
+        float* sc = (float*)p; p += align_up((size_t)N * 4);
+        LK(ctx, launch_quantize_weight_rows(src[w], N, (int)K, wq, sc, st));
+        ctx->fp8_blocks[b].lin[sgm][w] = spot_ctx::Fp8Linear{wq, sc};
+      }
+    }
+  return SPOT_OK;
+}
+
 spot_status spot_explore_host(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, const uint64_t* h_seeds,
                               const void* h_text_emb, const float* h_timesteps, int n_steps, const float* h_probe,
                               int k_select, float* h_latents, float* h_rewards, float* h_stats, int32_t* h_top,
@@ -957,7 +1039,7 @@ spot_status spot_qkv_rope_linear(const void* d_a, int n_seqs, int rows_per_seq, 
 
 spot_status spot_ln_modulate(spot_dtype dtype, const float* d_h, int64_t M, int64_t D, const float* d_shift,
                              const float* d_scale, float eps, void* d_out, void* cuda_stream) {
-  if (dtype != SPOT_F32 && dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  if (dtype != SPOT_F32 && dtype != SPOT_BF16 && dtype != SPOT_E4M3) return SPOT_ERR_DTYPE;
   if (M < 0 || D <= 0 || D % 128 || M > 0x7fffffff) return SPOT_ERR_SHAPE;
   if (M == 0) return SPOT_OK;
   if (!d_h || !d_shift || !d_scale || !d_out) return SPOT_ERR_NULL;
@@ -1035,6 +1117,49 @@ spot_status spot_sde_update(float* d_x, const float* d_v, const uint64_t* d_seed
   }
   return launch_sde_update(d_x, d_v, d_seeds, kSdeStreamBase + (uint32_t)step, cx, cv, cn, n_seqs, elems, nullptr, d_partials,
                            nullptr, d_logp, 1, st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
+spot_status spot_quantize_weight_rows(const void* d_w_bf16, int64_t N, int64_t K, void* d_wq, float* d_scale, void* cuda_stream) {
+  if (N < 0 || K <= 0 || K % 8 || K > 0x7fffffff) return SPOT_ERR_SHAPE;
+  if (N == 0) return SPOT_OK;
+  if (!d_w_bf16 || !d_wq || !d_scale) return SPOT_ERR_NULL;
+  if (!aligned16(d_w_bf16) || !aligned16(d_wq)) return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  return launch_quantize_weight_rows(d_w_bf16, N, (int)K, d_wq, d_scale, (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK
+                                                                                                                 : SPOT_ERR_CUDA;
+}
+
+spot_status spot_quantize_e4m3(spot_dtype dtype, const void* d_in, int64_t n, void* d_out, void* cuda_stream) {
+  if (dtype != SPOT_F32 && dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  if (n < 0) return SPOT_ERR_SHAPE;
+  if (n == 0) return SPOT_OK;
+  if (!d_in || !d_out) return SPOT_ERR_NULL;
+  if (!aligned16(d_in) || !aligned16(d_out)) return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  return launch_quantize_e4m3(dtype, d_in, n, d_out, (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
+spot_status spot_linear_fp8(spot_epilogue epi, const void* d_a, int64_t M, int64_t K, const void* d_wq, int64_t N,
+                            const float* d_w_scale, const void* d_bias, const float* d_gate, float* d_residual, void* d_out,
+                            void* cuda_stream) {
+  if (M < 0 || N <= 0 || K <= 0 || M > 0x7fffffff || N > 0x7fffffff || K > 0x7fffffff) return SPOT_ERR_SHAPE;
+  if (M == 0) return SPOT_OK;
+  if (!d_a || !d_wq || !d_w_scale || !d_bias) return SPOT_ERR_NULL;
+  const bool gate_res = epi == SPOT_EPI_GATE_RESIDUAL;
+  if (gate_res ? (!d_gate || !d_residual) : !d_out) return SPOT_ERR_NULL;
+  if (!aligned16(d_a) || !aligned16(d_wq) || !aligned16(d_w_scale) || !aligned16(d_bias) || !aligned16(d_out) ||
+      !aligned16(d_residual) || !aligned16(d_gate))
+    return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  GemmProblem p;
+  memset(&p, 0, sizeof(p));
+  p.A = d_a; p.a_map = plain_rows((int)M, K); p.W = d_wq; p.bias = d_bias; p.fp8 = 1; p.w_scale = d_w_scale;
+  p.M = (int)M; p.N = (int)N; p.K = (int)K;
+  if (gate_res) { p.gate = d_gate; p.resid = d_residual; p.resid_map = plain_rows((int)M, N); }
+  else { p.out = d_out; p.out_map = plain_rows((int)M, N); }
+  if (!tcgen05_gemm_supported(p)) return SPOT_ERR_SHAPE;
+  const Epilogue e = epi == SPOT_EPI_BIAS ? EPI_BIAS : (epi == SPOT_EPI_BIAS_GELU ? EPI_BIAS_GELU : EPI_GATE_RES);
+  return launch_gemm_tcgen05_v3(e, &p, 1, sm_count(), (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
 }
 
 }  // extern "C"

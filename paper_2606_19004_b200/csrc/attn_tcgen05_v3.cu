@@ -20,6 +20,7 @@
 //     waits for that read-out (o_free).
 // TMEM columns: [0,64) S_A0, [64,128) S_A1, [128,192) S_B0, [192,256) S_B1, [256,384) O_A, [384,512) O_B.
 // Tensor-pipe + MUFU bound: 4 S^2 d_h FLOP and S^2 ex2 per (sequence, head).
+#include <cuda_fp8.h>
 #include <string.h>
 
 #include "kernels.h"
@@ -55,8 +56,10 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
   return *reinterpret_cast<uint32_t*>(&v);
 }
 
+// OUT8: O is stored as E4M3 bytes (unit scale, saturating) - the A operand of the FP8 out-projection.
+template <bool OUT8>
 __global__ void __launch_bounds__(ATT_THREADS, 1)
-attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restrict__ out, int S, int H, int n_items,
+attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, void* __restrict__ out_v, int S, int H, int n_items,
                        float scale_log2) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw_addr = ptx::smem_u32(smem_raw);
@@ -296,7 +299,7 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
       const float inv = 1.f / l;
       const int qrow = q0 + t * BQ + row;
       const bool row_ok = qrow < S;
-      bf16* orow = out + ((long long)seq * S + qrow) * (long long)(H * DH) + head * DH;
+      const long long oidx = ((long long)seq * S + qrow) * (long long)(H * DH) + head * DH;
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         uint32_t ov[32];
@@ -308,14 +311,33 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
           if (lane == 0) ptx::mbar_arrive(o_free(t));
         }
         if (row_ok) {
+          if (OUT8) {
+            uint8_t* orow = reinterpret_cast<uint8_t*>(out_v) + oidx;
 #pragma unroll
-          for (int g4 = 0; g4 < 4; ++g4) {
-            uint4 pkt;
-            pkt.x = pack_bf16(__uint_as_float(ov[g4 * 8]) * inv, __uint_as_float(ov[g4 * 8 + 1]) * inv);
-            pkt.y = pack_bf16(__uint_as_float(ov[g4 * 8 + 2]) * inv, __uint_as_float(ov[g4 * 8 + 3]) * inv);
-            pkt.z = pack_bf16(__uint_as_float(ov[g4 * 8 + 4]) * inv, __uint_as_float(ov[g4 * 8 + 5]) * inv);
-            pkt.w = pack_bf16(__uint_as_float(ov[g4 * 8 + 6]) * inv, __uint_as_float(ov[g4 * 8 + 7]) * inv);
-            *reinterpret_cast<uint4*>(orow + c * 32 + g4 * 8) = pkt;
+            for (int g4 = 0; g4 < 2; ++g4) {
+              uint32_t w4[4];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                const int e = g4 * 16 + u * 4;
+                const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(__uint_as_float(ov[e]) * inv, __uint_as_float(ov[e + 1]) * inv),
+                                                             __NV_SATFINITE, __NV_E4M3);
+                const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(__uint_as_float(ov[e + 2]) * inv, __uint_as_float(ov[e + 3]) * inv),
+                                                             __NV_SATFINITE, __NV_E4M3);
+                w4[u] = lo | (hi << 16);
+              }
+              *reinterpret_cast<uint4*>(orow + c * 32 + g4 * 16) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+            }
+          } else {
+            bf16* orow = reinterpret_cast<bf16*>(out_v) + oidx;
+#pragma unroll
+            for (int g4 = 0; g4 < 4; ++g4) {
+              uint4 pkt;
+              pkt.x = pack_bf16(__uint_as_float(ov[g4 * 8]) * inv, __uint_as_float(ov[g4 * 8 + 1]) * inv);
+              pkt.y = pack_bf16(__uint_as_float(ov[g4 * 8 + 2]) * inv, __uint_as_float(ov[g4 * 8 + 3]) * inv);
+              pkt.z = pack_bf16(__uint_as_float(ov[g4 * 8 + 4]) * inv, __uint_as_float(ov[g4 * 8 + 5]) * inv);
+              pkt.w = pack_bf16(__uint_as_float(ov[g4 * 8 + 6]) * inv, __uint_as_float(ov[g4 * 8 + 7]) * inv);
+              *reinterpret_cast<uint4*>(orow + c * 32 + g4 * 8) = pkt;
+            }
           }
         }
       }
@@ -329,7 +351,8 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, bf16* __restr
 
 }  // namespace
 
-cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st) {
+cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st,
+                                   bool out_e4m3) {
   if (dh != DH) return cudaErrorInvalidValue;
   if (B <= 0) return cudaSuccess;
   CUtensorMap tm;
@@ -340,13 +363,15 @@ cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int
   SPOT_CUDA_TRY(spot_make_tmap_bf16(&tm, qkv, 3, dims, strides, box));
   static bool attr_set = false;
   if (!attr_set) {
-    SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_tcgen05_v3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ATT_SMEM));
+    SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_tcgen05_v3_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ATT_SMEM));
+    SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_tcgen05_v3_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ATT_SMEM));
     attr_set = true;
   }
   const long long items = (long long)((S + QT * BQ - 1) / (QT * BQ)) * H * B;
   if (items > 0x7fffffffLL / 128) return cudaErrorInvalidValue;
   const int grid = (int)(items < num_sms ? items : num_sms);       // persistent: one CTA per SM walks the item list
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)DH);
-  attn_tcgen05_v3_kernel<<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, (bf16*)out, S, H, (int)items, scale_log2);
+  if (out_e4m3) attn_tcgen05_v3_kernel<true><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, out, S, H, (int)items, scale_log2);
+  else attn_tcgen05_v3_kernel<false><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, out, S, H, (int)items, scale_log2);
   return cudaGetLastError();
 }

@@ -47,6 +47,11 @@ struct GemmProblem {
   const float* sin_t;
   int pos_off;
   float rms_eps;
+  // FP8 variant (tcgen05 v3 kernel only): A and W hold E4M3 bytes (a_map in elements = bytes),
+  // w_scale [N] fp32 = per-output-channel dequantisation scale applied to the accumulator before the bias;
+  // EPI_BIAS / EPI_BIAS_GELU then write E4M3 (out_map in bytes), EPI_QKV_ROPE bf16, EPI_GATE_RES the fp32 residual
+  int fp8;
+  const float* w_scale;
 };
 
 __device__ __forceinline__ float to_f32(float v) { return v; }

@@ -1,6 +1,7 @@
 // elementwise.cu - the HBM-bound kernels: K3 ln_modulate, K4 qk_norm_rope, K6 euler_update(+reward),
 // K7 time embedding / skinny Linear, K8 seed selection, and small plumbing kernels.
 // Readings S4-S12 of DESIGN.md; paper passages are cited at each kernel.
+#include <cuda_fp8.h>
 #include <string.h>
 
 #include "kernels.h"
@@ -119,6 +120,10 @@ __global__ void __launch_bounds__(256) ln_modulate_kernel(const LnProblem p0, co
     float y3 = (v[i].w - mean) * rstd * (1.f + sc.w) + sh.w;
     if constexpr (sizeof(TO) == 4) {
       *reinterpret_cast<float4*>(dst + col) = make_float4(y0, y1, y2, y3);
+    } else if constexpr (sizeof(TO) == 1) {               // E4M3, unit scale, saturating (DESIGN.md section 13 reading Q3)
+      const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(y0, y1), __NV_SATFINITE, __NV_E4M3);
+      const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(y2, y3), __NV_SATFINITE, __NV_E4M3);
+      *reinterpret_cast<uint32_t*>(dst + col) = lo | (hi << 16);
     } else {
       __nv_bfloat162 p0 = __floats2bfloat162_rn(y0, y1), p1 = __floats2bfloat162_rn(y2, y3);
       uint2 pk = make_uint2(*reinterpret_cast<uint32_t*>(&p0), *reinterpret_cast<uint32_t*>(&p1));
@@ -370,6 +375,7 @@ cudaError_t launch_ln_modulate2(spot_dtype odt, const LnProblem* probs, int n_pr
   if (p0.M < 0 || p1.M < 0) return cudaErrorInvalidValue;
   if (p0.M == 0) { p0 = p1; p1.M = 0; }
   if (p0.M == 0) return cudaSuccess;
+  if (odt == SPOT_E4M3) return ln_dispatch<uint8_t>(p0, p1, D, eps, st);
   return odt == SPOT_F32 ? ln_dispatch<float>(p0, p1, D, eps, st) : ln_dispatch<bf16>(p0, p1, D, eps, st);
 }
 

@@ -247,6 +247,11 @@ cudaError_t spot_make_tmap_bf16(CUtensorMap* out, const void* base, int rank, co
   return make_tmap(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, base, rank, dims, strides_bytes, box);
 }
 
+cudaError_t spot_make_tmap_u8(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
+                              const uint64_t* strides_bytes, const uint32_t* box) {
+  return make_tmap(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, base, rank, dims, strides_bytes, box);
+}
+
 cudaError_t spot_make_tmap_f32(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
                                const uint64_t* strides_bytes, const uint32_t* box) {
   return make_tmap(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, base, rank, dims, strides_bytes, box);
@@ -254,13 +259,15 @@ cudaError_t spot_make_tmap_f32(CUtensorMap* out, const void* base, int rank, con
 
 bool tcgen05_gemm_supported(const GemmProblem& p) {
   if (p.M <= 0 || p.N <= 0 || p.K <= 0) return false;
-  if (p.K % 8 || p.N % 32) return false;
+  const int es = p.fp8 ? 1 : 2;                     // bytes per operand element
+  if ((p.K * es) % 16 || p.N % 32) return false;
+  if (p.fp8 && (!p.w_scale || reinterpret_cast<uintptr_t>(p.w_scale) % 16)) return false;
   const RowMap& a = p.a_map;
   if (a.rows_per_seq <= 0 || p.M % a.rows_per_seq) return false;
-  if ((a.ld * 2) % 16 || (a.offset * 2) % 16 || (a.seq_stride * 2) % 16) return false;
+  if ((a.ld * es) % 16 || (a.offset * es) % 16 || (a.seq_stride * es) % 16) return false;
   if (reinterpret_cast<uintptr_t>(p.A) % 16 || reinterpret_cast<uintptr_t>(p.W) % 16) return false;
-  if (p.out && (p.out_map.rows_per_seq != a.rows_per_seq || p.out_map.ld % 8 || p.out_map.offset % 8 ||
-                p.out_map.seq_stride % 8 || reinterpret_cast<uintptr_t>(p.out) % 16))
+  if (p.out && (p.out_map.rows_per_seq != a.rows_per_seq || p.out_map.ld % 16 || p.out_map.offset % 16 ||
+                p.out_map.seq_stride % 16 || reinterpret_cast<uintptr_t>(p.out) % 16))
     return false;
   if (p.resid && (p.resid_map.rows_per_seq != a.rows_per_seq || p.resid_map.ld % 4 || p.resid_map.offset % 4 ||
                   p.resid_map.seq_stride % 4 || reinterpret_cast<uintptr_t>(p.resid) % 16))

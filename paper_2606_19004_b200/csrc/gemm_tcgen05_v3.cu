@@ -16,6 +16,7 @@
 //     thread owns one token row of the accumulator, so the per-head RMS is thread-local: pass 1 over TMEM sums the
 //     squares of (acc + bias), pass 2 scales by rsqrt(mean + eps) * gain, rotates pairs (2i, 2i+1) by the table
 //     angle of the token's joint position and stores bf16.  v heads take the plain bias path.
+#include <cuda_fp8.h>
 #include <stdlib.h>
 #include <string.h>
 
@@ -39,6 +40,7 @@ struct V3Problem {
   int group_m;              // rasterisation: tiles run n-major inside groups of group_m M-tiles (L2 residency)
   const bf16* bias;
   const float* gate;
+  const float* w_scale;     // FP8 variant: per-output-channel dequantisation scale
   // EPI_QKV_ROPE
   const bf16* q_gain;
   const bf16* k_gain;
@@ -97,6 +99,39 @@ __device__ __forceinline__ void add_bias32(const uint32_t (&v)[32], const bf16* 
     for (int j = 0; j < 8; ++j) y[g * 8 + j] = __uint_as_float(v[g * 8 + j]) + __bfloat162float(bb[j]);
   }
 }
+// FP8 variant: y = acc * w_scale[n] + bias[n]  (per-output-channel dequantisation, DESIGN.md section 13 reading Q4)
+__device__ __forceinline__ void scale_bias32(const uint32_t (&v)[32], const float* sp, const bf16* bp, float (&y)[32]) {
+  const uint4* p4 = reinterpret_cast<const uint4*>(bp);
+  const float4* s4 = reinterpret_cast<const float4*>(sp);
+#pragma unroll
+  for (int g = 0; g < 4; ++g) {
+    uint4 braw = __ldg(p4 + g);
+    const bf16* bb = reinterpret_cast<const bf16*>(&braw);
+    const float4 sa = __ldg(s4 + 2 * g), sb = __ldg(s4 + 2 * g + 1);
+    const float sc[8] = {sa.x, sa.y, sa.z, sa.w, sb.x, sb.y, sb.z, sb.w};
+#pragma unroll
+    for (int j = 0; j < 8; ++j) y[g * 8 + j] = fmaf(__uint_as_float(v[g * 8 + j]), sc[j], __bfloat162float(bb[j]));
+  }
+}
+template <bool FP8>
+__device__ __forceinline__ void acc_to_y(const uint32_t (&v)[32], const float* sp, const bf16* bp, float (&y)[32]) {
+  if (FP8) scale_bias32(v, sp, bp, y);
+  else add_bias32(v, bp, y);
+}
+__device__ __forceinline__ uint32_t pack4_e4m3(float a, float b, float c, float d) {
+  const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(a, b), __NV_SATFINITE, __NV_E4M3);
+  const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(c, d), __NV_SATFINITE, __NV_E4M3);
+  return lo | (hi << 16);
+}
+// 32 fp32 values -> 32 bytes of E4M3 = 16-byte chunks c0, c0+1 of this thread's 128-byte staging row
+__device__ __forceinline__ void stage_e4m3_32(uint32_t row_addr, int sw, int c0, const float (&y)[32]) {
+#pragma unroll
+  for (int g = 0; g < 2; ++g)
+    st_shared_v4(row_addr + (uint32_t)(((c0 + g) ^ sw) << 4), pack4_e4m3(y[16 * g], y[16 * g + 1], y[16 * g + 2], y[16 * g + 3]),
+                 pack4_e4m3(y[16 * g + 4], y[16 * g + 5], y[16 * g + 6], y[16 * g + 7]),
+                 pack4_e4m3(y[16 * g + 8], y[16 * g + 9], y[16 * g + 10], y[16 * g + 11]),
+                 pack4_e4m3(y[16 * g + 12], y[16 * g + 13], y[16 * g + 14], y[16 * g + 15]));
+}
 // 32 fp32 values -> 64 bytes of bf16 = 16-byte chunks c0 .. c0+3 of this thread's 128-byte staging row
 __device__ __forceinline__ void stage_bf16_32(uint32_t row_addr, int sw, int c0, const float (&y)[32]) {
 #pragma unroll
@@ -105,7 +140,10 @@ __device__ __forceinline__ void stage_bf16_32(uint32_t row_addr, int sw, int c0,
                  pack2(y[8 * g + 4], y[8 * g + 5]), pack2(y[8 * g + 6], y[8 * g + 7]));
 }
 
-template <int EPI>
+// FP8 = true: A and W are E4M3 (kind::f8f6f4, K = 32 per MMA; a 128-byte swizzled row then holds 128 elements, so a
+// stage is a 128-element K block and everything else - ring, descriptors, 32-byte advance per MMA - is unchanged);
+// accumulators are dequantised per output channel; EPI_BIAS / EPI_BIAS_GELU then store E4M3 (the next Linear's operand).
+template <int EPI, bool FP8>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
 gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmW0,
                        const __grid_constant__ CUtensorMap tmO0, const __grid_constant__ CUtensorMap tmA1,
@@ -159,8 +197,8 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
           ptx::mbar_wait(empty_bar(stage), phase ^ 1);
           const uint32_t leader_full = ptx::map_to_cta(full_bar(stage), 0);
           const uint32_t sa = smem_base + stage * STAGE_BYTES;
-          ptx::tma_load_3d_2cta(sa, mA, leader_full, kb * BLOCK_K, r0, seq);
-          ptx::tma_load_2d_2cta(sa + A_BYTES, mW, leader_full, kb * BLOCK_K, n0);
+          ptx::tma_load_3d_2cta(sa, mA, leader_full, kb * (FP8 ? 2 * BLOCK_K : BLOCK_K), r0, seq);
+          ptx::tma_load_2d_2cta(sa + A_BYTES, mW, leader_full, kb * (FP8 ? 2 * BLOCK_K : BLOCK_K), n0);
           // only the leader CTA arms its barrier, for the bytes of BOTH CTAs (see gemm_tcgen05_2cta.cu)
           if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
@@ -173,7 +211,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
     //  compiler fall back to per-lane ELECT / BRA.U.ANY loops around every UTCHMMA)
     if (ptx::elect_one()) {
       const int my_tiles = rank == 0 ? P.total_tiles : 0;
-      constexpr uint32_t idesc = ptx::make_idesc_bf16(PAIR_M, BLOCK_N, 0, 0);
+      constexpr uint32_t idesc = FP8 ? ptx::make_idesc_e4m3(PAIR_M, BLOCK_N) : ptx::make_idesc_bf16(PAIR_M, BLOCK_N, 0, 0);
       int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t acc_phase = 0;
       for (int t = pair; t < my_tiles; t += n_pairs) {
         const TileCoord c = decode_tile(P, t);
@@ -189,7 +227,8 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
           for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
             const uint64_t da = ptx::make_smem_desc(sa + k * UMMA_K * 2, 16, 1024);
             const uint64_t db = ptx::make_smem_desc(sb + k * UMMA_K * 2, 16, 1024);
-            ptx::mma_f16_ss_2cta(d_tmem, da, db, idesc, (kb | k) ? 1u : 0u);
+            if (FP8) ptx::mma_f8_ss_2cta(d_tmem, da, db, idesc, (kb | k) ? 1u : 0u);
+            else ptx::mma_f16_ss_2cta(d_tmem, da, db, idesc, (kb | k) ? 1u : 0u);
           }
           ptx::mma_commit_2cta(empty_bar(stage));
           if (kb == k_blocks - 1) ptx::mma_commit_2cta(tfull_bar(acc));
@@ -248,7 +287,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
           const uint32_t ra = acquire();
           ptx::tmem_ld_wait();
           float y[32];
-          add_bias32(v, q.bias + n0, y);
+          acc_to_y<FP8>(v, q.w_scale + n0, q.bias + n0, y);
           const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
 #pragma unroll
           for (int g = 0; g < 8; ++g) {
@@ -282,12 +321,36 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
                 ptx::tmem_ld_32x32(taddr0 + hh * 128 + c4 * 32, v);
                 ptx::tmem_ld_wait();
                 float y[32];
-                add_bias32(v, q.bias + hcol0 + c4 * 32, y);
+                acc_to_y<FP8>(v, q.w_scale + hcol0 + c4 * 32, q.bias + hcol0 + c4 * 32, y);
 #pragma unroll
                 for (int j = 0; j < 32; ++j) ss = fmaf(y[j], y[j], ss);
               }
               rinv = rsqrtf(ss * (1.f / 128.f) + q.rms_eps);
             }
+          }
+          if (FP8 && EPI != EPI_QKV_ROPE) {                  // E4M3 output: 128 columns = 128 bytes per row, one send per half tile
+            const uint32_t ra = acquire();
+#pragma unroll 1
+            for (int c4 = 0; c4 < 4; ++c4) {
+              const int n0 = hcol0 + c4 * 32;
+              float y[32];
+              if (n0 < q.N) {
+                uint32_t v[32];
+                ptx::tmem_ld_32x32(taddr0 + hh * 128 + c4 * 32, v);
+                ptx::tmem_ld_wait();
+                scale_bias32(v, q.w_scale + n0, q.bias + n0, y);
+                if (EPI == EPI_BIAS_GELU) {
+#pragma unroll
+                  for (int j = 0; j < 32; ++j) y[j] = gelu_tanh_fast(y[j]);
+                }
+              } else {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) y[j] = 0.f;
+              }
+              stage_e4m3_32(ra, sw, c4 * 2, y);
+            }
+            send(hcol0);
+            continue;
           }
 #pragma unroll 1
           for (int c2 = 0; c2 < 2; ++c2) {                    // 64 columns = 128 bytes of bf16 per row
@@ -302,8 +365,8 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {
               float y[32];
-              if (hf == 0) add_bias32(v0, q.bias + n0, y);
-              else if (second) add_bias32(v1, q.bias + n0 + 32, y);
+              if (hf == 0) acc_to_y<FP8>(v0, q.w_scale + n0, q.bias + n0, y);
+              else if (second) acc_to_y<FP8>(v1, q.w_scale + n0 + 32, q.bias + n0 + 32, y);
               else {
 #pragma unroll
                 for (int j = 0; j < 32; ++j) y[j] = 0.f;
@@ -366,9 +429,15 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
   CUtensorMap tm[6];
   memset(tm, 0, sizeof(tm));
   int tiles = 0, np = 0;
+  bool fp8 = false;
   for (int i = 0; i < n_probs; ++i) {
     const GemmProblem& g = probs[i];
     if (g.M <= 0) continue;
+    if (np > 0 && (g.fp8 != 0) != fp8) return cudaErrorInvalidValue;   // both problems of a launch share the operand type
+    fp8 = g.fp8 != 0;
+    const int es = fp8 ? 1 : 2;                     // bytes per operand element
+    const int bk = fp8 ? 2 * BLOCK_K : BLOCK_K;     // operand elements per 128-byte K block
+    const bool out8 = fp8 && (epi == EPI_BIAS || epi == EPI_BIAS_GELU);
     if (!tcgen05_gemm_supported(g)) return cudaErrorInvalidValue;
     if ((epi == EPI_GATE_RES) != (g.resid != nullptr)) return cudaErrorInvalidValue;
     if (epi != EPI_GATE_RES && !g.out) return cudaErrorInvalidValue;
@@ -380,7 +449,7 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
     q.m_tiles = nseq * q.tiles_per_seq;
     q.n_tiles = (g.N + BLOCK_N - 1) / BLOCK_N;
     q.N = g.N;
-    q.k_blocks = (g.K + BLOCK_K - 1) / BLOCK_K;
+    q.k_blocks = (g.K + bk - 1) / bk;
     q.tile_start = tiles;
     {
       // Rasterisation: tiles of one group sweep all N for group_m M-tiles, so a wave of 74 pair tiles touches
@@ -392,7 +461,7 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
       if (forced < 0) { const char* e = getenv("SPOT_GEMM_GROUP_M"); forced = e ? atoi(e) : 0; }
       int gm = 2;
       if (q.n_tiles >= 24) {
-        gm = (int)(25.0e6 / (2.0 * PAIR_M * (double)g.K));         // A panel of a group ~25 MB
+        gm = (int)(25.0e6 / ((double)es * PAIR_M * (double)g.K));  // A panel of a group ~25 MB
         if (gm > 16) gm = 16;
         if (gm < 2) gm = 2;
       }
@@ -400,24 +469,35 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
     }
     q.bias = (const bf16*)g.bias;
     q.gate = g.gate;
+    q.w_scale = g.w_scale;
     q.q_gain = (const bf16*)g.q_gain; q.k_gain = (const bf16*)g.k_gain;
     q.cos_t = g.cos_t; q.sin_t = g.sin_t; q.pos_off = g.pos_off; q.hidden = g.N / 3; q.rms_eps = g.rms_eps;
     tiles += q.m_tiles * q.n_tiles;
     const uint64_t adims[3] = {(uint64_t)g.K, (uint64_t)rps, (uint64_t)nseq};
-    const uint64_t astr[2] = {(uint64_t)g.a_map.ld * 2,
-                              (uint64_t)(nseq > 1 ? g.a_map.seq_stride : g.a_map.ld * (long long)rps) * 2};
-    const uint32_t abox[3] = {BLOCK_K, BLOCK_M, 1};
-    SPOT_CUDA_TRY(spot_make_tmap_bf16(&tm[3 * np], (const bf16*)g.A + g.a_map.offset, 3, adims, astr, abox));
+    const uint64_t astr[2] = {(uint64_t)g.a_map.ld * es,
+                              (uint64_t)(nseq > 1 ? g.a_map.seq_stride : g.a_map.ld * (long long)rps) * es};
+    const uint32_t abox[3] = {(uint32_t)bk, BLOCK_M, 1};
     const uint64_t wdims[2] = {(uint64_t)g.K, (uint64_t)g.N};
-    const uint64_t wstr[1] = {(uint64_t)g.K * 2};
-    const uint32_t wbox[2] = {BLOCK_K, HALF_N};
-    SPOT_CUDA_TRY(spot_make_tmap_bf16(&tm[3 * np + 1], g.W, 2, wdims, wstr, wbox));
+    const uint64_t wstr[1] = {(uint64_t)g.K * es};
+    const uint32_t wbox[2] = {(uint32_t)bk, HALF_N};
+    if (fp8) {
+      SPOT_CUDA_TRY(spot_make_tmap_u8(&tm[3 * np], (const uint8_t*)g.A + g.a_map.offset, 3, adims, astr, abox));
+      SPOT_CUDA_TRY(spot_make_tmap_u8(&tm[3 * np + 1], g.W, 2, wdims, wstr, wbox));
+    } else {
+      SPOT_CUDA_TRY(spot_make_tmap_bf16(&tm[3 * np], (const bf16*)g.A + g.a_map.offset, 3, adims, astr, abox));
+      SPOT_CUDA_TRY(spot_make_tmap_bf16(&tm[3 * np + 1], g.W, 2, wdims, wstr, wbox));
+    }
     const uint64_t odims[3] = {(uint64_t)g.N, (uint64_t)rps, (uint64_t)nseq};
     if (epi == EPI_GATE_RES) {
       const RowMap& m = g.resid_map;
       const uint64_t ostr[2] = {(uint64_t)m.ld * 4, (uint64_t)(nseq > 1 ? m.seq_stride : m.ld * (long long)rps) * 4};
       const uint32_t obox[3] = {32, 32, 1};
       SPOT_CUDA_TRY(spot_make_tmap_f32(&tm[3 * np + 2], g.resid + m.offset, 3, odims, ostr, obox));
+    } else if (out8) {
+      const RowMap& m = g.out_map;
+      const uint64_t ostr[2] = {(uint64_t)m.ld, (uint64_t)(nseq > 1 ? m.seq_stride : m.ld * (long long)rps)};
+      const uint32_t obox[3] = {128, 32, 1};
+      SPOT_CUDA_TRY(spot_make_tmap_u8(&tm[3 * np + 2], (uint8_t*)g.out + m.offset, 3, odims, ostr, obox));
     } else {
       const RowMap& m = g.out_map;
       const uint64_t ostr[2] = {(uint64_t)m.ld * 2, (uint64_t)(nseq > 1 ? m.seq_stride : m.ld * (long long)rps) * 2};
@@ -433,22 +513,28 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
   int pairs = num_sms / 2;
   if (tiles < pairs) pairs = tiles;
   const int grid = 2 * pairs;
-#define V3_LAUNCH(E)                                                                                              \
-  do {                                                                                                            \
-    static bool attr_set = false;                                                                                 \
-    if (!attr_set) {                                                                                              \
-      SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_v3_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                         (int)SMEM_BYTES));                                                       \
-      attr_set = true;                                                                                            \
-    }                                                                                                             \
-    gemm_tcgen05_v3_kernel<E><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], tm[4], tm[5], P); \
+#define V3_LAUNCH(E, F)                                                                                              \
+  do {                                                                                                               \
+    static bool attr_set = false;                                                                                    \
+    if (!attr_set) {                                                                                                 \
+      SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_v3_kernel<E, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                         (int)SMEM_BYTES));                                                          \
+      attr_set = true;                                                                                               \
+    }                                                                                                                \
+    gemm_tcgen05_v3_kernel<E, F><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], tm[4], tm[5], P); \
+  } while (0)
+#define V3_LAUNCH2(E)              \
+  do {                             \
+    if (fp8) V3_LAUNCH(E, true);   \
+    else V3_LAUNCH(E, false);      \
   } while (0)
   switch (epi) {
-    case EPI_BIAS: V3_LAUNCH(EPI_BIAS); break;
-    case EPI_BIAS_GELU: V3_LAUNCH(EPI_BIAS_GELU); break;
-    case EPI_GATE_RES: V3_LAUNCH(EPI_GATE_RES); break;
-    case EPI_QKV_ROPE: V3_LAUNCH(EPI_QKV_ROPE); break;
+    case EPI_BIAS: V3_LAUNCH2(EPI_BIAS); break;
+    case EPI_BIAS_GELU: V3_LAUNCH2(EPI_BIAS_GELU); break;
+    case EPI_GATE_RES: V3_LAUNCH2(EPI_GATE_RES); break;
+    case EPI_QKV_ROPE: V3_LAUNCH2(EPI_QKV_ROPE); break;
   }
+#undef V3_LAUNCH2
 #undef V3_LAUNCH
   return cudaGetLastError();
 }

@@ -61,6 +61,10 @@ cudaError_t launch_tc_gather(const float* src, float* dst, const int* idx, int d
 cudaError_t launch_tc_combine(float* h0, float* resid, const float* hc, const int* pos, int B, long long n_per_seq,
                               cudaStream_t st);
 
+// FP8 exploration variant (fp8.cu): per-output-channel weight quantisation, unit-scale activation cast
+cudaError_t launch_quantize_weight_rows(const void* w_bf16, long long N, int K, void* wq, float* scale, cudaStream_t st);
+cudaError_t launch_quantize_e4m3(spot_dtype dt, const void* in, long long n, void* out, cudaStream_t st);
+
 // plumbing
 cudaError_t launch_to_f32(spot_dtype dt, const void* in, float* out, long long n, cudaStream_t st);
 cudaError_t launch_from_f32(spot_dtype dt, const float* in, void* out, long long n, cudaStream_t st);
@@ -83,4 +87,5 @@ bool tcgen05_v3_qkv_rope_supported(const GemmProblem& p);
 bool tcgen05_attn_supported(int S, int H, int dh);
 cudaError_t launch_attn_tcgen05(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st);
 // v3: 64-key tiles, one pass over the scores, double-buffered S per query tile (the default)
-cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st);
+cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int H, int dh, int num_sms, cudaStream_t st,
+                                   bool out_e4m3 = false);   // out_e4m3: O stored as E4M3 bytes (operand of the FP8 out-projection)

@@ -156,6 +156,14 @@ __host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, int a_mn_ma
 
 }  // namespace ptx
 
+// Instruction descriptor for kind::f8f6f4 with E4M3 x E4M3 -> fp32: D fp32 (bit 4), a_format = b_format = 0 (E4M3),
+// both K-major, N >> 3 in [17,23), M >> 4 in [24,29).
+namespace ptx {
+__host__ __device__ constexpr uint32_t make_idesc_e4m3(int M, int N) {
+  return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+}  // namespace ptx
+
 // ---- host: cuTensorMapEncodeTiled through the runtime's driver entry point (no -lcuda) -----------
 typedef CUresult (*spot_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                          const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -167,6 +175,10 @@ cudaError_t spot_make_tmap_bf16(CUtensorMap* out, const void* base, int rank, co
 // same for an fp32 tensor (TMA store / reduce-add of the residual stream)
 cudaError_t spot_make_tmap_f32(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
                                const uint64_t* strides_bytes, const uint32_t* box);
+
+// one-byte element tensor (E4M3 operands of the FP8 variant), 128-byte swizzle
+cudaError_t spot_make_tmap_u8(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
+                              const uint64_t* strides_bytes, const uint32_t* box);
 
 // ---- TMA stores (shared -> global through a tensor map), bulk async-groups ---------------------------------
 namespace ptx {
@@ -239,6 +251,15 @@ __device__ __forceinline__ void mma_f16_ss_2cta(uint32_t d_tmem, uint64_t a_desc
   asm volatile(
       "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// kind::f8f6f4 with E4M3 operands (K = 32 per instruction): same descriptors, 2x the MACs per issued instruction
+__device__ __forceinline__ void mma_f8_ss_2cta(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                               uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(d_tmem),
       "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
       : "memory");
 }

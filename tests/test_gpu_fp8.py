@@ -1,0 +1,154 @@
+"""-m gpu parity of the low-precision (FP8 E4M3) exploration variant against oracle/fp8.py.
+
+Quantisation decides an integer (the E4M3 code) by floating point, so both sides take it in the kernel's precision:
+the scale s_n = amax / 448 and the quotient w / s_n are formed in fp32 on both sides and handed to the oracle's
+rounding function, and the codes are then compared bit for bit.  Where the VALUE being rounded differs between the
+two sides by accumulation order (GEMM and LayerNorm outputs written as E4M3), a value within that difference of a
+rounding boundary may land on the neighbouring code: those tests require (nearly) all codes equal and the rest to be
+adjacent codes.  Block- and rollout-level outputs keep the north-star bounds (2e-2 per block, 5e-2 final)."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_19004_b200 as spot
+from oracle import fp8, mmdit, philox, rollout
+from synth import CONFIGS, hash_normal, make_block_inputs, make_probe, make_text_emb
+from tests.gpu_common import device_weights, ensure_built, oracle_weights
+from tests.helpers import np64, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    ensure_built()
+
+
+def _f64(t):
+    return t.to(torch.float32).to("cpu", torch.float64).numpy()
+
+
+def _codes_close(got, ref, min_equal):
+    """got, ref: fp64 arrays of E4M3 values.  Nearly all equal; the rest are neighbouring codes (one grid step)."""
+    eq = got == ref
+    frac = eq.mean()
+    bad = ~eq
+    if bad.any():
+        step = np.exp2(np.maximum(np.floor(np.log2(np.maximum(np.abs(ref[bad]), 2.0 ** -6))), -6.0) - 3.0)
+        assert (np.abs(got[bad] - ref[bad]) <= 2.0 * step * 1.0001).all(), "codes differ by more than a neighbouring step"
+    assert frac >= min_equal, f"only {frac:.4f} of the codes are equal"
+    return frac
+
+
+def test_quantize_e4m3_bit_exact():
+    x = torch.cat([hash_normal(1101 + i, 1 << 16, s, torch.float32, "cuda") for i, s in enumerate((1e-3, 0.05, 1.0, 40.0, 400.0))])
+    x[:8] = torch.tensor([0.0, 448.0, 464.0, 1e9, -1e9, 2.0 ** -9, 2.0 ** -10, 1.0625], device="cuda")
+    q = spot.spot_quantize_e4m3(x)
+    assert (_f64(q) == fp8.e4m3(np64(x))).all()
+    xb = x[: 1 << 16].to(torch.bfloat16)
+    assert (_f64(spot.spot_quantize_e4m3(xb)) == fp8.e4m3(np64(xb))).all()
+    tail = x[:1001].contiguous()                                          # ragged length (not a multiple of 4)
+    assert (_f64(spot.spot_quantize_e4m3(tail)) == fp8.e4m3(np64(tail))).all()
+
+
+def test_quantize_weight_rows_bit_exact():
+    N, K = 96, 3072
+    w = hash_normal(1110, N * K, 0.02, torch.bfloat16, "cuda").reshape(N, K)
+    w[7] = 0
+    wq, s = spot.spot_quantize_weight_rows(w)
+    w32 = w.float().cpu().numpy()
+    amax = np.abs(w32).max(axis=1)
+    s_ref = np.where(amax > 0, amax / np.float32(448.0), np.float32(1.0)).astype(np.float32)      # fp32, as the kernel
+    assert (s.cpu().numpy() == s_ref).all()
+    q_ref = fp8.e4m3((w32 / s_ref[:, None]).astype(np.float32).astype(np.float64))
+    assert (_f64(wq) == q_ref).all()
+    wq64, s64 = fp8.quantize_weight(np64(w))                              # the oracle's own (fp64) scale: same codes up to ties
+    _codes_close(_f64(wq), wq64, 0.9999)
+    assert np.abs(s.cpu().numpy() / s64 - 1).max() < 2e-7
+
+
+@pytest.mark.parametrize("M,N,K", [(300, 512, 256), (128, 256, 128), (1024, 3072 + 32, 512), (77, 32, 16), (2048, 768, 3072)])
+def test_linear_fp8(M, N, K):
+    a = spot.spot_quantize_e4m3(hash_normal(1120, M * K, 1.0, torch.float32, "cuda").reshape(M, K))
+    wq, s = spot.spot_quantize_weight_rows(hash_normal(1121, N * K, 0.05, torch.bfloat16, "cuda").reshape(N, K))
+    b = hash_normal(1122, N, 0.1, torch.bfloat16, "cuda")
+    gate = hash_normal(1123, N, 0.5, torch.float32, "cuda")
+    resid = hash_normal(1124, M * N, 1.0, torch.float32, "cuda").reshape(M, N)
+    y = (_f64(a) @ _f64(wq).T) * np64(s) + np64(b)                        # exact: operands are E4M3 values
+    r = spot.spot_linear_fp8(a, wq, s, b, spot.EPI_GATE_RESIDUAL, gate=gate, residual=resid.clone())
+    assert rel_l2(np64(r), np64(resid) + np64(gate) * y) < 2e-5
+    o = spot.spot_linear_fp8(a, wq, s, b, spot.EPI_BIAS)
+    f = _codes_close(_f64(o), fp8.e4m3(y), 0.995)
+    og = spot.spot_linear_fp8(a, wq, s, b, spot.EPI_BIAS_GELU)
+    fg = _codes_close(_f64(og), fp8.e4m3(mmdit.gelu_tanh(y)), 0.98)       # tanh.approx moves a few more values across a tie
+    print(f"fp8 linear {M}x{N}x{K}: equal codes {f:.4f} (bias), {fg:.4f} (GELU)")
+    assert torch.equal(o.view(torch.uint8), spot.spot_linear_fp8(a, wq, s, b, spot.EPI_BIAS).view(torch.uint8))
+
+
+def test_ln_modulate_e4m3_output():
+    M, D = 131, 3072
+    h = hash_normal(1130, M * D, 2.0, torch.float32, "cuda").reshape(M, D) + 0.5
+    shift = hash_normal(1131, D, 0.3, torch.float32, "cuda")
+    scale = hash_normal(1132, D, 0.3, torch.float32, "cuda")
+    y = spot.spot_ln_modulate(h, shift, scale, 1e-6, torch.float8_e4m3fn)
+    ref = fp8.e4m3(mmdit.layer_norm(np64(h), 1e-6) * (1.0 + np64(scale)) + np64(shift))
+    _codes_close(_f64(y), ref, 0.999)
+
+
+@pytest.fixture(scope="module")
+def wide():
+    """Config-3 shapes (hidden 3072, 24 x 128 heads, 1024 + 256 tokens) at depth 2."""
+    s = CONFIGS[3].with_(n_blocks=2, seeds_per_prompt=4, n_steps=3)
+    w = device_weights(s)
+    ctx = spot.Context(s, w, max_seqs=4)
+    return s, w, ctx
+
+
+def test_block_forward_fp8_matches_fp8_oracle(wide):
+    s, w, ctx = wide
+    h_img, h_txt, temb = make_block_inputs(s, 2, "cuda")
+    _, blocks = oracle_weights(w)
+    cos, sin = mmdit.rope_table(s.grid_h, s.grid_w, s.n_txt, s.rope_pairs, s.rope_theta)
+    c = mmdit.silu(np64(temb))
+    ctx.enable_fp8(True)
+    try:
+        o_img, o_txt = spot.spot_dit_block_forward(ctx, 0, h_img, h_txt, temb)
+    finally:
+        ctx.enable_fp8(False)
+    b_img, b_txt = spot.spot_dit_block_forward(ctx, 0, h_img, h_txt, temb)      # the bf16 path on the same inputs
+    for b in range(2):
+        r_img, r_txt = fp8.block_forward_fp8(np64(h_img[b]), np64(h_txt[b]), c, blocks[0], n_heads=s.n_heads, cos=cos, sin=sin)
+        e_i, e_t = rel_l2(np64(o_img[b]), r_img), rel_l2(np64(o_txt[b]), r_txt)
+        d_i = rel_l2(np64(o_img[b]), np64(b_img[b]))
+        print(f"fp8 block, sequence {b}: vs fp8 oracle img {e_i:.3e} txt {e_t:.3e}; fp8 vs bf16 path img {d_i:.3e}")
+        assert e_i < 2e-2 and e_t < 2e-2
+        assert 1e-4 < d_i < 5e-2                                            # quantisation is visible, and small
+
+
+def test_rollout_fp8_matches_fp8_oracle_and_ranks_like_bf16(wide):
+    s, w, ctx = wide
+    text, probe = make_text_emb(s, "cuda"), make_probe(s, "cuda")
+    ts = [float(np.float32(t)) for t in s.timesteps]
+    seeds = torch.tensor([0, 1, 2, 3], dtype=torch.int64, device="cuda")
+    ref_bf16 = spot.spot_explore(ctx, seeds, text, ts, probe, 1, 4, 2)
+    lat_b, rew_b = ref_bf16["latents"].clone(), ref_bf16["rewards"].clone()
+    ctx.enable_fp8(True)
+    try:
+        out = spot.spot_explore(ctx, seeds, text, ts, probe, 1, 4, 2)
+        lat_q, rew_q = out["latents"].clone(), out["rewards"].clone()
+        again = spot.spot_explore(ctx, seeds, text, ts, probe, 1, 4, 2)
+        assert torch.equal(again["latents"], lat_q)                          # deterministic
+    finally:
+        ctx.enable_fp8(False)
+    g, blocks = oracle_weights(w)
+    qblocks = [fp8.quantize_block(bw) for bw in blocks]
+    cos, sin = mmdit.rope_table(s.grid_h, s.grid_w, s.n_txt, s.rope_pairs, s.rope_theta)
+    h_txt0 = mmdit.text_input(np64(text)[0], g)
+    x0 = philox.noise_from_seeds([0], s.n_img * s.latent_ch)[0].reshape(s.n_img, s.latent_ch).astype(np.float32).astype(np.float64)
+    xT = rollout.euler_denoise(x0, ts, lambda x, t: fp8.dit_velocity_fp8(x, t, h_txt0, g, blocks, qblocks, n_heads=s.n_heads, cos=cos, sin=sin))
+    e = rel_l2(np64(lat_q[0]), xT)
+    d = rel_l2(np64(lat_q), np64(lat_b))
+    print(f"fp8 rollout (depth 2, 3 steps): vs fp8 oracle {e:.3e}; fp8 vs bf16 latents {d:.3e}; rewards fp8 {rew_q.tolist()} bf16 {rew_b.tolist()}")
+    assert e < 5e-2
+    assert d < 5e-2
+    assert torch.argsort(rew_q).tolist() == torch.argsort(rew_b).tolist() or d < 1e-2
