@@ -66,6 +66,7 @@ struct Workspace {
   size_t t_dev, emb, hid, temb, cvec, mod, fmod, txt_norm, txt_h0, h_img, h_txt, ybuf, big, vel, stage, total;
   size_t st_seeds, st_text, st_probe, st_lat, st_rew, st_stats, st_top, st_bot;
   // cached-step variant only (carve(..., cached = true)): uncompacted h_img^0, previous modulated input, cached residual
+  size_t md_a, md_acc, md_ones, md_zero;   // tensor-core modulation path (conditioning): split c, accumulators, gate = 1, bias = 0
   size_t tc_h0, tc_mprev, tc_resid, tc_rowpart, tc_acc, tc_coeffs, tc_idx, tc_pos, tc_nact, tc_comp, tc_rel;
 };
 
@@ -85,6 +86,10 @@ Workspace carve(const spot_ctx* c, int B, int T, bool cached = false) {
   w.cvec = take(Tp * D * 4);
   w.mod = take(Tp * L * 2 * 6 * D * 4);
   w.fmod = take(Tp * 2 * D * 4);
+  w.md_a = take(2 * Tp * D * 2);
+  w.md_acc = take(2 * 2 * Tp * 6 * D * 4);             // [stream][2 T, 6 D] fp32, reused block after block
+  w.md_ones = take(6 * D * 4);
+  w.md_zero = take(6 * D * 2);
   w.txt_norm = take((size_t)B * NT * g.txt_dim * es);
   w.txt_h0 = take((size_t)B * NT * D * 4);
   w.h_img = take((size_t)B * NI * D * 4);
@@ -489,10 +494,40 @@ spot_status conditioning(spot_ctx* c, const Workspace& w, uint8_t* ws, int T, cu
   LK(c, launch_gemv(g.dtype, c->w.time_w2, c->w.time_b2, hid, T, D, D, temb, D, false, st));
   LK(c, launch_silu(temb, cv, (long long)T * D, st));
   const long long stride_t = (long long)L * 2 * 6 * D;
-  for (int b = 0; b < L; ++b)
-    for (int s = 0; s < 2; ++s)
-      LK(c, launch_gemv(g.dtype, c->blocks[b].s[s].mod_w, c->blocks[b].s[s].mod_b, cv, T, 6 * D, D,
-                        mod + ((long long)b * 2 + s) * 6 * D, stride_t, false, st));
+  // The 2 L modulation Linears stream 2 L * 6 D^2 weights (13.6 GB at config 3) once per call: HBM-bound.  The plain
+  // warp-per-row kernel re-reads c from L1 for every weight vector and reaches ~0.7 TB/s; on bf16 configs the same
+  // product goes through the tcgen05 GEMM instead, with c split into two bf16 rows (hi + lo = 16 mantissa bits) so the
+  // fp32 modulation vectors keep ~2^-17 relative accuracy: rows [hi; lo] x W^T accumulate into fp32 through the
+  // reduce-add epilogue (gate = 1, bias = 0), then hi + lo + bias.
+  GemmProblem mp[2];
+  memset(mp, 0, sizeof(mp));
+  mp[0].A = ws + w.md_a; mp[0].a_map = plain_rows(2 * T, D); mp[0].M = 2 * T; mp[0].N = 6 * D; mp[0].K = D;
+  mp[0].bias = ws + w.md_zero; mp[0].gate = (const float*)(ws + w.md_ones);
+  mp[0].resid = (float*)(ws + w.md_acc); mp[0].resid_map = plain_rows(2 * T, 6 * D);
+  mp[0].W = L > 0 ? c->blocks[0].s[0].mod_w : nullptr;
+  const bool tc_mod = g.dtype == SPOT_BF16 && c->gemm_impl == 0 && L > 0 && tcgen05_gemm_supported(mp[0]);
+  if (tc_mod) {
+    const size_t acc_bytes = (size_t)2 * T * 6 * D * 4;
+    LK(c, launch_split_hi_lo(cv, ws + w.md_a, (long long)T * D, st));
+    LK(c, launch_fill_f32((float*)(ws + w.md_ones), 1.f, 6 * D, st));
+    CK(c, cudaMemsetAsync(ws + w.md_zero, 0, (size_t)6 * D * 2, st));
+    mp[1] = mp[0];
+    mp[1].resid = (float*)(ws + w.md_acc + acc_bytes);
+    for (int b = 0; b < L; ++b) {
+      CK(c, cudaMemsetAsync(ws + w.md_acc, 0, 2 * acc_bytes, st));
+      mp[0].W = c->blocks[b].s[0].mod_w;
+      mp[1].W = c->blocks[b].s[1].mod_w;
+      LK(c, launch_gemm_tcgen05_v3(EPI_GATE_RES, mp, 2, c->num_sms, st));
+      for (int s = 0; s < 2; ++s)
+        LK(c, launch_mod_combine(mp[s].resid, c->blocks[b].s[s].mod_b, T, 6 * D, mod + ((long long)b * 2 + s) * 6 * D,
+                                 stride_t, st));
+    }
+  } else {
+    for (int b = 0; b < L; ++b)
+      for (int s = 0; s < 2; ++s)
+        LK(c, launch_gemv(g.dtype, c->blocks[b].s[s].mod_w, c->blocks[b].s[s].mod_b, cv, T, 6 * D, D,
+                          mod + ((long long)b * 2 + s) * 6 * D, stride_t, false, st));
+  }
   LK(c, launch_gemv(g.dtype, c->w.final_mod_w, c->w.final_mod_b, cv, T, 2 * D, D, fmod, 2 * D, false, st));
   return SPOT_OK;
 }

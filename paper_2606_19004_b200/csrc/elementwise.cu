@@ -469,3 +469,53 @@ cudaError_t launch_broadcast_prompts(const float* src, float* dst, int B, int K,
   broadcast_prompts_kernel<<<grid_for(total4, 256), 256, 0, st>>>((const float4*)src, (float4*)dst, K, n4, total4);
   return cudaGetLastError();
 }
+
+namespace {
+
+// c [rows, D] fp32 -> A [2 * rows, D] bf16: rows 0..rows-1 = hi = bf16(c), rows rows..2 rows-1 = lo = bf16(c - hi), so that
+// hi + lo carries 16 mantissa bits of c through a bf16 tensor-core GEMM (used for the modulation Linears, K7)
+__global__ void split_hi_lo_kernel(const float* __restrict__ c, bf16* __restrict__ a, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float x = c[i];
+  const bf16 hi = __float2bfloat16_rn(x);
+  a[i] = hi;
+  a[n + i] = __float2bfloat16_rn(x - __bfloat162float(hi));
+}
+
+__global__ void fill_f32_kernel(float* __restrict__ p, float v, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = v;
+}
+
+// out[t * stride_t + n] = acc[t, n] + acc[T + t, n] + bias[n]   (hi and lo halves of the split GEMM, then the bias)
+template <typename TB>
+__global__ void mod_combine_kernel(const float* __restrict__ acc, const TB* __restrict__ bias, int T, int N,
+                                   float* __restrict__ out, long long stride_t) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)T * N) return;
+  const int t = (int)(i / N), n = (int)(i - (long long)t * N);
+  out[(long long)t * stride_t + n] = (acc[(long long)t * N + n] + acc[(long long)(T + t) * N + n]) + to_f32(bias[n]);
+}
+
+}  // namespace
+
+cudaError_t launch_split_hi_lo(const float* c, void* a_bf16, long long n, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  split_hi_lo_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c, (bf16*)a_bf16, n);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_fill_f32(float* p, float v, long long n, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  fill_f32_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, v, n);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_mod_combine(const float* acc, const void* bias_bf16, int T, int N, float* out, long long stride_t,
+                               cudaStream_t st) {
+  const long long n = (long long)T * N;
+  if (n <= 0) return cudaSuccess;
+  mod_combine_kernel<bf16><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(acc, (const bf16*)bias_bf16, T, N, out, stride_t);
+  return cudaGetLastError();
+}

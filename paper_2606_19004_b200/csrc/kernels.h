@@ -11,6 +11,11 @@ cudaError_t launch_time_embed(const float* d_t, int T, float* d_e /*[T,256]*/, c
 cudaError_t launch_gemv(spot_dtype wdt, const void* W, const void* b, const float* X, int T, int N, int K,
                         float* out, long long out_stride_t, bool silu_out, cudaStream_t st);
 cudaError_t launch_silu(const float* in, float* out, long long n, cudaStream_t st);
+// K7 on the tensor cores: c = hi + lo (two bf16 rows per timestep) through the tcgen05 GEMM, then hi + lo + bias
+cudaError_t launch_split_hi_lo(const float* c, void* a_bf16, long long n, cudaStream_t st);
+cudaError_t launch_fill_f32(float* p, float v, long long n, cudaStream_t st);
+cudaError_t launch_mod_combine(const float* acc, const void* bias_bf16, int T, int N, float* out, long long stride_t,
+                               cudaStream_t st);
 
 // K3: LayerNorm (no affine) * (1 + scale) + shift, fp32 residual rows -> act dtype rows
 cudaError_t launch_ln_modulate(spot_dtype odt, const float* h, int M, int D, const float* shift, const float* scale,
