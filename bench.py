@@ -189,10 +189,17 @@ def run_kernels(args, shape):
         res[name] = {"bound": "tensor", "ms": ms, "flops": flops, "achieved": tf, "unit": "TFLOP/s",
                      "peak": peaks["bf16_tflops"], "frac": tf / peaks["bf16_tflops"]}
 
-    # K1 Philox + Box-Muller: 2^28 normals (16 seeds x 2^24), 4 B/element written
+    # K1 Philox + Box-Muller: 2^28 normals (16 seeds x 2^24).  ALU-bound, not HBM-bound: 226 SASS instructions per
+    # Philox block of 4 normals (10 rounds of 2 IMAD.WIDE + LOP3/IADD, then logf / sqrtf / sincospif per pair), so the
+    # roof is 148 SMs x 128 lanes x sm_max clock / 56.5 instructions per normal (K1)
     seeds = torch.arange(16, dtype=torch.int64, device="cuda")
     nz = torch.empty((16, 1 << 24), dtype=torch.float32, device="cuda")
-    hbm("K1_noise", lambda: spot.spot_noise_from_seeds(seeds, 1 << 24, 0, nz), 4.0 * 16 * (1 << 24))
+    ms = timed(lambda: spot.spot_noise_from_seeds(seeds, 1 << 24, 0, nz), 10)
+    n_norm = 16.0 * (1 << 24)
+    alu_peak = 148 * 128 * 1.965e9 / 56.5 / 1e9                       # G normals/s
+    res["K1_noise"] = {"bound": "alu", "ms": ms, "normals": n_norm, "achieved": n_norm / ms / 1e6, "unit": "Gnormal/s",
+                       "peak": alu_peak, "frac": n_norm / ms / 1e6 / alu_peak, "written_gbs": 4.0 * n_norm / ms / 1e6,
+                       "peak_kind": "derived: 148 SMs x 128 lanes x 1.965 GHz / 56.5 SASS instructions per normal"}
     del nz
     # K3 LN + modulate: fp32 residual rows in, bf16 out
     h = rnd(1, (M, D), torch.float32)

@@ -123,7 +123,8 @@ const char *spot_version(void);
  * seeds", :251 "deterministic random seed" per sample.  DESIGN.md S1-S3: Philox4x32-10 with
  * key = (lo32, hi32)(seed) and counter = (lo32(j), hi32(j), stream_id, 0) for the 4-element block
  * j = e/4, then Box-Muller on 24-bit uniforms.  d_out[b*elems_per_seed + e], fp32.
- * elems_per_seed must be a positive multiple of 4; d_out 16-byte aligned.  n_seeds == 0 is a no-op. */
+ * elems_per_seed must be a positive multiple of 4; d_out 16-byte aligned; n_seeds <= 65535 (one grid row per
+ * sequence); n_seeds == 0 is a no-op. */
 spot_status spot_noise_from_seeds(const uint64_t *d_seeds, int n_seeds, int64_t elems_per_seed,
                                   uint32_t stream_id, float *d_out, void *cuda_stream);
 /* The raw Philox words of the same elements (u32 per element), for bit-exact checks. */

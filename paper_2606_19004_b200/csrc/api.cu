@@ -709,7 +709,7 @@ extern "C" {
 
 static spot_status noise_common(const uint64_t* d_seeds, int n_seeds, int64_t elems, uint32_t stream_id, float* d_out,
                                 uint32_t* d_words, void* cuda_stream) {
-  if (n_seeds < 0 || elems <= 0 || (elems & 3)) return SPOT_ERR_SHAPE;
+  if (n_seeds < 0 || n_seeds > 65535 || elems <= 0 || (elems & 3)) return SPOT_ERR_SHAPE;
   if (n_seeds == 0) return SPOT_OK;
   const void* o = d_out ? (const void*)d_out : (const void*)d_words;
   if (!d_seeds || !o) return SPOT_ERR_NULL;

@@ -11,23 +11,22 @@
 
 namespace {
 
+// grid.y = sequence (no 64-bit division per element), grid.x strides over the sequence's Philox blocks
 template <bool WORDS>
 __global__ void __launch_bounds__(256) noise_kernel(const uint64_t* __restrict__ seeds, long long blocks_per_seed,
-                                                    long long total_blocks, uint32_t stream_id,
-                                                    float4* __restrict__ out, uint4* __restrict__ words) {
-  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+                                                    uint32_t stream_id, float4* __restrict__ out, uint4* __restrict__ words) {
+  const int b = blockIdx.y;
+  const uint64_t seed = seeds[b];
+  const uint2 key = make_uint2((uint32_t)seed, (uint32_t)(seed >> 32));
+  const long long base = (long long)b * blocks_per_seed;
   const long long stride = (long long)gridDim.x * blockDim.x;
-  for (; i < total_blocks; i += stride) {
-    long long b = i / blocks_per_seed;
-    unsigned long long j = (unsigned long long)(i - b * blocks_per_seed);
-    uint64_t seed = seeds[b];
-    uint4 w = philox4x32_10(make_uint4((uint32_t)j, (uint32_t)(j >> 32), stream_id, 0u),
-                            make_uint2((uint32_t)seed, (uint32_t)(seed >> 32)));
+  for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < blocks_per_seed; j += stride) {
+    const uint4 w = philox4x32_10(make_uint4((uint32_t)j, (uint32_t)((unsigned long long)j >> 32), stream_id, 0u), key);
     if (WORDS) {
-      words[i] = w;
+      words[base + j] = w;
     } else {
-      float2 a = box_muller(w.x, w.y), c = box_muller(w.z, w.w);
-      out[i] = make_float4(a.x, a.y, c.x, c.y);
+      const float2 a = box_muller(w.x, w.y), c = box_muller(w.z, w.w);
+      out[base + j] = make_float4(a.x, a.y, c.x, c.y);
     }
   }
 }
@@ -36,13 +35,16 @@ __global__ void __launch_bounds__(256) noise_kernel(const uint64_t* __restrict__
 
 cudaError_t launch_noise(const uint64_t* d_seeds, int n_seeds, long long elems_per_seed, uint32_t stream_id,
                          float* d_normals, uint32_t* d_words, cudaStream_t st) {
-  long long bps = elems_per_seed / 4, total = bps * n_seeds;
-  if (total == 0) return cudaSuccess;
-  long long want = (total + 255) / 256;
-  int grid = (int)(want < 148LL * 32 ? want : 148LL * 32);   // grid-stride: a multiple of the SM count when large
+  const long long bps = elems_per_seed / 4;
+  if (bps == 0 || n_seeds <= 0) return cudaSuccess;
+  if (n_seeds > 65535) return cudaErrorInvalidValue;
+  long long want = (bps + 255) / 256;
+  const long long cap = (148LL * 32 + n_seeds - 1) / n_seeds;      // ~32 blocks per SM over the whole grid
+  if (want > cap) want = cap < 1 ? 1 : cap;
+  const dim3 grid((unsigned)want, (unsigned)n_seeds);
   if (d_words)
-    noise_kernel<true><<<grid, 256, 0, st>>>(d_seeds, bps, total, stream_id, nullptr, (uint4*)d_words);
+    noise_kernel<true><<<grid, 256, 0, st>>>(d_seeds, bps, stream_id, nullptr, (uint4*)d_words);
   else
-    noise_kernel<false><<<grid, 256, 0, st>>>(d_seeds, bps, total, stream_id, (float4*)d_normals, nullptr);
+    noise_kernel<false><<<grid, 256, 0, st>>>(d_seeds, bps, stream_id, (float4*)d_normals, nullptr);
   return cudaGetLastError();
 }
