@@ -29,10 +29,15 @@ constexpr int BLOCK_M = 128 /*per CTA*/, PAIR_M = 256, BLOCK_N = 256, HALF_N = 1
 constexpr int STAGES = 6;
 constexpr uint32_t A_BYTES = BLOCK_M * BLOCK_K * 2, B_BYTES = HALF_N * BLOCK_K * 2, STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr uint32_t STG_BYTES = 32 * 128;                         // one staging buffer: 32 rows x 128 bytes
-constexpr uint32_t OFF_STG = STAGES * STAGE_BYTES;               // 4 warps x 2 buffers
-constexpr uint32_t OFF_BAR = OFF_STG + 4 * 2 * STG_BYTES;
+// Epilogue warps: 4 (one per TMEM lane quarter, two staging buffers each) or 8 (two per quarter: columns [0,128) and
+// [128,256), one buffer each).  Measured: 8 warps only pay where the epilogue is the pace-maker, i.e. the fused
+// QKV + RMSNorm + RoPE epilogue behind the half-as-long E4M3 mainloop (ncu 63 % tensor-pipe active with 4 warps; FP8
+// rollout 1566 -> 1519 ms); every other instantiation is 1-5 % faster with 4 warps.
+__host__ __device__ constexpr int epi_warps(int epi, bool fp8) { return (fp8 && epi == EPI_QKV_ROPE) ? 8 : 4; }
+constexpr int MAX_THREADS = 128 + 8 * 32;
+constexpr uint32_t OFF_STG = STAGES * STAGE_BYTES;               // 8 staging buffers: 4 warps x 2 or 8 warps x 1
+constexpr uint32_t OFF_BAR = OFF_STG + 8 * STG_BYTES;
 constexpr uint32_t SMEM_BYTES = OFF_BAR + 256 /*barriers*/ + 1024 /*align slack*/;
-constexpr int NUM_THREADS = 256;
 static_assert(SMEM_BYTES <= 232448, "shared memory budget");
 
 struct V3Problem {
@@ -144,7 +149,7 @@ __device__ __forceinline__ void stage_bf16_32(uint32_t row_addr, int sw, int c0,
 // stage is a 128-element K block and everything else - ring, descriptors, 32-byte advance per MMA - is unchanged);
 // accumulators are dequantised per output channel; EPI_BIAS / EPI_BIAS_GELU then store E4M3 (the next Linear's operand).
 template <int EPI, bool FP8>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(MAX_THREADS, 1)
 gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmW0,
                        const __grid_constant__ CUtensorMap tmO0, const __grid_constant__ CUtensorMap tmA1,
                        const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmO1,
@@ -170,7 +175,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
-    for (int a = 0; a < 2; ++a) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 8); }
+    for (int a = 0; a < 2; ++a) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 2 * epi_warps(EPI, FP8)); }
     ptx::fence_barrier_init();
   }
   if (warp == 2) { ptx::tmem_alloc_2cta(tmem_slot, 512); ptx::tmem_relinquish_2cta(); }
@@ -239,11 +244,13 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
     }
   } else if (warp >= 4) {
     // ===================== epilogue (both CTAs, own 128 TMEM lanes) =====================
-    const int q4 = warp & 3;
-    const uint32_t stg0 = smem_base + OFF_STG + (uint32_t)q4 * 2 * STG_BYTES;
+    constexpr int EW = epi_warps(EPI, FP8), NBUF = 8 / EW;
+    const int q4 = warp & 3, half = (warp - 4) >> 2;       // EW == 8: warps 8-11 take columns [128,256) of the tile
+    const int col_lo = EW == 8 ? half : 0, col_hi = EW == 8 ? half + 1 : 2;   // range of 128-column half tiles of this warp
+    const uint32_t stg0 = smem_base + OFF_STG + (uint32_t)(warp - 4) * NBUF * STG_BYTES;
+    int buf = 0;
     const uint32_t row_off = (uint32_t)lane * 128u;
     const int sw = lane & 7;
-    int buf = 0;
     int acc = 0; uint32_t acc_phase = 0;
     for (int t = pair; t < P.total_tiles; t += n_pairs) {
       const TileCoord c = decode_tile(P, t);
@@ -268,27 +275,28 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
           }
           ptx::bulk_commit();
         }
-        buf ^= 1;
+        if (NBUF == 2) buf ^= 1;
       };
-      // wait until the TMA engine has read the buffer filled two sends ago
+      // wait until the TMA engine has read the warp's staging buffer (called after the chunk's TMEM load was issued
+      // and right before the first shared-memory store, so the wait overlaps the load and the arithmetic)
       auto acquire = [&]() {
-        ptx::bulk_wait_read<1>();                         // the elected lane waits for its groups; trivially true elsewhere
+        ptx::bulk_wait_read<NBUF - 1>();                  // the elected lane waits for its groups; trivially true elsewhere
         __syncwarp();
         return stg0 + buf * STG_BYTES + row_off;
       };
 
       if (EPI == EPI_GATE_RES) {
 #pragma unroll 1
-        for (int ch = 0; ch < BLOCK_N / 32; ++ch) {
+        for (int ch = col_lo * 4; ch < col_hi * 4; ++ch) {
           const int n0 = ncol0 + ch * 32;
           if (n0 >= q.N) break;
           uint32_t v[32];
           ptx::tmem_ld_32x32(taddr0 + ch * 32, v);
-          const uint32_t ra = acquire();
           ptx::tmem_ld_wait();
           float y[32];
           acc_to_y<FP8>(v, q.w_scale + n0, q.bias + n0, y);
           const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
+          const uint32_t ra = acquire();
 #pragma unroll
           for (int g = 0; g < 8; ++g) {
             const float4 gt = __ldg(gp + g);
@@ -300,7 +308,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
       } else {
         const int row = row0 + lane;                          // row inside the sequence (may be past its end)
 #pragma unroll 1
-        for (int hh = 0; hh < BLOCK_N / 128; ++hh) {          // a 128-column half tile = one head of the QKV output
+        for (int hh = col_lo; hh < col_hi; ++hh) {            // a 128-column half tile = one head of the QKV output
           const int hcol0 = ncol0 + hh * 128;
           if (hcol0 >= q.N) break;
           float rinv = 0.f;
@@ -329,7 +337,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
             }
           }
           if (FP8 && EPI != EPI_QKV_ROPE) {                  // E4M3 output: 128 columns = 128 bytes per row, one send per half tile
-            const uint32_t ra = acquire();
+            uint32_t ra = 0;
 #pragma unroll 1
             for (int c4 = 0; c4 < 4; ++c4) {
               const int n0 = hcol0 + c4 * 32;
@@ -347,6 +355,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
 #pragma unroll
                 for (int j = 0; j < 32; ++j) y[j] = 0.f;
               }
+              if (c4 == 0) ra = acquire();
               stage_e4m3_32(ra, sw, c4 * 2, y);
             }
             send(hcol0);
@@ -360,7 +369,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
             uint32_t v0[32], v1[32];
             ptx::tmem_ld_32x32(taddr0 + hh * 128 + c2 * 64, v0);
             ptx::tmem_ld_32x32(taddr0 + hh * 128 + c2 * 64 + 32, v1);
-            const uint32_t ra = acquire();
+            uint32_t ra = 0;
             ptx::tmem_ld_wait();
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {
@@ -395,6 +404,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
                   }
                 }
               }
+              if (hf == 0) ra = acquire();                    // as late as possible: the previous chunk's TMA read overlaps the math
               stage_bf16_32(ra, sw, hf * 4, y);
             }
             send(n0);
@@ -521,7 +531,7 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
                                          (int)SMEM_BYTES));                                                          \
       attr_set = true;                                                                                               \
     }                                                                                                                \
-    gemm_tcgen05_v3_kernel<E, F><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], tm[4], tm[5], P); \
+    gemm_tcgen05_v3_kernel<E, F><<<grid, 128 + epi_warps(E, F) * 32, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], tm[4], tm[5], P); \
   } while (0)
 #define V3_LAUNCH2(E)              \
   do {                             \
