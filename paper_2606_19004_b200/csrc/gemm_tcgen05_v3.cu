@@ -3,10 +3,11 @@
 // tcgen05.mma.cta_group::2 (M 256, N 256, K 16), a 6-stage TMA ring of 128-byte-swizzled K-major tiles and two
 // 256-column TMEM accumulators, so the epilogue of tile i overlaps the mainloop of tile i + 1.
 //
-// What is new is the epilogue (warps 4-7 of each CTA, one TMEM lane quarter = 32 rows each):
+// What is new is the epilogue (warps 4-7 of each CTA, one TMEM lane quarter = 32 rows each; 8 warps, two per quarter, for
+// the fused QKV epilogue on E4M3 operands - see epi_warps below):
 //   * results leave the SM through shared memory and TMA instead of per-thread global accesses: each warp packs
 //     32 rows x 128 bytes into its own swizzled staging buffer (two buffers per warp, so the TMA engine drains
-//     one while the warp fills the other) and one lane issues cp.async.bulk.tensor (store) - full 128-byte
+//     one while the warp fills the other; the buffer is acquired as late as possible, behind the arithmetic) and one lane issues cp.async.bulk.tensor (store) - full 128-byte
 //     lines, rows past the end of a sequence clipped by the tensor map;
 //   * EPI_GATE_RES  h += gate * (y + bias): the tile of gate * (y + bias) is sent with cp.reduce.async.bulk.tensor
 //     .add.f32, so the fp32 residual stream is never loaded by the SM (the add happens in the memory system; every
