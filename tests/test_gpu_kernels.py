@@ -246,7 +246,7 @@ def test_euler_update_and_reward():
 # ------------------------------------------------------------------ K5 tcgen05 attention
 @pytest.mark.parametrize("B,S,H,scale", [(1, 128, 1, 1.0), (2, 256, 2, 1.0), (1, 200, 2, 1.0), (2, 1280, 3, 1.0),
                                          (1, 333, 1, 6.0), (1, 1280, 2, 5.0), (1, 64, 1, 1.0), (1, 37, 2, 3.0),
-                                         (1, 6656, 1, 1.0)])
+                                         (1, 6656, 1, 1.0), (3, 520, 5, 2.0)])
 def test_attention_tcgen05(B, S, H, scale):
     """TMA + tcgen05 flash attention vs the fp64 oracle: one tile, several tiles, ragged last query/key tile,
     and peaked softmax (logits ~ N(0, (scale^2 * sqrt(128))^2)) that forces the lazy-rescale path."""
