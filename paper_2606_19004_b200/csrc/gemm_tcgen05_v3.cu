@@ -17,6 +17,7 @@
 //     thread owns one token row of the accumulator, so the per-head RMS is thread-local: pass 1 over TMEM sums the
 //     squares of (acc + bias), pass 2 scales by rsqrt(mean + eps) * gain, rotates pairs (2i, 2i+1) by the table
 //     angle of the token's joint position and stores bf16.  v heads take the plain bias path.
+#pragma nv_diag_suppress 128   // "loop is not reachable": the E4M3 QKV instantiation leaves the generic epilogue through `continue`
 #include <cuda_fp8.h>
 #include <stdlib.h>
 #include <string.h>
@@ -35,6 +36,9 @@ constexpr uint32_t STG_BYTES = 32 * 128;                         // one staging 
 // QKV + RMSNorm + RoPE epilogue behind the half-as-long E4M3 mainloop (ncu 63 % tensor-pipe active with 4 warps; FP8
 // rollout 1566 -> 1519 ms); every other instantiation is 1-5 % faster with 4 warps.
 __host__ __device__ constexpr int epi_warps(int epi, bool fp8) { return (fp8 && epi == EPI_QKV_ROPE) ? 8 : 4; }
+// Ring depth: the E4M3 QKV instantiation gives its sixth stage (32 KB) to the epilogue's per-warp column constants.
+__host__ __device__ constexpr int ring_stages(int epi, bool fp8) { return (fp8 && epi == EPI_QKV_ROPE) ? STAGES - 1 : STAGES; }
+constexpr uint32_t OFF_COLC = (STAGES - 1) * STAGE_BYTES;        // [8 warps][scale, bias, gain][128 columns] fp32 (that instantiation only)
 constexpr int MAX_THREADS = 128 + 8 * 32;
 constexpr uint32_t OFF_STG = STAGES * STAGE_BYTES;               // 8 staging buffers: 4 warps x 2 or 8 warps x 1
 constexpr uint32_t OFF_BAR = OFF_STG + 8 * STG_BYTES;
@@ -146,6 +150,21 @@ __device__ __forceinline__ void stage_bf16_32(uint32_t row_addr, int sw, int c0,
                  pack2(y[8 * g + 4], y[8 * g + 5]), pack2(y[8 * g + 6], y[8 * g + 7]));
 }
 
+// Loads whose issue point is pinned (volatile asm keeps its program order): used to start a load long before its use.
+__device__ __forceinline__ float4 ldg_nc_f4(const float* p) {
+  float4 v;
+  asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ uint2 ldg_nc_u2(const void* p) {
+  uint2 v;
+  asm volatile("ld.global.nc.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+  return v;
+}
+struct ColConst { float4 s; uint2 b, g; };                       // scale, bias, gain of 4 consecutive columns (bf16 pairs raw)
+__device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+
 // FP8 = true: A and W are E4M3 (kind::f8f6f4, K = 32 per MMA; a 128-byte swizzled row then holds 128 elements, so a
 // stage is a 128-element K block and everything else - ring, descriptors, 32-byte advance per MMA - is unchanged);
 // accumulators are dequantised per output channel; EPI_BIAS / EPI_BIAS_GELU then store E4M3 (the next Linear's operand).
@@ -156,6 +175,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
                        const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmO1,
                        const V3Params P) {
   extern __shared__ uint8_t smem_raw[];
+  constexpr int NST = ring_stages(EPI, FP8);
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar_base = smem_base + OFF_BAR;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
@@ -175,7 +195,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
     if (P.n_probs > 1) { ptx::prefetch_tmap(&tmA1); ptx::prefetch_tmap(&tmW1); ptx::prefetch_tmap(&tmO1); }
   }
   if (warp == 1 && lane == 0) {
-    for (int s = 0; s < STAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < NST; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
     for (int a = 0; a < 2; ++a) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 2 * epi_warps(EPI, FP8)); }
     ptx::fence_barrier_init();
   }
@@ -207,7 +227,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
           ptx::tma_load_2d_2cta(sa + A_BYTES, mW, leader_full, kb * (FP8 ? 2 * BLOCK_K : BLOCK_K), n0);
           // only the leader CTA arms its barrier, for the bytes of BOTH CTAs (see gemm_tcgen05_2cta.cu)
           if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          if (++stage == NST) { stage = 0; phase ^= 1; }
         }
       }
     }
@@ -238,7 +258,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
           }
           ptx::mma_commit_2cta(empty_bar(stage));
           if (kb == k_blocks - 1) ptx::mma_commit_2cta(tfull_bar(acc));
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          if (++stage == NST) { stage = 0; phase ^= 1; }
         }
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
       }
@@ -253,6 +273,35 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
     const uint32_t row_off = (uint32_t)lane * 128u;
     const int sw = lane & 7;
     int acc = 0; uint32_t acc_phase = 0;
+    // E4M3 QKV instantiation: this warp's column constants [scale | bias | gain][128] fp32 in the unused sixth stage
+    const uint32_t colc_addr = smem_base + OFF_COLC + (uint32_t)(warp - 4) * 1536u;
+    const float4* colc = reinterpret_cast<const float4*>(smem_raw + (colc_addr - ptx::smem_u32(smem_raw)));
+    auto load_colconst = [&](int t, ColConst& cc) {          // lane l: columns 4l .. 4l+3 of this warp's head in tile t
+      const TileCoord c = decode_tile(P, t);
+      const V3Problem& q = P.p[c.prob];
+      const int hcol0 = c.nt * BLOCK_N + half * 128;
+      cc.s = make_float4(0.f, 0.f, 0.f, 0.f);
+      cc.b = make_uint2(0u, 0u);
+      cc.g = make_uint2(0x3f803f80u, 0x3f803f80u);
+      if (hcol0 < q.N) {
+        cc.s = ldg_nc_f4(q.w_scale + hcol0 + lane * 4);
+        cc.b = ldg_nc_u2(q.bias + hcol0 + lane * 4);
+        const int which = hcol0 / q.hidden;
+        if (which < 2) cc.g = ldg_nc_u2((which ? q.k_gain : q.q_gain) + lane * 4);
+      }
+    };
+    auto store_colconst = [&](const ColConst& cc) {
+      __syncwarp();
+      st_shared_v4(colc_addr + lane * 16, __float_as_uint(cc.s.x), __float_as_uint(cc.s.y), __float_as_uint(cc.s.z), __float_as_uint(cc.s.w));
+      st_shared_v4(colc_addr + 512 + lane * 16, __float_as_uint(bf16_lo(cc.b.x)), __float_as_uint(bf16_hi(cc.b.x)),
+                   __float_as_uint(bf16_lo(cc.b.y)), __float_as_uint(bf16_hi(cc.b.y)));
+      st_shared_v4(colc_addr + 1024 + lane * 16, __float_as_uint(bf16_lo(cc.g.x)), __float_as_uint(bf16_hi(cc.g.x)),
+                   __float_as_uint(bf16_lo(cc.g.y)), __float_as_uint(bf16_hi(cc.g.y)));
+      __syncwarp();
+    };
+    if constexpr (EPI == EPI_QKV_ROPE && FP8) {
+      if (pair < P.total_tiles) { ColConst first; load_colconst(pair, first); store_colconst(first); }
+    }
     for (int t = pair; t < P.total_tiles; t += n_pairs) {
       const TileCoord c = decode_tile(P, t);
       const V3Problem& q = P.p[c.prob];
@@ -260,8 +309,6 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
       const int seq = c.mt / q.tiles_per_seq;
       const int row0 = (c.mt - seq * q.tiles_per_seq) * PAIR_M + (int)rank * BLOCK_M + q4 * 32;   // first row of this warp
       const bool warp_ok = row0 < q.rps;                    // whole warp past the end of the sequence: nothing to store
-      ptx::mbar_wait(tfull_bar(acc), acc_phase);
-      ptx::tc_fence_after();
       const uint32_t taddr0 = tmem_base + acc * BLOCK_N + ((uint32_t)(q4 * 32) << 16);
       const int ncol0 = c.nt * BLOCK_N;
 
@@ -286,6 +333,106 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
         return stg0 + buf * STG_BYTES + row_off;
       };
 
+      if constexpr (EPI == EPI_QKV_ROPE && FP8) {
+        // Behind the half-as-long E4M3 mainloop this epilogue sets the pace, and what it waited for was global loads
+        // (ncu: 61 % of its samples on the long scoreboard - L1 is ~27 KB next to the 225 KB of shared memory, so the
+        // per-column vectors and the per-row rotation tables arrive from L2 at every 32-column chunk).  Here each warp
+        // owns one head (128 columns) of the tile: the column constants (scale, bias, gain) sit in shared memory,
+        // loaded one tile ahead; the rotation table is loaded two chunks ahead, the first two before the accumulator
+        // is even waited for.
+        const int hcol0 = ncol0 + half * 128;
+        const bool head_ok = hcol0 < q.N;
+        const int which = head_ok ? hcol0 / q.hidden : 2;       // 0 = q, 1 = k, 2 = v (warp-uniform)
+        const bool rope = which < 2;
+        ColConst nxt;
+        const bool have_next = t + n_pairs < P.total_tiles;
+        if (have_next) load_colconst(t + n_pairs, nxt);
+        float4 cA[4], sA[4], cB[4], sB[4];
+        const int row = row0 + lane;
+        const long long pos = q.pos_off + (row < q.rps ? row : 0);
+        const float* cs = q.cos_t + pos * 64;
+        const float* sn = q.sin_t + pos * 64;
+        if (rope) {
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            cA[g] = ldg_nc_f4(cs + 4 * g); sA[g] = ldg_nc_f4(sn + 4 * g);
+            cB[g] = ldg_nc_f4(cs + 16 + 4 * g); sB[g] = ldg_nc_f4(sn + 16 + 4 * g);
+          }
+        }
+        ptx::mbar_wait(tfull_bar(acc), acc_phase);
+        ptx::tc_fence_after();
+        if (head_ok) {
+          float rinv = 0.f;
+          if (rope) {                                          // pass 1: sum of squares of (scale * acc + bias) over the head
+            float ss0 = 0.f, ss1 = 0.f;
+#pragma unroll 1
+            for (int c4 = 0; c4 < 4; ++c4) {
+              uint32_t v[32];
+              ptx::tmem_ld_32x32(taddr0 + half * 128 + c4 * 32, v);
+              ptx::tmem_ld_wait();
+#pragma unroll
+              for (int g = 0; g < 8; ++g) {
+                const float4 sc = colc[c4 * 8 + g], bi = colc[32 + c4 * 8 + g];
+                const float y0 = fmaf(__uint_as_float(v[4 * g]), sc.x, bi.x), y1 = fmaf(__uint_as_float(v[4 * g + 1]), sc.y, bi.y);
+                const float y2 = fmaf(__uint_as_float(v[4 * g + 2]), sc.z, bi.z), y3 = fmaf(__uint_as_float(v[4 * g + 3]), sc.w, bi.w);
+                ss0 = fmaf(y0, y0, ss0); ss1 = fmaf(y1, y1, ss1);
+                ss0 = fmaf(y2, y2, ss0); ss1 = fmaf(y3, y3, ss1);
+              }
+            }
+            rinv = rsqrtf((ss0 + ss1) * (1.f / 128.f) + q.rms_eps);
+          }
+          uint32_t ra = 0;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {                         // pass 2, 32 columns at a time; two of them fill a staging row
+            uint32_t v[32];
+            ptx::tmem_ld_32x32(taddr0 + half * 128 + k * 32, v);
+            ptx::tmem_ld_wait();
+            float y[32];
+#pragma unroll
+            for (int g = 0; g < 8; ++g) {
+              const float4 sc = colc[k * 8 + g], bi = colc[32 + k * 8 + g];
+              y[4 * g] = fmaf(__uint_as_float(v[4 * g]), sc.x, bi.x);
+              y[4 * g + 1] = fmaf(__uint_as_float(v[4 * g + 1]), sc.y, bi.y);
+              y[4 * g + 2] = fmaf(__uint_as_float(v[4 * g + 2]), sc.z, bi.z);
+              y[4 * g + 3] = fmaf(__uint_as_float(v[4 * g + 3]), sc.w, bi.w);
+            }
+            if (rope) {
+              float4 (&cc)[4] = (k & 1) ? cB : cA;
+              float4 (&sd)[4] = (k & 1) ? sB : sA;
+#pragma unroll
+              for (int g = 0; g < 8; ++g) {                     // 4 columns = 2 rotation pairs
+                const float4 gn = colc[64 + k * 8 + g];
+                const float a0 = y[4 * g] * rinv * gn.x, b0 = y[4 * g + 1] * rinv * gn.y;
+                const float a1 = y[4 * g + 2] * rinv * gn.z, b1 = y[4 * g + 3] * rinv * gn.w;
+                const float c0 = (g & 1) ? cc[g >> 1].z : cc[g >> 1].x, s0 = (g & 1) ? sd[g >> 1].z : sd[g >> 1].x;
+                const float c1 = (g & 1) ? cc[g >> 1].w : cc[g >> 1].y, s1 = (g & 1) ? sd[g >> 1].w : sd[g >> 1].y;
+                y[4 * g] = a0 * c0 - b0 * s0;
+                y[4 * g + 1] = a0 * s0 + b0 * c0;
+                y[4 * g + 2] = a1 * c1 - b1 * s1;
+                y[4 * g + 3] = a1 * s1 + b1 * c1;
+              }
+              if (k < 2) {                                      // this buffer's next use is chunk k + 2
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                  cc[g] = ldg_nc_f4(cs + (k + 2) * 16 + 4 * g);
+                  sd[g] = ldg_nc_f4(sn + (k + 2) * 16 + 4 * g);
+                }
+              }
+            }
+            if ((k & 1) == 0) ra = acquire();
+            stage_bf16_32(ra, sw, (k & 1) * 4, y);
+            if (k & 1) send(hcol0 + (k >> 1) * 64);
+          }
+        }
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cluster(ptx::map_to_cta(tempty_bar(acc), 0));
+        if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+        if (have_next) store_colconst(nxt);                     // all lanes are past their reads of this tile's constants
+        continue;
+      }
+      ptx::mbar_wait(tfull_bar(acc), acc_phase);
+      ptx::tc_fence_after();
       if (EPI == EPI_GATE_RES) {
 #pragma unroll 1
         for (int ch = col_lo * 4; ch < col_hi * 4; ++ch) {
