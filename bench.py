@@ -245,6 +245,14 @@ def run_kernels(args, shape):
         res[name]["peak"] = 2.0 * peaks["bf16_tflops"]
         res[name]["frac"] = res[name]["achieved"] / res[name]["peak"]
         del a8, wq, resid
+    a8 = spot.spot_quantize_e4m3(rnd(10, (B, S, D), bf))
+    wq, ws = spot.spot_quantize_weight_rows(rnd(11, (3 * D, D), bf, 0.02))
+    b = rnd(12, (3 * D,), bf, 0.02)
+    name = "K2_fp8_gemm_qkv_rope_fused"
+    tensor(name, lambda: spot.spot_qkv_rope_linear_fp8(a8, wq, ws, b, gains[0], gains[1], cs, sn, 0, 1e-6), 2.0 * M * 3 * D * D)
+    res[name]["peak"] = 2.0 * peaks["bf16_tflops"]
+    res[name]["frac"] = res[name]["achieved"] / res[name]["peak"]
+    del a8, wq
     print(json.dumps({"mode": "kernels", "workload": shape.name, "rows": M, "l2": "512 MiB written between iterations",
                       "peaks": peaks, "kernels": res}))
 

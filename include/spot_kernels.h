@@ -80,12 +80,19 @@ spot_status spot_sde_update(float *d_x, const float *d_v, const uint64_t *d_seed
  * spot_quantize_e4m3: elementwise e4m3(x) with unit scale (round to nearest even, saturating at +-448), n elements.
  * spot_linear_fp8: as spot_linear with d_a [M, K] and d_wq [N, K] E4M3 bytes, y = d_w_scale[n] * acc + bias (bias bf16);
  *   SPOT_EPI_BIAS / SPOT_EPI_BIAS_GELU write d_out [M, N] as E4M3 bytes, SPOT_EPI_GATE_RESIDUAL updates the fp32
- *   residual.  K % 16 == 0, N % 32 == 0. */
+ *   residual.  K % 16 == 0, N % 32 == 0.
+ * spot_qkv_rope_linear_fp8: spot_qkv_rope_linear on E4M3 operands: [q | k | v] = d_w_scale[n] * (d_a d_wq^T) + bias with
+ *   d_a [n_seqs * rows_per_seq, K] and d_wq [3 * hidden, K] E4M3 bytes, then QK-RMSNorm + RoPE as there; d_out stays
+ *   bf16 (attention runs in bf16, reading Q1).  This is the QKV launch of the FP8 rollout.  K % 16 == 0. */
 spot_status spot_quantize_weight_rows(const void *d_w_bf16, int64_t N, int64_t K, void *d_wq, float *d_scale, void *cuda_stream);
 spot_status spot_quantize_e4m3(spot_dtype dtype, const void *d_in, int64_t n, void *d_out, void *cuda_stream);
 spot_status spot_linear_fp8(spot_epilogue epi, const void *d_a, int64_t M, int64_t K, const void *d_wq, int64_t N,
                             const float *d_w_scale, const void *d_bias, const float *d_gate, float *d_residual, void *d_out,
                             void *cuda_stream);
+spot_status spot_qkv_rope_linear_fp8(const void *d_a, int n_seqs, int rows_per_seq, int64_t K, const void *d_wq,
+                                     const float *d_w_scale, int64_t hidden, const void *d_bias, const void *d_q_gain,
+                                     const void *d_k_gain, const float *d_cos, const float *d_sin, int pos_off, float eps,
+                                     void *d_out, void *cuda_stream);
 
 /* The RoPE table the context built at spot_create (S5): copies cos and sin [S, d_h/2] fp32 to HOST. */
 spot_status spot_rope_table(const spot_ctx *ctx, float *h_cos, float *h_sin);

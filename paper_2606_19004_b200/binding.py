@@ -101,6 +101,7 @@ def load_library() -> C.CDLL:
         "spot_explore_host": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_linear": [i32, i32, i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp],
         "spot_qkv_rope_linear": [vp, i32, i32, i64, vp, i64, vp, vp, vp, vp, vp, i32, f32, vp, vp],
+        "spot_qkv_rope_linear_fp8": [vp, i32, i32, i64, vp, vp, i64, vp, vp, vp, vp, vp, i32, f32, vp, vp],
         "spot_ln_modulate": [i32, vp, i64, i64, vp, vp, f32, vp, vp],
         "spot_qk_norm_rope": [i32, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, f32, vp],
         "spot_attention": [i32, i32, vp, vp, i32, i32, i32, i32, vp],
@@ -425,6 +426,18 @@ def spot_qkv_rope_linear(a: torch.Tensor, w: torch.Tensor, bias: torch.Tensor, q
     out = torch.empty((n_seqs, rps, 3 * hidden), dtype=a.dtype, device=a.device)
     _check(load_library().spot_qkv_rope_linear(_ptr(a), n_seqs, rps, K, _ptr(w), hidden, _ptr(bias), _ptr(q_gain), _ptr(k_gain),
                                                _ptr(cos), _ptr(sin), pos_off, eps, _ptr(out), _stream()), "spot_qkv_rope_linear")
+    return out
+
+
+def spot_qkv_rope_linear_fp8(a: torch.Tensor, wq: torch.Tensor, w_scale: torch.Tensor, bias: torch.Tensor, q_gain: torch.Tensor,
+                             k_gain: torch.Tensor, cos: torch.Tensor, sin: torch.Tensor, pos_off: int, eps: float) -> torch.Tensor:
+    """a [n_seqs, rows_per_seq, K] and wq [3 * hidden, K] E4M3 -> [n_seqs, rows_per_seq, 3 * hidden] bf16 (the FP8 rollout's QKV launch)."""
+    n_seqs, rps, K = a.shape
+    hidden = wq.shape[0] // 3
+    out = torch.empty((n_seqs, rps, 3 * hidden), dtype=torch.bfloat16, device=a.device)
+    _check(load_library().spot_qkv_rope_linear_fp8(_ptr(a), n_seqs, rps, K, _ptr(wq), _ptr(w_scale), hidden, _ptr(bias), _ptr(q_gain),
+                                                   _ptr(k_gain), _ptr(cos), _ptr(sin), pos_off, eps, _ptr(out), _stream()),
+           "spot_qkv_rope_linear_fp8")
     return out
 
 

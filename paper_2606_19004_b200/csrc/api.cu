@@ -1048,9 +1048,10 @@ spot_status spot_linear(spot_dtype dtype, spot_impl impl, spot_epilogue epi, con
   return launch_gemm_simt(dtype, dtype, dtype, e, p, st) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
 }
 
-spot_status spot_qkv_rope_linear(const void* d_a, int n_seqs, int rows_per_seq, int64_t K, const void* d_w, int64_t hidden,
-                                 const void* d_bias, const void* d_q_gain, const void* d_k_gain, const float* d_cos,
-                                 const float* d_sin, int pos_off, float eps, void* d_out, void* cuda_stream) {
+static spot_status qkv_rope_linear(const void* d_a, int n_seqs, int rows_per_seq, int64_t K, const void* d_w,
+                                   const float* d_w_scale, int64_t hidden, const void* d_bias, const void* d_q_gain,
+                                   const void* d_k_gain, const float* d_cos, const float* d_sin, int pos_off, float eps,
+                                   void* d_out, void* cuda_stream, bool fp8) {
   if (n_seqs < 0 || rows_per_seq <= 0 || K <= 0 || hidden <= 0 || hidden % 128 || pos_off < 0 || K > 0x7fffffff ||
       3 * hidden > 0x7fffffff || (long long)n_seqs * rows_per_seq > 0x7fffffff)
     return SPOT_ERR_SHAPE;
@@ -1067,9 +1068,29 @@ spot_status spot_qkv_rope_linear(const void* d_a, int n_seqs, int rows_per_seq, 
   p.A = d_a; p.a_map = RowMap{rows_per_seq, (long long)rows_per_seq * K, 0, K}; p.W = d_w; p.bias = d_bias;
   p.M = M; p.N = (int)N; p.K = (int)K; p.out = d_out; p.out_map = RowMap{rows_per_seq, (long long)rows_per_seq * N, 0, N};
   p.q_gain = d_q_gain; p.k_gain = d_k_gain; p.cos_t = d_cos; p.sin_t = d_sin; p.pos_off = pos_off; p.rms_eps = eps;
+  if (fp8) {
+    if (!d_w_scale) return SPOT_ERR_NULL;
+    if (!aligned16(d_w_scale)) return SPOT_ERR_ALIGN;
+    p.fp8 = 1; p.w_scale = d_w_scale;
+  }
   if (!tcgen05_gemm_supported(p) || !tcgen05_v3_qkv_rope_supported(p)) return SPOT_ERR_SHAPE;
   return launch_gemm_tcgen05_v3(EPI_QKV_ROPE, &p, 1, sm_count(), (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK
                                                                                                            : SPOT_ERR_CUDA;
+}
+
+spot_status spot_qkv_rope_linear(const void* d_a, int n_seqs, int rows_per_seq, int64_t K, const void* d_w, int64_t hidden,
+                                 const void* d_bias, const void* d_q_gain, const void* d_k_gain, const float* d_cos,
+                                 const float* d_sin, int pos_off, float eps, void* d_out, void* cuda_stream) {
+  return qkv_rope_linear(d_a, n_seqs, rows_per_seq, K, d_w, nullptr, hidden, d_bias, d_q_gain, d_k_gain, d_cos, d_sin, pos_off,
+                         eps, d_out, cuda_stream, false);
+}
+
+spot_status spot_qkv_rope_linear_fp8(const void* d_a, int n_seqs, int rows_per_seq, int64_t K, const void* d_wq,
+                                     const float* d_w_scale, int64_t hidden, const void* d_bias, const void* d_q_gain,
+                                     const void* d_k_gain, const float* d_cos, const float* d_sin, int pos_off, float eps,
+                                     void* d_out, void* cuda_stream) {
+  return qkv_rope_linear(d_a, n_seqs, rows_per_seq, K, d_wq, d_w_scale, hidden, d_bias, d_q_gain, d_k_gain, d_cos, d_sin,
+                         pos_off, eps, d_out, cuda_stream, true);
 }
 
 spot_status spot_ln_modulate(spot_dtype dtype, const float* d_h, int64_t M, int64_t D, const float* d_shift,

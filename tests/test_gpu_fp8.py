@@ -85,6 +85,37 @@ def test_linear_fp8(M, N, K):
     assert torch.equal(o.view(torch.uint8), spot.spot_linear_fp8(a, wq, s, b, spot.EPI_BIAS).view(torch.uint8))
 
 
+@pytest.mark.parametrize("n_seqs,rps,H,K,pos_off", [(2, 200, 2, 256, 9), (3, 77, 1, 64, 5), (5, 1280, 24, 512, 0), (4, 256, 24, 256, 1024)])
+def test_qkv_rope_linear_fp8(n_seqs, rps, H, K, pos_off):
+    """The FP8 rollout's QKV launch (E4M3 operands, per-channel dequantisation, QK-RMSNorm + RoPE in the epilogue, bf16 out)
+    vs exact arithmetic on the same E4M3 values.  The large cases give every CTA pair several tiles (the epilogue keeps its
+    column constants one tile ahead and its rotation table two chunks ahead) with ragged row tiles and an odd head count."""
+    dh, hidden = 128, H * 128
+    S = pos_off + rps + 3
+    a = spot.spot_quantize_e4m3(hash_normal(1140, n_seqs * rps * K, 1.0, torch.float32, "cuda").reshape(n_seqs, rps, K))
+    wq, ws = spot.spot_quantize_weight_rows(hash_normal(1141, 3 * hidden * K, 0.05, torch.bfloat16, "cuda").reshape(3 * hidden, K))
+    b = hash_normal(1142, 3 * hidden, 0.1, torch.bfloat16, "cuda")
+    qg = hash_normal(1143, dh, 0.3, torch.bfloat16, "cuda") + 1.0
+    kg = hash_normal(1144, dh, 0.3, torch.bfloat16, "cuda") + 1.0
+    ang = hash_normal(1145, S * 64, 2.0, torch.float32, "cuda").reshape(S, 64)
+    cos, sin = torch.cos(ang), torch.sin(ang)
+    out = spot.spot_qkv_rope_linear_fp8(a, wq, ws, b, qg, kg, cos, sin, pos_off, 1e-6)
+    y = ((_f64(a).reshape(-1, K) @ _f64(wq).T) * np64(ws) + np64(b)).reshape(n_seqs, rps, 3, H, dh)
+    c64, s64 = np64(cos)[pos_off:pos_off + rps], np64(sin)[pos_off:pos_off + rps]
+    ref = y.copy()
+    for part, gn in ((0, qg), (1, kg)):
+        for i in range(n_seqs):
+            ref[i, :, part] = mmdit.apply_rope(mmdit.rms_norm(y[i, :, part], np64(gn), 1e-6), c64, s64)
+    got = np64(out).reshape(n_seqs, rps, 3, H, dh)
+    for part in range(3):
+        err = rel_l2(got[:, :, part], ref[:, :, part])
+        assert err < 4e-3, (part, err)                                    # bf16 output rounding: 2^-9 / sqrt(3) = 1.1e-3
+    # per element: within bf16 rounding of the exact value (catches a single misplaced column constant or rotation pair)
+    tol = 2.0 ** -8 * np.abs(ref) + 1e-3
+    assert (np.abs(got - ref) <= tol).all()
+    assert torch.equal(out, spot.spot_qkv_rope_linear_fp8(a, wq, ws, b, qg, kg, cos, sin, pos_off, 1e-6))
+
+
 def test_ln_modulate_e4m3_output():
     M, D = 131, 3072
     h = hash_normal(1130, M * D, 2.0, torch.float32, "cuda").reshape(M, D) + 0.5
