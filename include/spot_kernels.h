@@ -68,6 +68,14 @@ spot_status spot_attention(spot_dtype dtype, spot_impl impl, const void *d_qkv, 
 spot_status spot_euler_update(float *d_x, const float *d_v, float dt, int n_seqs, int64_t elems, const float *d_probe,
                               float *d_rewards, float *d_partials, void *cuda_stream);
 
+/* A7 alone: per-prompt statistics and top/bottom-k selection of rewards that are already on the device (spot.h
+ * spot_seed_rewards states the ordering rules).  This is the step every rank repeats after the all-gather of the reward
+ * shards in the multi-GPU path.  d_rewards [n_prompts * seeds_per_prompt] fp32; d_stats
+ * [n_prompts, 2]; d_top / d_bottom [n_prompts, k_select] int32 (may be NULL when k_select == 0).
+ * 0 <= 2 * k_select <= seeds_per_prompt <= 1024, else SPOT_ERR_SHAPE. */
+spot_status spot_select_seeds(const float *d_rewards, int n_prompts, int seeds_per_prompt, int k_select, float *d_stats,
+                              int32_t *d_top, int32_t *d_bottom, void *cuda_stream);
+
 /* One stochastic sampler step on [n_seqs, elems] fp32 (spot.h spot_dit_denoise_sde): x <- mean +
  * sigma sqrt(-dt) xi with xi from Philox stream 256 + step of d_seeds[b]; d_logp[b] = the step's log-probability.
  * noise_level == 0 degenerates to the Euler update (d_logp = 0).  d_partials: [n_seqs, ceil(elems / 4096)] fp32 scratch. */

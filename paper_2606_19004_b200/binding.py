@@ -86,6 +86,7 @@ def load_library() -> C.CDLL:
         "spot_dit_block_forward": [vp, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_dit_denoise": [vp, i32, i32, vp, vp, vp, i32, vp, sz, vp],
         "spot_seed_rewards": [vp, i32, i32, vp, vp, i32, vp, vp, vp, vp, vp],
+        "spot_select_seeds": [vp, i32, i32, i32, vp, vp, vp, vp],
         "spot_explore": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_workspace_bytes_cached": [vp, i32, i32, C.POINTER(sz)],
         "spot_dit_denoise_cached": [vp, i32, i32, vp, vp, vp, i32, C.POINTER(SpotCacheConfig), vp, vp, vp, sz, vp],
@@ -299,6 +300,17 @@ def spot_seed_rewards(ctx: Context, latents: torch.Tensor, probe: torch.Tensor, 
                                             _ptr(rewards), _ptr(stats), _ptr(top), _ptr(bottom), _stream()),
            "spot_seed_rewards", ctx)
     return rewards, stats, top[:, :k_select], bottom[:, :k_select]
+
+
+def spot_select_seeds(rewards: torch.Tensor, n_prompts: int, seeds_per_prompt: int, k_select: int):
+    """A7 on rewards already on the device: (stats [P, 2], top [P, k], bottom [P, k])."""
+    dev = rewards.device
+    stats = torch.empty((n_prompts, 2), dtype=torch.float32, device=dev)
+    top = torch.empty((n_prompts, max(k_select, 1)), dtype=torch.int32, device=dev)
+    bottom = torch.empty((n_prompts, max(k_select, 1)), dtype=torch.int32, device=dev)
+    _check(load_library().spot_select_seeds(_ptr(rewards), n_prompts, seeds_per_prompt, k_select, _ptr(stats), _ptr(top),
+                                            _ptr(bottom), _stream()), "spot_select_seeds")
+    return stats, top[:, :k_select], bottom[:, :k_select]
 
 
 def spot_explore(ctx: Context, seeds: torch.Tensor, text_emb: torch.Tensor, timesteps: Sequence[float],

@@ -1093,6 +1093,17 @@ spot_status spot_qkv_rope_linear_fp8(const void* d_a, int n_seqs, int rows_per_s
                          pos_off, eps, d_out, cuda_stream, true);
 }
 
+spot_status spot_select_seeds(const float* d_rewards, int n_prompts, int seeds_per_prompt, int k_select, float* d_stats,
+                              int32_t* d_top, int32_t* d_bottom, void* cuda_stream) {
+  if (!d_rewards || !d_stats) return SPOT_ERR_NULL;
+  if (n_prompts <= 0 || seeds_per_prompt <= 0 || seeds_per_prompt > 1024 || k_select < 0 || 2 * k_select > seeds_per_prompt)
+    return SPOT_ERR_SHAPE;
+  if (k_select > 0 && (!d_top || !d_bottom)) return SPOT_ERR_NULL;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  return launch_seed_select(d_rewards, n_prompts, seeds_per_prompt, k_select, d_stats, d_top, d_bottom,
+                            (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
 spot_status spot_ln_modulate(spot_dtype dtype, const float* d_h, int64_t M, int64_t D, const float* d_shift,
                              const float* d_scale, float eps, void* d_out, void* cuda_stream) {
   if (dtype != SPOT_F32 && dtype != SPOT_BF16 && dtype != SPOT_E4M3) return SPOT_ERR_DTYPE;

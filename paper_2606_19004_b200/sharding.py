@@ -50,3 +50,46 @@ def max_over_ranks(value: float, device: str | torch.device = "cpu", group: Opti
     t = torch.tensor([float(value)], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
     return float(t.item())
+
+
+def shard_prompt_index(lo: int, hi: int, seeds_per_prompt: int) -> List[int]:
+    """Prompt of every sequence of the shard [lo, hi): sequence b belongs to prompt b // K (a shard may start and end
+    inside a prompt group)."""
+    return [b // seeds_per_prompt for b in range(lo, hi)]
+
+
+def explore_shard(ctx, seeds: torch.Tensor, text_emb: torch.Tensor, timesteps, probe: torch.Tensor, n_prompts: int,
+                  seeds_per_prompt: int, rank: int, world: int) -> dict:
+    """This rank's slice of one exploration call (sequence b -> rank floor(b * world / B)): noise,
+    T Euler steps and rewards of sequences [lo, hi) through the C ABI.  The slice runs as hi - lo one-seed prompt groups
+    with the text rows gathered per sequence (a row copy; h_txt0 is then projected per sequence, 2 * N_txt * D^2 FLOP
+    each), so it may cut through a prompt group; a sequence's result does not depend on its batch (spot.h "Determinism"),
+    hence the shards together are bit-identical to the unsharded call.  Returns {"lo", "hi", "latents", "rewards"}."""
+    from . import binding
+    B = n_prompts * seeds_per_prompt
+    assert seeds.numel() == B and text_emb.shape[0] == n_prompts
+    lo, hi = shard_range(B, rank, world)
+    s = ctx.shape
+    if hi == lo:
+        return {"lo": lo, "hi": hi, "latents": torch.empty((0, s.n_img, s.latent_ch), dtype=torch.float32, device=seeds.device),
+                "rewards": torch.empty(0, dtype=torch.float32, device=seeds.device)}
+    idx = torch.tensor(shard_prompt_index(lo, hi, seeds_per_prompt), dtype=torch.long, device=text_emb.device)
+    local_text = text_emb.index_select(0, idx).contiguous()
+    out = binding.spot_explore(ctx, seeds[lo:hi].contiguous(), local_text, timesteps, probe, hi - lo, 1, 0)
+    return {"lo": lo, "hi": hi, "latents": out["latents"], "rewards": out["rewards"]}
+
+
+def explore_sharded(ctx, seeds: torch.Tensor, text_emb: torch.Tensor, timesteps, probe: torch.Tensor, n_prompts: int,
+                    seeds_per_prompt: int, k_select: int, group: Optional[dist.ProcessGroup] = None) -> dict:
+    """One exploration call spread over the ranks of `group` (strong scaling of a fixed P x K batch): every rank holds
+    the full seeds / text / probe and the replicated weights, computes its shard (explore_shard), the fp32 rewards are
+    all-gathered (the path's only exchange: 4 B per sequence) and the selection runs redundantly on every rank.
+    Returns rewards [P * K], stats, top, bottom (identical on all ranks) and this rank's latents with their range."""
+    from . import binding
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    rank = dist.get_rank(group) if dist.is_initialized() else 0
+    shard = explore_shard(ctx, seeds, text_emb, timesteps, probe, n_prompts, seeds_per_prompt, rank, world)
+    rewards = gather_rewards(shard["rewards"], n_prompts * seeds_per_prompt, group)
+    stats, top, bottom = binding.spot_select_seeds(rewards, n_prompts, seeds_per_prompt, k_select)
+    return {"rewards": rewards, "stats": stats, "top": top, "bottom": bottom, "local_latents": shard["latents"],
+            "local_range": (shard["lo"], shard["hi"])}

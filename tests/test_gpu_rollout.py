@@ -207,3 +207,33 @@ def test_cfg3_lite_rollout_bf16():
     assert e_lat < 5e-2 and e_rew < 5e-2
     if abs(rew[0] - rew[1]) > 2 * 5e-2 * np.abs(rew).max():
         assert out["top"][0, 0].item() == int(np.argmax(rew))
+
+
+@pytest.mark.parametrize("world,wide", [(1, False), (3, False), (8, False), (4, True)])
+def test_sharded_exploration_is_bit_identical(world, wide):
+    """sequences sharded over `world` ranks (run here one after the other on the one GPU - no rank
+    waits on another), rewards reassembled, selection repeated: bit-identical to the unsharded call, including shards
+    that cut through a prompt group and empty shards (world 8 > some shard sizes of P x K = 2 x 3)."""
+    from paper_2606_19004_b200 import sharding
+    s = CONFIGS[3].with_(n_blocks=2, n_steps=2) if wide else CONFIGS[1]      # wide: the bf16 tcgen05 kernels at full width
+    w = device_weights(s)
+    P, K, k_sel = 2, 3, 1
+    ctx = spot.Context(s, w, max_seqs=P * K)
+    text = make_text_emb(s.with_(n_prompts=P), "cuda")
+    probe = make_probe(s, "cuda")
+    ts = [float(np.float32(t)) for t in s.timesteps]
+    seeds = torch.tensor([11, 12, 13, 21, 22, 23], dtype=torch.int64, device="cuda")
+    full = spot.spot_explore(ctx, seeds, text, ts, probe, P, K, k_sel)
+    full = {k: v.clone() for k, v in full.items()}
+    shards = [sharding.explore_shard(ctx, seeds, text, ts, probe, P, K, r, world) for r in range(world)]
+    assert [sh["lo"] for sh in shards] + [P * K] == [sharding.shard_range(P * K, r, world)[0] for r in range(world)] + [P * K]
+    rewards = torch.cat([sh["rewards"].clone() for sh in shards])
+    latents = torch.cat([sh["latents"].clone() for sh in shards])
+    assert torch.equal(rewards, full["rewards"]) and torch.equal(latents, full["latents"])
+    stats, top, bottom = spot.spot_select_seeds(rewards, P, K, k_sel)
+    assert torch.equal(stats, full["stats"]) and torch.equal(top, full["top"][:, :k_sel]) and torch.equal(bottom, full["bottom"][:, :k_sel])
+    if world == 1:                                            # the collective-free single-process form of the public call
+        out = sharding.explore_sharded(ctx, seeds, text, ts, probe, P, K, k_sel)
+        assert torch.equal(out["rewards"], full["rewards"]) and torch.equal(out["top"], top) and out["local_range"] == (0, P * K)
+    with pytest.raises(spot.SpotError):
+        spot.spot_select_seeds(rewards, P, K, 2)              # 2 * k_select > K

@@ -46,6 +46,20 @@ def _worker(rank, world, port, n_units, k_select, q):
         dist.destroy_process_group()
 
 
+def test_shard_prompt_index_cuts_through_groups():
+    """explore_shard runs its slice as one-seed prompt groups: sequence b keeps the text of prompt b // K."""
+    P, K, world = 3, 5, 4
+    seen = []
+    for r in range(world):
+        lo, hi = sharding.shard_range(P * K, r, world)
+        idx = sharding.shard_prompt_index(lo, hi, K)
+        assert len(idx) == hi - lo and all(0 <= p < P for p in idx)
+        seen += idx
+    assert seen == [b // K for b in range(P * K)]
+    assert sharding.shard_prompt_index(4, 6, 5) == [0, 1]              # a shard that straddles two prompt groups
+    assert sharding.shard_prompt_index(7, 7, 5) == []
+
+
 @pytest.mark.parametrize("n_units", [16, 17])
 def test_two_rank_gather_and_selection(n_units):
     world, port = 2, 29500 + (os.getpid() % 2000) + n_units
