@@ -5,6 +5,7 @@ path.  Cost: ~40 min to generate the 20.4 G weights on 8 cores + ~15 min of fp64
 
     python tests/golden/make_cfg3_golden.py [--blocks L] [--steps T] [--seed S] [--out NAME]
     python tests/golden/make_cfg3_golden.py --config 5 --prompt 7 --seed 229 --out cfg5_p7     (config 5, prompt 7)
+    python tests/golden/make_cfg3_golden.py --precision fp8 --out cfg3_seed0_fp8               (FP8 variant, oracle/fp8.py)
 
 The GPU test (tests/test_gpu_fullsize.py) regenerates the same weights on the device, checks their
 per-block checksums against the ones stored here, runs the 16-seed batch and compares seed S.
@@ -21,7 +22,7 @@ import torch
 ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 sys.path.insert(0, ROOT)
 
-from oracle import mmdit, philox, rollout  # noqa: E402
+from oracle import fp8, mmdit, philox, rollout  # noqa: E402
 from synth import CONFIGS, make_probe, make_text_emb, tensor_checksum  # noqa: E402
 from synth.manifest import make_block_weights, make_global_weights  # noqa: E402
 
@@ -38,6 +39,8 @@ def main():
     ap.add_argument("--out", default="cfg3_seed0")
     ap.add_argument("--config", type=int, default=3, choices=[3, 5])
     ap.add_argument("--prompt", type=int, default=0)
+    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp8"],
+                    help="fp8: the low-precision exploration variant as oracle/fp8.py states it (DESIGN.md section 13)")
     a = ap.parse_args()
     s = CONFIGS[a.config]
     if a.blocks is not None:
@@ -47,10 +50,19 @@ def main():
     here = os.path.dirname(os.path.abspath(__file__))
     t0 = time.time()
     gw = make_global_weights(s)
-    blocks, sums = [], []
+    blocks, sums, qblocks = [], [], []
     for b in range(s.n_blocks):
         bw = make_block_weights(s, b)
         sums.append({k: tensor_checksum(v) for k, v in sorted(bw.items())})
+        if a.precision == "fp8":
+            # quantise once with the oracle's quantiser and keep the codes as 1-byte tensors (exact: the values are
+            # E4M3-representable); the bf16 copies of the four Linears are dropped (20 GB instead of 40.8 GB)
+            q = {}
+            for st in ("img", "txt"):
+                for ln in fp8.BLOCK_LINEARS:
+                    wq, sc = fp8.quantize_weight(np64(bw.pop(f"{st}.{ln}_w")))
+                    q[f"{st}.{ln}"] = (torch.from_numpy(wq).to(torch.float8_e4m3fn), sc)
+            qblocks.append(q)
         blocks.append(bw)                                  # kept as bf16 (40.8 GB at full depth)
         print(f"block {b} generated ({time.time() - t0:.0f} s)", flush=True)
     gsum = {k: tensor_checksum(v) for k, v in sorted(gw.items())}
@@ -71,8 +83,15 @@ def main():
 
     hist = []
 
+    def fp8_lin(bi):                                       # the `lin` hook of oracle/fp8.py, codes widened per call
+        def lin(x, name):
+            wq8, sc = qblocks[bi][name]
+            return fp8.linear_fp8(x, wq8.to(torch.float64).numpy(), sc, np64(blocks[bi][f"{name}_b"]))
+        return lin
+
     def vel(x, t):
-        v = mmdit.dit_velocity(x, t, h0, g, LazyBlocks(), n_heads=s.n_heads, cos=cos, sin=sin, ln_eps=s.ln_eps, rms_eps=s.rms_eps)
+        v = mmdit.dit_velocity(x, t, h0, g, LazyBlocks(), n_heads=s.n_heads, cos=cos, sin=sin, ln_eps=s.ln_eps, rms_eps=s.rms_eps,
+                               block_lin=fp8_lin if a.precision == "fp8" else None)
         print(f"  velocity at t={t:.3f} done ({time.time() - t1:.0f} s)", flush=True)
         return v
 
@@ -80,7 +99,7 @@ def main():
     reward = rollout.probe_reward(xT, np64(probe))
     np.save(os.path.join(here, a.out + "_latent.npy"), xT.astype(np.float32))
     meta = {"written_by": "tests/golden/make_cfg3_golden.py (oracle/ + synth/ only)", "config": s.name, "n_blocks": s.n_blocks,
-            "n_steps": s.n_steps, "seed": a.seed, "prompt": a.prompt, "timesteps": ts, "reward": reward,
+            "n_steps": s.n_steps, "precision": a.precision, "seed": a.seed, "prompt": a.prompt, "timesteps": ts, "reward": reward,
             "latent_l2": float(np.linalg.norm(xT)), "x0_l2": float(np.linalg.norm(x0)),
             "per_step_l2": [float(np.linalg.norm(h)) for h in hist],
             "per_step_head": [[float(v) for v in h.reshape(-1)[:16]] for h in hist],
