@@ -156,61 +156,87 @@ namespace {
 
 // ------------------------------------------------------------------------------------------------
 // K4: q <- RoPE(RMSNorm(q) * g_q), k likewise, in place on qkv [B, S, 3, H, d_h] (north_star (c);
-// DESIGN.md S4 step 4-5, S5).  A warp owns one (token, head): lanes 0-15 hold q, lanes 16-31 hold k,
-// EPL = d_h / 16 consecutive elements per lane (16 bytes for bf16 d_h = 128, and for fp32 d_h = 64),
-// so every global access is a 128-bit load/store and the RMS reduction is 4 shuffles.
+// DESIGN.md S4 step 4-5, S5).  A warp owns HPW consecutive heads of one token: lanes 0-15 hold q,
+// lanes 16-31 hold k, EPL = d_h / 16 consecutive elements per lane (16 bytes for bf16 d_h = 128, and
+// for fp32 d_h = 64), so every global access is a 128-bit load/store and the RMS reduction is 4
+// shuffles.  The HPW row loads are issued back to back before any arithmetic (HPW x 16 B in flight
+// per thread), and the gain and the rotation pair of the token are read once per warp, as 128-bit
+// loads, and reused for the HPW heads.
 // Algorithmic bytes: read + write of q and k = 4 * sizeof(T) * d_h per (token, head).
-template <typename T, int EPL>
-__global__ void __launch_bounds__(256) qk_norm_rope_kernel(T* __restrict__ qkv, long long n_tok_heads, int S, int H,
+template <typename T, int EPL, int HPW>
+__global__ void __launch_bounds__(256) qk_norm_rope_kernel(T* __restrict__ qkv, long long n_warps, int S, int H,
                                                            int n_txt, const T* __restrict__ qg_img,
                                                            const T* __restrict__ kg_img, const T* __restrict__ qg_txt,
                                                            const T* __restrict__ kg_txt, const float* __restrict__ cos_t,
                                                            const float* __restrict__ sin_t, float eps) {
   constexpr int DH = EPL * 16;
+  constexpr bool VEC = sizeof(T) * EPL == 16;
   const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (w >= n_tok_heads) return;
+  if (w >= n_warps) return;
   const int lane = threadIdx.x & 31, part = lane >> 4, sub = lane & 15;
-  const long long tok = w / H;
-  const int head = (int)(w - tok * H), s = (int)(tok % S);
-  T* ptr = qkv + (tok * 3 + part) * (long long)(H * DH) + head * DH + sub * EPL;
+  const int groups = H / HPW;
+  const long long tok = w / groups;
+  const int head0 = (int)(w - tok * groups) * HPW, s = (int)(tok % S);
+  T* ptr = qkv + (tok * 3 + part) * (long long)(H * DH) + head0 * DH + sub * EPL;
   const T* gain = (s < n_txt ? (part ? kg_txt : qg_txt) : (part ? kg_img : qg_img)) + sub * EPL;
-  float x[EPL], g[EPL];
-  if constexpr (sizeof(T) * EPL == 16) {
-    uint4 raw = *reinterpret_cast<const uint4*>(ptr);
-    uint4 graw = *reinterpret_cast<const uint4*>(gain);
+  const float* cs = cos_t + (long long)s * (DH / 2) + sub * (EPL / 2);
+  const float* sn = sin_t + (long long)s * (DH / 2) + sub * (EPL / 2);
+  float x[HPW][EPL], g[EPL], c[EPL / 2], d[EPL / 2];
+  if constexpr (VEC) {
+    uint4 raw[HPW];
 #pragma unroll
-    for (int j = 0; j < EPL; ++j) {
-      x[j] = to_f32(reinterpret_cast<const T*>(&raw)[j]);
-      g[j] = to_f32(reinterpret_cast<const T*>(&graw)[j]);
+    for (int h = 0; h < HPW; ++h) raw[h] = *reinterpret_cast<const uint4*>(ptr + h * DH);
+    const uint4 graw = __ldg(reinterpret_cast<const uint4*>(gain));
+#pragma unroll
+    for (int j = 0; j < EPL; ++j) g[j] = to_f32(reinterpret_cast<const T*>(&graw)[j]);
+#pragma unroll
+    for (int h = 0; h < HPW; ++h)
+#pragma unroll
+      for (int j = 0; j < EPL; ++j) x[h][j] = to_f32(reinterpret_cast<const T*>(&raw[h])[j]);
+  } else {
+#pragma unroll
+    for (int h = 0; h < HPW; ++h)
+#pragma unroll
+      for (int j = 0; j < EPL; ++j) x[h][j] = to_f32(ptr[h * DH + j]);
+#pragma unroll
+    for (int j = 0; j < EPL; ++j) g[j] = to_f32(gain[j]);
+  }
+  if constexpr (EPL % 8 == 0) {  // EPL / 2 floats per table = whole float4s, 16-byte aligned
+#pragma unroll
+    for (int j = 0; j < EPL / 8; ++j) {
+      const float4 cv = __ldg(reinterpret_cast<const float4*>(cs) + j);
+      const float4 dv = __ldg(reinterpret_cast<const float4*>(sn) + j);
+      c[4 * j] = cv.x; c[4 * j + 1] = cv.y; c[4 * j + 2] = cv.z; c[4 * j + 3] = cv.w;
+      d[4 * j] = dv.x; d[4 * j + 1] = dv.y; d[4 * j + 2] = dv.z; d[4 * j + 3] = dv.w;
     }
   } else {
 #pragma unroll
-    for (int j = 0; j < EPL; ++j) { x[j] = to_f32(ptr[j]); g[j] = to_f32(gain[j]); }
+    for (int j = 0; j < EPL / 2; ++j) { c[j] = __ldg(cs + j); d[j] = __ldg(sn + j); }
   }
-  float q = 0.f;
 #pragma unroll
-  for (int j = 0; j < EPL; ++j) q += x[j] * x[j];
+  for (int h = 0; h < HPW; ++h) {
+    float q = 0.f;
 #pragma unroll
-  for (int o = 8; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
-  const float r = rsqrtf(q / (float)DH + eps);
-  const float* cs = cos_t + (long long)s * (DH / 2) + sub * (EPL / 2);
-  const float* sn = sin_t + (long long)s * (DH / 2) + sub * (EPL / 2);
-  float y[EPL];
+    for (int j = 0; j < EPL; ++j) q += x[h][j] * x[h][j];
 #pragma unroll
-  for (int j = 0; j < EPL / 2; ++j) {
-    float a = x[2 * j] * r * g[2 * j], b = x[2 * j + 1] * r * g[2 * j + 1];
-    float c = cs[j], d = sn[j];
-    y[2 * j] = a * c - b * d;
-    y[2 * j + 1] = a * d + b * c;
-  }
-  if constexpr (sizeof(T) * EPL == 16) {
-    uint4 o;
+    for (int o = 8; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+    const float r = rsqrtf(q / (float)DH + eps);
+    float y[EPL];
 #pragma unroll
-    for (int j = 0; j < EPL; ++j) reinterpret_cast<T*>(&o)[j] = from_f32<T>(y[j]);
-    *reinterpret_cast<uint4*>(ptr) = o;
-  } else {
+    for (int j = 0; j < EPL / 2; ++j) {
+      float a = x[h][2 * j] * r * g[2 * j], b = x[h][2 * j + 1] * r * g[2 * j + 1];
+      y[2 * j] = a * c[j] - b * d[j];
+      y[2 * j + 1] = a * d[j] + b * c[j];
+    }
+    if constexpr (VEC) {
+      uint4 o;
 #pragma unroll
-    for (int j = 0; j < EPL; ++j) ptr[j] = from_f32<T>(y[j]);
+      for (int j = 0; j < EPL; ++j) reinterpret_cast<T*>(&o)[j] = from_f32<T>(y[j]);
+      *reinterpret_cast<uint4*>(ptr + h * DH) = o;
+    } else {
+#pragma unroll
+      for (int j = 0; j < EPL; ++j) ptr[h * DH + j] = from_f32<T>(y[j]);
+    }
   }
 }
 
@@ -408,19 +434,28 @@ cudaError_t launch_rmsnorm_rows(spot_dtype dt, const void* in, const void* gain,
 cudaError_t launch_qk_norm_rope(spot_dtype dt, void* qkv, int B, int S, int H, int dh, int n_txt,
                                 const void* qg_img, const void* kg_img, const void* qg_txt, const void* kg_txt,
                                 const float* cos_t, const float* sin_t, float eps, cudaStream_t st) {
-  const long long n = (long long)B * S * H;
-  if (n <= 0) return cudaSuccess;
+  const long long n_heads = (long long)B * S * H;
+  if (n_heads <= 0) return cudaSuccess;
+  const int hpw = H % 4 == 0 ? 4 : H % 2 == 0 ? 2 : 1;  // heads per warp
+  const long long n = n_heads / hpw;
   const long long blocks = (n + 7) / 8;
   if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+#define QK_LAUNCH(T, EPL, HPW)                                                                                  \
+  qk_norm_rope_kernel<T, EPL, HPW><<<(int)blocks, 256, 0, st>>>((T*)qkv, n, S, H, n_txt, (const T*)qg_img,      \
+                                                                (const T*)kg_img, (const T*)qg_txt,             \
+                                                                (const T*)kg_txt, cos_t, sin_t, eps)
 #define QK_CASE(T, EPL)                                                                                        \
-  qk_norm_rope_kernel<T, EPL><<<(int)blocks, 256, 0, st>>>((T*)qkv, n, S, H, n_txt, (const T*)qg_img,           \
-                                                           (const T*)kg_img, (const T*)qg_txt, (const T*)kg_txt, \
-                                                           cos_t, sin_t, eps)
+  do {                                                                                                         \
+    if (hpw == 4) QK_LAUNCH(T, EPL, 4);                                                                        \
+    else if (hpw == 2) QK_LAUNCH(T, EPL, 2);                                                                   \
+    else QK_LAUNCH(T, EPL, 1);                                                                                 \
+  } while (0)
   if (dt == SPOT_F32 && dh == 64) QK_CASE(float, 4);
   else if (dt == SPOT_F32 && dh == 128) QK_CASE(float, 8);
   else if (dt == SPOT_BF16 && dh == 64) QK_CASE(bf16, 4);
   else if (dt == SPOT_BF16 && dh == 128) QK_CASE(bf16, 8);
   else return cudaErrorInvalidValue;
+#undef QK_LAUNCH
 #undef QK_CASE
   return cudaGetLastError();
 }

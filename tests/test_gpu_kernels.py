@@ -73,8 +73,10 @@ def test_ln_modulate(dtype, D, M, tol):
 
 # ------------------------------------------------------------------ K4
 @pytest.mark.parametrize("dtype,dh,H,tol", [(torch.float32, 64, 4, 1e-5), (torch.bfloat16, 128, 3, 4e-3),
-                                            (torch.float32, 128, 2, 1e-5), (torch.bfloat16, 64, 2, 4e-3)])
+                                            (torch.float32, 128, 2, 1e-5), (torch.bfloat16, 64, 2, 4e-3),
+                                            (torch.bfloat16, 128, 24, 4e-3), (torch.float32, 64, 6, 1e-5)])
 def test_qk_norm_rope(dtype, dh, H, tol):
+    # H = 3 / 2, 6 / 4, 24 take the 1-, 2- and 4-heads-per-warp instantiations of K4
     B, gh, gw, n_txt = 2, 5, 7, 9
     S = n_txt + gh * gw
     pairs = (dh // 16, (dh // 2 - dh // 16) // 2, dh // 2 - dh // 16 - (dh // 2 - dh // 16) // 2)
