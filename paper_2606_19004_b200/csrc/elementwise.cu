@@ -79,8 +79,11 @@ __global__ void silu_kernel(const float* __restrict__ in, float* __restrict__ ou
 // registers (NV float4 per lane), mean and variance are two exact passes over registers, the
 // output is written once in the activation dtype.  Algorithmic bytes: 4 D read + sizeof(T) D write.
 // Up to two problems (the image and the text stream of a block) share one launch: rows [0, M0) belong to p[0].
+// Launched with LN_ROWS_PER_CTA warps per CTA; for rows of up to 3072 elements the register cap of 6 resident CTAs
+// (168: the 96 row registers plus a window of the scale / shift loads) keeps 12 warps on an SM.
+constexpr int LN_ROWS_PER_CTA = 2;
 template <typename TO, int NV>
-__global__ void __launch_bounds__(256) ln_modulate_kernel(const LnProblem p0, const LnProblem p1, int D, float eps) {
+__global__ void __launch_bounds__(32 * LN_ROWS_PER_CTA, NV <= 24 ? 6 : 4) ln_modulate_kernel(const LnProblem p0, const LnProblem p1, int D, float eps) {
   int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   const bool second = row >= p0.M;
@@ -385,9 +388,10 @@ cudaError_t launch_silu(const float* in, float* out, long long n, cudaStream_t s
 
 template <typename TO>
 static cudaError_t ln_dispatch(const LnProblem& p0, const LnProblem& p1, int D, float eps, cudaStream_t st) {
-  // 2 rows per CTA: at ~150 registers per thread (the row lives in registers) 6 such CTAs = 12 warps fit an SM, against 8 warps
-  // with one 256-thread CTA; measured 5.50 vs 4.95 TB/s at config 3 (a CTA per row with the row spread over 256 threads: 4.55)
-  constexpr int blk = 64;
+  // 2 rows per CTA, 6 CTAs = 12 warps per SM (the launch bounds cap the kernel at 168 registers; left alone the compiler
+  // hoists every scale / shift load and takes 248, i.e. 8 warps): 5.94 TB/s at config 3, against 5.59 uncapped, 4.95 with one
+  // 256-thread CTA and 4.55 with a CTA per row spread over 256 threads
+  constexpr int blk = 32 * LN_ROWS_PER_CTA;
   const int wpb = blk / 32, grid = (p0.M + p1.M + wpb - 1) / wpb;
 #define LN_CASE(nv)                                                                                     \
   case nv:                                                                                              \
