@@ -117,6 +117,13 @@ def cpu_threads() -> int:
     return os.cpu_count() or 1
 
 
+def workload_config(shape) -> dict:
+    """The keys of `config` that name the workload; both arms print them."""
+    return {"workload": shape.name, "n_prompts": shape.n_prompts, "seeds_per_prompt": shape.seeds_per_prompt,
+            "euler_steps": shape.n_steps, "blocks": shape.n_blocks, "hidden": shape.hidden,
+            "image_tokens": shape.n_img, "text_tokens": shape.n_txt}
+
+
 def run_reference(args, shape):
     """--impl reference: the fp64 oracle timed on the host cores (rank 0 only)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -140,7 +147,7 @@ def run_reference(args, shape):
               "(work is linear in seeds, steps, blocks)")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": {"workload": shape.name, "sample": sample},
+            "dtype": "f64", "data": "synthetic", "config": {**workload_config(shape), "sample": sample},
             "cpu_baseline": {"value": value, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -160,6 +167,7 @@ def run_kernels(args, shape):
     B, S, D, F, H, dh = shape.n_seqs, shape.seq, shape.hidden, shape.mlp_hidden, shape.n_heads, shape.head_dim
     M = B * S
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    flush_words = flush.view(torch.int32)
     bf = torch.bfloat16
 
     def rnd(tid, shp, dtype, scale=1.0):
@@ -172,7 +180,10 @@ def run_kernels(args, shape):
         torch.cuda.synchronize()
         ts = []
         for _ in range(iters):
-            flush.zero_()
+            flush.zero_()                     # 512 MiB written: nothing of the kernel's operands is left in L2 ...
+            if args.flush == "clean":
+                flush_words.sum()             # ... then read back, so that L2 holds CLEAN lines: otherwise the write-back of
+            # up to 126 MB of dirty flush lines lands inside the timed kernel (10 us of a 60 us kernel, none of it its own)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
             fn()
@@ -259,13 +270,16 @@ def run_kernels(args, shape):
     res[name]["peak"] = 2.0 * peaks["bf16_tflops"]
     res[name]["frac"] = res[name]["achieved"] / res[name]["peak"]
     del a8, wq
-    print(json.dumps({"mode": "kernels", "workload": shape.name, "rows": M, "l2": "512 MiB written between iterations",
+    print(json.dumps({"mode": "kernels", "workload": shape.name, "rows": M, "l2": "512 MiB written" + (", then read back (clean lines)," if args.flush == "clean" else "") + " between iterations",
                       "peaks": peaks, "kernels": res}))
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--kernels", action="store_true", help="time every kernel alone against its roofline")
+    ap.add_argument("--flush", choices=["clean", "dirty"], default="clean",
+                    help="--kernels: L2 flush between iterations: 512 MiB written and read back (clean lines, default) or only "
+                         "written (the timed kernel then also pays the write-back of the flush's dirty lines)")
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
@@ -442,8 +456,7 @@ def main():
                 "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "fp8_e4m3 block Linears (bf16 attention, fp32 residual): exploration variant, not the headline" if fp8 else "bf16",
                 "data": "synthetic",
-                "config": {"workload": shape.name, "n_prompts": P, "seeds_per_prompt": K, "euler_steps": T, "blocks": L,
-                           "hidden": D, "image_tokens": shape.n_img, "text_tokens": shape.n_txt,
+                "config": {**workload_config(shape),
                            "l2": "inputs (40.8 GB of weights streamed every Euler step) are larger than L2",
                            "parallelism": f"replicas x{world}, disjoint seed groups"},
                 "seeds_per_s": world * B / (ms_step / 1e3), "tflops_per_gpu": tflops,
