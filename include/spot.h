@@ -99,7 +99,11 @@ typedef enum {
                              * 4 = as 0 but K4 (QK-norm+RoPE) as its own kernel */
   SPOT_OPT_ATTN_IMPL = 1,   /* 0 = auto (tcgen05 for bf16, d_h = 128: one-pass kernel, 64-key tiles), 1 = SIMT attention, 2 = previous two-pass tcgen05 kernel */
   SPOT_OPT_TIMING = 2,      /* 1 = bracket every tcgen05 GEMM launch with CUDA events on the launch stream */
-  SPOT_OPT_FP8 = 3          /* 1 = the four Linears of every block run on E4M3 operands (after spot_fp8_prepare) */
+  SPOT_OPT_FP8 = 3,         /* 1 = the four Linears of every block run on E4M3 operands (after spot_fp8_prepare) */
+  SPOT_OPT_CHUNK_SEQS = 4   /* sequences per pass of the block stack in spot_dit_denoise / spot_explore / spot_explore_host: larger
+                             * batches run as consecutive chunks of this many sequences (PAPER.md:338 caps an exploration batch at
+                             * 32 sequences); 0 = the whole batch in one pass; default 32.  Results do not depend on it, bit for
+                             * bit (see "Determinism").  The cached and the stochastic rollouts always take the whole batch. */
 } spot_option;
 
 /* Validates cfg and w, builds the RoPE table (S5) and returns a context.  max_seqs bounds

@@ -19,7 +19,7 @@ _lib: Optional[C.CDLL] = None
 SPOT_F32, SPOT_BF16 = 0, 1
 EPI_BIAS, EPI_BIAS_GELU, EPI_GATE_RESIDUAL = 0, 1, 2
 IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_2CTA, IMPL_TCGEN05_TMA = 0, 1, 2, 3, 4
-OPT_GEMM_IMPL, OPT_ATTN_IMPL, OPT_TIMING, OPT_FP8 = 0, 1, 2, 3
+OPT_GEMM_IMPL, OPT_ATTN_IMPL, OPT_TIMING, OPT_FP8, OPT_CHUNK_SEQS = 0, 1, 2, 3, 4
 SPOT_E4M3 = 2     # storage type of the FP8 variant's activations / quantised weights (torch.float8_e4m3fn)
 STATUS_NAMES = ["SPOT_OK", "SPOT_ERR_NULL", "SPOT_ERR_SHAPE", "SPOT_ERR_DTYPE", "SPOT_ERR_ALIGN",
                 "SPOT_ERR_WORKSPACE", "SPOT_ERR_ARCH", "SPOT_ERR_CUDA", "SPOT_ERR_UNIMPLEMENTED"]

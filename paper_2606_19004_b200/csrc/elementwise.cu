@@ -342,12 +342,12 @@ __global__ void from_f32_kernel(const float* __restrict__ in, T* __restrict__ ou
 }
 // dst[b, :] = src[b / K, :]  (the prompt's text stream h_txt^0 is shared by its K seeds)
 __global__ void broadcast_prompts_kernel(const float4* __restrict__ src, float4* __restrict__ dst, int K,
-                                         long long n4, long long total4) {
+                                         long long n4, long long total4, int first_seq) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long stride = (long long)gridDim.x * blockDim.x;
   for (; i < total4; i += stride) {
     long long b = i / n4, e = i - b * n4;
-    dst[i] = src[(b / K) * n4 + e];
+    dst[i] = src[((b + first_seq) / K) * n4 + e];   // dst row b holds sequence first_seq + b of the call
   }
 }
 
@@ -510,10 +510,11 @@ cudaError_t launch_from_f32(spot_dtype dt, const float* in, void* out, long long
   return cudaGetLastError();
 }
 
-cudaError_t launch_broadcast_prompts(const float* src, float* dst, int B, int K, long long n_per_prompt, cudaStream_t st) {
+cudaError_t launch_broadcast_prompts(const float* src, float* dst, int B, int K, long long n_per_prompt, cudaStream_t st,
+                                     int first_seq) {
   const long long n4 = n_per_prompt / 4, total4 = n4 * B;
   if (total4 <= 0) return cudaSuccess;
-  broadcast_prompts_kernel<<<grid_for(total4, 256), 256, 0, st>>>((const float4*)src, (float4*)dst, K, n4, total4);
+  broadcast_prompts_kernel<<<grid_for(total4, 256), 256, 0, st>>>((const float4*)src, (float4*)dst, K, n4, total4, first_seq);
   return cudaGetLastError();
 }
 

@@ -73,7 +73,8 @@ cudaError_t launch_quantize_e4m3(spot_dtype dt, const void* in, long long n, voi
 // plumbing
 cudaError_t launch_to_f32(spot_dtype dt, const void* in, float* out, long long n, cudaStream_t st);
 cudaError_t launch_from_f32(spot_dtype dt, const float* in, void* out, long long n, cudaStream_t st);
-cudaError_t launch_broadcast_prompts(const float* src, float* dst, int B, int K, long long n_per_prompt, cudaStream_t st);
+cudaError_t launch_broadcast_prompts(const float* src, float* dst, int B, int K, long long n_per_prompt, cudaStream_t st,
+                                     int first_seq = 0);
 
 // K9: SIMT GEMM / attention (gemm_simt.cu, attn_simt.cu).  ta/tout: dtype of A and of the output
 // matrix (EPI_BIAS / EPI_BIAS_GELU); W and bias have dtype tw.

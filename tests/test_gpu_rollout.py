@@ -107,6 +107,33 @@ def test_cfg1_two_prompts_and_host_api(cfg1):
     assert torch.equal(h_out["top"], out["top"][:, :2].cpu()) and torch.equal(h_out["stats"], out["stats"].cpu())
 
 
+def test_cfg1_chunked_passes_are_bit_identical(cfg1):
+    """SPOT_OPT_CHUNK_SEQS (spot.h): a batch above the chunk size runs as consecutive chunks through all steps; chunks that
+    cut through a prompt group (3 of 2 x 4 sequences), a ragged last chunk, one sequence per pass and the whole batch in one
+    pass all give the same bits, and the one-pass result is the oracle's."""
+    s, w, ctx, text, probe = cfg1
+    ts = f32_timesteps(s)
+    text2 = make_text_emb(s.with_(n_prompts=2), "cuda")
+    seeds = [10, 11, 12, 13, 20, 21, 22, 23]
+    try:
+        spot.spot_set_option(ctx, spot.OPT_CHUNK_SEQS, 0)
+        whole = {k: v.clone() for k, v in spot.spot_explore(ctx, _seeds(seeds), text2, ts, probe, 2, 4, 2).items()}
+        lat, _ = oracle_explore(s, w, text2[1], probe, seeds[4:], ts)
+        assert rel_l2(np64(whole["latents"][4:]), lat) < 1e-4
+        for chunk in (1, 3, 4, 5, 8, 32):
+            spot.spot_set_option(ctx, spot.OPT_CHUNK_SEQS, chunk)
+            out = spot.spot_explore(ctx, _seeds(seeds), text2, ts, probe, 2, 4, 2)
+            for k in whole:
+                assert torch.equal(out[k], whole[k]), (chunk, k)
+            lat2 = spot.spot_noise_from_seeds(_seeds(seeds), s.n_img * s.latent_ch).reshape(8, s.n_img, s.latent_ch)
+            spot.spot_dit_denoise(ctx, lat2, text2, ts, 2, 4)
+            assert torch.equal(lat2, whole["latents"]), chunk
+        with pytest.raises(spot.SpotError):
+            spot.spot_set_option(ctx, spot.OPT_CHUNK_SEQS, -1)
+    finally:
+        spot.spot_set_option(ctx, spot.OPT_CHUNK_SEQS, 32)
+
+
 def test_seed_rewards_selection_with_ties(cfg1):
     s, w, ctx, _, _ = cfg1
     E = s.n_img * s.latent_ch
