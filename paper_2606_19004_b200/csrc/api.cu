@@ -695,10 +695,15 @@ spot_status denoise_cached_core(spot_ctx* c, int P, int K, float* lat, const voi
     if (n_act > 0) {
       LK(c, launch_tc_gather(h0, hc, d_idx, 1, n_act, per_img, st));
       if (NT > 0) LK(c, launch_tc_gather(txt_h0, h_txt, d_idx, K, n_act, per_txt, st));
-      for (int b = 0; b < L; ++b) {
-        const float* m = mod + ((long long)i * L + b) * 2 * 6 * D;
-        rs = block_core(c, b, n_act, hc, h_txt, m, m + 6 * D, ybuf, big, b == L - 1, st);
-        if (rs != SPOT_OK) return rs;
+      // the compacted batch goes through the block stack in chunks of at most chunk_seqs sequences (see denoise_core)
+      const int chunk = (c->chunk_seqs <= 0 || c->chunk_seqs > n_act) ? n_act : c->chunk_seqs;
+      for (int a0 = 0; a0 < n_act; a0 += chunk) {
+        const int nc = n_act - a0 < chunk ? n_act - a0 : chunk;
+        for (int b = 0; b < L; ++b) {
+          const float* m = mod + ((long long)i * L + b) * 2 * 6 * D;
+          rs = block_core(c, b, nc, hc + a0 * per_img, h_txt + a0 * per_txt, m, m + 6 * D, ybuf, big, b == L - 1, st);
+          if (rs != SPOT_OK) return rs;
+        }
       }
     }
     LK(c, launch_tc_combine(h0, resid, hc, d_pos, B, per_img, st));

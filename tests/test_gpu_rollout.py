@@ -128,6 +128,15 @@ def test_cfg1_chunked_passes_are_bit_identical(cfg1):
             lat2 = spot.spot_noise_from_seeds(_seeds(seeds), s.n_img * s.latent_ch).reshape(8, s.n_img, s.latent_ch)
             spot.spot_dit_denoise(ctx, lat2, text2, ts, 2, 4)
             assert torch.equal(lat2, whole["latents"]), chunk
+        # cached-step exploration: the compacted batch of every step is chunked the same way
+        cached = {}
+        for chunk in (0, 3):
+            spot.spot_set_option(ctx, spot.OPT_CHUNK_SEQS, chunk)
+            cached[chunk] = spot.spot_explore_cached(ctx, _seeds(seeds), text2, ts, probe, 2, 4, 2, threshold=3.0, coeffs=[1.0])
+        comp = cached[0]["computed"]
+        assert int(comp.sum()) == 2 * 8 and comp[:, 0].all() and comp[:, -1].all()   # first and last step computed, rest reused
+        for k in cached[0]:
+            assert torch.equal(cached[0][k], cached[3][k]), k
         with pytest.raises(spot.SpotError):
             spot.spot_set_option(ctx, spot.OPT_CHUNK_SEQS, -1)
     finally:
