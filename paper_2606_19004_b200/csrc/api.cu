@@ -588,9 +588,9 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
     LK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
   }
   // The batch runs as consecutive chunks of at most chunk_seqs sequences (an exploration batch is capped at 32
-  // sequences), each through all T steps: a chunk's activations (0.5 GB for the fc1 output of 16 sequences) stay closer to the
-  // 126 MB L2 than those of 256 sequences, which costs less HBM power under the cap (config 5: 26.2 -> 23.9 s), and a
-  // sequence's arithmetic does not depend on its batch, so the result is the same bit for bit.  Conditioning and h_txt^0
+  // sequences), each through all T steps: measured 9 % faster per sequence at config 5 than one pass over 256 sequences
+  // (26.2 -> 23.9 s; DESIGN.md section 5 "Chunked passes"), and a sequence's arithmetic does not depend on its batch, so
+  // the result is the same bit for bit.  Conditioning and h_txt^0
   // above are shared by all chunks.  The stochastic rollout keeps the whole batch (its log-probabilities are laid out per call).
   const int chunk = (sde || c->chunk_seqs <= 0 || c->chunk_seqs > B) ? B : c->chunk_seqs;
   const long long n_part = (E + REWARD_CHUNK - 1) / REWARD_CHUNK;
