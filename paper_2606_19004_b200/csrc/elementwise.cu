@@ -196,6 +196,20 @@ __global__ void __launch_bounds__(256) qk_norm_rope_kernel(T* __restrict__ qkv, 
     for (int h = 0; h < HPW; ++h)
 #pragma unroll
       for (int j = 0; j < EPL; ++j) x[h][j] = to_f32(reinterpret_cast<const T*>(&raw[h])[j]);
+  } else if constexpr (sizeof(T) * EPL == 32) {  // fp32, d_h = 128: two 128-bit accesses per lane and row
+    static_assert(sizeof(T) == 4, "32 bytes per lane is the fp32 d_h = 128 case");
+#pragma unroll
+    for (int h = 0; h < HPW; ++h)
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const float4 v = *reinterpret_cast<const float4*>(ptr + h * DH + 4 * k);
+        x[h][4 * k] = v.x; x[h][4 * k + 1] = v.y; x[h][4 * k + 2] = v.z; x[h][4 * k + 3] = v.w;
+      }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const float4 v = __ldg(reinterpret_cast<const float4*>(gain) + k);
+      g[4 * k] = v.x; g[4 * k + 1] = v.y; g[4 * k + 2] = v.z; g[4 * k + 3] = v.w;
+    }
   } else {
 #pragma unroll
     for (int h = 0; h < HPW; ++h)
@@ -236,6 +250,10 @@ __global__ void __launch_bounds__(256) qk_norm_rope_kernel(T* __restrict__ qkv, 
 #pragma unroll
       for (int j = 0; j < EPL; ++j) reinterpret_cast<T*>(&o)[j] = from_f32<T>(y[j]);
       *reinterpret_cast<uint4*>(ptr + h * DH) = o;
+    } else if constexpr (sizeof(T) * EPL == 32) {
+#pragma unroll
+      for (int k = 0; k < 2; ++k)
+        *reinterpret_cast<float4*>(ptr + h * DH + 4 * k) = make_float4(y[4 * k], y[4 * k + 1], y[4 * k + 2], y[4 * k + 3]);
     } else {
 #pragma unroll
       for (int j = 0; j < EPL; ++j) ptr[h * DH + j] = from_f32<T>(y[j]);
