@@ -33,6 +33,15 @@ def test_exports_every_declared_symbol(lib):
     assert lib.spot_status_string(2).decode().startswith("SPOT_ERR_SHAPE")
 
 
+def test_option_constants_match_the_header():
+    """The binding's OPT_* integers are the values of `spot_option` in include/spot.h."""
+    text = open(os.path.join(ROOT, "include", "spot.h")).read()
+    enum = dict((k, int(v)) for k, v in re.findall(r"\b(SPOT_OPT_[A-Z0-9_]+)\s*=\s*(\d+)", text))
+    assert len(enum) >= 5
+    for name, value in enum.items():
+        assert getattr(binding, name[len("SPOT_"):]) == value, name
+
+
 def _cfg_struct(s, **over):
     kw = dict(n_blocks=s.n_blocks, hidden=s.hidden, n_heads=s.n_heads, head_dim=s.head_dim, mlp_hidden=s.mlp_hidden,
               grid_h=s.grid_h, grid_w=s.grid_w, n_txt=s.n_txt, latent_ch=s.latent_ch, txt_dim=s.txt_dim,
