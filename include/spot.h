@@ -103,8 +103,8 @@ typedef enum {
   SPOT_OPT_CHUNK_SEQS = 4   /* sequences per pass of the block stack in spot_dit_denoise / spot_explore / spot_explore_host: larger
                              * batches run as consecutive chunks of this many sequences (PAPER.md:338 caps an exploration batch at
                              * 32 sequences); 0 = the whole batch in one pass; default 32.  Results do not depend on it, bit for
-                             * bit (see "Determinism").  The cached rollout chunks the compacted batch of computing sequences per step; the
-                             * stochastic rollout always takes the whole batch. */
+                             * bit (see "Determinism").  Applies to the stochastic rollout (spot_dit_denoise_sde) as well; the
+                             * cached rollout chunks each step's compacted batch of computing sequences. */
 } spot_option;
 
 /* Validates cfg and w, builds the RoPE table (S5) and returns a context.  max_seqs bounds

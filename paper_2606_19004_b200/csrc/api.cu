@@ -591,8 +591,8 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
   // sequences), each through all T steps: measured 9 % faster per sequence at config 5 than one pass over 256 sequences
   // (26.2 -> 23.9 s; DESIGN.md section 5 "Chunked passes"), and a sequence's arithmetic does not depend on its batch, so
   // the result is the same bit for bit.  Conditioning and h_txt^0
-  // above are shared by all chunks.  The stochastic rollout keeps the whole batch (its log-probabilities are laid out per call).
-  const int chunk = (sde || c->chunk_seqs <= 0 || c->chunk_seqs > B) ? B : c->chunk_seqs;
+  // above are shared by all chunks; the stochastic step takes its seeds, partial sums and log-probability rows at the chunk's offset.
+  const int chunk = (c->chunk_seqs <= 0 || c->chunk_seqs > B) ? B : c->chunk_seqs;
   const long long n_part = (E + REWARD_CHUNK - 1) / REWARD_CHUNK;
   for (int b0 = 0; b0 < B; b0 += chunk) {
     const int Bc = B - b0 < chunk ? B - b0 : chunk;
@@ -620,8 +620,9 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
       const bool last = i == T - 1;
       double cx, cv, cn;
       if (sde && i >= sde->lo && i < sde->hi && sde_coeffs(h_t[i], h_t[i + 1], sde->noise_level, &cx, &cv, &cn))
-        LK(c, launch_sde_update(lat_c, vel, sde->seeds, kSdeStreamBase + (uint32_t)i, cx, cv, cn, Bc, E, last ? probe : nullptr,
-                                c->d_partials2, partials_c, sde->logp + i, T, st));
+        LK(c, launch_sde_update(lat_c, vel, sde->seeds + b0, kSdeStreamBase + (uint32_t)i, cx, cv, cn, Bc, E,
+                                last ? probe : nullptr, c->d_partials2 + (long long)b0 * n_part, partials_c,
+                                sde->logp + (long long)b0 * T + i, T, st));
       else
         LK(c, launch_euler_update(lat_c, vel, h_t[i + 1] - h_t[i], Bc, E, last ? probe : nullptr, partials_c, st));
     }

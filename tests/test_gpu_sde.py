@@ -93,6 +93,14 @@ def test_cfg1_denoise_sde_matches_oracle():
     spot.spot_dit_denoise_sde(ctx, _seeds(seeds), lat_a, text, ts, 1, 3, a, (2, 2))
     spot.spot_dit_denoise(ctx, lat_b, text, ts, 1, 3)
     assert torch.equal(lat_a, lat_b)
+    # SPOT_OPT_CHUNK_SEQS: the stochastic rollout in chunks of 2 + 1 sequences gives the bits of the one-pass call
+    try:
+        spot.spot_set_option(ctx, spot.OPT_CHUNK_SEQS, 2)
+        lat_c = spot.spot_noise_from_seeds(_seeds(seeds), s.n_img * s.latent_ch).reshape(3, s.n_img, s.latent_ch)
+        out_c, logp_c = spot.spot_dit_denoise_sde(ctx, _seeds(seeds), lat_c, text, ts, 1, 3, a, window)
+        assert torch.equal(out_c, out) and torch.equal(logp_c, logp)
+    finally:
+        spot.spot_set_option(ctx, spot.OPT_CHUNK_SEQS, 32)
 
 
 def test_denoise_sde_bf16_full_width_reduced_depth():
