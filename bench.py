@@ -458,6 +458,7 @@ def main():
                 "data": "synthetic",
                 "config": {**workload_config(shape),
                            "l2": "inputs (40.8 GB of weights streamed every Euler step) are larger than L2",
+                           "chunk_seqs": 32,     # SPOT_OPT_CHUNK_SEQS default: batches above it run chunk by chunk (spot.h)
                            "parallelism": f"replicas x{world}, disjoint seed groups"},
                 "seeds_per_s": world * B / (ms_step / 1e3), "tflops_per_gpu": tflops,
                 "frac_of_bf16_peak": {"burst": tflops / peaks["bf16_tflops"], "sustained": tflops / peaks["bf16_tflops_sustained"],
