@@ -230,6 +230,7 @@ def run_kernels(args, shape):
     hbm("K4_qk_norm_rope", lambda: spot.spot_qk_norm_rope(qkv, shape.n_txt, gains, cs, sn, 1e-6), 2.0 * 2 * B * S * H * dh * 2)
     # K5 attention
     tensor("K5_attention", lambda: spot.spot_attention(qkv, spot.IMPL_TCGEN05), 4.0 * S * S * dh * H * B)
+    qkv_attn = qkv
     tensor("K5_attention_prev_two_pass", lambda: spot.spot_attention(qkv, spot.IMPL_TCGEN05_2CTA), 4.0 * S * S * dh * H * B)
     del qkv
     # K6 Euler update (+ reward): 2^26 elements so that the working set exceeds L2
@@ -270,6 +271,22 @@ def run_kernels(args, shape):
     res[name]["peak"] = 2.0 * peaks["bf16_tflops"]
     res[name]["frac"] = res[name]["achieved"] / res[name]["peak"]
     del a8, wq
+    # K5 sustained, measured last so that its heat does not colour the other rows: the same launch repeated back to back
+    # for about 1.5 s (no flush: 377 MB of q, k, v per launch > L2), one event pair around all of them: the rate under
+    # the power cap, against the SUSTAINED bf16 peak
+    n_rep = 4000
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n_rep):
+        spot.spot_attention(qkv_attn, spot.IMPL_TCGEN05)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / n_rep
+    fl = 4.0 * S * S * dh * H * B
+    res["K5_attention_sustained"] = {"bound": "tensor", "ms": ms, "flops": fl, "achieved": fl / ms / 1e9, "unit": "TFLOP/s",
+                                     "peak": peaks["bf16_tflops_sustained"], "frac": fl / ms / 1e9 / peaks["bf16_tflops_sustained"],
+                                     "peak_kind": f"measured sustained bf16; {n_rep} launches back to back"}
     print(json.dumps({"mode": "kernels", "workload": shape.name, "rows": M, "l2": "512 MiB written" + (", then read back (clean lines)," if args.flush == "clean" else "") + " between iterations",
                       "peaks": peaks, "kernels": res}))
 
