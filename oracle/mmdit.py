@@ -21,6 +21,27 @@ import numpy as np
 
 Array = np.ndarray
 
+# Optional host threads for the full-size golden runs (tests/golden/make_cfg3_golden.py).  They only change WHO
+# evaluates an independent piece (an attention head, a block of rows of an elementwise map, a sequence), never the
+# arithmetic or its order inside a piece; tests/test_oracle_mmdit.py pins the threaded results bit for bit to the
+# serial ones.  Default 1 = plain serial code, which is also what bench.py times as the CPU baseline.
+_WORKERS = 1
+
+
+def set_workers(n: int) -> None:
+    global _WORKERS
+    _WORKERS = max(1, int(n))
+
+
+def _pmap(fn, items, workers=None):
+    items = list(items)
+    w = _WORKERS if workers is None else workers
+    if w <= 1 or len(items) <= 1:
+        return [fn(i) for i in items]
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(w) as ex:
+        return list(ex.map(fn, items))
+
 
 def linear(x: Array, w: Array, b: Array | None, mode: str = "blas") -> Array:
     """y = x W^T + b ; x [n, in], W [out, in]."""
@@ -39,7 +60,10 @@ def silu(x: Array) -> Array:
 
 def gelu_tanh(x: Array) -> Array:
     """GELU_tanh(x) = x/2 (1 + tanh(sqrt(2/pi) (x + 0.044715 x^3)))  (reading S4)."""
-    return 0.5 * x * (1.0 + np.tanh(math.sqrt(2.0 / math.pi) * (x + 0.044715 * x ** 3)))
+    f = lambda x: 0.5 * x * (1.0 + np.tanh(math.sqrt(2.0 / math.pi) * (x + 0.044715 * x ** 3)))
+    if _WORKERS > 1 and x.ndim == 2 and x.shape[0] >= 2 * _WORKERS:
+        return np.concatenate(_pmap(f, np.array_split(x, _WORKERS, axis=0)), axis=0)      # elementwise: rows are independent
+    return f(x)
 
 
 def layer_norm(x: Array, eps: float) -> Array:
@@ -112,12 +136,15 @@ def attention(q: Array, k: Array, v: Array) -> Array:
     """softmax(Q K^T / sqrt(d_h)) V per head, all S keys, no mask (C5 step 6). q,k,v [S, H, d_h]."""
     S, H, dh = q.shape
     out = np.empty_like(q)
-    for h in range(H):
+
+    def head(h):
         logits = (q[:, h, :] @ k[:, h, :].T) / math.sqrt(dh)
         logits = logits - logits.max(axis=1, keepdims=True)
         p = np.exp(logits)
         p = p / p.sum(axis=1, keepdims=True)
         out[:, h, :] = p @ v[:, h, :]
+
+    _pmap(head, range(H))                                   # heads are independent; serial unless set_workers(n > 1)
     return out
 
 
@@ -194,3 +221,28 @@ def dit_velocity(x: Array, t: float, h_txt0: Array, g: Dict[str, Array], blocks:
     scale_f, shift_f = m_f[:D], m_f[D:]
     y = layer_norm(h_img, ln_eps) * (1.0 + scale_f) + shift_f
     return linear(y, g["proj_w"], g["proj_b"], mode)
+
+
+def dit_velocity_multi(xs: Sequence[Array], t: float, h_txt0s: Sequence[Array], g: Dict[str, Array], blocks, *,
+                       n_heads: int, cos: Array, sin: Array, ln_eps: float = 1e-6, rms_eps: float = 1e-6,
+                       mode: str = "blas", block_lin=None, workers: int = 1) -> List[Array]:
+    """dit_velocity for several INDEPENDENT sequences at the same t ("K samples from each of P prompts",
+    PAPER.md:61), with the loop over blocks outermost and the loop over sequences inside it, so that a driver which
+    can only hold one block's fp64 weights at a time (tests/golden/make_cfg3_golden.py) widens each block once per
+    pass instead of once per sequence.  Sequence j sees exactly the operations of dit_velocity(xs[j], t,
+    h_txt0s[j], ...) in the same order - no arithmetic is shared between sequences - and the test
+    test_dit_velocity_multi_is_dit_velocity pins the two bit for bit.  `workers` > 1 hands the sequences of a block to
+    host threads (same pin)."""
+    _, c = time_conditioning(t, g, mode)
+    h_img = [linear(x, g["img_in_w"], g["img_in_b"], mode) for x in xs]
+    h_txt = list(h_txt0s)
+    for bi, bw in enumerate(blocks):
+        lin = None if block_lin is None else block_lin(bi)
+        res = _pmap(lambda j: block_forward(h_img[j], h_txt[j], c, bw, n_heads=n_heads, cos=cos, sin=sin,
+                                            ln_eps=ln_eps, rms_eps=rms_eps, mode=mode, lin=lin), range(len(xs)), workers)
+        for j, (hi, ht) in enumerate(res):
+            h_img[j], h_txt[j] = hi, ht
+    m_f = linear(c[None, :], g["final_mod_w"], g["final_mod_b"], mode)[0]
+    D = h_img[0].shape[1]
+    scale_f, shift_f = m_f[:D], m_f[D:]
+    return [linear(layer_norm(h, ln_eps) * (1.0 + scale_f) + shift_f, g["proj_w"], g["proj_b"], mode) for h in h_img]

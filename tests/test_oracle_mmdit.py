@@ -5,6 +5,7 @@ Every check compares the oracle with something other than itself: a torch librar
 a brute-force Python loop, a closed form or an invariant.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -260,6 +261,111 @@ def test_text_input_and_final_layer_shapes():
     # zero projection => zero velocity
     g0 = dict(g, proj_w=np.zeros_like(g["proj_w"]), proj_b=np.zeros_like(g["proj_b"]))
     assert (mmdit.dit_velocity(x, 0.75, h0, g0, blocks, n_heads=s.n_heads, cos=cos, sin=sin) == 0).all()
+
+
+# ------------------------------------------------------------------ C4 / C7: conditioning and the final layer
+def _read_hand_case():
+    rows = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "final_layer_hand.txt")):
+        if line.strip() and not line.startswith("#"):
+            k, *v = line.split()
+            rows[k] = np.asarray([float(t) for t in v])
+    return rows
+
+
+def _hand_case_weights():
+    w1 = np.zeros((4, 256))
+    w1[0, 0] = 1.0
+    return {"time_w1": w1, "time_b1": np.array([0.0, 1.0, 0.0, 0.0]), "time_w2": np.diag([2.0, -1.0, 1.0, 1.0]),
+            "time_b2": np.array([0.0, 0.0, 0.0, 1.0]), "img_in_w": np.eye(4), "img_in_b": np.zeros(4),
+            "final_mod_w": np.concatenate([np.eye(4), 0.5 * np.eye(4)]),
+            "final_mod_b": np.array([0.25, -0.5, 0.0, 1.0, 0.1, 0.2, -0.3, 0.4]),
+            "proj_w": np.array([[1.0, 0, 0, 0], [0, 2.0, 0, 0], [0, 0, 1.0, 1.0], [0, 0, 0, -1.0]]),
+            "proj_b": np.array([0.0, 0.0, 0.0, 10.0])}
+
+
+def test_time_conditioning_and_final_layer_hand_worked_case():
+    """tests/golden/final_layer_hand.txt: numbers worked out with decimal arithmetic.  Fails if scale_f / shift_f are
+    swapped, if temb instead of SiLU(temb) feeds the modulation, if the LN epsilon is not 1e-6 inside the root, if
+    W1 / W2 / the biases of the time MLP are composed differently, or if proj is applied transposed."""
+    r = _read_hand_case()
+    g = _hand_case_weights()
+    temb, c = mmdit.time_conditioning(0.0, g)
+    assert np.abs(temb - r["temb"]).max() < 1e-15 and np.abs(c - r["c"]).max() < 1e-15
+    x = np.stack([r["x0"], r["x1"]])
+    none = np.zeros((0, 4))
+    v = mmdit.dit_velocity(x, 0.0, none, g, [], n_heads=1, cos=None, sin=None, ln_eps=1e-6)
+    assert np.abs(v - np.stack([r["v0"], r["v1"]])).max() < 1e-13
+    vm = mmdit.dit_velocity_multi([x[:1], x[1:]], 0.0, [none, none], g, [], n_heads=1, cos=None, sin=None, ln_eps=1e-6)
+    assert np.abs(np.concatenate(vm) - np.stack([r["v0"], r["v1"]])).max() < 1e-13
+    # the case is sensitive to the epsilon: row x0 has variance 1e-6
+    v_bad = mmdit.dit_velocity(x, 0.0, none, g, [], n_heads=1, cos=None, sin=None, ln_eps=1e-5)
+    assert np.abs(v_bad[0] - r["v0"]).max() > 0.1
+
+
+def _torch_velocity(x, t, h_txt0, g, blocks, s, cos, sin, *, swap=False, raw_temb=False, final_eps=None):
+    """Independent statement of v = DiT(x, t, text) with torch library routines (fp64); the keyword arguments build
+    the plausible MISTAKES the pin must reject."""
+    T = lambda a: torch.from_numpy(np.ascontiguousarray(a))
+    D = s.hidden
+    freqs = torch.pow(torch.tensor(10000.0, dtype=torch.float64), -torch.arange(128, dtype=torch.float64) / 128.0)
+    ang = 1000.0 * t * freqs
+    e = torch.cat([torch.cos(ang), torch.sin(ang)])
+    temb = F.linear(F.silu(F.linear(e, T(g["time_w1"]), T(g["time_b1"]))), T(g["time_w2"]), T(g["time_b2"]))
+    c = temb if raw_temb else F.silu(temb)
+    h_img, h_txt = F.linear(T(x), T(g["img_in_w"]), T(g["img_in_b"])).numpy(), h_txt0
+    for bw in blocks:
+        h_img, h_txt = _torch_joint_block(h_img, h_txt, c.numpy(), bw, s, cos, sin)
+    a, b = F.linear(c, T(g["final_mod_w"]), T(g["final_mod_b"])).chunk(2)
+    scale, shift = (b, a) if swap else (a, b)
+    y = F.layer_norm(T(h_img), (D,), eps=s.ln_eps if final_eps is None else final_eps) * (1 + scale) + shift
+    return F.linear(y, T(g["proj_w"]), T(g["proj_b"])).numpy()
+
+
+def test_velocity_against_torch_library_statement_and_its_mutants():
+    """Pins dit_velocity end to end (time MLP -> c = SiLU(temb) -> img_in -> blocks -> final modulation split
+    (scale_f, shift_f) -> LN with ln_eps -> proj) against torch library routines, with ln_eps != rms_eps and
+    weights large enough that every term matters; each plausible mistake moves the result by > 1e-3."""
+    s = CONFIGS[1].with_(ln_eps=1e-2)
+    g, blocks = weights_np64(make_weights(s))
+    for k in g:
+        g[k] = g[k] * (8.0 if k.startswith(("final_mod", "time_")) else 3.0)
+    te = np64(make_text_emb(s))[0]
+    h0 = mmdit.text_input(te, g, s.rms_eps)
+    cos, sin = mmdit.rope_table(s.grid_h, s.grid_w, s.n_txt, s.rope_pairs, s.rope_theta)
+    x = RNG.normal(size=(s.n_img, s.latent_ch)) * 0.05        # small rows: the LN epsilon matters
+    for t in (0.75, 0.1):
+        v = mmdit.dit_velocity(x, t, h0, g, blocks, n_heads=s.n_heads, cos=cos, sin=sin, ln_eps=s.ln_eps, rms_eps=s.rms_eps)
+        ref = _torch_velocity(x, t, h0, g, blocks, s, cos, sin)
+        assert rel_l2(v, ref) < 1e-12
+        for mistake in (dict(swap=True), dict(raw_temb=True), dict(final_eps=s.rms_eps)):
+            assert rel_l2(_torch_velocity(x, t, h0, g, blocks, s, cos, sin, **mistake), ref) > 1e-3, mistake
+    # temb / c themselves
+    temb, c = mmdit.time_conditioning(0.3, g)
+    assert np.abs(c - F.silu(torch.from_numpy(temb)).numpy()).max() < 1e-14 and np.abs(c - temb).max() > 1e-3
+
+
+def test_dit_velocity_multi_is_dit_velocity():
+    """The blocks-outermost loop order used by the full-size golden script gives, per sequence, the bits of dit_velocity."""
+    s = CONFIGS[1]
+    g, blocks = weights_np64(make_weights(s))
+    cos, sin = mmdit.rope_table(s.grid_h, s.grid_w, s.n_txt, s.rope_pairs, s.rope_theta)
+    h0s = [mmdit.text_input(np64(make_text_emb(s, prompts=[p]))[0], g) for p in (0, 1, 0)]
+    xs = [RNG.normal(size=(s.n_img, s.latent_ch)) for _ in range(3)]
+    vm = mmdit.dit_velocity_multi(xs, 0.6, h0s, g, iter(blocks), n_heads=s.n_heads, cos=cos, sin=sin)
+    for j in range(3):
+        assert (vm[j] == mmdit.dit_velocity(xs[j], 0.6, h0s[j], g, blocks, n_heads=s.n_heads, cos=cos, sin=sin)).all()
+    assert not (vm[0] == vm[2]).all() and rel_l2(vm[0], vm[1]) > 1e-6
+    # host threads (over sequences; over heads and row blocks) change nothing, bit for bit
+    vt = mmdit.dit_velocity_multi(xs, 0.6, h0s, g, iter(blocks), n_heads=s.n_heads, cos=cos, sin=sin, workers=3)
+    mmdit.set_workers(4)
+    try:
+        vw = mmdit.dit_velocity(xs[1], 0.6, h0s[1], g, blocks, n_heads=s.n_heads, cos=cos, sin=sin)
+        u = RNG.normal(size=(1280, 96)) * 3.0
+        gw = mmdit.gelu_tanh(u)
+    finally:
+        mmdit.set_workers(1)
+    assert all((vt[j] == vm[j]).all() for j in range(3)) and (vw == vm[1]).all() and (gw == mmdit.gelu_tanh(u)).all()
 
 
 def test_parameter_count_matches_20b():
