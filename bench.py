@@ -6,10 +6,18 @@ of the 60-block MMDiT -> probe rewards -> top/bottom-k selection (spot_explore).
 of BASELINE.json (512x512, 60 blocks, 1 prompt x 16 seeds, 10 Euler steps, bf16), the configuration the
 metric's ">= 50 % of dense BF16 peak" target is quoted on.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg4|cfg5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3|cfg4|cfg5] [--scaling weak|strong]
+                    [--impl reference] [--dry-run]
 
-N > 1 is launched by torch.distributed.run (one rank per GPU); ranks hold replicated weights and disjoint
-seed groups (weak scaling, no data-path collective; the K fp32 rewards are all-gathered once per step).
+N > 1 runs one rank per GPU over NCCL.  Either the caller starts the ranks (python -m torch.distributed.run
+--nproc-per-node N ... bench.py --gpus N: WORLD_SIZE must then equal --gpus) or, when WORLD_SIZE is not set,
+bench.py re-executes itself under torch.distributed.run with N ranks on 127.0.0.1.  It refuses to run when fewer
+than N CUDA devices are visible, and prints n_gpus = the number of ranks that actually joined the process group.
+  --scaling weak   (default) replicated weights, every rank explores its own P x K batch with disjoint seeds;
+  --scaling strong ONE P x K batch, sequence b on rank floor(b N / B) (sharding.explore_sharded).
+Both have no data-path collective; the fp32 rewards are all-gathered once per step.
+  --dry-run        host logic only (gloo, a stub step, no GPU, no library): the launcher / sharding / timing /
+                   JSON plumbing of the N > 1 path, used by the -m "not gpu" tests.
 """
 from __future__ import annotations
 
@@ -35,7 +43,7 @@ METRIC = "image-tokens*steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of gemm_tcgen05_v3_kernel, averaged over its four uses in a
 # block (QKV+RoPE 1.071 GB, out-proj 0.646 GB, fc1 1.451 GB, fc2 2.680 GB) - profiles/r1_ncu_full_gemm_v3.txt (config 3)
 GEMM_DRAM_TRAFFIC_PER_LAUNCH = {"cfg3": 1.462e9}
-WORKLOADS = {"cfg3": 3, "cfg4": 4, "cfg5": 5}
+WORKLOADS = {"cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
 
 
 def load_peaks():
@@ -291,6 +299,210 @@ def run_kernels(args, shape):
                       "peaks": peaks, "kernels": res}))
 
 
+def free_port() -> int:
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        return so.getsockname()[1]
+
+
+def ensure_ranks(args) -> int:
+    """Makes `--gpus N` mean N ranks.  Returns the world size of THIS process (after a re-exec under
+    torch.distributed.run when the caller did not start the ranks); exits loudly on any mismatch."""
+    env_world = os.environ.get("WORLD_SIZE")
+    if args.gpus < 1:
+        sys.exit("bench.py: --gpus must be >= 1")
+    if args.impl == "reference":                 # the oracle arm: rank 0 alone works, the other ranks (if any) exit 0
+        return int(env_world or "1")
+    if not args.dry_run and args.impl != "reference":
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            sys.exit(f"bench.py: --gpus {args.gpus} but only {have} CUDA device(s) are visible: refusing to print a "
+                     f"line for fewer GPUs than asked for")
+    if env_world is None and args.gpus > 1:
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__), *sys.argv[1:]]
+        print("bench.py: starting", args.gpus, "ranks:", " ".join(cmd), file=sys.stderr, flush=True)
+        sys.exit(subprocess.call(cmd))
+    world = int(env_world or "1")
+    if world != args.gpus:
+        sys.exit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: start the ranks with --nproc-per-node {args.gpus} "
+                 f"(or leave WORLD_SIZE unset and bench.py starts them itself)")
+    return world
+
+
+def parallelism_label(scaling: str, world: int, B: int) -> str:
+    if scaling == "strong":
+        return f"dp{world} strong: one batch of {B} sequences, sequence b on rank floor(b*{world}/{B}), weights replicated"
+    return f"dp{world} weak: replicated weights, {B} sequences per rank with disjoint seeds"
+
+
+def job_seeds(shape, scaling: str, rank: int, world: int):
+    """Seeds of this rank.  weak: the job explores world * B sequences, rank r owns [r*B, (r+1)*B); strong: the B seeds of
+    the config, all ranks hold all of them (explore_sharded slices)."""
+    from paper_2606_19004_b200 import sharding
+    B = shape.n_seqs
+    if scaling == "strong":
+        return [int(v) for v in shape.seeds]
+    lo, hi = sharding.shard_range(world * B, rank, world)
+    assert hi - lo == B
+    return [int(shape.seeds[i % B]) + (i // B) * B for i in range(lo, hi)]
+
+
+def run_dry(args, shape, world):
+    """--dry-run: the N > 1 host logic with a stub step on CPU (gloo)."""
+    import torch.distributed as dist
+    from paper_2606_19004_b200 import sharding
+    rank = int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    joined = torch.ones(1)
+    if world > 1:
+        dist.all_reduce(joined)
+    B, T = shape.n_seqs, shape.n_steps
+    seeds = job_seeds(shape, args.scaling, rank, world)
+    n_job = B if args.scaling == "strong" else world * B
+    lo, hi = sharding.shard_range(B, rank, world) if args.scaling == "strong" else (0, B)
+    full = None
+
+    def step():
+        nonlocal full
+        time.sleep(0.002 * (hi - lo))                                   # the stub: "compute" this rank's sequences
+        local = torch.tensor([((s * 2654435761) % 1000) / 1000.0 for s in seeds[lo:hi]], dtype=torch.float32)
+        full = sharding.gather_rewards(local, n_job) if world > 1 else local
+
+    for _ in range(args.warmup):
+        step()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    ms = sharding.max_over_ranks((time.perf_counter() - t0) * 1e3) / args.steps
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": n_job * shape.n_img * T / (ms / 1e3), "unit": METRIC, "dry_run": True,
+                          "n_gpus": int(joined.item()), "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+                          "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None, "dtype": "stub", "data": "synthetic",
+                          "config": {**workload_config(shape), "parallelism": parallelism_label(args.scaling, world, B)},
+                          "rewards_gathered": int(full.numel()), "gpu_launches": 0}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def run_block(args, shape):
+    """--workload cfg2 (BASELINE.json configs[1]; BASELINE.md section 3 "report TFLOP/s"): north-star call (2),
+    spot_dit_block_forward, on ONE full-width joint block with B = 8 sequences.  A step = one block evaluation; the
+    block's weights (0.68 GB) and intermediates (qkv 189 MB, MLP hidden 252 MB, fp32-free bf16 I/O 126 MB) exceed L2, and
+    512 MiB are written and read back between timed iterations anyway (config.l2)."""
+    import paper_2606_19004_b200 as spot
+    from paper_2606_19004_b200 import build as spot_build
+    from synth.manifest import make_block_inputs
+    assert int(os.environ.get("WORLD_SIZE", "1")) == 1, "cfg2 is a single-GPU line"
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: the product path has no CPU fallback"
+    torch.cuda.set_device(0)
+    spot_build.build()
+    spot.load_library()
+    peaks = load_peaks()
+    B = shape.n_seqs
+    w = make_weights(shape, device="cuda", blocks=[0])
+    ctx = spot.Context(shape, w, max_seqs=B)
+    h_img, h_txt, temb = make_block_inputs(shape, B, "cuda")
+    o_img, o_txt = torch.empty_like(h_img), torch.empty_like(h_txt)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    S, D, F = shape.seq, shape.hidden, shape.mlp_hidden
+    flops = B * (2.0 * S * D * (3 * D + D + 2 * F) + 4.0 * S * S * D)
+    gemm_flops = B * 2.0 * S * D * (3 * D + D + 2 * F)
+
+    def step():
+        spot.spot_dit_block_forward(ctx, 0, h_img, h_txt, temb, o_img, o_txt)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+    spot.spot_get_counters(ctx, reset=True)
+    spot.spot_set_option(ctx, spot.OPT_TIMING, 1)
+    sampler = ClockSampler(0)
+    sampler.start()
+    ts = []
+    for _ in range(args.steps):
+        flush.zero_()
+        flush.view(torch.int32).sum()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step()
+        e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    counters = spot.spot_get_counters(ctx, reset=True)
+    spot.spot_set_option(ctx, spot.OPT_TIMING, 0)
+    # sustained: the same call back to back for about a second (what a rollout sees), one event pair
+    n_rep = 300
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n_rep):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms_sus = e0.elapsed_time(e1) / n_rep
+    ms = statistics.median(ts)
+    # e2e: pinned host buffers -> device, the call, outputs -> pinned host, all inside the timed region
+    hp = [t.cpu().pin_memory() for t in (h_img, h_txt, temb)]
+    ho = [torch.empty_like(t, device="cpu").pin_memory() for t in (o_img, o_txt)]
+
+    def e2e_step():
+        for dst, src in zip((h_img, h_txt, temb), hp):
+            dst.copy_(src, non_blocking=True)
+        step()
+        for dst, src in zip(ho, (o_img, o_txt)):
+            dst.copy_(src, non_blocking=True)
+        torch.cuda.synchronize()
+
+    e2e_step()
+    w0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()
+    e_ms = (time.perf_counter() - w0) * 1e3 / args.steps
+    units = B * shape.n_img
+    tf = flops / ms / 1e9
+    gemm_tf = gemm_flops * counters["gemm_timed"] / max(1, counters["gemm_launches"]) * args.steps / (counters["gemm_ms"] / 1e3) / 1e12 \
+        if counters["gemm_ms"] > 0 else None
+    line = {"metric": METRIC, "value": units / (ms / 1e3), "unit": METRIC, "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup),
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {**workload_config(shape), "note": "one joint block (spot_dit_block_forward); a step = one block evaluation of 8 sequences",
+                       "l2": "512 MiB written and read back between timed iterations; the block's working set exceeds L2 as well"},
+            "tflops_per_gpu": tf, "ms_at_100pct_of_burst_peak": flops / peaks["bf16_tflops"] / 1e9,
+            "frac_of_bf16_peak": {"burst": tf / peaks["bf16_tflops"], "sustained": tf / peaks["bf16_tflops_sustained"],
+                                  "nominal_2250": tf / 2250.0, "peaks": peaks["source"]},
+            "sustained": {"ms_per_step": ms_sus, "tflops": flops / ms_sus / 1e9, "launches_back_to_back": n_rep,
+                          "frac_of_sustained_peak": flops / ms_sus / 1e9 / peaks["bf16_tflops_sustained"]},
+            "clocks": clocks, "gpu_launches": counters["launches"],
+            "e2e": {"value": units / (e_ms / 1e3), "unit": METRIC, "ms_per_step": e_ms,
+                    "h2d_bytes_per_step": sum(t.numel() * t.element_size() for t in hp),
+                    "d2h_bytes_per_step": sum(t.numel() * t.element_size() for t in ho),
+                    "note": "pinned host tensors copied by the binding's caller around the device-pointer C-ABI call"},
+            "roofline": {"bound": "tensor", "kernel": "gemm_tcgen05_v3_kernel", "achieved": gemm_tf, "peak": peaks["bf16_tflops"],
+                         "peak_kind": f"{peaks['source']} burst bf16 (kernel timed in a 2 ms call after an L2 flush)", "unit": "TFLOP/s",
+                         "frac": gemm_tf / peaks["bf16_tflops"] if gemm_tf else None, "traffic": None,
+                         "launches_timed": counters["gemm_timed"], "avg_launch_ms": counters["gemm_ms"] / max(1, counters["gemm_timed"])},
+            "cpu_baseline": None}
+    if not args.no_cpu_baseline:
+        from oracle import mmdit
+        from tests.helpers import np64
+        bw = {k: np64(v) for k, v in w["blocks"][0].items()}
+        cos, sin = mmdit.rope_table(shape.grid_h, shape.grid_w, shape.n_txt, shape.rope_pairs, shape.rope_theta)
+        c = mmdit.silu(np64(temb))
+        hi, ht = np64(h_img[:2]), np64(h_txt[:2])
+        t0 = time.perf_counter()
+        for b in range(2):
+            mmdit.block_forward(hi[b], ht[b], c, bw, n_heads=shape.n_heads, cos=cos, sin=sin, ln_eps=shape.ln_eps, rms_eps=shape.rms_eps)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": 2 * shape.n_img / dt, "unit": METRIC, "cores": cpu_threads(), "kind": "oracle", "seconds": dt,
+                                "sample": "2 of the 8 sequences through the block (work is linear in sequences)"}
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--kernels", action="store_true", help="time every kernel alone against its roofline")
@@ -302,6 +514,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="spot", choices=["spot", "reference"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank its own P x K batch (disjoint seeds); strong = ONE P x K batch sharded over "
+                         "the ranks through sharding.explore_sharded (SURVEY.md 8(e))")
+    ap.add_argument("--dry-run", action="store_true", help="host logic only: gloo, stub step, no GPU (tests)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--gemm-impl", type=int, default=0,
@@ -315,23 +531,38 @@ def main():
                          "adds the effective denoising steps; no e2e leg")
     args = ap.parse_args()
     shape = CONFIGS[WORKLOADS[args.workload]]
+    world = ensure_ranks(args)
     if args.impl == "reference":
         return run_reference(args, shape)
+    if args.dry_run:
+        return run_dry(args, shape, world)
     if args.kernels:
         return run_kernels(args, shape)
+    if args.precision == "fp8" and args.gemm_impl not in (0,):
+        sys.exit("bench.py: --precision fp8 runs only on the default GEMM (--gemm-impl 0); other values would run bf16 Linears")
+    if args.workload == "cfg2":
+        return run_block(args, shape)
 
     import paper_2606_19004_b200 as spot
     from paper_2606_19004_b200 import build as spot_build
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device: the product path has no CPU fallback"
     torch.cuda.set_device(local_rank)
     dist = None
+    nccl_log = None
     if world > 1:
         import torch.distributed as dist
+        if "NCCL_DEBUG" not in os.environ:                       # keep the communicator's own record (ranks, NVLS, rings) ...
+            os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+            nccl_log = os.path.join(ROOT, "gpurun_out", f"nccl_n{world}_rank%p.log")
+            os.environ.update(NCCL_DEBUG="INFO", NCCL_DEBUG_SUBSYS="INIT", NCCL_DEBUG_FILE=nccl_log)   # ... out of stdout
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    joined = torch.ones(1, device="cuda")
+    if dist is not None:
+        dist.all_reduce(joined)                                  # n_gpus of the line = ranks that really joined
+    assert int(joined.item()) == world
     if rank == 0:
         spot_build.build()
     if dist is not None:
@@ -352,20 +583,23 @@ def main():
         spot.spot_set_option(ctx, spot.OPT_GEMM_IMPL, args.gemm_impl)
     ts = [float(np.float32(t)) for t in shape.timesteps]
     k_sel = K // 2
-    # weak scaling: the job explores world * B sequences; rank r owns the contiguous shard [r*B, (r+1)*B)
     from paper_2606_19004_b200 import sharding
-    lo, hi = sharding.shard_range(world * B, rank, world)
-    assert hi - lo == B
-    seeds = torch.tensor([int(shape.seeds[i % B]) + (i // B) * B for i in range(lo, hi)], dtype=torch.int64, device="cuda")
+    strong = args.scaling == "strong"
+    seeds = torch.tensor(job_seeds(shape, args.scaling, rank, world), dtype=torch.int64, device="cuda")
+    n_job = B if strong else world * B                              # sequences the whole job explores per step
     out = None
 
     cached = args.cache_threshold is not None
     fp8 = args.precision == "fp8"
-    if cached or fp8:
+    if cached or fp8 or strong:
         args.no_e2e = True
+        assert not (strong and (cached or fp8)), "--scaling strong times the plain bf16 rollout"
 
     def step():
         nonlocal out
+        if strong:
+            out = sharding.explore_sharded(ctx, seeds, text, ts, probe, P, K, k_sel)     # shard + all-gather + selection
+            return
         if cached:
             out = spot.spot_explore_cached(ctx, seeds, text, ts, probe, P, K, k_sel, args.cache_threshold, None, out)
         else:
@@ -406,16 +640,17 @@ def main():
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         ms_total = tt.item()
     ms_step = ms_total / args.steps
-    units_per_step = world * B * shape.n_img * T                     # image tokens x Euler steps, all ranks
+    units_per_step = n_job * shape.n_img * T                         # image tokens x Euler steps, all ranks
     value = units_per_step / (ms_step / 1e3)
     eff_frac = float(out["computed"].sum().item()) / (B * T) if cached else 1.0     # share of (sequence, step) pairs computed
-    flops_step = shape.flops_per_rollout() * eff_frac
-    tflops = flops_step / (ms_step / 1e3) / 1e12                     # per GPU
+    my_seqs = B if not strong else sharding.shard_sizes(B, world)[rank]
+    flops_step = shape.flops_per_rollout() * eff_frac * (n_job / B) / world          # per GPU (mean over ranks)
+    tflops = flops_step / (ms_step / 1e3) / 1e12
 
     # roofline of the dominant kernel (tcgen05 GEMM): algorithmic GEMM FLOPs / event-timed GEMM device time
     S, D, F, L = shape.seq, shape.hidden, shape.mlp_hidden, shape.n_blocks
     lin_per_seq_block = 2 * D * (3 * D + D + 2 * F)                   # per token
-    gemm_flops_step = eff_frac * T * B * (L * S * lin_per_seq_block - shape.n_txt * 2 * D * (D + 2 * F))   # last block: no text tail
+    gemm_flops_step = eff_frac * T * my_seqs * (L * S * lin_per_seq_block - shape.n_txt * 2 * D * (D + 2 * F))   # last block: no text tail (this rank)
     timed_frac = counters["gemm_timed"] / max(1, counters["gemm_launches"])
     gemm_ms = counters["gemm_ms"]
     gemm_tflops = (gemm_flops_step * args.steps * timed_frac) / (gemm_ms / 1e3) / 1e12 if gemm_ms > 0 else None
@@ -458,7 +693,7 @@ def main():
         assert torch.equal(h_out["rewards"], out["rewards"].cpu()), "host and device entry points disagree"
 
     cpu_baseline = None
-    if rank == 0 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
         nb = SAMPLE_BLOCKS
         w_host = {"global": {k: v.cpu() for k, v in weights["global"].items()},
                   "blocks": [{k: v.cpu() for k, v in b.items()} for b in weights["blocks"][:nb]]}
@@ -469,19 +704,21 @@ def main():
                                   "(work is linear in seeds, steps, blocks)"}
 
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        line = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": int(joined.item()), "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_step, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
                 "dtype": "fp8_e4m3 block Linears (bf16 attention, fp32 residual): exploration variant, not the headline" if fp8 else "bf16",
                 "data": "synthetic",
                 "config": {**workload_config(shape),
                            "l2": "inputs (40.8 GB of weights streamed every Euler step) are larger than L2",
                            "chunk_seqs": 32,     # SPOT_OPT_CHUNK_SEQS default: batches above it run chunk by chunk (spot.h)
-                           "parallelism": f"replicas x{world}, disjoint seed groups"},
-                "seeds_per_s": world * B / (ms_step / 1e3), "tflops_per_gpu": tflops,
+                           "parallelism": parallelism_label(args.scaling, world, B)},
+                "seeds_per_s": n_job / (ms_step / 1e3), "tflops_per_gpu": tflops,
                 "frac_of_bf16_peak": {"burst": tflops / peaks["bf16_tflops"], "sustained": tflops / peaks["bf16_tflops_sustained"],
                                       "nominal_2250": tflops / 2250.0, "peaks": peaks["source"]},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": counters["launches"], "roofline": roofline,
                 "cpu_baseline": cpu_baseline, "weight_gen_s": gen_s}
+        if nccl_log:
+            line["nccl_log"] = os.path.relpath(nccl_log, ROOT)
         rk = lambda v: torch.argsort(torch.argsort(v)).double()
         if fp8:
             line["fp8"] = {"reward_rank_correlation_vs_bf16_per_prompt":
