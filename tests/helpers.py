@@ -20,3 +20,20 @@ def rel_l2(a, b):
     a = np.asarray(a, dtype=np.float64).reshape(-1)
     b = np.asarray(b, dtype=np.float64).reshape(-1)
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+BF16_U = 2.0 ** -8          # unit roundoff of one round-to-nearest bf16 store (8 significand bits)
+
+
+def elem_excess(got, ref, rel, abs_rms):
+    """Per-element parity: max over elements of |got - ref| / (rel * |ref| + abs_rms * rms(ref)).  <= 1 means EVERY
+    element is within `rel` of the oracle (one output rounding) plus an absolute floor scaled by the tensor's rms
+    (accumulation-order error of elements that cancel to near zero).  A whole-tensor rel-L2 cannot see one wrong
+    element in 10^5; this can: a wrong element is off by ~rms(ref), hundreds of times the bound."""
+    got = np.asarray(got, dtype=np.float64).reshape(-1)
+    ref = np.asarray(ref, dtype=np.float64).reshape(-1)
+    if ref.size == 0:
+        return 0.0
+    rms = float(np.sqrt(np.mean(ref * ref)))
+    bound = rel * np.abs(ref) + abs_rms * max(rms, 1e-300)
+    return float((np.abs(got - ref) / bound).max())

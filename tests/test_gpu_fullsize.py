@@ -17,10 +17,10 @@ import pytest
 import torch
 
 import paper_2606_19004_b200 as spot
-from oracle import rollout
+from oracle import philox, rollout
 from synth import CONFIGS, make_probe, make_text_emb, make_weights, tensor_checksum
 from tests.gpu_common import device_weights, ensure_built, f32_timesteps, oracle_explore
-from tests.helpers import np64, rel_l2
+from tests.helpers import elem_excess, np64, rel_l2
 
 pytestmark = pytest.mark.gpu
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
@@ -53,6 +53,28 @@ def full_model():
     return s, w
 
 
+def _x0(s, seed):
+    """The initial latent as the CUDA path stores it (fp32), from the ORACLE's generator."""
+    x = philox.noise_from_seeds([int(seed)], s.n_img * s.latent_ch)[0].reshape(s.n_img, s.latent_ch)
+    return x.astype(np.float32).astype(np.float64)
+
+
+def _update_errors(s, seed, got, ref):
+    """What the model contributed, x_T - x_0, on its own scale: the final latent is dominated by the initial noise
+    (|x_0| 256 of |x_T| 297 at config 3), so a bound on x_T alone is about half as strict as it reads.
+    Returns (rel-L2 of the update, worst element of the update in units of 5e-2 |ref update| + 2.5e-2 rms(update))."""
+    x0 = _x0(s, seed)
+    return rel_l2(got - x0, ref - x0), elem_excess(got - x0, ref - x0, 5e-2, 2.5e-2)
+
+
+def _alone_equals_in_batch(ctx, s, text_rows, ts, probe, seeds, out, positions):
+    """Bit-identity of a sequence run alone (and of a pair of them) with the same sequence inside the batch, at the given
+    batch positions: carries the golden seed's parity to the other seeds, rows and chunks of the launch."""
+    for i in positions:
+        alone = spot.spot_explore(ctx, _seeds([seeds[i]]), text_rows(i), ts, probe, 1, 1, 0)
+        assert torch.equal(alone["latents"][0], out["latents"][i]) and torch.equal(alone["rewards"][0], out["rewards"][i]), i
+
+
 def _check_weights(meta, w, text, probe):
     assert {k: tensor_checksum(v) for k, v in sorted(w["global"].items())} == meta["global_checksums"]
     for b, want in enumerate(meta["block_checksums"]):
@@ -80,6 +102,9 @@ def test_cfg3_full_size_against_golden(full_model):
           f"(reward {out['rewards'][i].item():.6f} vs oracle {meta['reward']:.6f})")
     assert e_lat < 5e-2
     assert abs(out["rewards"][i].item() - meta["reward"]) < 5e-2 * max(np.abs(np64(out["rewards"])).max(), 1e-30)
+    e_upd, ex_upd = _update_errors(s, meta["seed"], np64(out["latents"][i]), lat_ref)
+    print(f"cfg3 full size: x_T - x_0 rel-L2 {e_upd:.3e}, worst element at {ex_upd:.2f} of its bound")
+    assert e_upd < 5e-2 and ex_upd <= 1.0
     # properties at full size --------------------------------------------------------------------------------
     lat = np64(out["latents"])
     rew = np64(out["rewards"])
@@ -89,9 +114,11 @@ def test_cfg3_full_size_against_golden(full_model):
     assert out["top"].cpu().tolist() == sel["top"].tolist() and out["bottom"].cpu().tolist() == sel["bottom"].tolist()
     assert abs(out["stats"][0, 1].item() - sel["std"][0]) < 1e-5 * max(1.0, sel["std"][0])
     assert np.isfinite(lat).all() and np.std(rew) > 0
-    # seed independence: the sampled seed alone gives the same bits as inside the 16-seed batch
-    alone = spot.spot_explore(ctx, _seeds([meta["seed"]]), text, ts, probe, 1, 1, 0)
-    assert torch.equal(alone["latents"][0], out["latents"][i]) and torch.equal(alone["rewards"][0], out["rewards"][i])
+    # seed independence: a seed alone gives the same bits as inside the 16-seed batch - the golden seed, the first, a
+    # middle and the last row of the batch
+    _alone_equals_in_batch(ctx, s, lambda j: text, ts, probe, list(s.seeds), out, sorted({i, 0, 7, K - 1}))
+    pair = spot.spot_explore(ctx, _seeds([s.seeds[K - 1], s.seeds[5]]), text, ts, probe, 1, 2, 1)     # other order, other batch size
+    assert torch.equal(pair["latents"][0], out["latents"][K - 1]) and torch.equal(pair["latents"][1], out["latents"][5])
     # so every other seed of the batch is covered by the same code path that the golden seed verified
 
 
@@ -160,6 +187,88 @@ def test_cfg5_prompt_independence_and_golden(full_model):
         print(f"cfg5 full size, seed {meta['seed']}: latents rel-L2 {e_lat:.3e}, reward {out['rewards'][i].item():.6f} vs {meta['reward']:.6f}")
         assert e_lat < 5e-2
         assert abs(out["rewards"][i].item() - meta["reward"]) < 5e-2 * np.abs(rew).max()
+        e_upd, ex_upd = _update_errors(s, meta["seed"], np64(out["latents"][i]), lat_ref)
+        print(f"cfg5 full size: x_T - x_0 rel-L2 {e_upd:.3e}, worst element at {ex_upd:.2f} of its bound")
+        assert e_upd < 5e-2 and ex_upd <= 1.0
+    # rows at chunk boundaries of the 256-sequence launch (SPOT_OPT_CHUNK_SEQS = 32): last row of chunk 0, first row of
+    # chunk 1, a middle row, the very last row - each alone is bit-identical to itself inside the batch
+    _alone_equals_in_batch(ctx, s, lambda j: text[j // K:j // K + 1].contiguous(), ts, probe, list(s.seeds), out, [31, 32, 100, P * K - 1])
+    # ---- all stored oracle seeds of prompt 7 (tests/golden/cfg5_p7_a / _b: 16 seeds each, make_cfg3_golden.py --seeds):
+    # rewards, sigma_g and top / bottom-k against ORACLE rewards under reading S12
+    metas = [_load_multi(n) for n in ("cfg5_p7_a", "cfg5_p7_b")]
+    metas = [m for m in metas if m is not None]
+    if metas:
+        o_seeds = [sd for m, _ in metas for sd in m["seeds"]]
+        o_rew = np.asarray([r for m, _ in metas for r in m["rewards"]])
+        o_lat = np.concatenate([l for _, l in metas])
+        idx = [list(s.seeds).index(sd) for sd in o_seeds]
+        assert all(j // K == g for j in idx) and metas[0][0]["n_blocks"] == s.n_blocks and metas[0][0]["n_steps"] == s.n_steps
+        _check_weights(metas[0][0], w, text[g:g + 1], probe)
+        g_rew = np64(out["rewards"])[idx]
+        scale = np.abs(o_rew).max()
+        worst_lat = max(rel_l2(np64(out["latents"][j]), o_lat[n]) for n, j in enumerate(idx))
+        worst_upd = max(_update_errors(s, o_seeds[n], np64(out["latents"][j]), o_lat[n])[0] for n, j in enumerate(idx))
+        e_rew = np.abs(g_rew - o_rew).max() / scale
+        n = len(idx)
+        o_sel = rollout.select_seeds(o_rew[None, :], n // 2)
+        st, top, bottom = spot.spot_select_seeds(out["rewards"][idx].contiguous(), 1, n, n // 2)       # the CUDA selection on the CUDA rewards
+        sig_err = abs(st[0, 1].item() - o_sel["std"][0]) / o_sel["std"][0]
+        gap = 2 * 5e-2 * scale                                                                          # reading S12
+        excl_s12 = sum(1 for a in range(n) for b in range(a + 1, n) if abs(o_rew[a] - o_rew[b]) <= gap)
+        gap_meas = 2 * np.abs(g_rew - o_rew).max()
+        excl_meas = sum(1 for a in range(n) for b in range(a + 1, n) if abs(o_rew[a] - o_rew[b]) <= gap_meas)
+        same_sets = set(top[0].tolist()) == set(o_sel["top"][0].tolist()) and set(bottom[0].tolist()) == set(o_sel["bottom"][0].tolist())
+        same_order = top[0].tolist() == o_sel["top"][0].tolist() and bottom[0].tolist() == o_sel["bottom"][0].tolist()
+        print(f"cfg5 prompt {g}: {n} of {K} seeds against oracle rewards: worst latents rel-L2 {worst_lat:.3e}, worst x_T - x_0 "
+              f"rel-L2 {worst_upd:.3e}, rewards max err {e_rew:.3e} of max|r|, sigma_g rel err {sig_err:.3e}; top/bottom-{n // 2} "
+              f"sets identical: {same_sets}, in the same order: {same_order}; pairs excluded under S12 (gap <= {gap:.3f}): "
+              f"{excl_s12} of {n * (n - 1) // 2}; pairs closer than twice the measured reward error ({gap_meas:.2e}): {excl_meas}")
+        assert worst_lat < 5e-2 and worst_upd < 5e-2 and e_rew < 5e-2 and sig_err < 5e-2
+        for name, got, ref in (("top", top[0].tolist(), o_sel["top"][0].tolist()), ("bottom", bottom[0].tolist(), o_sel["bottom"][0].tolist())):
+            for a in set(ref) - set(got):               # a seed the oracle selects and the CUDA path does not ...
+                for b in set(got) - set(ref):           # ... may only have lost its place to one within the S12 gap
+                    assert abs(o_rew[a] - o_rew[b]) <= gap, (name, a, b)
+        if excl_meas == 0:
+            assert same_order                           # no pair is closer than the reward error: the order is unique
+
+
+def _load_multi(name):
+    path = os.path.join(GOLDEN, name + ".json")
+    if not os.path.exists(path):
+        return None
+    return json.load(open(path)), np.load(os.path.join(GOLDEN, name + "_latent.npy")).astype(np.float64)
+
+
+def test_cfg4_full_size_against_golden(full_model):
+    """Config 4 (1280 x 1280: 6400 image + 256 text tokens, 52 key tiles per attention item, 4 seeds, 8 Euler steps) at
+    FULL depth against the oracle's result for seed 0 (tests/golden/cfg4_seed0*, make_cfg3_golden.py --config 4;
+    BASELINE.json configs[3], "1280 x 1280")."""
+    _, w = full_model
+    s = CONFIGS[4]
+    meta, lat_ref = _load_golden("cfg4_seed0")
+    assert meta["n_blocks"] == s.n_blocks and meta["n_steps"] == s.n_steps and meta["config"] == s.name
+    text, probe = make_text_emb(s, "cuda"), make_probe(s, "cuda")
+    _check_weights(meta, w, text, probe)
+    ctx = spot.Context(s, w, max_seqs=s.n_seqs)
+    ts = f32_timesteps(s)
+    assert ts == meta["timesteps"]
+    K = s.seeds_per_prompt
+    out = spot.spot_explore(ctx, _seeds(s.seeds), text, ts, probe, 1, K, K // 2)      # bench.py --workload cfg4's launch
+    torch.cuda.synchronize()
+    i = list(s.seeds).index(meta["seed"])
+    e_lat = rel_l2(np64(out["latents"][i]), lat_ref)
+    e_upd, ex_upd = _update_errors(s, meta["seed"], np64(out["latents"][i]), lat_ref)
+    rew = np64(out["rewards"])
+    print(f"cfg4 full size, seed {meta['seed']}: latents rel-L2 {e_lat:.3e}, x_T - x_0 rel-L2 {e_upd:.3e} (worst element at "
+          f"{ex_upd:.2f} of its bound), reward {rew[i]:.6f} vs oracle {meta['reward']:.6f}")
+    assert e_lat < 5e-2 and e_upd < 5e-2 and ex_upd <= 1.0
+    assert abs(rew[i] - meta["reward"]) < 5e-2 * max(np.abs(rew).max(), 1e-30)
+    lat = np64(out["latents"])
+    ref_rew = np.array([rollout.probe_reward(lat[b], np64(probe)) for b in range(K)])
+    assert np.abs(rew - ref_rew).max() < 1e-5 * max(1.0, np.abs(ref_rew).max())
+    sel = rollout.select_seeds(rew[None, :], K // 2)
+    assert out["top"].cpu().tolist() == sel["top"].tolist() and out["bottom"].cpu().tolist() == sel["bottom"].tolist()
+    _alone_equals_in_batch(ctx, s, lambda j: text, ts, probe, list(s.seeds), out, [i, K - 1])
 
 
 def test_cfg4_shape_reduced_depth_against_live_oracle():
