@@ -222,15 +222,20 @@ spot_status spot_explore_cached(spot_ctx *ctx, int n_prompts, int seeds_per_prom
  * FlowGRPO", Table 2 (:477-482) "SDE window".  DESIGN.md section 11 (readings D1-D4): steps window_lo <= i < window_hi
  * of the grid take the marginal-preserving reverse-SDE step of the rectified flow
  *     mean = x (1 + sigma^2/(2 t_i) dt) + v (1 + sigma^2 (1 - t_i)/(2 t_i)) dt,   x_next = mean + sigma sqrt(-dt) xi,
- *     sigma = noise_level * sqrt(t/(1-t))  (t = t_i, or t_{i+1} when t_i == 1),  dt = t_{i+1} - t_i < 0,
- * with xi ~ N(0, I) from Philox stream 256 + i of the sequence's seed (same generator as (1)); all other steps are the
- * Euler steps of (3).  d_logp [P*K, n_steps] fp32 receives log N(x_next; mean, sigma^2 (-dt) I) averaged over the
+ *     sigma = noise_level * sqrt(t_i/(1-t')),  t' = t_i, or t_{i+1} when t_i == 1 (FlowGRPO's rule for the singular first
+ *     step: only the denominator moves),  dt = t_{i+1} - t_i < 0,
+ * with xi ~ N(0, I) from Philox stream 256 + j of the sequence's seed (same generator as (1)), j = first_step + i the
+ * GLOBAL index of the step: a rollout split over several calls (resume after a preemption) passes the
+ * number of steps already taken as first_step, so that it neither reuses a noise stream nor shifts the window - the
+ * window test is window_lo <= j < window_hi as well, and a split rollout is bit-identical to the unsplit one.  All other
+ * steps are the Euler steps of (3).  d_logp [P*K, n_steps] fp32 receives log N(x_next; mean, sigma^2 (-dt) I) averaged over the
  * elements of the latent (0 for deterministic steps) - the per-step log-probability GRPO consumes.
- * Requires 1 >= t_0 > t_1 > ... > t_T >= 0, noise_level >= 0, 0 <= window_lo <= window_hi.  Workspace as (3). */
+ * Requires 1 >= t_0 > t_1 > ... > t_T >= 0, noise_level >= 0, 0 <= window_lo <= window_hi, first_step >= 0 (else
+ * SPOT_ERR_SHAPE).  Workspace as (3). */
 spot_status spot_dit_denoise_sde(spot_ctx *ctx, int n_prompts, int seeds_per_prompt, const uint64_t *d_seeds,
                                  float *d_latents, const void *d_text_emb, const float *h_timesteps, int n_steps,
-                                 float noise_level, int window_lo, int window_hi, float *d_logp,
-                                 void *d_workspace, size_t ws_bytes, void *cuda_stream);
+                                 float noise_level, int window_lo, int window_hi, int first_step,
+                                 float *d_logp, void *d_workspace, size_t ws_bytes, void *cuda_stream);
 
 /* ---- Low-precision exploration variant: FP8 (E4M3) block Linears ----------------------------------------------
  * PAPER.md:67 (s2.2): "first running a cheap exploratory rollout e.g., with reduced denoising steps or a quantized

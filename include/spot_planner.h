@@ -24,7 +24,7 @@ typedef struct spot_planner spot_planner;
 typedef struct { int32_t d, s; } spot_action;
 
 /* Action grid = d_values x s_values (all > 0, each list without duplicates); n_prompts = C; t_step > 0 seconds per
- * denoising step per sequence; beta > 0; window = W_b >= 1. */
+ * denoising step per sequence; beta >= 0 (0 = greedy on the window means; the paper sweeps beta in {0, 0.5, 1.0}); window = W_b >= 1. */
 spot_status spot_planner_create(const int32_t *d_values, int n_d, const int32_t *s_values, int n_s, int n_prompts,
                                 double t_step, double beta, int window, spot_planner **out);
 spot_status spot_planner_destroy(spot_planner *p);

@@ -18,7 +18,8 @@ with noise level a.  One Euler-Maruyama step from t_i to t_{i+1} (dt = t_{i+1} -
       x_next  = mean + sigma sqrt(-dt) xi ,   xi ~ N(0, I)
       log p   = mean_e[ -(x_next - mean)^2 / (2 sigma^2 (-dt)) ] - log(sigma sqrt(-dt)) - log(2 pi)/2
 
-sigma is singular at t = 1: there the schedule is evaluated at t_{i+1} instead of t_i (reading D2).  xi of step i comes
+sigma is singular at t = 1: there FlowGRPO replaces the t in the DENOMINATOR by t_{i+1}, sigma = a sqrt(t_i / (1 - t_{i+1}))
+(reading D2).  xi of step i comes
 from Philox stream SDE_STREAM_BASE + i of the sequence's seed (reading D3; C2 of SURVEY.md reserves a stream for it).
 Steps outside the window, and steps with sigma = 0, are plain Euler steps with log p = 0 (reading D4).
 """
@@ -36,9 +37,9 @@ SDE_STREAM_BASE = 256
 
 
 def sde_sigma(t_i: float, t_next: float, noise_level: float) -> float:
-    """sigma = a sqrt(t / (1 - t)), evaluated at t_next when t_i == 1 (reading D2)."""
-    t = t_i if t_i < 1.0 else t_next
-    return noise_level * math.sqrt(t / (1.0 - t))
+    """sigma = a sqrt(t_i / (1 - t')), t' = t_i, or t_next when t_i == 1 (reading D2: only the denominator moves)."""
+    td = t_i if t_i < 1.0 else t_next
+    return noise_level * math.sqrt(t_i / (1.0 - td))
 
 
 def sde_step(x: Array, v: Array, t_i: float, t_next: float, noise_level: float, xi: Array) -> Tuple[Array, float]:
@@ -62,8 +63,9 @@ def step_noise(seed: int, step: int, shape: Sequence[int]) -> Array:
 
 def denoise_sde(x0: Array, seed: int, timesteps: Sequence[float], velocity: Callable[[Array, float], Array],
                 noise_level: float, window: Tuple[int, int], noise_cast=None,
-                history: List[Array] | None = None) -> Tuple[Array, Array]:
-    """T steps over `timesteps` (length T + 1); steps i with window[0] <= i < window[1] are stochastic.
+                history: List[Array] | None = None, first_step: int = 0) -> Tuple[Array, Array]:
+    """T steps over `timesteps` (length T + 1); steps with window[0] <= j < window[1] are stochastic, j = first_step + i
+    the global step index (a resumed rollout passes the number of steps already taken; noise stream = base + j).
     Returns (x_T, logp [T]).  `noise_cast` models the storage precision of xi (the CUDA path makes it in fp32)."""
     T = len(timesteps) - 1
     x = np.array(x0, dtype=np.float64, copy=True)
@@ -71,8 +73,9 @@ def denoise_sde(x0: Array, seed: int, timesteps: Sequence[float], velocity: Call
     for i in range(T):
         t_i, t_n = float(timesteps[i]), float(timesteps[i + 1])
         v = velocity(x, t_i)
-        if window[0] <= i < window[1]:
-            xi = step_noise(seed, i, x.shape)
+        j = first_step + i
+        if window[0] <= j < window[1]:
+            xi = step_noise(seed, j, x.shape)
             if noise_cast is not None:
                 xi = noise_cast(xi)
             x, logp[i] = sde_step(x, v, t_i, t_n, noise_level, xi)

@@ -92,7 +92,7 @@ def load_library() -> C.CDLL:
         "spot_dit_denoise_cached": [vp, i32, i32, vp, vp, vp, i32, C.POINTER(SpotCacheConfig), vp, vp, vp, sz, vp],
         "spot_explore_cached": [vp, i32, i32, vp, vp, vp, i32, vp, i32, C.POINTER(SpotCacheConfig), vp, vp, vp, vp, vp, vp, vp,
                                 vp, sz, vp],
-        "spot_dit_denoise_sde": [vp, i32, i32, vp, vp, vp, vp, i32, f32, i32, i32, vp, vp, sz, vp],
+        "spot_dit_denoise_sde": [vp, i32, i32, vp, vp, vp, vp, i32, f32, i32, i32, i32, vp, vp, sz, vp],
         "spot_sde_update": [vp, vp, vp, i32, f32, f32, f32, i32, i64, vp, vp, vp],
         "spot_fp8_bytes": [vp, C.POINTER(sz)],
         "spot_fp8_prepare": [vp, vp, sz, vp],
@@ -380,15 +380,16 @@ def spot_dit_denoise_cached(ctx: Context, latents: torch.Tensor, text_emb: torch
 
 def spot_dit_denoise_sde(ctx: Context, seeds: torch.Tensor, latents: torch.Tensor, text_emb: torch.Tensor,
                          timesteps: Sequence[float], n_prompts: int, seeds_per_prompt: int, noise_level: float,
-                         window: Sequence[int]):
-    """In place on latents; returns (latents, logp [B, T] fp32 device).  PAPER.md:227, Table 2 "SDE window"."""
+                         window: Sequence[int], first_step: int = 0):
+    """In place on latents; returns (latents, logp [B, T] fp32 device).  PAPER.md:227, Table 2 "SDE window".
+    `first_step`: global index of this call's first step (a resumed rollout passes the steps already taken)."""
     B = n_prompts * seeds_per_prompt
     arr, T = _timesteps(timesteps)
     logp = torch.empty((B, T), dtype=torch.float32, device=latents.device)
     ws = ctx.workspace(B, T)
     _check(load_library().spot_dit_denoise_sde(ctx.handle, n_prompts, seeds_per_prompt, _ptr(seeds), _ptr(latents), _ptr(text_emb),
                                                C.cast(arr, C.c_void_p), T, float(noise_level), int(window[0]), int(window[1]),
-                                               _ptr(logp), _ptr(ws), ws.numel(), _stream()), "spot_dit_denoise_sde", ctx)
+                                               int(first_step), _ptr(logp), _ptr(ws), ws.numel(), _stream()), "spot_dit_denoise_sde", ctx)
     return latents, logp
 
 

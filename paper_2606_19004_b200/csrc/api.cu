@@ -321,6 +321,7 @@ spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
   if (!ctx) return SPOT_ERR_NULL;
   if (opt == SPOT_OPT_GEMM_IMPL) {
     if (value < 0 || value > 4) return SPOT_ERR_SHAPE;
+    if (value != 0 && ctx->fp8) return SPOT_ERR_SHAPE;   // the E4M3 Linears exist on the default GEMM only
     ctx->gemm_impl = value;
     return SPOT_OK;
   }
@@ -336,8 +337,9 @@ spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
   }
   if (value != 0 && value != 1) return SPOT_ERR_SHAPE;
   if (opt == SPOT_OPT_FP8) {
-    if (value && (ctx->fp8_blocks.size() != ctx->blocks.size() || ctx->cfg.dtype != SPOT_BF16 || ctx->cfg.head_dim != 128))
-      return SPOT_ERR_SHAPE;                     // spot_fp8_prepare first; bf16 configs with d_h = 128 only
+    if (value && (ctx->fp8_blocks.size() != ctx->blocks.size() || ctx->cfg.dtype != SPOT_BF16 || ctx->cfg.head_dim != 128 ||
+                  ctx->gemm_impl != 0))
+      return SPOT_ERR_SHAPE;                     // spot_fp8_prepare first; bf16 configs with d_h = 128, default GEMM only
     ctx->fp8 = value;
     return SPOT_OK;
   }
@@ -545,14 +547,15 @@ struct SdeRun {
   float noise_level;
   int lo, hi;
   float* logp;             // device, [B, T] (zero for deterministic steps)
+  int first_step;          // global index of the call's step 0: noise stream and window test use first_step + i
 };
 constexpr uint32_t kSdeStreamBase = 256;
 
 // cx, cv, cn of the step t_i -> t_next (readings D1-D2); returns false when sigma == 0 (a deterministic step)
 bool sde_coeffs(float t_i, float t_next, float noise_level, double* cx, double* cv, double* cn) {
   const double t = (double)t_i, tn = (double)t_next, dt = tn - t;
-  const double ts = t < 1.0 ? t : tn;
-  const double sig = (double)noise_level * sqrt(ts / (1.0 - ts));
+  const double td = t < 1.0 ? t : tn;                       // FlowGRPO: at t = 1 only the denominator takes t_next
+  const double sig = (double)noise_level * sqrt(t / (1.0 - td));
   if (!(sig > 0.0) || !(dt < 0.0)) return false;
   *cx = 1.0 + sig * sig / (2.0 * t) * dt;
   *cv = (1.0 + sig * sig * (1.0 - t) / (2.0 * t)) * dt;
@@ -619,8 +622,9 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
       LK(c, launch_gemm_simt(dt, dt, SPOT_F32, EPI_BIAS, pr, st));
       const bool last = i == T - 1;
       double cx, cv, cn;
-      if (sde && i >= sde->lo && i < sde->hi && sde_coeffs(h_t[i], h_t[i + 1], sde->noise_level, &cx, &cv, &cn))
-        LK(c, launch_sde_update(lat_c, vel, sde->seeds + b0, kSdeStreamBase + (uint32_t)i, cx, cv, cn, Bc, E,
+      const int j = sde ? sde->first_step + i : i;           // global step index
+      if (sde && j >= sde->lo && j < sde->hi && sde_coeffs(h_t[i], h_t[i + 1], sde->noise_level, &cx, &cv, &cn))
+        LK(c, launch_sde_update(lat_c, vel, sde->seeds + b0, kSdeStreamBase + (uint32_t)j, cx, cv, cn, Bc, E,
                                 last ? probe : nullptr, c->d_partials2 + (long long)b0 * n_part, partials_c,
                                 sde->logp + (long long)b0 * T + i, T, st));
       else
@@ -912,12 +916,12 @@ spot_status spot_explore_cached(spot_ctx* ctx, int n_prompts, int seeds_per_prom
 
 spot_status spot_dit_denoise_sde(spot_ctx* ctx, int n_prompts, int seeds_per_prompt, const uint64_t* d_seeds,
                                  float* d_latents, const void* d_text_emb, const float* h_timesteps, int n_steps,
-                                 float noise_level, int window_lo, int window_hi, float* d_logp, void* d_workspace,
-                                 size_t ws_bytes, void* cuda_stream) {
+                                 float noise_level, int window_lo, int window_hi, int first_step, float* d_logp,
+                                 void* d_workspace, size_t ws_bytes, void* cuda_stream) {
   spot_status s = check_rollout_args(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps);
   if (s != SPOT_OK) return s;
   if (!d_seeds || !d_logp) return SPOT_ERR_NULL;
-  if (!(noise_level >= 0.f) || window_lo < 0 || window_hi < window_lo) return SPOT_ERR_SHAPE;
+  if (!(noise_level >= 0.f) || window_lo < 0 || window_hi < window_lo || first_step < 0) return SPOT_ERR_SHAPE;
   for (int i = 0; i < n_steps; ++i)
     if (!(h_timesteps[i] > 0.f && h_timesteps[i] <= 1.f && h_timesteps[i + 1] < h_timesteps[i] && h_timesteps[i + 1] >= 0.f))
       return SPOT_ERR_SHAPE;                                 // the schedule sigma = a sqrt(t/(1-t)) needs 1 >= t_i > t_{i+1} >= 0
@@ -926,7 +930,7 @@ spot_status spot_dit_denoise_sde(spot_ctx* ctx, int n_prompts, int seeds_per_pro
   if (s != SPOT_OK) return s;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (n_steps > 0) CK(ctx, cudaMemsetAsync(d_logp, 0, (size_t)B * n_steps * 4, st));
-  SdeRun run{d_seeds, noise_level, window_lo, window_hi, d_logp};
+  SdeRun run{d_seeds, noise_level, window_lo, window_hi, d_logp, first_step};
   return denoise_core(ctx, n_prompts, seeds_per_prompt, d_latents, d_text_emb, h_timesteps, n_steps, (uint8_t*)d_workspace,
                       nullptr, nullptr, st, &run);
 }

@@ -31,7 +31,7 @@ spot_status spot_planner_create(const int32_t* d_values, int n_d, const int32_t*
                                 double t_step, double beta, int window, spot_planner** out) {
   if (!d_values || !s_values || !out) return SPOT_ERR_NULL;
   *out = nullptr;
-  if (n_d <= 0 || n_s <= 0 || n_prompts <= 0 || !(t_step > 0.0) || !(beta > 0.0) || window < 1) return SPOT_ERR_SHAPE;
+  if (n_d <= 0 || n_s <= 0 || n_prompts <= 0 || !(t_step > 0.0) || !(beta >= 0.0) || window < 1) return SPOT_ERR_SHAPE;
   for (int i = 0; i < n_d; ++i) {
     if (d_values[i] <= 0) return SPOT_ERR_SHAPE;
     for (int j = 0; j < i; ++j) if (d_values[j] == d_values[i]) return SPOT_ERR_SHAPE;

@@ -156,6 +156,23 @@ def test_block_forward_fp8_matches_fp8_oracle(wide):
         assert 1e-4 < d_i < 5e-2                                            # quantisation is visible, and small
 
 
+def test_fp8_and_alternative_gemm_kernels_are_exclusive(wide):
+    """The E4M3 Linears exist on the default GEMM only: asking for both must fail instead of silently running bf16."""
+    s, w, ctx = wide
+    ctx.enable_fp8(True)
+    try:
+        with pytest.raises(spot.SpotError):
+            spot.spot_set_option(ctx, spot.OPT_GEMM_IMPL, 4)
+    finally:
+        ctx.enable_fp8(False)
+    spot.spot_set_option(ctx, spot.OPT_GEMM_IMPL, 4)
+    try:
+        with pytest.raises(spot.SpotError):
+            ctx.enable_fp8(True)
+    finally:
+        spot.spot_set_option(ctx, spot.OPT_GEMM_IMPL, 0)
+
+
 def test_rollout_fp8_matches_fp8_oracle_and_ranks_like_bf16(wide):
     s, w, ctx = wide
     text, probe = make_text_emb(s, "cuda"), make_probe(s, "cuda")

@@ -87,6 +87,11 @@ def test_cfg1_denoise_sde_matches_oracle():
         assert rel_l2(np64(out[b]), ref) < 1e-4
         assert np.abs(np64(logp[b]) - ref_lp).max() < 1e-4 * max(1.0, np.abs(ref_lp).max())
         assert logp[b, 4].item() == 0.0                          # outside the window: deterministic step
+    # a rollout split over two calls with first_step = steps already taken is the unsplit rollout, bit for bit
+    lat_s = spot.spot_noise_from_seeds(_seeds(seeds), s.n_img * s.latent_ch).reshape(3, s.n_img, s.latent_ch)
+    _, lp1 = spot.spot_dit_denoise_sde(ctx, _seeds(seeds), lat_s, text, ts[:3], 1, 3, a, window)
+    _, lp2 = spot.spot_dit_denoise_sde(ctx, _seeds(seeds), lat_s, text, ts[2:], 1, 3, a, window, first_step=2)
+    assert torch.equal(lat_s, out) and torch.equal(torch.cat([lp1, lp2], 1), logp)
     # an empty window is the plain deterministic denoise, bit for bit
     lat_a = spot.spot_noise_from_seeds(_seeds(seeds), s.n_img * s.latent_ch).reshape(3, s.n_img, s.latent_ch)
     lat_b = lat_a.clone()

@@ -74,7 +74,8 @@ def test_log_probability_matches_scipy():
 def test_sigma_schedule_and_singular_endpoint():
     assert abs(sde.sde_sigma(0.5, 0.4, 0.7) - 0.7) < 1e-15                    # t/(1-t) = 1
     assert abs(sde.sde_sigma(0.8, 0.7, 1.0) - 2.0) < 1e-12                    # sqrt(0.8/0.2)
-    assert abs(sde.sde_sigma(1.0, 0.9, 1.0) - 3.0) < 1e-12                    # evaluated at t_next: sqrt(0.9/0.1)
+    # t = 1: FlowGRPO keeps t in the numerator and moves only the denominator to t_next: sqrt(1/0.1), not sqrt(0.9/0.1)
+    assert abs(sde.sde_sigma(1.0, 0.9, 1.0) - math.sqrt(10.0)) < 1e-12
     assert sde.sde_sigma(0.3, 0.2, 0.0) == 0.0
 
 
@@ -87,3 +88,18 @@ def test_step_noise_is_the_pinned_philox_stream():
         for b in range(a + 1, 3):
             assert abs(np.corrcoef(big[a], big[b])[0, 1]) < 0.02
     assert abs(np.corrcoef(big[0], philox.noise_from_seeds([9], 1 << 16, 0)[0])[0, 1]) < 0.02    # and from the initial latent
+
+
+def test_resumed_rollout_uses_global_step_indices():
+    """A rollout split into two calls (in-flight latents are committed on preemption and resumed) must draw
+    the noise of GLOBAL step j from stream base + j and test the window on j: split == unsplit exactly."""
+    rng = np.random.default_rng(11)
+    x0 = rng.normal(size=(8, 4))
+    vel = lambda x, t: -0.3 * x + t
+    ts = [1.0, 0.8, 0.6, 0.4, 0.2, 0.0]
+    full, lp = sde.denoise_sde(x0, 5, ts, vel, 0.6, (1, 4))
+    a, lpa = sde.denoise_sde(x0, 5, ts[:3], vel, 0.6, (1, 4))
+    b, lpb = sde.denoise_sde(a, 5, ts[2:], vel, 0.6, (1, 4), first_step=2)
+    assert (b == full).all() and (np.concatenate([lpa, lpb]) == lp).all()
+    wrong, _ = sde.denoise_sde(a, 5, ts[2:], vel, 0.6, (1, 4))                # forgetting the offset reuses streams 256, 257
+    assert np.abs(wrong - full).max() > 1e-3

@@ -112,6 +112,27 @@ def test_c_planner_matches_oracle_on_random_run():
         assert abs(st["mean"] - sum(op.history[a_o][-3:]) / st["n_i"]) < 1e-12
 
 
+def test_beta_zero_is_greedy_on_window_means():
+    """PAPER.md:486 sweeps beta in {0, 0.5, 1.0}: beta = 0 is accepted and selects the best window mean (after every
+    action was tried once: untried actions still score +inf)."""
+    d_vals, s_vals = [4, 8], [12, 16]
+    cp = spot.Planner(d_vals, s_vals, 8, 1.0, beta=0.0, window=2)
+    op = orc.Planner(d_vals, s_vals, 8, 1.0, 0.0, 2)
+    fb = {(4, 12): 1.0, (8, 12): 1.4, (4, 16): 1.2, (8, 16): 1.3}
+    for it in range(8):
+        a_c, u_c = cp.spot_planner_select(1e6, 8)
+        a_o, u_o = op.select(1e6, 8)
+        assert a_c == a_o
+        if it >= 4:
+            assert a_c == (8, 12) and abs(u_c - 1.4) < 1e-12 and abs(u_o - 1.4) < 1e-12      # no exploration bonus
+        cp.spot_planner_update(a_c, fb[a_c])
+        op.update(a_o, fb[a_o])
+    with pytest.raises(spot.SpotError):
+        spot.Planner(d_vals, s_vals, 8, 1.0, beta=-0.1)
+    with pytest.raises(spot.SpotError):
+        spot.Planner(d_vals, s_vals, 8, 1.0, beta=float("nan"))
+
+
 def test_c_planner_argument_errors():
     with pytest.raises(spot.SpotError):
         spot.Planner([4, 4], [12], 8, 1.0)                 # duplicate d
