@@ -35,5 +35,16 @@ def elem_excess(got, ref, rel, abs_rms):
     if ref.size == 0:
         return 0.0
     rms = float(np.sqrt(np.mean(ref * ref)))
-    bound = rel * np.abs(ref) + abs_rms * max(rms, 1e-300)
-    return float((np.abs(got - ref) / bound).max())
+    return bound_excess(got, ref, rel * np.abs(ref) + abs_rms * max(rms, 1e-300))
+
+
+def bound_excess(got, ref, bound):
+    """max over elements of |got - ref| / bound (bound: array of per-element bounds)."""
+    got, ref, bound = (np.asarray(a, dtype=np.float64).reshape(-1) for a in (got, ref, bound))
+    if ref.size == 0:
+        return 0.0
+    r = np.abs(got - ref) / bound
+    i = int(np.argmax(r))
+    if r[i] > 1.0:
+        print(f"  bound_excess: worst element #{i}: got {got[i]:.6e} ref {ref[i]:.6e} |err| {abs(got[i] - ref[i]):.3e} bound {bound[i]:.3e}")
+    return float(r[i])

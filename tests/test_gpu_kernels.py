@@ -117,7 +117,7 @@ def test_attention_simt(dtype, S, H, dh, scale, tol):
     out = spot.spot_attention(qkv, spot.IMPL_SIMT)
     ref = _attn_ref(qkv)
     assert rel_l2(np64(out), ref) < tol
-    ex = elem_excess(np64(out), ref, 2 * BF16_U, 4e-3) if dtype == torch.bfloat16 else elem_excess(np64(out), ref, 1e-4, 1e-5)
+    ex = elem_excess(np64(out), ref, 2 * BF16_U, 1.5e-2) if dtype == torch.bfloat16 else elem_excess(np64(out), ref, 1e-4, 1e-5)
     assert ex <= 1.0, ex
 
 
@@ -283,9 +283,12 @@ def test_attention_tcgen05(B, S, H, scale):
     out = spot.spot_attention(qkv, spot.IMPL_TCGEN05)
     ref = _attn_ref(qkv)
     err = rel_l2(np64(out), ref)
-    # per element: P is rounded to bf16 before P V (each weight within 2^-9, a convex combination keeps that relative to
-    # the |v| it mixes => absolute floor in units of rms(o)), then one bf16 rounding of o
-    ex = elem_excess(np64(out), ref, 2 * BF16_U, 6e-3)
+    # per element: the weights P are rounded to bf16 before P V, independent relative errors of rms ~2^-9 each, so an output
+    # element (a near-cancelling average of many v) carries an ABSOLUTE error of sigma ~ 2.2e-3 rms(o) whatever its own
+    # size (measured rel-L2 2.0-2.3e-3 = that sigma); the floor is 7 sigma (the largest of up to 10^6 Gaussian errors sits
+    # near 5 sigma), plus two bf16 roundings relative to the element (P scale and the store of o).  A wrong element -
+    # a mis-clipped tile corner, a bad TMEM lane - is off by ~rms(o) = 450 sigma.
+    ex = elem_excess(np64(out), ref, 2 * BF16_U, 1.5e-2)
     print(f"attention tcgen05 B={B} S={S} H={H} scale={scale}: rel-L2 {err:.3e}, worst element at {ex:.2f} of its bound")
     assert err < 8e-3
     assert ex <= 1.0, ex

@@ -204,13 +204,21 @@ def test_cfg2_block_forward_bf16(cfg2):
     print(f"cfg2 block update rel-L2: img {d_img:.3e} txt {d_txt:.3e}")
     # the block's output is h + update rounded ONCE to bf16 (config 2 has bf16 I/O and |h| ~ 1 dominates |update|), so the
     # update inherits that rounding, rho = 2^-9/sqrt(3) * rms(out)/rms(update); what the block itself contributes must stay
-    # under the north-star's per-block 2e-2 measured on the UPDATE (stricter than on the output)
-    from tests.helpers import BF16_U, elem_excess
+    # under the north-star's per-block 2e-2 measured on the UPDATE (stricter than on the output).
+    # Per element: the error of element (row r, channel c) comes from the bf16 roundings of the block's intermediates
+    # carried through the Linears, ~ 2^-9 gate_c |a_r| |w_c|: it scales with the ROW (token activations) and with the
+    # CHANNEL (gate, weight row), which differ by an order of magnitude across the tensor.  Bound: one output rounding
+    # + 2e-2 |update| + 4e-2 rms_r(update) rms_c(update) / rms(update)  (the rank-1 scale of the update; the error's
+    # measured rms is 3e-3 of it, so this is a > 10 sigma floor, and a wrong element is off by ~25 x the floor).
+    from tests.helpers import BF16_U, bound_excess
     for name, d, got, ref, h_in in (("img", d_img, np64(o_img[check]), r_img, np64(h_img[check])),
                                     ("txt", d_txt, np64(o_txt[check]), r_txt, np64(h_txt[check]))):
-        upd_rms, out_rms = float(np.sqrt(np.mean((ref - h_in) ** 2))), float(np.sqrt(np.mean(ref ** 2)))
+        upd = ref - h_in
+        upd_rms, out_rms = float(np.sqrt(np.mean(upd ** 2))), float(np.sqrt(np.mean(ref ** 2)))
         rho = 2.0 ** -9 / np.sqrt(3.0) * out_rms / upd_rms
-        ex = elem_excess(got, ref, 1.05 * BF16_U, 2e-2 * upd_rms / out_rms)      # every element: one rounding + 2e-2 rms(update)
+        col_rms = np.sqrt(np.mean(upd ** 2, axis=(0, 1), keepdims=True))
+        row_rms = np.sqrt(np.mean(upd ** 2, axis=2, keepdims=True))
+        ex = bound_excess(got, ref, 1.05 * BF16_U * np.abs(ref) + 2e-2 * np.abs(upd) + 4e-2 * row_rms * col_rms / upd_rms)
         print(f"cfg2 block {name}: update rel-L2 {d:.3e} (output-rounding share {rho:.3e}), worst element at {ex:.2f} of its bound")
         assert d < 1.2 * rho + 2e-2, (name, d, rho)
         assert ex <= 1.0, (name, ex)
