@@ -1,7 +1,7 @@
 // attn_tcgen05_v3.cu - K5, third version: flash-style joint text+image attention O = softmax(Q K^T / sqrt(d_h)) V over
 // all S keys, no mask (north_star (d); S4 step 6, S6), bf16, d_h = 128.
 //
-// What changed against attn_tcgen05.cu (v2) and why (profiles/r1_ncu_full_attn_ln_qk.txt: tensor pipe 37 % active):
+// What changed against attn_tcgen05.cu (v2) and why (its ncu capture in round 1: tensor pipe 37 % active):
 //   * v2 read every score tile from tensor memory TWICE (row max, then exp) and its S tile aliased P, so the chain
 //     S -> softmax -> P -> PV -> next S of a query tile was serial.  TMEM reads are the scarce resource (the 128 x 128
 //     fp32 S tile is 64 KB), so v3 streams keys in tiles of 64: a thread's 64 scores fit in registers (ONE pass), and
@@ -34,7 +34,9 @@ constexpr uint32_t Q_TILE = 2 * Q_SUB;                 // [128 x 128]
 constexpr uint32_t KV_SUB = 64 * 128;                  // [64 rows x 64 cols]
 constexpr uint32_t KV_TILE = 2 * KV_SUB;               // [64 x 128]
 constexpr uint32_t OFF_Q = 0, OFF_K = QT * Q_TILE, OFF_V = OFF_K + KV_STAGES * KV_TILE, OFF_BAR = OFF_V + KV_STAGES * KV_TILE;
-constexpr uint32_t ATT_SMEM = OFF_BAR + 512 + 1024;
+// epilogue staging: one [32 rows x 128 bytes] buffer per softmax warp, 128-byte swizzled, handed to TMA stores
+constexpr uint32_t OFF_STG = OFF_BAR + 1024, STG_BYTES = 32 * 128;
+constexpr uint32_t ATT_SMEM = OFF_STG + QT * 4 * STG_BYTES + 1024;        // 226 KB of the 227 KB a CTA may have
 constexpr int ATT_THREADS = 64 + QT * 128;
 constexpr float RESCALE_THRESHOLD = 8.0f;
 
@@ -51,6 +53,9 @@ __device__ __forceinline__ void mma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uin
       "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
   __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
   return *reinterpret_cast<uint32_t*>(&v);
@@ -59,8 +64,8 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 // OUT8: O is stored as E4M3 bytes (unit scale, saturating) - the A operand of the FP8 out-projection.
 template <bool OUT8>
 __global__ void __launch_bounds__(ATT_THREADS, 1)
-attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, void* __restrict__ out_v, int S, int H, int n_items,
-                       float scale_log2) {
+attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, const __grid_constant__ CUtensorMap tm_out, int S, int H,
+                       int n_items, float scale_log2) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw_addr = ptx::smem_u32(smem_raw);
   const uint32_t base = (raw_addr + 1023u) & ~1023u;
@@ -83,7 +88,7 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, void* __restr
   const int n_kv = (S + BKV - 1) / BKV;
   const int n_qt = (S + QT * BQ - 1) / (QT * BQ);           // work item = (sequence, head, pair of query tiles)
 
-  if (warp == 0 && lane == 0) ptx::prefetch_tmap(&tm_qkv);
+  if (warp == 0 && lane == 0) { ptx::prefetch_tmap(&tm_qkv); ptx::prefetch_tmap(&tm_out); }
   if (warp == 1) {
     if (lane == 0) {
       ptx::mbar_init(q_full, 1);
@@ -204,7 +209,6 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, void* __restr
     // ===================== softmax / correction / epilogue: 2 warpgroups x 128 rows =====================
     const int t = (warp - 2) >> 2;                      // query tile of this warpgroup
     const int quarter = warp & 3;                       // TMEM lane quarter this warp may access
-    const int row = quarter * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     const uint32_t tmem_s = tmem_base + t * 128 + lane_addr, tmem_o = tmem_base + 256 + t * DH + lane_addr;
     int it = 0;
@@ -292,14 +296,30 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, void* __restr
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(p_full(t, b));
       }
-      // epilogue: O / l -> bf16.  (pv_done's parity is only unambiguous one phase back - the softmax of tile g runs at
-      // most one P V ahead of it - so the end of the item's LAST P V has its own barrier.)
+      // epilogue: O / l -> bf16 (or E4M3).  (pv_done's parity is only unambiguous one phase back - the softmax of tile g
+      // runs at most one P V ahead of it - so the end of the item's LAST P V has its own barrier.)
+      // A thread owns a query ROW, so storing from registers sends 32 scattered 16-byte pieces per instruction (measured:
+      // 4400-6000 cycles per item and query tile, 12-18 % of an S = 1280 item).  Instead each warp stages its 32 rows x
+      // 128 bytes in 128-byte-swizzled shared memory and one lane hands them to a TMA store, which also clips rows >= S.
       ptx::mbar_wait(o_final(t), (uint32_t)(it & 1));
       ptx::tc_fence_after();
       const float inv = 1.f / l;
-      const int qrow = q0 + t * BQ + row;
-      const bool row_ok = qrow < S;
-      const long long oidx = ((long long)seq * S + qrow) * (long long)(H * DH) + head * DH;
+      const int row0 = q0 + t * BQ + quarter * 32;        // first row of this warp
+      const uint32_t stg = base + OFF_STG + (uint32_t)(warp - 2) * STG_BYTES;
+      const uint32_t stg_row = stg + (uint32_t)lane * 128u;
+      const int sw = lane & 7;
+      auto send = [&](int col) {                          // staging buffer -> out[seq, row0 .. row0 + 31, col ..]
+        ptx::fence_proxy_async_smem();
+        __syncwarp();
+        if (ptx::elect_one()) {                           // the same lane every time: it owns the bulk async-groups
+          if (row0 < S) ptx::tma_store_3d(&tm_out, stg, col, row0, seq);
+          ptx::bulk_commit();
+        }
+      };
+      auto acquire = [&]() {                              // the TMA engine has read the previous contents
+        ptx::bulk_wait_read<0>();
+        __syncwarp();
+      };
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         uint32_t ov[32];
@@ -310,38 +330,37 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, void* __restr
           __syncwarp();
           if (lane == 0) ptx::mbar_arrive(o_free(t));
         }
-        if (row_ok) {
-          if (OUT8) {
-            uint8_t* orow = reinterpret_cast<uint8_t*>(out_v) + oidx;
+        if (OUT8) {                                       // 128 E4M3 bytes per row: one buffer, one store
+          if (c == 0) acquire();
 #pragma unroll
-            for (int g4 = 0; g4 < 2; ++g4) {
-              uint32_t w4[4];
+          for (int g4 = 0; g4 < 2; ++g4) {
+            uint32_t w4[4];
 #pragma unroll
-              for (int u = 0; u < 4; ++u) {
-                const int e = g4 * 16 + u * 4;
-                const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(__uint_as_float(ov[e]) * inv, __uint_as_float(ov[e + 1]) * inv),
-                                                             __NV_SATFINITE, __NV_E4M3);
-                const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(__uint_as_float(ov[e + 2]) * inv, __uint_as_float(ov[e + 3]) * inv),
-                                                             __NV_SATFINITE, __NV_E4M3);
-                w4[u] = lo | (hi << 16);
-              }
-              *reinterpret_cast<uint4*>(orow + c * 32 + g4 * 16) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+            for (int u = 0; u < 4; ++u) {
+              const int e = g4 * 16 + u * 4;
+              const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(__uint_as_float(ov[e]) * inv, __uint_as_float(ov[e + 1]) * inv),
+                                                           __NV_SATFINITE, __NV_E4M3);
+              const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(__uint_as_float(ov[e + 2]) * inv, __uint_as_float(ov[e + 3]) * inv),
+                                                           __NV_SATFINITE, __NV_E4M3);
+              w4[u] = lo | (hi << 16);
             }
-          } else {
-            bf16* orow = reinterpret_cast<bf16*>(out_v) + oidx;
-#pragma unroll
-            for (int g4 = 0; g4 < 4; ++g4) {
-              uint4 pkt;
-              pkt.x = pack_bf16(__uint_as_float(ov[g4 * 8]) * inv, __uint_as_float(ov[g4 * 8 + 1]) * inv);
-              pkt.y = pack_bf16(__uint_as_float(ov[g4 * 8 + 2]) * inv, __uint_as_float(ov[g4 * 8 + 3]) * inv);
-              pkt.z = pack_bf16(__uint_as_float(ov[g4 * 8 + 4]) * inv, __uint_as_float(ov[g4 * 8 + 5]) * inv);
-              pkt.w = pack_bf16(__uint_as_float(ov[g4 * 8 + 6]) * inv, __uint_as_float(ov[g4 * 8 + 7]) * inv);
-              *reinterpret_cast<uint4*>(orow + c * 32 + g4 * 8) = pkt;
-            }
+            st_shared_v4(stg_row + (uint32_t)(((c * 2 + g4) ^ sw) << 4), w4[0], w4[1], w4[2], w4[3]);
           }
+          if (c == 3) send(head * DH);
+        } else {                                          // 256 bf16 bytes per row: two buffers' worth, two stores
+          if ((c & 1) == 0) acquire();
+#pragma unroll
+          for (int g4 = 0; g4 < 4; ++g4)
+            st_shared_v4(stg_row + (uint32_t)((((c & 1) * 4 + g4) ^ sw) << 4),
+                         pack_bf16(__uint_as_float(ov[g4 * 8]) * inv, __uint_as_float(ov[g4 * 8 + 1]) * inv),
+                         pack_bf16(__uint_as_float(ov[g4 * 8 + 2]) * inv, __uint_as_float(ov[g4 * 8 + 3]) * inv),
+                         pack_bf16(__uint_as_float(ov[g4 * 8 + 4]) * inv, __uint_as_float(ov[g4 * 8 + 5]) * inv),
+                         pack_bf16(__uint_as_float(ov[g4 * 8 + 6]) * inv, __uint_as_float(ov[g4 * 8 + 7]) * inv));
+          if (c & 1) send(head * DH + (c >> 1) * 64);
         }
       }
     }
+    ptx::bulk_wait<0>();                                  // every store of this warp has completed before the CTA exits
   }
 
   ptx::tc_fence_before();
@@ -361,6 +380,15 @@ cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int
   const uint64_t strides[2] = {(uint64_t)3 * H * DH * 2, (uint64_t)S * 3 * H * DH * 2};
   const uint32_t box[3] = {64, 64, 1};
   SPOT_CUDA_TRY(spot_make_tmap_bf16(&tm, qkv, 3, dims, strides, box));
+  // output [B, S, H * d_h] as bf16 (box 64 columns x 32 rows) or E4M3 bytes (box 128 x 32): one warp's staging buffer
+  CUtensorMap tmo;
+  memset(&tmo, 0, sizeof(tmo));
+  const uint64_t es = out_e4m3 ? 1 : 2;
+  const uint64_t odims[3] = {(uint64_t)H * DH, (uint64_t)S, (uint64_t)B};
+  const uint64_t ostrides[2] = {(uint64_t)H * DH * es, (uint64_t)S * H * DH * es};
+  const uint32_t obox[3] = {out_e4m3 ? 128u : 64u, 32u, 1u};
+  if (out_e4m3) SPOT_CUDA_TRY(spot_make_tmap_u8(&tmo, out, 3, odims, ostrides, obox));
+  else SPOT_CUDA_TRY(spot_make_tmap_bf16(&tmo, out, 3, odims, ostrides, obox));
   static bool attr_set = false;
   if (!attr_set) {
     SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_tcgen05_v3_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ATT_SMEM));
@@ -371,7 +399,7 @@ cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int
   if (items > 0x7fffffffLL / 128) return cudaErrorInvalidValue;
   const int grid = (int)(items < num_sms ? items : num_sms);       // persistent: one CTA per SM walks the item list
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)DH);
-  if (out_e4m3) attn_tcgen05_v3_kernel<true><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, out, S, H, (int)items, scale_log2);
-  else attn_tcgen05_v3_kernel<false><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, out, S, H, (int)items, scale_log2);
+  if (out_e4m3) attn_tcgen05_v3_kernel<true><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, tmo, S, H, (int)items, scale_log2);
+  else attn_tcgen05_v3_kernel<false><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, tmo, S, H, (int)items, scale_log2);
   return cudaGetLastError();
 }
