@@ -224,7 +224,10 @@ def run_kernels(args, shape):
     alu_peak = 148 * 128 * 1.965e9 / 56.5 / 1e9                       # G normals/s
     res["K1_noise"] = {"bound": "alu", "ms": ms, "normals": n_norm, "achieved": n_norm / ms / 1e6, "unit": "Gnormal/s",
                        "peak": alu_peak, "frac": n_norm / ms / 1e6 / alu_peak, "written_gbs": 4.0 * n_norm / ms / 1e6,
-                       "peak_kind": "derived: 148 SMs x 128 lanes x 1.965 GHz / 56.5 SASS instructions per normal"}
+                       "frac_of_hbm_peak": 4.0 * n_norm / ms / 1e6 / peaks["hbm_gbs"],
+                       "peak_kind": "derived, and generous: 148 SMs x 128 lanes x 1.965 GHz / 56.5 SASS instructions per normal counts the "
+                                    "MUFU-rate instructions (lg2, sqrt, sin, cos: 16 per clock and SM) at the full issue rate; against the "
+                                    "HBM write roof the kernel is at frac_of_hbm_peak.  It runs once per rollout (4 MB at config 3: ~0 % of a step)"}
     del nz
     # K3 LN + modulate: fp32 residual rows in, bf16 out
     h = rnd(1, (M, D), torch.float32)

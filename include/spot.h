@@ -108,7 +108,9 @@ typedef enum {
 } spot_option;
 
 /* Validates cfg and w, builds the RoPE table (S5) and returns a context.  max_seqs bounds
- * n_seqs / n_prompts*seeds_per_prompt of later calls.  Does not synchronise. */
+ * n_seqs / n_prompts*seeds_per_prompt of later calls.  Allocates four small device buffers (RoPE cos / sin, reward
+ * partial sums) with cudaMalloc and fills the table with blocking cudaMemcpy: the call synchronises with the device
+ * like any cudaMalloc / pageable cudaMemcpy does; it is setup, not part of the timed path.  Launches no kernel. */
 spot_status spot_create(const spot_config *cfg, const spot_weights *w, int max_seqs, spot_ctx **out);
 spot_status spot_destroy(spot_ctx *ctx);
 spot_status spot_set_option(spot_ctx *ctx, spot_option opt, int value);

@@ -1,0 +1,90 @@
+"""Pins for oracle/nvfp4.py (CPU only).  E2M1 rounding: every representable value, every midpoint (ties to the even code)
+and random data against a brute-force nearest-neighbour search over the written-out value table (a different method from
+the oracle's binade arithmetic); the block scales ride on fp8.e4m3, pinned against torch's float8_e4m3fn cast in
+test_oracle_fp8.py; the block quantiser by a hand-worked block, its error bounds and exactness on representable input;
+the quantised Linear by identity with the dequantised product and by its error against the exact Linear."""
+import numpy as np
+
+from oracle import fp8, mmdit, nvfp4
+from synth import CONFIGS, make_block_inputs, make_weights
+from tests.helpers import np64, rel_l2, weights_np64
+
+TABLE = [0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0]          # E2M1 magnitudes in code order 0..7 (OCP MX specification)
+
+
+def _brute_e2m1(v):
+    """Nearest table entry; on an exact tie the EVEN code; saturate."""
+    a = min(abs(v), 6.0)
+    best = min(range(8), key=lambda c: (abs(TABLE[c] - a), c % 2))      # distance first, even code wins a tie
+    return np.sign(v) * TABLE[best]
+
+
+def test_e2m1_table_midpoints_and_random():
+    grid = np.array(TABLE)
+    assert (nvfp4.e2m1(grid) == grid).all() and (nvfp4.e2m1(-grid) == -grid).all()
+    mids = 0.5 * (grid[:-1] + grid[1:])
+    assert nvfp4.e2m1(mids).tolist() == [0.0, 1.0, 1.0, 2.0, 2.0, 4.0, 4.0]       # 0.25->0 0.75->1 1.25->1 1.75->2 2.5->2 3.5->4 5->4
+    assert nvfp4.e2m1(np.array([6.0, 7.0, 1e9, -1e9, 5.0001, 4.9999])).tolist() == [6.0, 6.0, 6.0, -6.0, 6.0, 4.0]
+    rng = np.random.default_rng(0)
+    x = np.concatenate([rng.normal(size=20000) * s for s in (0.2, 1.0, 3.0)] + [mids, -mids, np.nextafter(mids, 10), np.nextafter(mids, -10)])
+    assert (nvfp4.e2m1(x) == np.array([_brute_e2m1(v) for v in x])).all()
+
+
+def test_quantize_rows_hand_block_and_bounds():
+    # one block whose maximum is 3: sf = e4m3(3 / 6) = 0.5, codes = x / 0.5 rounded to the E2M1 grid
+    x = np.array([[3.0, -1.5, 0.75, 0.5, 0.25, 0.1, 0.0, -3.0, 2.0, 1.0, 0.6, 0.4, 2.9, 2.2, -0.13, 1.3]])
+    q, sf = nvfp4.quantize_rows(x)
+    assert sf.tolist() == [[0.5]]
+    assert q.tolist() == [[6.0, -3.0, 1.5, 1.0, 0.5, 0.0, 0.0, -6.0, 4.0, 2.0, 1.0, 1.0, 6.0, 4.0, -0.5, 3.0]]
+    #                        3/.5  -1.5/.5 1.5  1.0  0.5  .2->0      -6    4    2    1.2->1 .8->1 5.8->6 4.4->4 -.26->-.5 2.6->3
+    rng = np.random.default_rng(3)
+    x = rng.normal(size=(32, 256)) * np.exp(rng.normal(size=(32, 1)))
+    x[3, 16:32] = 0.0                                                     # a zero block: scale 0, codes 0
+    q, sf = nvfp4.quantize_rows(x)
+    assert (sf[3, 1] == 0) and (q[3, 16:32] == 0).all()
+    assert (fp8.e4m3(sf) == sf).all() and (nvfp4.e2m1(q) == q).all()      # scales are E4M3 values, codes E2M1 values
+    deq = nvfp4.dequantize(q, sf)
+    amax = np.abs(x).reshape(32, 16, 16).max(axis=2)
+    # the scale is amax/6 rounded to E4M3 (<= 2^-4 relative), the largest gap of the grid is 2 (between 4 and 6):
+    # |x - deq| <= sf (half that gap) + the clipping when the scale rounded down, amax * 2^-4
+    assert (np.abs(x - deq).reshape(32, 16, 16).max(axis=2) <= sf * 1.0 + amax * 2.0 ** -4 + 1e-12).all()
+    assert 0.05 < rel_l2(deq, x) < 0.15
+    q2, sf2 = nvfp4.quantize_rows(deq)                                    # representable input is a fixed point
+    assert (nvfp4.dequantize(q2, sf2) == deq).all()
+
+
+def test_weight_quantisation_and_linear():
+    rng = np.random.default_rng(4)
+    w = rng.normal(size=(48, 256)) * 0.02
+    w[5] = 0.0
+    q, sf, s = nvfp4.quantize_weight(w)
+    assert s[5] == 1.0 and (q[5] == 0).all()
+    assert np.allclose(s[np.arange(48) != 5], np.abs(w).max(axis=1)[np.arange(48) != 5] / (6 * 448), rtol=1e-6)
+    assert sf.max() <= 448.0 and sf.max() > 300.0                          # the row maximum's block scale sits at the top of E4M3
+    x = rng.normal(size=(64, 256))
+    b = rng.normal(size=48) * 0.1
+    y = nvfp4.linear_nvfp4(x, q, sf, s, b)
+    xq, xsf = nvfp4.quantize_rows(x)
+    ref = np.zeros((64, 48))                                               # reading N5 written as the explicit block sum
+    for blk in range(16):
+        sl = slice(16 * blk, 16 * blk + 16)
+        ref += (xq[:, sl] @ q[:, sl].T) * xsf[:, blk:blk + 1] * sf[:, blk][None, :]
+    assert np.abs(y - (ref * s + b)).max() < 1e-12
+    assert 0.08 < rel_l2(y - b, x @ w.T) < 0.2                             # one mantissa bit on both operands
+
+
+def test_block_nvfp4_is_close_and_mixed_with_fp8():
+    s = CONFIGS[1]
+    g, blocks = weights_np64(make_weights(s))
+    h_img, h_txt, temb = (np64(t) for t in make_block_inputs(s, 1))
+    cos, sin = mmdit.rope_table(s.grid_h, s.grid_w, s.n_txt, s.rope_pairs, s.rope_theta)
+    c = mmdit.silu(temb)
+    kw = dict(n_heads=s.n_heads, cos=cos, sin=sin)
+    bw = blocks[0]
+    ref = mmdit.block_forward(h_img[0], h_txt[0], c, bw, **kw)
+    q8 = fp8.block_forward_fp8(h_img[0], h_txt[0], c, bw, **kw)
+    q4 = nvfp4.block_forward_nvfp4(h_img[0], h_txt[0], c, bw, **kw)
+    qw = nvfp4.quantize_block(bw)
+    assert len(qw["img.fc1"]) == 3 and len(qw["img.qkv"]) == 2             # MLP in NVFP4, attention Linears in FP8
+    for a4, a8, r in zip(q4, q8, ref):
+        assert rel_l2(a8, r) < rel_l2(a4, r) < 0.15                        # coarser than FP8, still a small perturbation
