@@ -102,6 +102,25 @@ spot_status spot_qkv_rope_linear_fp8(const void *d_a, int n_seqs, int rows_per_s
                                      const void *d_k_gain, const float *d_cos, const float *d_sin, int pos_off, float eps,
                                      void *d_out, void *cuda_stream);
 
+/* NVFP4 building blocks of the 4-bit exploration variant (spot.h).  NVFP4 = E2M1
+ * values {0, .5, 1, 1.5, 2, 3, 4, 6} with sign in blocks of 16 consecutive elements along K, one E4M3 scale per block.
+ * spot_nvfp4_sizes: bytes of the code matrix [rows, K / 2] (element k in the low / high nibble for k even / odd) and of
+ *   the scale-factor buffer (512-byte atoms of 128 rows x 4 blocks; see csrc/nvfp4.cu) for a [rows, K] matrix.
+ * spot_nvfp4_row_scale: d_scale[r] = max_k |W_rk| / (6 * 448) (1 for a zero row) - the second-level scale of a weight row.
+ * spot_nvfp4_quantize: d_src [rows, K] bf16 (each row divided by d_row_scale[r] first when that pointer is not NULL) ->
+ *   block scale sf = e4m3(max|x| / 6), codes e2m1(x / sf), all in fp32 with IEEE division.  rows % 128 == 0, K % 64 == 0.
+ * spot_linear_nvfp4: y[m, n] = d_w_scale[n] * sum_blocks sfa sfw sum_k a w + bias[n] on the block-scaled tensor-core path
+ *   (kind::mxf4nvf4), fp32 accumulation; SPOT_EPI_BIAS / SPOT_EPI_BIAS_GELU write d_out [M, N] bf16,
+ *   SPOT_EPI_GATE_RESIDUAL updates the fp32 residual [M, N].  M % 128 == 0, N % 256 == 0, K % 256 == 0, else
+ *   SPOT_ERR_SHAPE. */
+spot_status spot_nvfp4_sizes(int64_t rows, int64_t K, size_t *codes_bytes, size_t *sf_bytes);
+spot_status spot_nvfp4_row_scale(const void *d_w_bf16, int64_t rows, int64_t K, float *d_scale, void *cuda_stream);
+spot_status spot_nvfp4_quantize(const void *d_src_bf16, int64_t rows, int64_t K, const float *d_row_scale, void *d_codes,
+                                void *d_sf, void *cuda_stream);
+spot_status spot_linear_nvfp4(spot_epilogue epi, const void *d_a_codes, const void *d_a_sf, int64_t M, int64_t K,
+                              const void *d_w_codes, const void *d_w_sf, const float *d_w_scale, int64_t N,
+                              const void *d_bias, const float *d_gate, float *d_residual, void *d_out, void *cuda_stream);
+
 /* The RoPE table the context built at spot_create (S5): copies cos and sin [S, d_h/2] fp32 to HOST. */
 spot_status spot_rope_table(const spot_ctx *ctx, float *h_cos, float *h_sin);
 

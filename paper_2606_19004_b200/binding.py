@@ -99,6 +99,10 @@ def load_library() -> C.CDLL:
         "spot_quantize_weight_rows": [vp, i64, i64, vp, vp, vp],
         "spot_quantize_e4m3": [i32, vp, i64, vp, vp],
         "spot_linear_fp8": [i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp, vp],
+        "spot_nvfp4_sizes": [i64, i64, C.POINTER(sz), C.POINTER(sz)],
+        "spot_nvfp4_row_scale": [vp, i64, i64, vp, vp],
+        "spot_nvfp4_quantize": [vp, i64, i64, vp, vp, vp, vp],
+        "spot_linear_nvfp4": [i32, vp, vp, i64, i64, vp, vp, vp, i64, vp, vp, vp, vp, vp],
         "spot_explore_host": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_linear": [i32, i32, i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp],
         "spot_qkv_rope_linear": [vp, i32, i32, i64, vp, i64, vp, vp, vp, vp, vp, i32, f32, vp, vp],
@@ -468,6 +472,48 @@ def spot_quantize_e4m3(x: torch.Tensor) -> torch.Tensor:
     out = torch.empty(x.shape, dtype=torch.float8_e4m3fn, device=x.device)
     _check(load_library().spot_quantize_e4m3(_dt(x.dtype), _ptr(x), x.numel(), _ptr(out), _stream()), "spot_quantize_e4m3")
     return out
+
+
+def spot_nvfp4_quantize(x: torch.Tensor, row_scale: Optional[torch.Tensor] = None):
+    """bf16 [rows, K] -> (codes uint8 [rows, K / 2], scale-factor atoms uint8 [rows / 128 * K / 64 * 512]) (DESIGN.md section
+    13b readings N3 / N4; each row is divided by row_scale[r] first when given).  rows % 128 == 0, K % 64 == 0."""
+    rows, K = x.shape
+    cb, sb = C.c_size_t(), C.c_size_t()
+    _check(load_library().spot_nvfp4_sizes(rows, K, C.byref(cb), C.byref(sb)), "spot_nvfp4_sizes")
+    codes = torch.empty((rows, K // 2), dtype=torch.uint8, device=x.device)
+    sf = torch.zeros(int(sb.value), dtype=torch.uint8, device=x.device)
+    assert codes.numel() == int(cb.value)
+    _check(load_library().spot_nvfp4_quantize(_ptr(x), rows, K, _ptr(row_scale), _ptr(codes), _ptr(sf), _stream()), "spot_nvfp4_quantize")
+    return codes, sf
+
+
+def spot_nvfp4_quantize_weight(w: torch.Tensor):
+    """bf16 [N, K] -> (codes, scale-factor atoms, fp32 per-row scale s_n = max|W_n| / (6 * 448)) (reading N4)."""
+    N, K = w.shape
+    scale = torch.empty(N, dtype=torch.float32, device=w.device)
+    _check(load_library().spot_nvfp4_row_scale(_ptr(w), N, K, _ptr(scale), _stream()), "spot_nvfp4_row_scale")
+    codes, sf = spot_nvfp4_quantize(w, scale)
+    return codes, sf, scale
+
+
+def nvfp4_sf_index(rows: int, K: int) -> torch.Tensor:
+    """[rows, K / 16] -> byte offset of the scale factor of (row r, block b) in the atom buffer (layout of csrc/nvfp4.cu)."""
+    r = torch.arange(rows).view(-1, 1)
+    b = torch.arange(K // 16).view(1, -1)
+    return ((r // 128) * (K // 64) + b // 4) * 512 + (r % 32) * 16 + ((r % 128) // 32) * 4 + b % 4
+
+
+def spot_linear_nvfp4(a_codes: torch.Tensor, a_sf: torch.Tensor, w_codes: torch.Tensor, w_sf: torch.Tensor, w_scale: torch.Tensor,
+                      bias: torch.Tensor, epi: int = EPI_BIAS, gate: Optional[torch.Tensor] = None,
+                      residual: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Block-scaled 4-bit Linear on quantised operands; EPI_BIAS / EPI_BIAS_GELU return bf16 [M, N], EPI_GATE_RESIDUAL updates
+    `residual` (fp32)."""
+    M, K = a_codes.shape[0], a_codes.shape[1] * 2
+    N = w_codes.shape[0]
+    out = None if epi == EPI_GATE_RESIDUAL else torch.empty((M, N), dtype=torch.bfloat16, device=a_codes.device)
+    _check(load_library().spot_linear_nvfp4(epi, _ptr(a_codes), _ptr(a_sf), M, K, _ptr(w_codes), _ptr(w_sf), _ptr(w_scale), N,
+                                            _ptr(bias), _ptr(gate), _ptr(residual), _ptr(out), _stream()), "spot_linear_nvfp4")
+    return residual if epi == EPI_GATE_RESIDUAL else out
 
 
 def spot_linear_fp8(a: torch.Tensor, wq: torch.Tensor, w_scale: torch.Tensor, bias: torch.Tensor, epi: int = EPI_BIAS,

@@ -1258,4 +1258,55 @@ spot_status spot_linear_fp8(spot_epilogue epi, const void* d_a, int64_t M, int64
   return launch_gemm_tcgen05_v3(e, &p, 1, sm_count(), (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
 }
 
+// ---- NVFP4 building blocks -----------------------------------------------------------------
+spot_status spot_nvfp4_sizes(int64_t rows, int64_t K, size_t* codes_bytes, size_t* sf_bytes) {
+  if (!codes_bytes || !sf_bytes) return SPOT_ERR_NULL;
+  if (rows < 0 || K <= 0 || K % 64) return SPOT_ERR_SHAPE;
+  *codes_bytes = nvfp4_codes_bytes(rows, K);
+  *sf_bytes = nvfp4_sf_bytes(rows, K);
+  return SPOT_OK;
+}
+
+spot_status spot_nvfp4_row_scale(const void* d_w_bf16, int64_t rows, int64_t K, float* d_scale, void* cuda_stream) {
+  if (rows < 0 || K <= 0 || K % 8 || rows > 0x7fffffff || K > 0x7fffffff) return SPOT_ERR_SHAPE;
+  if (rows == 0) return SPOT_OK;
+  if (!d_w_bf16 || !d_scale) return SPOT_ERR_NULL;
+  if (!aligned16(d_w_bf16)) return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  return launch_nvfp4_row_scale(d_w_bf16, (int)rows, (int)K, d_scale, (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
+spot_status spot_nvfp4_quantize(const void* d_src_bf16, int64_t rows, int64_t K, const float* d_row_scale, void* d_codes,
+                                void* d_sf, void* cuda_stream) {
+  if (rows < 0 || K <= 0 || K % 64 || rows % 128 || rows > 0x7fffffff || K > 0x7fffffff) return SPOT_ERR_SHAPE;
+  if (rows == 0) return SPOT_OK;
+  if (!d_src_bf16 || !d_codes || !d_sf) return SPOT_ERR_NULL;
+  if (!aligned16(d_src_bf16) || !aligned16(d_codes) || !aligned16(d_sf)) return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  return launch_nvfp4_quantize(d_src_bf16, plain_rows((int)rows, K), (int)rows, (int)K, d_row_scale, d_codes, d_sf,
+                               (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
+spot_status spot_linear_nvfp4(spot_epilogue epi, const void* d_a_codes, const void* d_a_sf, int64_t M, int64_t K,
+                              const void* d_w_codes, const void* d_w_sf, const float* d_w_scale, int64_t N,
+                              const void* d_bias, const float* d_gate, float* d_residual, void* d_out, void* cuda_stream) {
+  if (M < 0 || N <= 0 || K <= 0 || M > 0x7fffffff || N > 0x7fffffff || K > 0x7fffffff) return SPOT_ERR_SHAPE;
+  if (M == 0) return SPOT_OK;
+  if (!d_a_codes || !d_a_sf || !d_w_codes || !d_w_sf || !d_w_scale || !d_bias) return SPOT_ERR_NULL;
+  const bool gate_res = epi == SPOT_EPI_GATE_RESIDUAL;
+  if (gate_res ? (!d_gate || !d_residual) : !d_out) return SPOT_ERR_NULL;
+  if (!aligned16(d_a_codes) || !aligned16(d_a_sf) || !aligned16(d_w_codes) || !aligned16(d_w_sf) || !aligned16(d_w_scale) ||
+      !aligned16(d_bias) || !aligned16(d_out) || !aligned16(d_residual) || !aligned16(d_gate))
+    return SPOT_ERR_ALIGN;
+  if (device_state() != 1) return SPOT_ERR_ARCH;
+  Nvfp4Problem p;
+  memset(&p, 0, sizeof(p));
+  p.a_codes = d_a_codes; p.a_sf = d_a_sf; p.w_codes = d_w_codes; p.w_sf = d_w_sf; p.w_scale = d_w_scale; p.bias = d_bias;
+  p.M = (int)M; p.N = (int)N; p.K = (int)K;
+  if (gate_res) { p.gate = d_gate; p.resid = d_residual; } else p.out = d_out;
+  if (!nvfp4_gemm_supported(p)) return SPOT_ERR_SHAPE;
+  const Epilogue e = epi == SPOT_EPI_BIAS ? EPI_BIAS : (epi == SPOT_EPI_BIAS_GELU ? EPI_BIAS_GELU : EPI_GATE_RES);
+  return launch_gemm_nvfp4(e, &p, 1, sm_count(), (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;
+}
+
 }  // extern "C"

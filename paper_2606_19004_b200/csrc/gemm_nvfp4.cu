@@ -1,0 +1,273 @@
+// gemm_nvfp4.cu - the MLP Linears of the NVFP4 exploration variant on the block-scaled 4-bit tensor-core path
+// (reading N5; "a cheap exploratory rollout ... with a quantized model"):
+//     y[m, n] = s_n * sum_b sfa[m, b] sfw[n, b] sum_{k in block b} a[m, k] w[n, k]  (+ bias, epilogue)
+// a, w: E2M1 codes (two per byte, K-major), sfa / sfw: E4M3 scale factors per 16 elements of K in the 512-byte atoms
+// nvfp4.cu writes, s_n: fp32 per output channel.
+//
+//   warp 0      producer: per 256-element K block one TMA load of the A tile [128 rows x 128 bytes] and of the W tile
+//               [256 x 128 bytes] (128-byte swizzle) plus three plain bulk copies of their scale-factor atoms (4 atoms of
+//               512 bytes for A, 2 x 4 for W) into a 3-stage ring
+//   warp 1      issuer (elect.sync): per K block 12 x tcgen05.cp 32x128b.warpx4 (scale factors shared -> tensor memory;
+//               executes in issue order with the MMAs, so no barrier in between) and 4 x tcgen05.mma
+//               kind::mxf4nvf4.block_scale.block16, M128 N256 K64, accumulating into 256 tensor-memory columns
+//   warp 2      tensor-memory allocator;  warps 4-7 epilogue: tcgen05.ld, * s_n + bias, then
+//                 EPI_BIAS_GELU -> tanh-GELU -> bf16 rows (fc1)      EPI_GATE_RES -> h += gate * y on the fp32 residual (fc2)
+// One CTA per SM, tiles 128 x 256 round-robin; ONE accumulator (the scale factors take the tensor-memory columns a
+// second one would need), so the epilogue of a tile is not overlapped with the next tile's MMAs.  This is the first,
+// correctness-first version of the path: its parity with oracle/nvfp4.py is the contract, its speed is reported as is.
+#include <string.h>
+
+#include "kernels.h"
+#include "tcgen05.cuh"
+
+namespace {
+
+constexpr int BLOCK_M = 128, BLOCK_N = 256, BLOCK_K = 256 /* E2M1 elements = 128 bytes */, UMMA_K = 64, STAGES = 3;
+constexpr uint32_t A_BYTES = BLOCK_M * 128, B_BYTES = BLOCK_N * 128, SFA_BYTES = 4 * 512, SFB_BYTES = 2 * 4 * 512;
+constexpr uint32_t OFF_SFA = A_BYTES + B_BYTES, OFF_SFB = OFF_SFA + SFA_BYTES;
+constexpr uint32_t STAGE_BYTES = 56 * 1024;                          // 54 KB used, padded to keep 1024-byte alignment
+constexpr uint32_t TX_BYTES = A_BYTES + B_BYTES + SFA_BYTES + SFB_BYTES;
+constexpr uint32_t OFF_BAR = STAGES * STAGE_BYTES;
+constexpr uint32_t SMEM_BYTES = OFF_BAR + 256 + 1024;
+constexpr int NUM_THREADS = 256;
+constexpr uint32_t TM_SF = 256, SF_COLS_PER_STAGE = 4 * (4 + 8);     // tensor-memory columns: [0,256) accumulator, then scale factors
+
+struct NvProblem {
+  int m_tiles, n_tiles, k_blocks, tile_start, M, N;
+  const uint8_t* sfa;       // atoms [M / 128][K / 64][512]
+  const uint8_t* sfw;       // atoms [N / 128][K / 64][512]
+  const float* w_scale;     // [N]
+  const bf16* bias;         // [N]
+  bf16* out;                // EPI_BIAS_GELU: [M, N] bf16
+  const float* gate;        // EPI_GATE_RES
+  float* resid;             // EPI_GATE_RES: [M, N] fp32, updated in place
+};
+struct NvParams {
+  NvProblem p[2];
+  int n_probs, total_tiles;
+};
+
+__device__ __forceinline__ float gelu_tanh_fast(float x) {
+  const float k0 = 0.7978845608028654f, k1 = 0.7978845608028654f * 0.044715f;
+  const float inner = x * fmaf(k1, x * x, k0);
+  float th;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(inner));
+  const float hx = 0.5f * x;
+  return fmaf(hx, th, hx);
+}
+
+template <int EPI>
+__global__ void __launch_bounds__(NUM_THREADS, 1)
+gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmW0,
+                  const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmW1, const NvParams P) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + OFF_BAR;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  const uint32_t tfull_bar = bar_base + 8u * (2 * STAGES), tempty_bar = bar_base + 8u * (2 * STAGES + 1);
+  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 2);
+  volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmA0); ptx::prefetch_tmap(&tmW0);
+    if (P.n_probs > 1) { ptx::prefetch_tmap(&tmA1); ptx::prefetch_tmap(&tmW1); }
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    ptx::mbar_init(tfull_bar, 1);
+    ptx::mbar_init(tempty_bar, 4);
+    ptx::fence_barrier_init();
+  }
+  if (warp == 2) { ptx::tmem_alloc(tmem_slot, 512); ptx::tmem_relinquish(); }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  auto tile_of = [&](int t, int& prob, int& mt, int& nt) {
+    prob = (P.n_probs > 1 && t >= P.p[1].tile_start) ? 1 : 0;
+    const NvProblem& q = P.p[prob];
+    t -= q.tile_start;
+    // n-major inside pairs of M tiles: neighbouring CTAs share their A rows or their W rows in L2
+    const int per_group = 2 * q.n_tiles, g = t / per_group, first_m = 2 * g;
+    const int gm = min(2, q.m_tiles - first_m), r = t - g * per_group;
+    mt = first_m + r % gm;
+    nt = r / gm;
+  };
+
+  if (warp == 0) {
+    // ===================== producer =====================
+    if (ptx::elect_one()) {
+      int stage = 0; uint32_t phase = 0;
+      for (int t = blockIdx.x; t < P.total_tiles; t += gridDim.x) {
+        int prob, mt, nt;
+        tile_of(t, prob, mt, nt);
+        const NvProblem& q = P.p[prob];
+        const CUtensorMap* mA = prob ? &tmA1 : &tmA0;
+        const CUtensorMap* mW = prob ? &tmW1 : &tmW0;
+        const long long ka = (long long)q.k_blocks * 4;           // K / 64 atoms per 128 rows
+        for (int kb = 0; kb < q.k_blocks; ++kb) {
+          ptx::mbar_wait(empty_bar(stage), phase ^ 1);
+          ptx::mbar_arrive_expect_tx(full_bar(stage), TX_BYTES);
+          const uint32_t sa = smem_base + stage * STAGE_BYTES;
+          ptx::tma_load_2d(sa, mA, full_bar(stage), kb * 128, mt * BLOCK_M);
+          ptx::tma_load_2d(sa + A_BYTES, mW, full_bar(stage), kb * 128, nt * BLOCK_N);
+          ptx::bulk_load_1d(sa + OFF_SFA, q.sfa + ((long long)mt * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
+          ptx::bulk_load_1d(sa + OFF_SFB, q.sfw + ((long long)(2 * nt) * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
+          ptx::bulk_load_1d(sa + OFF_SFB + SFA_BYTES, q.sfw + ((long long)(2 * nt + 1) * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== scale-factor copies + MMA issue =====================
+    if (ptx::elect_one()) {
+      constexpr uint32_t idesc = ptx::make_idesc_nvfp4(BLOCK_M, BLOCK_N);
+      int stage = 0; uint32_t phase = 0, acc_phase = 0;
+      for (int t = blockIdx.x; t < P.total_tiles; t += gridDim.x) {
+        int prob, mt, nt;
+        tile_of(t, prob, mt, nt);
+        const int k_blocks = P.p[prob].k_blocks;
+        ptx::mbar_wait(tempty_bar, acc_phase ^ 1);                  // the epilogue has drained the accumulator
+        ptx::tc_fence_after();
+        for (int kb = 0; kb < k_blocks; ++kb) {
+          ptx::mbar_wait(full_bar(stage), phase);
+          ptx::tc_fence_after();
+          const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
+          const uint32_t tsf = tmem_base + TM_SF + stage * SF_COLS_PER_STAGE;
+#pragma unroll
+          for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+            // scale factors of this K = 64 step: A rows 0-127 -> 4 columns, W rows 0-127 / 128-255 -> 4 + 4 columns
+            const uint32_t sfa_t = tsf + k * 12, sfb_t = sfa_t + 4;
+            ptx::tmem_cp_32x128b_warpx4(sfa_t, ptx::make_smem_desc_noswizzle(sa + OFF_SFA + k * 512, 128, 128));
+            ptx::tmem_cp_32x128b_warpx4(sfb_t, ptx::make_smem_desc_noswizzle(sa + OFF_SFB + k * 512, 128, 128));
+            ptx::tmem_cp_32x128b_warpx4(sfb_t + 4, ptx::make_smem_desc_noswizzle(sa + OFF_SFB + SFA_BYTES + k * 512, 128, 128));
+            ptx::mma_nvfp4_ss(tmem_base, ptx::make_smem_desc(sa + k * 32, 16, 1024), ptx::make_smem_desc(sb + k * 32, 16, 1024), idesc,
+                              sfa_t, sfb_t, (kb | k) ? 1u : 0u);
+          }
+          ptx::mma_commit(empty_bar(stage));
+          if (kb == k_blocks - 1) ptx::mma_commit(tfull_bar);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+        acc_phase ^= 1;
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue =====================
+    const int q4 = warp & 3;                      // tensor-memory lane quarter of this warp
+    uint32_t acc_phase = 0;
+    for (int t = blockIdx.x; t < P.total_tiles; t += gridDim.x) {
+      int prob, mt, nt;
+      tile_of(t, prob, mt, nt);
+      const NvProblem& q = P.p[prob];
+      const long long r = (long long)mt * BLOCK_M + q4 * 32 + lane;
+      ptx::mbar_wait(tfull_bar, acc_phase);
+      ptx::tc_fence_after();
+      const uint32_t taddr0 = tmem_base + ((uint32_t)(q4 * 32) << 16);
+#pragma unroll 1
+      for (int ch = 0; ch < BLOCK_N / 32; ++ch) {
+        const int n0 = nt * BLOCK_N + ch * 32;
+        uint32_t v[32];
+        ptx::tmem_ld_32x32(taddr0 + ch * 32, v);
+        ptx::tmem_ld_wait();
+        float y[32];
+        const uint4* bp = reinterpret_cast<const uint4*>(q.bias + n0);
+        const float4* sp = reinterpret_cast<const float4*>(q.w_scale + n0);
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+          const uint4 braw = __ldg(bp + g);
+          const bf16* bb = reinterpret_cast<const bf16*>(&braw);
+          const float4 s0 = __ldg(sp + 2 * g), s1 = __ldg(sp + 2 * g + 1);
+          const float sc[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+#pragma unroll
+          for (int j = 0; j < 8; ++j) y[g * 8 + j] = fmaf(__uint_as_float(v[g * 8 + j]), sc[j], __bfloat162float(bb[j]));
+        }
+        if (EPI == EPI_GATE_RES) {
+          float4* rp = reinterpret_cast<float4*>(q.resid + r * q.N + n0);
+          const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
+#pragma unroll
+          for (int g = 0; g < 8; ++g) {
+            float4 h = rp[g];
+            const float4 gt = __ldg(gp + g);
+            h.x = fmaf(gt.x, y[4 * g], h.x); h.y = fmaf(gt.y, y[4 * g + 1], h.y);
+            h.z = fmaf(gt.z, y[4 * g + 2], h.z); h.w = fmaf(gt.w, y[4 * g + 3], h.w);
+            rp[g] = h;
+          }
+        } else {
+          uint4* op = reinterpret_cast<uint4*>(q.out + r * q.N + n0);
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            float z[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) z[j] = EPI == EPI_BIAS_GELU ? gelu_tanh_fast(y[8 * g + j]) : y[8 * g + j];
+            uint4 pk;
+            __nv_bfloat162 p0 = __floats2bfloat162_rn(z[0], z[1]), p1 = __floats2bfloat162_rn(z[2], z[3]);
+            __nv_bfloat162 p2 = __floats2bfloat162_rn(z[4], z[5]), p3 = __floats2bfloat162_rn(z[6], z[7]);
+            pk.x = *reinterpret_cast<uint32_t*>(&p0); pk.y = *reinterpret_cast<uint32_t*>(&p1);
+            pk.z = *reinterpret_cast<uint32_t*>(&p2); pk.w = *reinterpret_cast<uint32_t*>(&p3);
+            op[g] = pk;
+          }
+        }
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(tempty_bar);
+      acc_phase ^= 1;
+    }
+  }
+
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem_base, 512); }
+}
+
+}  // namespace
+
+bool nvfp4_gemm_supported(const Nvfp4Problem& p) {
+  return p.M > 0 && p.N > 0 && p.K > 0 && p.M % BLOCK_M == 0 && p.N % BLOCK_N == 0 && p.K % BLOCK_K == 0 && p.a_codes && p.a_sf &&
+         p.w_codes && p.w_sf && p.w_scale && p.bias && spot_get_encode_tiled() != nullptr;
+}
+
+cudaError_t launch_gemm_nvfp4(Epilogue epi, const Nvfp4Problem* probs, int n_probs, int num_sms, cudaStream_t st) {
+  if (n_probs < 1 || n_probs > 2 || (epi != EPI_BIAS && epi != EPI_BIAS_GELU && epi != EPI_GATE_RES)) return cudaErrorInvalidValue;
+  NvParams P;
+  memset(&P, 0, sizeof(P));
+  CUtensorMap tm[4];
+  memset(tm, 0, sizeof(tm));
+  int tiles = 0, np = 0;
+  for (int i = 0; i < n_probs; ++i) {
+    const Nvfp4Problem& g = probs[i];
+    if (g.M == 0) continue;
+    if (!nvfp4_gemm_supported(g)) return cudaErrorInvalidValue;
+    if ((epi == EPI_GATE_RES) != (g.resid != nullptr) || (epi != EPI_GATE_RES && !g.out)) return cudaErrorInvalidValue;
+    NvProblem& q = P.p[np];
+    q.m_tiles = g.M / BLOCK_M; q.n_tiles = g.N / BLOCK_N; q.k_blocks = g.K / BLOCK_K; q.tile_start = tiles; q.M = g.M; q.N = g.N;
+    q.sfa = (const uint8_t*)g.a_sf; q.sfw = (const uint8_t*)g.w_sf; q.w_scale = g.w_scale; q.bias = (const bf16*)g.bias;
+    q.out = (bf16*)g.out; q.gate = g.gate; q.resid = g.resid;
+    tiles += q.m_tiles * q.n_tiles;
+    const uint64_t adims[2] = {(uint64_t)g.K / 2, (uint64_t)g.M}, wdims[2] = {(uint64_t)g.K / 2, (uint64_t)g.N};
+    const uint64_t str[1] = {(uint64_t)g.K / 2};
+    const uint32_t abox[2] = {128, BLOCK_M}, wbox[2] = {128, BLOCK_N};
+    SPOT_CUDA_TRY(spot_make_tmap_u8(&tm[2 * np], g.a_codes, 2, adims, str, abox));
+    SPOT_CUDA_TRY(spot_make_tmap_u8(&tm[2 * np + 1], g.w_codes, 2, wdims, str, wbox));
+    ++np;
+  }
+  if (np == 0) return cudaSuccess;
+  if (np == 1) { tm[2] = tm[0]; tm[3] = tm[1]; }
+  P.n_probs = np;
+  P.total_tiles = tiles;
+  static bool attr_set = false;
+  if (!attr_set) {
+    SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_nvfp4_kernel<EPI_BIAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
+    SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_nvfp4_kernel<EPI_BIAS_GELU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
+    SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_nvfp4_kernel<EPI_GATE_RES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
+    attr_set = true;
+  }
+  const int grid = tiles < num_sms ? tiles : num_sms;
+  if (epi == EPI_BIAS) gemm_nvfp4_kernel<EPI_BIAS><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], P);
+  else if (epi == EPI_BIAS_GELU) gemm_nvfp4_kernel<EPI_BIAS_GELU><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], P);
+  else gemm_nvfp4_kernel<EPI_GATE_RES><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], P);
+  return cudaGetLastError();
+}

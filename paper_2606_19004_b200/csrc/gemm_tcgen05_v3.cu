@@ -617,7 +617,9 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
       // narrow outputs want short ones.  SPOT_GEMM_GROUP_M overrides (A/B timing only).
       static int forced = -1;
       if (forced < 0) { const char* e = getenv("SPOT_GEMM_GROUP_M"); forced = e ? atoi(e) : 0; }
-      int gm = 2;
+      static int narrow = -1;                       // A/B only: group height of the narrow-output GEMMs (out-proj, fc2)
+      if (narrow < 0) { const char* e = getenv("SPOT_GEMM_GROUP_M_NARROW"); narrow = e ? atoi(e) : 0; }
+      int gm = narrow > 0 ? narrow : 2;
       if (q.n_tiles >= 24) {
         gm = (int)(25.0e6 / ((double)es * PAIR_M * (double)g.K));  // A panel of a group ~25 MB
         if (gm > 16) gm = 16;

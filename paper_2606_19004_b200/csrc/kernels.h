@@ -66,6 +66,26 @@ cudaError_t launch_tc_gather(const float* src, float* dst, const int* idx, int d
 cudaError_t launch_tc_combine(float* h0, float* resid, const float* hc, const int* pos, int B, long long n_per_seq,
                               cudaStream_t st);
 
+// NVFP4 exploration variant (nvfp4.cu, gemm_nvfp4.cu): E2M1 codes [rows, K / 2] + E4M3 block scales in
+// 512-byte atoms (128 rows x 4 blocks of 16), fp32 per-row second-level scale for weights
+struct Nvfp4Problem {
+  const void* a_codes; const void* a_sf;     // activations [M, K / 2], atoms [M / 128][K / 64][512]
+  const void* w_codes; const void* w_sf;     // weights     [N, K / 2], atoms [N / 128][K / 64][512]
+  const float* w_scale;                      // [N] fp32
+  const void* bias;                          // [N] bf16
+  int M, N, K;
+  void* out;                                 // EPI_BIAS / EPI_BIAS_GELU: [M, N] bf16
+  const float* gate;                         // EPI_GATE_RES: [N] fp32
+  float* resid;                              // EPI_GATE_RES: [M, N] fp32 residual, updated in place
+};
+size_t nvfp4_codes_bytes(long long rows, long long K);
+size_t nvfp4_sf_bytes(long long rows, long long K);
+cudaError_t launch_nvfp4_quantize(const void* src_bf16, RowMap map, int rows, int K, const float* row_scale, void* codes,
+                                  void* sf, cudaStream_t st);
+cudaError_t launch_nvfp4_row_scale(const void* w_bf16, int rows, int K, float* scale, cudaStream_t st);
+bool nvfp4_gemm_supported(const Nvfp4Problem& p);
+cudaError_t launch_gemm_nvfp4(Epilogue epi, const Nvfp4Problem* probs, int n_probs, int num_sms, cudaStream_t st);
+
 // FP8 exploration variant (fp8.cu): per-output-channel weight quantisation, unit-scale activation cast
 cudaError_t launch_quantize_weight_rows(const void* w_bf16, long long N, int K, void* wq, float* scale, cudaStream_t st);
 cudaError_t launch_quantize_e4m3(spot_dtype dt, const void* in, long long n, void* out, cudaStream_t st);

@@ -164,6 +164,48 @@ __host__ __device__ constexpr uint32_t make_idesc_e4m3(int M, int N) {
 }
 }  // namespace ptx
 
+// ---- block-scaled 4-bit MMA (kind::mxf4nvf4, NVFP4: E2M1 values, one E4M3 scale per 16 elements along K) --------
+namespace ptx {
+// Shared-memory descriptor WITHOUT swizzle (layout type 0): K-major core matrices of 8 rows x 16 bytes; SBO = distance
+// between core matrices along M/N, LBO = along K.  Used as the source of tcgen05.cp for the scale factors.
+__device__ __forceinline__ uint64_t make_smem_desc_noswizzle(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr >> 4) & 0x3FFF);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;
+  return d;
+}
+// Instruction descriptor of the block-scaled kinds: b_sf_id [4,6), a_format [7,10), b_format [10,13) (kind::mxf4nvf4:
+// 1 = E2M1), a/b major bits 15/16 (0 = K-major), N >> 3 in [17,23), scale format bit 23 (0 = E4M3, 1 = E8M0),
+// M >> 4 in [24,29), a_sf_id [29,31), bit 31: K = 64 (0) per instruction.  The accumulator is always fp32.
+__host__ __device__ constexpr uint32_t make_idesc_nvfp4(int M, int N) {
+  return (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+// 512 bytes of scale factors (32 rows x 16 bytes in shared memory) -> 4 columns of tensor memory, the same 32 lanes
+// replicated into all four lane quarters (the layout the block-scaled MMA reads its scale factors in).  Executes in
+// issue order with the tcgen05.mma of the same thread.
+__device__ __forceinline__ void tmem_cp_32x128b_warpx4(uint32_t taddr, uint64_t sdesc) {
+  asm volatile("tcgen05.cp.cta_group::1.32x128b.warpx4 [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+// D[tmem] (+)= (A * SFA)[smem desc] * (B * SFB)[smem desc], E2M1 operands (K = 64 per instruction), E4M3 scale factors
+// per 16 elements in tensor memory at sfa / sfb (4 columns per 128 rows), fp32 accumulate, one thread issues.
+__device__ __forceinline__ void mma_nvfp4_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t sfa,
+                                             uint32_t sfb, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::mxf4nvf4.block_scale.block16 [%0], %1, %2, %3, [%5], [%6], p;\n\t}\n" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(sfa), "r"(sfb)
+      : "memory");
+}
+// plain (non-tensor) bulk copy global -> shared, completion on an mbarrier (16-byte granularity)
+__device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(reinterpret_cast<uint64_t>(src)), "r"(bytes), "r"(bar)
+               : "memory");
+}
+}  // namespace ptx
+
 // ---- host: cuTensorMapEncodeTiled through the runtime's driver entry point (no -lcuda) -----------
 typedef CUresult (*spot_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                          const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
