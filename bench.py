@@ -526,7 +526,7 @@ def main():
     ap.add_argument("--gemm-impl", type=int, default=0,
                     help="0 auto (CTA pair + TMA-store epilogue, K4 fused), 2 one-CTA tcgen05, 3 CTA pair with per-thread "
                          "epilogue, 4 as 0 with K4 as its own kernel (A/B testing)")
-    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp8"],
+    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp8", "nvfp4"],
                     help="fp8 = the low-precision exploration variant (E4M3 block Linears, DESIGN.md section 13): NOT the "
                          "headline configuration; the line says dtype fp8 and adds the reward rank correlation with bf16")
     ap.add_argument("--cache-threshold", type=float, default=None,
@@ -541,7 +541,7 @@ def main():
         return run_dry(args, shape, world)
     if args.kernels:
         return run_kernels(args, shape)
-    if args.precision == "fp8" and args.gemm_impl not in (0,):
+    if args.precision != "bf16" and args.gemm_impl not in (0,):
         sys.exit("bench.py: --precision fp8 runs only on the default GEMM (--gemm-impl 0); other values would run bf16 Linears")
     if args.workload == "cfg2":
         return run_block(args, shape)
@@ -593,7 +593,8 @@ def main():
     out = None
 
     cached = args.cache_threshold is not None
-    fp8 = args.precision == "fp8"
+    fp8 = args.precision in ("fp8", "nvfp4")
+    nvfp4 = args.precision == "nvfp4"
     if cached or fp8 or strong:
         args.no_e2e = True
         assert not (strong and (cached or fp8)), "--scaling strong times the plain bf16 rollout"
@@ -618,7 +619,9 @@ def main():
     full_rewards = None
     if cached or fp8:                            # the full bf16 rollout's rewards, for the rank correlation of PAPER.md:340
         full_rewards = spot.spot_explore(ctx, seeds, text, ts, probe, P, K, k_sel)["rewards"].clone()
-    if fp8:
+    if nvfp4:
+        ctx.enable_nvfp4(True)
+    elif fp8:
         ctx.enable_fp8(True)
     for _ in range(args.warmup):
         step()
@@ -709,7 +712,8 @@ def main():
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": int(joined.item()), "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_step, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
-                "dtype": "fp8_e4m3 block Linears (bf16 attention, fp32 residual): exploration variant, not the headline" if fp8 else "bf16",
+                "dtype": ("nvfp4 MLP Linears + fp8_e4m3 QKV / out-proj (bf16 attention, fp32 residual): exploration variant, not the headline" if nvfp4
+                          else "fp8_e4m3 block Linears (bf16 attention, fp32 residual): exploration variant, not the headline" if fp8 else "bf16"),
                 "data": "synthetic",
                 "config": {**workload_config(shape),
                            "l2": "inputs (40.8 GB of weights streamed every Euler step) are larger than L2",

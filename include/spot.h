@@ -100,6 +100,7 @@ typedef enum {
   SPOT_OPT_ATTN_IMPL = 1,   /* 0 = auto (tcgen05 for bf16, d_h = 128: one-pass kernel, 64-key tiles), 1 = SIMT attention, 2 = previous two-pass tcgen05 kernel */
   SPOT_OPT_TIMING = 2,      /* 1 = bracket every tcgen05 GEMM launch with CUDA events on the launch stream */
   SPOT_OPT_FP8 = 3,         /* 1 = the four Linears of every block run on E4M3 operands (after spot_fp8_prepare) */
+  SPOT_OPT_NVFP4 = 5,       /* 1 = on top of SPOT_OPT_FP8, fc1 / fc2 of every block run on NVFP4 operands (after spot_nvfp4_prepare) */
   SPOT_OPT_CHUNK_SEQS = 4   /* sequences per pass of the block stack in spot_dit_denoise / spot_explore / spot_explore_host: larger
                              * batches run as consecutive chunks of this many sequences (PAPER.md:338 caps an exploration batch at
                              * 32 sequences); 0 = the whole batch in one pass; default 32.  Results do not depend on it, bit for
@@ -254,6 +255,21 @@ spot_status spot_dit_denoise_sde(spot_ctx *ctx, int n_prompts, int seeds_per_pro
  * bf16 configs with head_dim 128 only (SPOT_ERR_DTYPE / SPOT_ERR_SHAPE otherwise). */
 spot_status spot_fp8_bytes(const spot_ctx *ctx, size_t *bytes);
 spot_status spot_fp8_prepare(spot_ctx *ctx, void *d_buffer, size_t bytes, void *cuda_stream);
+
+/* ---- 4-bit exploration variant: NVFP4 MLP Linears on top of the FP8 variant ----------------------------------------
+ * Same passages.  DESIGN.md section 13b (readings N1-N5): fc1 and fc2 of every block and stream -
+ * two thirds of the block's Linear FLOPs - take BOTH operands as NVFP4: E2M1 values {0, .5, 1, 1.5, 2, 3, 4, 6} with
+ * sign in blocks of 16 consecutive elements along K, one E4M3 scale factor per block,
+ *   activations  sf_b = e4m3(max_b |x| / 6),  q = e2m1(x / sf_b)   (made per call from the bf16 LN / GELU outputs),
+ *   weights      the same on W_n / s_n with s_n = max_k |W_nk| / (6 * 448) fp32 per output channel (spot_nvfp4_prepare),
+ *   y_n = s_n * sum_b sfx_b sfw_nb sum_{k in b} qx_k qw_nk + b_n on tcgen05.mma kind::mxf4nvf4.block_scale, fp32 accumulation;
+ * QKV and out-proj stay on the FP8 path, everything else is unchanged.  spot_nvfp4_bytes / spot_nvfp4_prepare work like
+ * their FP8 counterparts; spot_set_option(ctx, SPOT_OPT_NVFP4, 1) needs SPOT_OPT_FP8 = 1 and the prepared buffer
+ * (SPOT_ERR_SHAPE otherwise) and enlarges the workspace (query spot_workspace_bytes again).  hidden and mlp_hidden must
+ * be multiples of 256 and every call's image / text row counts (n_seqs * n_img, n_seqs * n_txt) multiples of 128
+ * (SPOT_ERR_SHAPE otherwise).  Switching SPOT_OPT_FP8 off switches this off too. */
+spot_status spot_nvfp4_bytes(const spot_ctx *ctx, size_t *bytes);
+spot_status spot_nvfp4_prepare(spot_ctx *ctx, void *d_buffer, size_t bytes, void *cuda_stream);
 
 #ifdef __cplusplus
 }

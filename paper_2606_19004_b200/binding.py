@@ -19,7 +19,7 @@ _lib: Optional[C.CDLL] = None
 SPOT_F32, SPOT_BF16 = 0, 1
 EPI_BIAS, EPI_BIAS_GELU, EPI_GATE_RESIDUAL = 0, 1, 2
 IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_2CTA, IMPL_TCGEN05_TMA = 0, 1, 2, 3, 4
-OPT_GEMM_IMPL, OPT_ATTN_IMPL, OPT_TIMING, OPT_FP8, OPT_CHUNK_SEQS = 0, 1, 2, 3, 4
+OPT_GEMM_IMPL, OPT_ATTN_IMPL, OPT_TIMING, OPT_FP8, OPT_CHUNK_SEQS, OPT_NVFP4 = 0, 1, 2, 3, 4, 5
 SPOT_E4M3 = 2     # storage type of the FP8 variant's activations / quantised weights (torch.float8_e4m3fn)
 STATUS_NAMES = ["SPOT_OK", "SPOT_ERR_NULL", "SPOT_ERR_SHAPE", "SPOT_ERR_DTYPE", "SPOT_ERR_ALIGN",
                 "SPOT_ERR_WORKSPACE", "SPOT_ERR_ARCH", "SPOT_ERR_CUDA", "SPOT_ERR_UNIMPLEMENTED"]
@@ -96,6 +96,8 @@ def load_library() -> C.CDLL:
         "spot_sde_update": [vp, vp, vp, i32, f32, f32, f32, i32, i64, vp, vp, vp],
         "spot_fp8_bytes": [vp, C.POINTER(sz)],
         "spot_fp8_prepare": [vp, vp, sz, vp],
+        "spot_nvfp4_bytes": [vp, C.POINTER(sz)],
+        "spot_nvfp4_prepare": [vp, vp, sz, vp],
         "spot_quantize_weight_rows": [vp, i64, i64, vp, vp, vp],
         "spot_quantize_e4m3": [i32, vp, i64, vp, vp],
         "spot_linear_fp8": [i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp, vp],
@@ -216,6 +218,21 @@ class Context:
             self._fp8_buf = torch.empty(int(n.value), dtype=torch.uint8, device="cuda")
             _check(lib.spot_fp8_prepare(self.handle, _ptr(self._fp8_buf), self._fp8_buf.numel(), _stream()), "spot_fp8_prepare", self)
         _check(lib.spot_set_option(self.handle, OPT_FP8, 1 if on else 0), "spot_set_option", self)
+
+    def enable_nvfp4(self, on: bool = True) -> None:
+        """4-bit exploration variant: FP8 variant + fc1 / fc2 on NVFP4 operands.  on=True switches both
+        on; on=False switches both off (back to bf16)."""
+        lib = load_library()
+        if on:
+            self.enable_fp8(True)
+            if getattr(self, "_nvfp4_buf", None) is None:
+                n = C.c_size_t()
+                _check(lib.spot_nvfp4_bytes(self.handle, C.byref(n)), "spot_nvfp4_bytes", self)
+                self._nvfp4_buf = torch.empty(int(n.value), dtype=torch.uint8, device="cuda")
+                _check(lib.spot_nvfp4_prepare(self.handle, _ptr(self._nvfp4_buf), self._nvfp4_buf.numel(), _stream()), "spot_nvfp4_prepare", self)
+        _check(lib.spot_set_option(self.handle, OPT_NVFP4, 1 if on else 0), "spot_set_option", self)
+        if not on:
+            _check(lib.spot_set_option(self.handle, OPT_FP8, 0), "spot_set_option", self)
 
     def workspace(self, n_seqs: int, n_steps: int, cached: bool = False) -> torch.Tensor:
         n = spot_workspace_bytes(self, n_seqs, n_steps, cached)

@@ -33,6 +33,11 @@ struct spot_ctx {
   struct Fp8Block { Fp8Linear lin[2][4]; };   // [stream][qkv, out, fc1, fc2]
   std::vector<Fp8Block> fp8_blocks;
   int fp8;                       // 1: block Linears run on E4M3 operands (SPOT_OPT_FP8; needs spot_fp8_prepare)
+  // NVFP4 exploration variant: fc1 / fc2 of every block as E2M1 codes + E4M3 block scales + fp32 row scale
+  struct Nv4Linear { const uint8_t* codes; const uint8_t* sf; const float* scale; };
+  struct Nv4Block { Nv4Linear lin[2][2]; };   // [stream][fc1, fc2]
+  std::vector<Nv4Block> nv4_blocks;
+  int nvfp4;                     // 1: the MLP Linears run on the block-scaled 4-bit path (SPOT_OPT_NVFP4; on top of SPOT_OPT_FP8)
   int chunk_seqs;                // sequences per pass of the block stack (SPOT_OPT_CHUNK_SEQS); 0 = whole batch
   int n_img() const { return cfg.grid_h * cfg.grid_w; }
   int seq() const { return cfg.n_txt + n_img(); }
@@ -67,6 +72,7 @@ struct Workspace {
   size_t t_dev, emb, hid, temb, cvec, mod, fmod, txt_norm, txt_h0, h_img, h_txt, ybuf, big, vel, stage, total;
   size_t st_seeds, st_text, st_probe, st_lat, st_rew, st_stats, st_top, st_bot;
   // cached-step variant only (carve(..., cached = true)): uncompacted h_img^0, previous modulated input, cached residual
+  size_t nv_codes[2], nv_sf[2];            // NVFP4 variant only: quantised MLP activations of the image / text stream
   size_t md_a, md_acc, md_ones, md_zero;   // tensor-core modulation path (conditioning): split c, accumulators, gate = 1, bias = 0
   size_t tc_h0, tc_mprev, tc_resid, tc_rowpart, tc_acc, tc_coeffs, tc_idx, tc_pos, tc_nact, tc_comp, tc_rel;
 };
@@ -107,6 +113,15 @@ Workspace carve(const spot_ctx* c, int B, int T, bool cached = false) {
   w.st_stats = take((size_t)B * 2 * 4);
   w.st_top = take((size_t)B * 4);
   w.st_bot = take((size_t)B * 4);
+  w.nv_codes[0] = w.nv_codes[1] = w.nv_sf[0] = w.nv_sf[1] = 0;
+  if (c->nvfp4) {
+    const size_t Kmax = (size_t)(D > (size_t)g.mlp_hidden ? D : g.mlp_hidden);
+    const size_t rows[2] = {(size_t)B * NI, (size_t)B * NT};
+    for (int s = 0; s < 2; ++s) {
+      w.nv_codes[s] = take(nvfp4_codes_bytes((long long)rows[s], (long long)Kmax));
+      w.nv_sf[s] = take(nvfp4_sf_bytes((long long)rows[s], (long long)Kmax));
+    }
+  }
   w.tc_h0 = w.tc_mprev = w.tc_resid = w.tc_rowpart = w.tc_acc = w.tc_coeffs = w.tc_idx = w.tc_pos = w.tc_nact = w.tc_comp =
       w.tc_rel = 0;
   if (cached) {
@@ -282,6 +297,7 @@ spot_status spot_create(const spot_config* cfg, const spot_weights* w, int max_s
   c->n_launches = c->gemm_launches = 0;
   c->timing = 0;
   c->fp8 = 0;
+  c->nvfp4 = 0;
   c->ev_used = 0;
   c->d_cos = c->d_sin = c->d_partials = c->d_partials2 = nullptr;
   int dev = 0;
@@ -341,6 +357,13 @@ spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
                   ctx->gemm_impl != 0))
       return SPOT_ERR_SHAPE;                     // spot_fp8_prepare first; bf16 configs with d_h = 128, default GEMM only
     ctx->fp8 = value;
+    if (!value) ctx->nvfp4 = 0;                  // the 4-bit MLP rides on the FP8 variant
+    return SPOT_OK;
+  }
+  if (opt == SPOT_OPT_NVFP4) {
+    if (value && (!ctx->fp8 || ctx->nv4_blocks.size() != ctx->blocks.size() || ctx->cfg.hidden % 256 || ctx->cfg.mlp_hidden % 256))
+      return SPOT_ERR_SHAPE;                     // SPOT_OPT_FP8 and spot_nvfp4_prepare first; widths in multiples of 256
+    ctx->nvfp4 = value;
     return SPOT_OK;
   }
   if (opt == SPOT_OPT_GEMM_IMPL) ctx->gemm_impl = value;
@@ -411,8 +434,11 @@ StreamMaps stream_maps(const spot_ctx* c, int B, int stream /*0 img, 1 txt*/) {
 // 2-8).  mod_img / mod_txt: [6D] fp32 = (shift1, scale1, gate1, shift2, scale2, gate2).  When
 // img_only_tail is set (last block of a denoise pass, S16) the text stream's out-proj and MLP,
 // whose result nobody reads, are skipped.
+struct Nv4Scratch { uint8_t* codes[2]; uint8_t* sf[2]; };   // quantised MLP activations per stream (NVFP4 variant)
+
 spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt, const float* mod_img,
-                       const float* mod_txt, void* ybuf, void* big, bool img_only_tail, cudaStream_t st) {
+                       const float* mod_txt, void* ybuf, void* big, bool img_only_tail, cudaStream_t st,
+                       const Nv4Scratch* nv = nullptr) {
   const spot_config& g = c->cfg;
   const spot_dtype dt = g.dtype;
   const int D = g.hidden, F = g.mlp_hidden, S = c->seq();
@@ -472,7 +498,32 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
   if (rs != SPOT_OK) return rs;
   // (8) y2 = LN(h)(1 + scale2) + shift2 ; u = GELU(y2 W1^T + b) ; h += gate2 * (u W2^T + b)
   for (int s = 0; s < ns; ++s) lp[s] = LnProblem{h[s], sm[s].rows, mod[s] + 3 * D, mod[s] + 4 * D, ybuf, sm[s].y};
-  LK(c, launch_ln_modulate2(adt, lp, ns, D, g.ln_eps, st));
+  const bool nv4 = f8 && c->nvfp4 != 0;
+  LK(c, launch_ln_modulate2(nv4 ? dt : adt, lp, ns, D, g.ln_eps, st));
+  if (nv4) {
+    // NVFP4 variant: y2 (bf16) -> E2M1 codes + E4M3 block scales -> fc1 on the block-scaled 4-bit
+    // tensor-core path with the GELU epilogue -> u (bf16, dense per stream in `big`) -> codes + scales -> fc2 with the
+    // gate-residual epilogue on the fp32 residual stream.
+    if (!nv) return SPOT_ERR_WORKSPACE;
+    const spot_ctx::Nv4Block& nb = c->nv4_blocks[block];
+    Nvfp4Problem np[2];
+    bf16* u[2] = {(bf16*)big, (bf16*)big + (long long)sm[0].rows * F};
+    for (int s = 0; s < ns; ++s) {
+      memset(&np[s], 0, sizeof(Nvfp4Problem));
+      np[s].a_codes = nv->codes[s]; np[s].a_sf = nv->sf[s]; np[s].w_codes = nb.lin[s][0].codes; np[s].w_sf = nb.lin[s][0].sf;
+      np[s].w_scale = nb.lin[s][0].scale; np[s].bias = bw.s[s].fc1_b; np[s].M = sm[s].rows; np[s].N = F; np[s].K = D; np[s].out = u[s];
+      if (np[s].M > 0 && !nvfp4_gemm_supported(np[s])) return SPOT_ERR_SHAPE;   // rows in multiples of 128, widths of 256
+      LK(c, launch_nvfp4_quantize(ybuf, sm[s].y, sm[s].rows, D, nullptr, nv->codes[s], nv->sf[s], st));
+    }
+    LK(c, launch_gemm_nvfp4(EPI_BIAS_GELU, np, ns, c->num_sms, st));
+    for (int s = 0; s < ns; ++s) {
+      LK(c, launch_nvfp4_quantize(u[s], plain_rows(sm[s].rows, F), sm[s].rows, F, nullptr, nv->codes[s], nv->sf[s], st));
+      np[s].w_codes = nb.lin[s][1].codes; np[s].w_sf = nb.lin[s][1].sf; np[s].w_scale = nb.lin[s][1].scale; np[s].bias = bw.s[s].fc2_b;
+      np[s].N = D; np[s].K = F; np[s].out = nullptr; np[s].gate = mod[s] + 5 * D; np[s].resid = h[s];
+    }
+    LK(c, launch_gemm_nvfp4(EPI_GATE_RES, np, ns, c->num_sms, st));
+    return SPOT_OK;
+  }
   for (int s = 0; s < ns; ++s) {
     memset(&pr[s], 0, sizeof(GemmProblem));
     pr[s].A = ybuf; pr[s].a_map = sm[s].y; pr[s].W = bw.s[s].fc1_w; pr[s].bias = bw.s[s].fc1_b;
@@ -580,6 +631,7 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
   if (rs != SPOT_OK) return rs;
   float* txt_h0 = (float*)(ws + w.txt_h0); float* h_img = (float*)(ws + w.h_img); float* h_txt = (float*)(ws + w.h_txt);
   void* ybuf = ws + w.ybuf; void* big = ws + w.big; float* vel = (float*)(ws + w.vel);
+  Nv4Scratch nvs{{ws + w.nv_codes[0], ws + w.nv_codes[1]}, {ws + w.nv_sf[0], ws + w.nv_sf[1]}};
   const float* mod = (const float*)(ws + w.mod); const float* fmod = (const float*)(ws + w.fmod);
   GemmProblem pr;
   // h_txt^0 = RMSNorm(text_emb) Wtxt^T + b, once per prompt (C7)
@@ -610,7 +662,7 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
       LK(c, launch_broadcast_prompts(txt_h0, h_txt, Bc, K, (long long)NT * D, st, b0));
       for (int b = 0; b < L; ++b) {
         const float* m = mod + ((long long)i * L + b) * 2 * 6 * D;
-        rs = block_core(c, b, Bc, h_img, h_txt, m, m + 6 * D, ybuf, big, b == L - 1, st);
+        rs = block_core(c, b, Bc, h_img, h_txt, m, m + 6 * D, ybuf, big, b == L - 1, st, c->nvfp4 ? &nvs : nullptr);
         if (rs != SPOT_OK) return rs;
       }
       // v = (LN(h_img)(1 + scale_f) + shift_f) Wp^T + b
@@ -667,6 +719,7 @@ spot_status denoise_cached_core(spot_ctx* c, int P, int K, float* lat, const voi
   int* d_idx = (int*)(ws + w.tc_idx); int* d_pos = (int*)(ws + w.tc_pos); int* d_nact = (int*)(ws + w.tc_nact);
   int* d_comp = (int*)(ws + w.tc_comp); float* d_rel = (float*)(ws + w.tc_rel);
   void* ybuf = ws + w.ybuf; void* big = ws + w.big; float* vel = (float*)(ws + w.vel);
+  Nv4Scratch nvs{{ws + w.nv_codes[0], ws + w.nv_codes[1]}, {ws + w.nv_sf[0], ws + w.nv_sf[1]}};
   const float* mod = (const float*)(ws + w.mod); const float* fmod = (const float*)(ws + w.fmod);
   std::vector<int> h_idx((size_t)B + 1), h_comp((size_t)B);
   std::vector<float> h_relv((size_t)B);
@@ -706,7 +759,8 @@ spot_status denoise_cached_core(spot_ctx* c, int P, int K, float* lat, const voi
         const int nc = n_act - a0 < chunk ? n_act - a0 : chunk;
         for (int b = 0; b < L; ++b) {
           const float* m = mod + ((long long)i * L + b) * 2 * 6 * D;
-          rs = block_core(c, b, nc, hc + a0 * per_img, h_txt + a0 * per_txt, m, m + 6 * D, ybuf, big, b == L - 1, st);
+          rs = block_core(c, b, nc, hc + a0 * per_img, h_txt + a0 * per_txt, m, m + 6 * D, ybuf, big, b == L - 1, st,
+                          c->nvfp4 ? &nvs : nullptr);
           if (rs != SPOT_OK) return rs;
         }
       }
@@ -784,7 +838,9 @@ spot_status spot_dit_block_forward(spot_ctx* ctx, int block, int n_seqs, const v
                         mod + (long long)sgm * 6 * D, 0, false, st));
   LK(ctx, launch_to_f32(g.dtype, d_h_img, h_img, n_img, st));
   LK(ctx, launch_to_f32(g.dtype, d_h_txt, h_txt, n_txt, st));
-  s = block_core(ctx, block, n_seqs, h_img, h_txt, mod, mod + 6 * D, ws + w.ybuf, ws + w.big, false, st);
+  Nv4Scratch nvs{{ws + w.nv_codes[0], ws + w.nv_codes[1]}, {ws + w.nv_sf[0], ws + w.nv_sf[1]}};
+  s = block_core(ctx, block, n_seqs, h_img, h_txt, mod, mod + 6 * D, ws + w.ybuf, ws + w.big, false, st,
+                 ctx->nvfp4 ? &nvs : nullptr);
   if (s != SPOT_OK) return s;
   LK(ctx, launch_from_f32(g.dtype, h_img, d_out_img, n_img, st));
   LK(ctx, launch_from_f32(g.dtype, h_txt, d_out_txt, n_txt, st));
@@ -984,6 +1040,47 @@ spot_status spot_fp8_prepare(spot_ctx* ctx, void* d_buffer, size_t bytes, void* 
         float* sc = (float*)p; p += align_up((size_t)N * 4);
         LK(ctx, launch_quantize_weight_rows(src[w], N, (int)K, wq, sc, st));
         ctx->fp8_blocks[b].lin[sgm][w] = spot_ctx::Fp8Linear{wq, sc};
+      }
+    }
+  return SPOT_OK;
+}
+
+// ---- NVFP4 exploration variant: fc1 / fc2 of every block ---------------------------------------
+spot_status spot_nvfp4_bytes(const spot_ctx* ctx, size_t* bytes) {
+  if (!ctx || !bytes) return SPOT_ERR_NULL;
+  if (ctx->cfg.dtype != SPOT_BF16) return SPOT_ERR_DTYPE;
+  const long long D = ctx->cfg.hidden, F = ctx->cfg.mlp_hidden;
+  if (D % 256 || F % 256) return SPOT_ERR_SHAPE;
+  const size_t fc1 = align_up(nvfp4_codes_bytes(F, D)) + align_up(nvfp4_sf_bytes(F, D)) + align_up((size_t)F * 4);
+  const size_t fc2 = align_up(nvfp4_codes_bytes(D, F)) + align_up(nvfp4_sf_bytes(D, F)) + align_up((size_t)D * 4);
+  *bytes = (fc1 + fc2) * 2 * (size_t)ctx->cfg.n_blocks;
+  return SPOT_OK;
+}
+
+spot_status spot_nvfp4_prepare(spot_ctx* ctx, void* d_buffer, size_t bytes, void* cuda_stream) {
+  if (!ctx || !d_buffer) return SPOT_ERR_NULL;
+  if (!aligned16(d_buffer)) return SPOT_ERR_ALIGN;
+  size_t need = 0;
+  spot_status s = spot_nvfp4_bytes(ctx, &need);
+  if (s != SPOT_OK) return s;
+  if (bytes < need) return SPOT_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  uint8_t* p = (uint8_t*)d_buffer;
+  const long long D = ctx->cfg.hidden, F = ctx->cfg.mlp_hidden;
+  ctx->nvfp4 = 0;
+  ctx->nv4_blocks.assign(ctx->blocks.size(), spot_ctx::Nv4Block());
+  for (size_t b = 0; b < ctx->blocks.size(); ++b)
+    for (int sgm = 0; sgm < 2; ++sgm) {
+      const spot_stream_weights& sw = ctx->blocks[b].s[sgm];
+      const void* src[2] = {sw.fc1_w, sw.fc2_w};
+      const long long N[2] = {F, D}, K[2] = {D, F};
+      for (int w = 0; w < 2; ++w) {
+        uint8_t* codes = p; p += align_up(nvfp4_codes_bytes(N[w], K[w]));
+        uint8_t* sf = p; p += align_up(nvfp4_sf_bytes(N[w], K[w]));
+        float* sc = (float*)p; p += align_up((size_t)N[w] * 4);
+        LK(ctx, launch_nvfp4_row_scale(src[w], (int)N[w], (int)K[w], sc, st));
+        LK(ctx, launch_nvfp4_quantize(src[w], plain_rows((int)N[w], K[w]), (int)N[w], (int)K[w], sc, codes, sf, st));
+        ctx->nv4_blocks[b].lin[sgm][w] = spot_ctx::Nv4Linear{codes, sf, sc};
       }
     }
   return SPOT_OK;

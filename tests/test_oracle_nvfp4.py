@@ -88,3 +88,21 @@ def test_block_nvfp4_is_close_and_mixed_with_fp8():
     assert len(qw["img.fc1"]) == 3 and len(qw["img.qkv"]) == 2             # MLP in NVFP4, attention Linears in FP8
     for a4, a8, r in zip(q4, q8, ref):
         assert rel_l2(a8, r) < rel_l2(a4, r) < 0.15                        # coarser than FP8, still a small perturbation
+
+
+def test_small_input_differences_are_amplified_by_a_4bit_quantiser():
+    """Why GPU-vs-oracle parity of the COMPOSED NVFP4 path cannot be at the bf16 path's 2e-2 (N6):
+    perturbing the input of one NVFP4 Linear by 2e-3 (a bf16 rounding) re-rounds every value near a code boundary and moves
+    the output by > 10 x as much; the exact Linear moves by the perturbation itself."""
+    rng = np.random.default_rng(0)
+    x = rng.normal(size=(128, 1024))
+    w = rng.normal(size=(256, 1024)) * 0.02
+    b = np.zeros(256)
+    q, sf, s = nvfp4.quantize_weight(w)
+    y, exact = nvfp4.linear_nvfp4(x, q, sf, s, b), x @ w.T
+    noise = rel_l2(y, exact)
+    for eps, lo in ((2e-3, 1.5e-2), (1e-2, 4e-2)):
+        xp = x * (1 + eps * rng.normal(size=x.shape))
+        moved = np.linalg.norm(nvfp4.linear_nvfp4(xp, q, sf, s, b) - y) / np.linalg.norm(exact)
+        assert abs(rel_l2(xp @ w.T, exact) - eps) < 0.2 * eps           # the exact Linear: as much as the input
+        assert lo < moved < noise                                        # the 4-bit Linear: an order of magnitude more
