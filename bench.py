@@ -41,8 +41,10 @@ from synth import CONFIGS, make_probe, make_text_emb, make_weights  # noqa: E402
 
 METRIC = "image-tokens*steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of gemm_tcgen05_v3_kernel, averaged over its four uses in a
-# block (QKV+RoPE 1.071 GB, out-proj 0.646 GB, fc1 1.451 GB, fc2 2.680 GB) - profiles/r1_ncu_full_gemm_v3.txt (config 3)
-GEMM_DRAM_TRAFFIC_PER_LAUNCH = {"cfg3": 1.462e9}
+# block, from one `ncu --set full` capture per workload (profiles/r2_ncu_full_gemm.txt, commands in profiles/r2_ncu.md):
+#   cfg3 (16 seqs): QKV+RoPE 0.939, out-proj 0.623, fc1 1.273, fc2 2.488 GB;  cfg4 (4 x 6656 tokens): 1.229, 0.823, 1.608, 3.570 GB;
+#   cfg5 (a chunk of 32 seqs): 2.036, 1.250, 2.837, 6.162 GB
+GEMM_DRAM_TRAFFIC_PER_LAUNCH = {"cfg3": 1.331e9, "cfg4": 1.807e9, "cfg5": 3.071e9}
 WORKLOADS = {"cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
 
 
@@ -282,6 +284,24 @@ def run_kernels(args, shape):
     res[name]["peak"] = 2.0 * peaks["bf16_tflops"]
     res[name]["frac"] = res[name]["achieved"] / res[name]["peak"]
     del a8, wq
+    # NVFP4 exploration variant: block-scaled 4-bit GEMMs of the MLP and the activation quantiser;
+    # peak = measured bf16 burst x 4 (nominal fp4 : bf16 ratio)
+    for name, (N, K, epi) in {"K2_nvfp4_gemm_fc1": (F, D, spot.EPI_BIAS_GELU), "K2_nvfp4_gemm_fc2": (D, F, spot.EPI_GATE_RESIDUAL)}.items():
+        if M % 128 or N % 256 or K % 256:
+            continue
+        act = rnd(10, (M, K), bf)
+        ac, asf = spot.spot_nvfp4_quantize(act)
+        wc, wsf, wsc = spot.spot_nvfp4_quantize_weight(rnd(11, (N, K), bf, 0.02))
+        b = rnd(12, (N,), bf, 0.02)
+        gate, resid = rnd(13, (N,), torch.float32, 0.1), torch.zeros((M, N), dtype=torch.float32, device="cuda")
+        tensor(name, lambda: spot.spot_linear_nvfp4(ac, asf, wc, wsf, wsc, b, epi, gate=gate, residual=resid), 2.0 * M * N * K)
+        res[name]["peak"] = 4.0 * peaks["bf16_tflops"]
+        res[name]["frac"] = res[name]["achieved"] / res[name]["peak"]
+        cb, sb = torch.empty_like(ac), torch.empty_like(asf)
+        lib = spot.load_library()
+        hbm("K12_nvfp4_quantize_K%d" % K, lambda: lib.spot_nvfp4_quantize(act.data_ptr(), M, K, None, cb.data_ptr(), sb.data_ptr(),
+                                                                         torch.cuda.current_stream().cuda_stream), M * K * (2.0 + 0.5 + 1.0 / 16))
+        del act, ac, asf, wc, wsf, resid, cb, sb
     # K5 sustained, measured last so that its heat does not colour the other rows: the same launch repeated back to back
     # for about 1.5 s (no flush: 377 MB of q, k, v per launch > L2), one event pair around all of them: the rate under
     # the power cap, against the SUSTAINED bf16 peak
@@ -522,6 +542,9 @@ def main():
                          "the ranks through sharding.explore_sharded (SURVEY.md 8(e))")
     ap.add_argument("--dry-run", action="store_true", help="host logic only: gloo, stub step, no GPU (tests)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--gap-probe", action="store_true",
+                    help="after the timed region: one more rollout with an event pair around EVERY kernel launch (SPOT_OPT_TIMING = 2); "
+                         "the line gains launch_gaps = share of a rollout's wall time in which no kernel of the library runs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--gemm-impl", type=int, default=0,
                     help="0 auto (CTA pair + TMA-store epilogue, K4 fused), 2 one-CTA tcgen05, 3 CTA pair with per-thread "
@@ -657,6 +680,8 @@ def main():
     S, D, F, L = shape.seq, shape.hidden, shape.mlp_hidden, shape.n_blocks
     lin_per_seq_block = 2 * D * (3 * D + D + 2 * F)                   # per token
     gemm_flops_step = eff_frac * T * my_seqs * (L * S * lin_per_seq_block - shape.n_txt * 2 * D * (D + 2 * F))   # last block: no text tail (this rank)
+    if nvfp4:      # the event-timed kernel (gemm_tcgen05_v3) runs only QKV and out-proj here; fc1 / fc2 are gemm_nvfp4_kernel launches
+        gemm_flops_step = eff_frac * T * my_seqs * (L * S * 2 * D * 4 * D - shape.n_txt * 2 * D * D)
     timed_frac = counters["gemm_timed"] / max(1, counters["gemm_launches"])
     gemm_ms = counters["gemm_ms"]
     gemm_tflops = (gemm_flops_step * args.steps * timed_frac) / (gemm_ms / 1e3) / 1e12 if gemm_ms > 0 else None
@@ -665,7 +690,7 @@ def main():
     roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_v3_kernel", "achieved": gemm_tflops,
                 "peak": gemm_peak, "peak_kind": peak_kind,
                 "unit": "TFLOP/s", "frac": (gemm_tflops / gemm_peak) if gemm_tflops else None,
-                "traffic": GEMM_DRAM_TRAFFIC_PER_LAUNCH.get(args.workload), "launches_timed": counters["gemm_timed"],
+                "traffic": None if fp8 else GEMM_DRAM_TRAFFIC_PER_LAUNCH.get(args.workload), "launches_timed": counters["gemm_timed"],
                 "avg_launch_ms": gemm_ms / max(1, counters["gemm_timed"]), "share_of_step": gemm_ms / ms_total / max(timed_frac, 1e-9),
                 "flops_per_launch": gemm_flops_step / max(1, counters["gemm_launches"] / args.steps)}
 
@@ -698,6 +723,19 @@ def main():
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
         assert torch.equal(h_out["rewards"], out["rewards"].cpu()), "host and device entry points disagree"
 
+    gaps = None
+    if args.gap_probe and not strong:
+        spot.spot_get_counters(ctx, reset=True)
+        spot.spot_set_option(ctx, spot.OPT_TIMING, 2)
+        sync_all()
+        step()
+        sync_all()
+        cg = spot.spot_get_counters(ctx, reset=True)
+        spot.spot_set_option(ctx, spot.OPT_TIMING, 0)
+        gaps = {"kernel_ms_sum": cg["gemm_ms"], "launches": cg["gemm_timed"], "rollout_ms": ms_step,
+                "idle_share": 1.0 - cg["gemm_ms"] / ms_step,
+                "how": "sum of CUDA-event durations around every kernel launch of one extra rollout, against ms_per_step of the timed region"}
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         nb = SAMPLE_BLOCKS
@@ -724,6 +762,8 @@ def main():
                                       "nominal_2250": tflops / 2250.0, "peaks": peaks["source"]},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": counters["launches"], "roofline": roofline,
                 "cpu_baseline": cpu_baseline, "weight_gen_s": gen_s}
+        if gaps:
+            line["launch_gaps"] = gaps
         if nccl_log:
             line["nccl_log"] = os.path.relpath(nccl_log, ROOT)
         rk = lambda v: torch.argsort(torch.argsort(v)).double()

@@ -98,7 +98,8 @@ typedef enum {
                              * 1 = SIMT FFMA GEMM, 2 = 1-CTA tcgen05, 3 = CTA-pair tcgen05 with per-thread epilogue,
                              * 4 = as 0 but K4 (QK-norm+RoPE) as its own kernel */
   SPOT_OPT_ATTN_IMPL = 1,   /* 0 = auto (tcgen05 for bf16, d_h = 128: one-pass kernel, 64-key tiles), 1 = SIMT attention, 2 = previous two-pass tcgen05 kernel */
-  SPOT_OPT_TIMING = 2,      /* 1 = bracket every tcgen05 GEMM launch with CUDA events on the launch stream */
+  SPOT_OPT_TIMING = 2,      /* 1 = bracket every tcgen05 GEMM launch with CUDA events on the launch stream; 2 = bracket EVERY kernel
+                             * launch (gap probe: spot_get_counters then returns the summed device time of all kernels) */
   SPOT_OPT_FP8 = 3,         /* 1 = the four Linears of every block run on E4M3 operands (after spot_fp8_prepare) */
   SPOT_OPT_NVFP4 = 5,       /* 1 = on top of SPOT_OPT_FP8, fc1 / fc2 of every block run on NVFP4 operands (after spot_nvfp4_prepare) */
   SPOT_OPT_CHUNK_SEQS = 4   /* sequences per pass of the block stack in spot_dit_denoise / spot_explore / spot_explore_host: larger
@@ -264,7 +265,7 @@ spot_status spot_fp8_prepare(spot_ctx *ctx, void *d_buffer, size_t bytes, void *
  *   weights      the same on W_n / s_n with s_n = max_k |W_nk| / (6 * 448) fp32 per output channel (spot_nvfp4_prepare),
  *   y_n = s_n * sum_b sfx_b sfw_nb sum_{k in b} qx_k qw_nk + b_n on tcgen05.mma kind::mxf4nvf4.block_scale, fp32 accumulation;
  * QKV and out-proj stay on the FP8 path, everything else is unchanged.  spot_nvfp4_bytes / spot_nvfp4_prepare work like
- * their FP8 counterparts; spot_set_option(ctx, SPOT_OPT_NVFP4, 1) needs SPOT_OPT_FP8 = 1 and the prepared buffer
+ * their FP8 counterparts; spot_set_option(ctx, SPOT_OPT_NVFP4, 1) needs SPOT_OPT_FP8 switched on and the prepared buffer
  * (SPOT_ERR_SHAPE otherwise) and enlarges the workspace (query spot_workspace_bytes again).  hidden and mlp_hidden must
  * be multiples of 256 and every call's image / text row counts (n_seqs * n_img, n_seqs * n_txt) multiples of 128
  * (SPOT_ERR_SHAPE otherwise).  Switching SPOT_OPT_FP8 off switches this off too. */

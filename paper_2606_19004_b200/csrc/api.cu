@@ -150,11 +150,26 @@ Workspace carve(const spot_ctx* c, int B, int T, bool cached = false) {
     }                                                  \
   } while (0)
 
-// LK = CK for a kernel launcher: also counts the launch (reported by spot_get_counters).
-#define LK(ctx, expr)       \
-  do {                      \
-    ++(ctx)->n_launches;    \
-    CK(ctx, expr);          \
+// SPOT_OPT_TIMING = 2: an event pair around EVERY kernel launch (gap probe: wall time of a rollout minus the summed
+// kernel time = what launch gaps cost).  Returns false when the event pool is exhausted or an event call failed.
+bool launch_event(spot_ctx* c, cudaStream_t st) {
+  if (c->ev_used + 1 > kMaxTimingEvents) return false;
+  while (c->ev.size() < c->ev_used + 1) {
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return false;
+    c->ev.push_back(e);
+  }
+  return cudaEventRecord(c->ev[c->ev_used++], st) == cudaSuccess;
+}
+
+// LK = CK for a kernel launcher: also counts the launch (reported by spot_get_counters).  Used where the launch stream
+// is in scope as `st`.
+#define LK(ctx, expr)                                                        \
+  do {                                                                       \
+    ++(ctx)->n_launches;                                                     \
+    const bool _probe = (ctx)->timing == 2 && launch_event((ctx), st);       \
+    CK(ctx, expr);                                                           \
+    if (_probe && !launch_event((ctx), st)) return SPOT_ERR_CUDA;            \
   } while (0)
 
 // Linear layer dispatch: tcgen05 when the context runs bf16 and every problem qualifies, else SIMT.
@@ -165,7 +180,7 @@ spot_status run_gemm(spot_ctx* c, Epilogue epi, GemmProblem* probs, int n, spot_
   for (int i = 0; i < n && tc; ++i)
     if (probs[i].M > 0 && !tcgen05_gemm_supported(probs[i])) tc = false;
   if (tc) {
-    const bool timed = c->timing && c->ev_used + 2 <= kMaxTimingEvents;
+    const bool timed = c->timing == 1 && c->ev_used + 2 <= kMaxTimingEvents;
     if (timed) {
       while (c->ev.size() < c->ev_used + 2) {
         cudaEvent_t e;
@@ -349,6 +364,11 @@ spot_status spot_set_option(spot_ctx* ctx, spot_option opt, int value) {
   if (opt == SPOT_OPT_CHUNK_SEQS) {
     if (value < 0) return SPOT_ERR_SHAPE;
     ctx->chunk_seqs = value;
+    return SPOT_OK;
+  }
+  if (opt == SPOT_OPT_TIMING) {
+    if (value < 0 || value > 2) return SPOT_ERR_SHAPE;
+    ctx->timing = value;
     return SPOT_OK;
   }
   if (value != 0 && value != 1) return SPOT_ERR_SHAPE;
