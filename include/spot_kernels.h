@@ -111,15 +111,19 @@ spot_status spot_qkv_rope_linear_fp8(const void *d_a, int n_seqs, int rows_per_s
  *   block scale sf = e4m3(max|x| / 6), codes e2m1(x / sf), all in fp32 with IEEE division.  rows % 128 == 0, K % 64 == 0.
  * spot_linear_nvfp4: y[m, n] = d_w_scale[n] * sum_blocks sfa sfw sum_k a w + bias[n] on the block-scaled tensor-core path
  *   (kind::mxf4nvf4), fp32 accumulation; SPOT_EPI_BIAS / SPOT_EPI_BIAS_GELU write d_out [M, N] bf16,
- *   SPOT_EPI_GATE_RESIDUAL updates the fp32 residual [M, N].  M % 128 == 0, N % 256 == 0, K % 256 == 0, else
- *   SPOT_ERR_SHAPE. */
+ *   SPOT_EPI_GATE_RESIDUAL updates the fp32 residual [M, N].  With SPOT_EPI_BIAS_GELU and d_out_sf != NULL the epilogue
+ *   quantises instead (what the rollout's fc1 does): d_out receives the E2M1 codes of GELU(y) [M, N / 2] and d_out_sf their
+ *   E4M3 block scales (atoms for a [M, N] matrix), reading N3 applied to the fp32 value - the bf16 tensor is never written.
+ *   M % 128 == 0, K % 256 == 0, N % 192 == 0 (tiles 128 x 192, two accumulators: epilogue overlapped) or N % 256 == 0
+ *   (tiles 128 x 256), else SPOT_ERR_SHAPE. */
 spot_status spot_nvfp4_sizes(int64_t rows, int64_t K, size_t *codes_bytes, size_t *sf_bytes);
 spot_status spot_nvfp4_row_scale(const void *d_w_bf16, int64_t rows, int64_t K, float *d_scale, void *cuda_stream);
 spot_status spot_nvfp4_quantize(const void *d_src_bf16, int64_t rows, int64_t K, const float *d_row_scale, void *d_codes,
                                 void *d_sf, void *cuda_stream);
 spot_status spot_linear_nvfp4(spot_epilogue epi, const void *d_a_codes, const void *d_a_sf, int64_t M, int64_t K,
                               const void *d_w_codes, const void *d_w_sf, const float *d_w_scale, int64_t N,
-                              const void *d_bias, const float *d_gate, float *d_residual, void *d_out, void *cuda_stream);
+                              const void *d_bias, const float *d_gate, float *d_residual, void *d_out, void *d_out_sf,
+                              void *cuda_stream);
 
 /* The RoPE table the context built at spot_create (S5): copies cos and sin [S, d_h/2] fp32 to HOST. */
 spot_status spot_rope_table(const spot_ctx *ctx, float *h_cos, float *h_sin);

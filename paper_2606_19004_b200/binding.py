@@ -104,7 +104,7 @@ def load_library() -> C.CDLL:
         "spot_nvfp4_sizes": [i64, i64, C.POINTER(sz), C.POINTER(sz)],
         "spot_nvfp4_row_scale": [vp, i64, i64, vp, vp],
         "spot_nvfp4_quantize": [vp, i64, i64, vp, vp, vp, vp],
-        "spot_linear_nvfp4": [i32, vp, vp, i64, i64, vp, vp, vp, i64, vp, vp, vp, vp, vp],
+        "spot_linear_nvfp4": [i32, vp, vp, i64, i64, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp],
         "spot_explore_host": [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp],
         "spot_linear": [i32, i32, i32, vp, i64, i64, vp, i64, vp, vp, vp, vp, vp],
         "spot_qkv_rope_linear": [vp, i32, i32, i64, vp, i64, vp, vp, vp, vp, vp, i32, f32, vp, vp],
@@ -522,14 +522,25 @@ def nvfp4_sf_index(rows: int, K: int) -> torch.Tensor:
 
 def spot_linear_nvfp4(a_codes: torch.Tensor, a_sf: torch.Tensor, w_codes: torch.Tensor, w_sf: torch.Tensor, w_scale: torch.Tensor,
                       bias: torch.Tensor, epi: int = EPI_BIAS, gate: Optional[torch.Tensor] = None,
-                      residual: Optional[torch.Tensor] = None) -> torch.Tensor:
+                      residual: Optional[torch.Tensor] = None, quantize_out: bool = False):
     """Block-scaled 4-bit Linear on quantised operands; EPI_BIAS / EPI_BIAS_GELU return bf16 [M, N], EPI_GATE_RESIDUAL updates
-    `residual` (fp32)."""
+    `residual` (fp32).  quantize_out (EPI_BIAS_GELU only): the epilogue quantises GELU(y) to NVFP4 and the call returns
+    (codes uint8 [M, N / 2], scale-factor atoms) instead - what the rollout's fc1 does."""
     M, K = a_codes.shape[0], a_codes.shape[1] * 2
     N = w_codes.shape[0]
-    out = None if epi == EPI_GATE_RESIDUAL else torch.empty((M, N), dtype=torch.bfloat16, device=a_codes.device)
+    dev = a_codes.device
+    sf_out = None
+    if quantize_out:
+        cb, sb = C.c_size_t(), C.c_size_t()
+        _check(load_library().spot_nvfp4_sizes(M, N, C.byref(cb), C.byref(sb)), "spot_nvfp4_sizes")
+        out = torch.empty((M, N // 2), dtype=torch.uint8, device=dev)
+        sf_out = torch.zeros(int(sb.value), dtype=torch.uint8, device=dev)
+    else:
+        out = None if epi == EPI_GATE_RESIDUAL else torch.empty((M, N), dtype=torch.bfloat16, device=dev)
     _check(load_library().spot_linear_nvfp4(epi, _ptr(a_codes), _ptr(a_sf), M, K, _ptr(w_codes), _ptr(w_sf), _ptr(w_scale), N,
-                                            _ptr(bias), _ptr(gate), _ptr(residual), _ptr(out), _stream()), "spot_linear_nvfp4")
+                                            _ptr(bias), _ptr(gate), _ptr(residual), _ptr(out), _ptr(sf_out), _stream()), "spot_linear_nvfp4")
+    if quantize_out:
+        return out, sf_out
     return residual if epi == EPI_GATE_RESIDUAL else out
 
 

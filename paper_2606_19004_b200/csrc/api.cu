@@ -72,7 +72,7 @@ struct Workspace {
   size_t t_dev, emb, hid, temb, cvec, mod, fmod, txt_norm, txt_h0, h_img, h_txt, ybuf, big, vel, stage, total;
   size_t st_seeds, st_text, st_probe, st_lat, st_rew, st_stats, st_top, st_bot;
   // cached-step variant only (carve(..., cached = true)): uncompacted h_img^0, previous modulated input, cached residual
-  size_t nv_codes[2], nv_sf[2];            // NVFP4 variant only: quantised MLP activations of the image / text stream
+  size_t nv_codes[2], nv_sf[2], nv_codes2[2], nv_sf2[2];   // NVFP4 variant only: quantised y2 and u of the image / text stream
   size_t md_a, md_acc, md_ones, md_zero;   // tensor-core modulation path (conditioning): split c, accumulators, gate = 1, bias = 0
   size_t tc_h0, tc_mprev, tc_resid, tc_rowpart, tc_acc, tc_coeffs, tc_idx, tc_pos, tc_nact, tc_comp, tc_rel;
 };
@@ -113,13 +113,14 @@ Workspace carve(const spot_ctx* c, int B, int T, bool cached = false) {
   w.st_stats = take((size_t)B * 2 * 4);
   w.st_top = take((size_t)B * 4);
   w.st_bot = take((size_t)B * 4);
-  w.nv_codes[0] = w.nv_codes[1] = w.nv_sf[0] = w.nv_sf[1] = 0;
+  w.nv_codes[0] = w.nv_codes[1] = w.nv_sf[0] = w.nv_sf[1] = w.nv_codes2[0] = w.nv_codes2[1] = w.nv_sf2[0] = w.nv_sf2[1] = 0;
   if (c->nvfp4) {
-    const size_t Kmax = (size_t)(D > (size_t)g.mlp_hidden ? D : g.mlp_hidden);
     const size_t rows[2] = {(size_t)B * NI, (size_t)B * NT};
     for (int s = 0; s < 2; ++s) {
-      w.nv_codes[s] = take(nvfp4_codes_bytes((long long)rows[s], (long long)Kmax));
-      w.nv_sf[s] = take(nvfp4_sf_bytes((long long)rows[s], (long long)Kmax));
+      w.nv_codes[s] = take(nvfp4_codes_bytes((long long)rows[s], (long long)D));
+      w.nv_sf[s] = take(nvfp4_sf_bytes((long long)rows[s], (long long)D));
+      w.nv_codes2[s] = take(nvfp4_codes_bytes((long long)rows[s], (long long)g.mlp_hidden));
+      w.nv_sf2[s] = take(nvfp4_sf_bytes((long long)rows[s], (long long)g.mlp_hidden));
     }
   }
   w.tc_h0 = w.tc_mprev = w.tc_resid = w.tc_rowpart = w.tc_acc = w.tc_coeffs = w.tc_idx = w.tc_pos = w.tc_nact = w.tc_comp =
@@ -454,7 +455,8 @@ StreamMaps stream_maps(const spot_ctx* c, int B, int stream /*0 img, 1 txt*/) {
 // 2-8).  mod_img / mod_txt: [6D] fp32 = (shift1, scale1, gate1, shift2, scale2, gate2).  When
 // img_only_tail is set (last block of a denoise pass, S16) the text stream's out-proj and MLP,
 // whose result nobody reads, are skipped.
-struct Nv4Scratch { uint8_t* codes[2]; uint8_t* sf[2]; };   // quantised MLP activations per stream (NVFP4 variant)
+// quantised MLP activations per stream (NVFP4 variant): y2 (fc1's operand) and u (fc2's operand, written by fc1's epilogue)
+struct Nv4Scratch { uint8_t* codes[2]; uint8_t* sf[2]; uint8_t* codes2[2]; uint8_t* sf2[2]; };
 
 spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt, const float* mod_img,
                        const float* mod_txt, void* ybuf, void* big, bool img_only_tail, cudaStream_t st,
@@ -527,17 +529,18 @@ spot_status block_core(spot_ctx* c, int block, int B, float* h_img, float* h_txt
     if (!nv) return SPOT_ERR_WORKSPACE;
     const spot_ctx::Nv4Block& nb = c->nv4_blocks[block];
     Nvfp4Problem np[2];
-    bf16* u[2] = {(bf16*)big, (bf16*)big + (long long)sm[0].rows * F};
     for (int s = 0; s < ns; ++s) {
       memset(&np[s], 0, sizeof(Nvfp4Problem));
       np[s].a_codes = nv->codes[s]; np[s].a_sf = nv->sf[s]; np[s].w_codes = nb.lin[s][0].codes; np[s].w_sf = nb.lin[s][0].sf;
-      np[s].w_scale = nb.lin[s][0].scale; np[s].bias = bw.s[s].fc1_b; np[s].M = sm[s].rows; np[s].N = F; np[s].K = D; np[s].out = u[s];
+      np[s].w_scale = nb.lin[s][0].scale; np[s].bias = bw.s[s].fc1_b; np[s].M = sm[s].rows; np[s].N = F; np[s].K = D; np[s].out = nv->codes2[s];
       if (np[s].M > 0 && !nvfp4_gemm_supported(np[s])) return SPOT_ERR_SHAPE;   // rows in multiples of 128, widths of 256
       LK(c, launch_nvfp4_quantize(ybuf, sm[s].y, sm[s].rows, D, nullptr, nv->codes[s], nv->sf[s], st));
     }
+    // fc1's epilogue quantises u itself (codes + scales straight into fc2's operand buffers `u2`): u is never stored
+    for (int s = 0; s < ns; ++s) { np[s].out = nv->codes2[s]; np[s].out_sf = nv->sf2[s]; }
     LK(c, launch_gemm_nvfp4(EPI_BIAS_GELU, np, ns, c->num_sms, st));
     for (int s = 0; s < ns; ++s) {
-      LK(c, launch_nvfp4_quantize(u[s], plain_rows(sm[s].rows, F), sm[s].rows, F, nullptr, nv->codes[s], nv->sf[s], st));
+      np[s].a_codes = nv->codes2[s]; np[s].a_sf = nv->sf2[s]; np[s].out_sf = nullptr;
       np[s].w_codes = nb.lin[s][1].codes; np[s].w_sf = nb.lin[s][1].sf; np[s].w_scale = nb.lin[s][1].scale; np[s].bias = bw.s[s].fc2_b;
       np[s].N = D; np[s].K = F; np[s].out = nullptr; np[s].gate = mod[s] + 5 * D; np[s].resid = h[s];
     }
@@ -651,7 +654,8 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
   if (rs != SPOT_OK) return rs;
   float* txt_h0 = (float*)(ws + w.txt_h0); float* h_img = (float*)(ws + w.h_img); float* h_txt = (float*)(ws + w.h_txt);
   void* ybuf = ws + w.ybuf; void* big = ws + w.big; float* vel = (float*)(ws + w.vel);
-  Nv4Scratch nvs{{ws + w.nv_codes[0], ws + w.nv_codes[1]}, {ws + w.nv_sf[0], ws + w.nv_sf[1]}};
+  Nv4Scratch nvs{{ws + w.nv_codes[0], ws + w.nv_codes[1]}, {ws + w.nv_sf[0], ws + w.nv_sf[1]},
+                 {ws + w.nv_codes2[0], ws + w.nv_codes2[1]}, {ws + w.nv_sf2[0], ws + w.nv_sf2[1]}};
   const float* mod = (const float*)(ws + w.mod); const float* fmod = (const float*)(ws + w.fmod);
   GemmProblem pr;
   // h_txt^0 = RMSNorm(text_emb) Wtxt^T + b, once per prompt (C7)
@@ -739,7 +743,8 @@ spot_status denoise_cached_core(spot_ctx* c, int P, int K, float* lat, const voi
   int* d_idx = (int*)(ws + w.tc_idx); int* d_pos = (int*)(ws + w.tc_pos); int* d_nact = (int*)(ws + w.tc_nact);
   int* d_comp = (int*)(ws + w.tc_comp); float* d_rel = (float*)(ws + w.tc_rel);
   void* ybuf = ws + w.ybuf; void* big = ws + w.big; float* vel = (float*)(ws + w.vel);
-  Nv4Scratch nvs{{ws + w.nv_codes[0], ws + w.nv_codes[1]}, {ws + w.nv_sf[0], ws + w.nv_sf[1]}};
+  Nv4Scratch nvs{{ws + w.nv_codes[0], ws + w.nv_codes[1]}, {ws + w.nv_sf[0], ws + w.nv_sf[1]},
+                 {ws + w.nv_codes2[0], ws + w.nv_codes2[1]}, {ws + w.nv_sf2[0], ws + w.nv_sf2[1]}};
   const float* mod = (const float*)(ws + w.mod); const float* fmod = (const float*)(ws + w.fmod);
   std::vector<int> h_idx((size_t)B + 1), h_comp((size_t)B);
   std::vector<float> h_relv((size_t)B);
@@ -858,7 +863,8 @@ spot_status spot_dit_block_forward(spot_ctx* ctx, int block, int n_seqs, const v
                         mod + (long long)sgm * 6 * D, 0, false, st));
   LK(ctx, launch_to_f32(g.dtype, d_h_img, h_img, n_img, st));
   LK(ctx, launch_to_f32(g.dtype, d_h_txt, h_txt, n_txt, st));
-  Nv4Scratch nvs{{ws + w.nv_codes[0], ws + w.nv_codes[1]}, {ws + w.nv_sf[0], ws + w.nv_sf[1]}};
+  Nv4Scratch nvs{{ws + w.nv_codes[0], ws + w.nv_codes[1]}, {ws + w.nv_sf[0], ws + w.nv_sf[1]},
+                 {ws + w.nv_codes2[0], ws + w.nv_codes2[1]}, {ws + w.nv_sf2[0], ws + w.nv_sf2[1]}};
   s = block_core(ctx, block, n_seqs, h_img, h_txt, mod, mod + 6 * D, ws + w.ybuf, ws + w.big, false, st,
                  ctx->nvfp4 ? &nvs : nullptr);
   if (s != SPOT_OK) return s;
@@ -1406,7 +1412,8 @@ spot_status spot_nvfp4_quantize(const void* d_src_bf16, int64_t rows, int64_t K,
 
 spot_status spot_linear_nvfp4(spot_epilogue epi, const void* d_a_codes, const void* d_a_sf, int64_t M, int64_t K,
                               const void* d_w_codes, const void* d_w_sf, const float* d_w_scale, int64_t N,
-                              const void* d_bias, const float* d_gate, float* d_residual, void* d_out, void* cuda_stream) {
+                              const void* d_bias, const float* d_gate, float* d_residual, void* d_out, void* d_out_sf,
+                              void* cuda_stream) {
   if (M < 0 || N <= 0 || K <= 0 || M > 0x7fffffff || N > 0x7fffffff || K > 0x7fffffff) return SPOT_ERR_SHAPE;
   if (M == 0) return SPOT_OK;
   if (!d_a_codes || !d_a_sf || !d_w_codes || !d_w_sf || !d_w_scale || !d_bias) return SPOT_ERR_NULL;
@@ -1421,6 +1428,11 @@ spot_status spot_linear_nvfp4(spot_epilogue epi, const void* d_a_codes, const vo
   p.a_codes = d_a_codes; p.a_sf = d_a_sf; p.w_codes = d_w_codes; p.w_sf = d_w_sf; p.w_scale = d_w_scale; p.bias = d_bias;
   p.M = (int)M; p.N = (int)N; p.K = (int)K;
   if (gate_res) { p.gate = d_gate; p.resid = d_residual; } else p.out = d_out;
+  if (d_out_sf) {
+    if (epi != SPOT_EPI_BIAS_GELU || N % 64) return SPOT_ERR_SHAPE;
+    if (!aligned16(d_out_sf)) return SPOT_ERR_ALIGN;
+    p.out_sf = d_out_sf;
+  }
   if (!nvfp4_gemm_supported(p)) return SPOT_ERR_SHAPE;
   const Epilogue e = epi == SPOT_EPI_BIAS ? EPI_BIAS : (epi == SPOT_EPI_BIAS_GELU ? EPI_BIAS_GELU : EPI_GATE_RES);
   return launch_gemm_nvfp4(e, &p, 1, sm_count(), (cudaStream_t)cuda_stream) == cudaSuccess ? SPOT_OK : SPOT_ERR_CUDA;

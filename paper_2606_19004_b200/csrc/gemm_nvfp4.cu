@@ -5,16 +5,21 @@
 // nvfp4.cu writes, s_n: fp32 per output channel.
 //
 //   warp 0      producer: per 256-element K block one TMA load of the A tile [128 rows x 128 bytes] and of the W tile
-//               [256 x 128 bytes] (128-byte swizzle) plus three plain bulk copies of their scale-factor atoms (4 atoms of
-//               512 bytes for A, 2 x 4 for W) into a 3-stage ring
+//               [BN x 128 bytes] (128-byte swizzle) plus three plain bulk copies of their scale-factor atoms (4 atoms of
+//               512 bytes for A, 2 x 4 for W) into a 4-stage (BN = 192) or 3-stage (BN = 256) ring
 //   warp 1      issuer (elect.sync): per K block 12 x tcgen05.cp 32x128b.warpx4 (scale factors shared -> tensor memory;
 //               executes in issue order with the MMAs, so no barrier in between) and 4 x tcgen05.mma
-//               kind::mxf4nvf4.block_scale.block16, M128 N256 K64, accumulating into 256 tensor-memory columns
+//               kind::mxf4nvf4.block_scale.block16, M128 N = BN K64, accumulating into BN tensor-memory columns
 //   warp 2      tensor-memory allocator;  warps 4-7 epilogue: tcgen05.ld, * s_n + bias, then
 //                 EPI_BIAS_GELU -> tanh-GELU -> bf16 rows (fc1)      EPI_GATE_RES -> h += gate * y on the fp32 residual (fc2)
-// One CTA per SM, tiles 128 x 256 round-robin; ONE accumulator (the scale factors take the tensor-memory columns a
-// second one would need), so the epilogue of a tile is not overlapped with the next tile's MMAs.  This is the first,
-// correctness-first version of the path: its parity with oracle/nvfp4.py is the contract, its speed is reported as is.
+// One CTA per SM, tiles round-robin.  Tile width BN = 192 when N is a multiple of 192 (the rollout's 3072 and 12288 are):
+// TWO 192-column accumulators (384 tensor-memory columns) + two 48-column scale-factor slots = 480 of 512, so the epilogue
+// of a tile overlaps the next tile's MMAs; a 192-row W tile starts 0 or 64 rows into a 128-row scale atom, so both atoms it
+// touches are copied and the MMA's scale address is offset by 0 or 2 columns.  Otherwise BN = 256 with ONE accumulator.
+// EPI_GELU_NVFP4 (fc1 in the rollout) does not write u at all: the epilogue thread owns a row and 32 consecutive columns =
+// two whole 16-element blocks, so it forms the block scales and E2M1 codes of u in registers and stores 16 bytes of codes
+// and 2 scale bytes - fc2's operand in the layout nvfp4.cu documents (reading N3 applied to the fp32 GELU value).
+#include <cuda_fp8.h>
 #include <string.h>
 
 #include "kernels.h"
@@ -22,15 +27,23 @@
 
 namespace {
 
-constexpr int BLOCK_M = 128, BLOCK_N = 256, BLOCK_K = 256 /* E2M1 elements = 128 bytes */, UMMA_K = 64, STAGES = 3;
-constexpr uint32_t A_BYTES = BLOCK_M * 128, B_BYTES = BLOCK_N * 128, SFA_BYTES = 4 * 512, SFB_BYTES = 2 * 4 * 512;
-constexpr uint32_t OFF_SFA = A_BYTES + B_BYTES, OFF_SFB = OFF_SFA + SFA_BYTES;
-constexpr uint32_t STAGE_BYTES = 56 * 1024;                          // 54 KB used, padded to keep 1024-byte alignment
-constexpr uint32_t TX_BYTES = A_BYTES + B_BYTES + SFA_BYTES + SFB_BYTES;
-constexpr uint32_t OFF_BAR = STAGES * STAGE_BYTES;
-constexpr uint32_t SMEM_BYTES = OFF_BAR + 256 + 1024;
+constexpr int BLOCK_M = 128, BLOCK_K = 256 /* E2M1 elements = 128 bytes */, UMMA_K = 64;
+constexpr uint32_t A_BYTES = BLOCK_M * 128, SFA_BYTES = 4 * 512, SFB_BYTES = 2 * 4 * 512;
 constexpr int NUM_THREADS = 256;
-constexpr uint32_t TM_SF = 256, SF_COLS_PER_STAGE = 4 * (4 + 8);     // tensor-memory columns: [0,256) accumulator, then scale factors
+constexpr uint32_t SF_COLS_PER_SLOT = 4 * (4 + 8);                    // scale factors of one K block: 4 K = 64 steps x (A 4 + W 8 columns)
+constexpr int EPI_GELU_NVFP4 = 16;                                    // internal epilogue id: bias -> tanh-GELU -> NVFP4 codes + scales
+
+template <int BN>
+struct Cfg {
+  static constexpr int NACC = BN == 192 ? 2 : 1;                      // accumulators in tensor memory
+  static constexpr int STAGES = BN == 192 ? 4 : 3;
+  static constexpr uint32_t B_BYTES = BN * 128, OFF_SFA = A_BYTES + B_BYTES, OFF_SFB = OFF_SFA + SFA_BYTES;
+  static constexpr uint32_t STAGE_BYTES = (OFF_SFB + SFB_BYTES + 1023) / 1024 * 1024;
+  static constexpr uint32_t TX_BYTES = A_BYTES + B_BYTES + SFA_BYTES + SFB_BYTES;
+  static constexpr uint32_t OFF_BAR = STAGES * STAGE_BYTES, SMEM_BYTES = OFF_BAR + 256 + 1024;
+  static constexpr uint32_t TM_SF = NACC * BN;                        // first scale-factor column
+  static constexpr int SF_SLOTS = BN == 192 ? 2 : 3;
+};
 
 struct NvProblem {
   int m_tiles, n_tiles, k_blocks, tile_start, M, N;
@@ -38,7 +51,8 @@ struct NvProblem {
   const uint8_t* sfw;       // atoms [N / 128][K / 64][512]
   const float* w_scale;     // [N]
   const bf16* bias;         // [N]
-  bf16* out;                // EPI_BIAS_GELU: [M, N] bf16
+  bf16* out;                // EPI_BIAS / EPI_BIAS_GELU: [M, N] bf16;  EPI_GELU_NVFP4: codes [M, N / 2]
+  uint8_t* out_sf;          // EPI_GELU_NVFP4: scale-factor atoms [M / 128][N / 64][512]
   const float* gate;        // EPI_GATE_RES
   float* resid;             // EPI_GATE_RES: [M, N] fp32, updated in place
 };
@@ -56,17 +70,40 @@ __device__ __forceinline__ float gelu_tanh_fast(float x) {
   return fmaf(hx, th, hx);
 }
 
-template <int EPI>
+// nearest E4M3 value (RNE, saturating) of v as fp32, and its byte
+__device__ __forceinline__ float e4m3_round(float v, uint32_t* code) {
+  const __nv_fp8_storage_t c = __nv_cvt_float_to_fp8(v, __NV_SATFINITE, __NV_E4M3);
+  *code = (uint32_t)c;
+  return __half2float(__half(__nv_cvt_fp8_to_halfraw(c, __NV_E4M3)));
+}
+// eight fp32 -> eight E2M1 codes in one 32-bit word, element i in nibble i (RNE, ties to the even code, saturating)
+__device__ __forceinline__ uint32_t e2m1x8(const float* v) {
+  uint32_t r;
+  asm("{\n\t.reg .b8 b0, b1, b2, b3;\n\t"
+      "cvt.rn.satfinite.e2m1x2.f32 b0, %2, %1;\n\t"
+      "cvt.rn.satfinite.e2m1x2.f32 b1, %4, %3;\n\t"
+      "cvt.rn.satfinite.e2m1x2.f32 b2, %6, %5;\n\t"
+      "cvt.rn.satfinite.e2m1x2.f32 b3, %8, %7;\n\t"
+      "mov.b32 %0, {b0, b1, b2, b3};\n\t}\n"
+      : "=r"(r)
+      : "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]));
+  return r;
+}
+
+template <int EPI, int BN>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmW0,
                   const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmW1, const NvParams P) {
+  using C = Cfg<BN>;
+  constexpr int STAGES = C::STAGES, NACC = C::NACC;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bar_base = smem_base + OFF_BAR;
+  const uint32_t bar_base = smem_base + C::OFF_BAR;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
-  const uint32_t tfull_bar = bar_base + 8u * (2 * STAGES), tempty_bar = bar_base + 8u * (2 * STAGES + 1);
-  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 2);
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + 2 + a); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
   volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -76,8 +113,7 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
-    ptx::mbar_init(tfull_bar, 1);
-    ptx::mbar_init(tempty_bar, 4);
+    for (int a = 0; a < 2; ++a) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 4); }
     ptx::fence_barrier_init();
   }
   if (warp == 2) { ptx::tmem_alloc(tmem_slot, 512); ptx::tmem_relinquish(); }
@@ -108,15 +144,17 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
         const CUtensorMap* mA = prob ? &tmA1 : &tmA0;
         const CUtensorMap* mW = prob ? &tmW1 : &tmW0;
         const long long ka = (long long)q.k_blocks * 4;           // K / 64 atoms per 128 rows
+        const int n0 = nt * BN, atom0 = n0 >> 7;                  // first W row of the tile and the scale atom it falls into
+        const int atom1 = min(atom0 + 1, ((q.N + 127) >> 7) - 1); // (the last tile's second atom may not exist: its columns are not read)
         for (int kb = 0; kb < q.k_blocks; ++kb) {
           ptx::mbar_wait(empty_bar(stage), phase ^ 1);
-          ptx::mbar_arrive_expect_tx(full_bar(stage), TX_BYTES);
-          const uint32_t sa = smem_base + stage * STAGE_BYTES;
+          ptx::mbar_arrive_expect_tx(full_bar(stage), C::TX_BYTES);
+          const uint32_t sa = smem_base + stage * C::STAGE_BYTES;
           ptx::tma_load_2d(sa, mA, full_bar(stage), kb * 128, mt * BLOCK_M);
-          ptx::tma_load_2d(sa + A_BYTES, mW, full_bar(stage), kb * 128, nt * BLOCK_N);
-          ptx::bulk_load_1d(sa + OFF_SFA, q.sfa + ((long long)mt * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
-          ptx::bulk_load_1d(sa + OFF_SFB, q.sfw + ((long long)(2 * nt) * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
-          ptx::bulk_load_1d(sa + OFF_SFB + SFA_BYTES, q.sfw + ((long long)(2 * nt + 1) * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
+          ptx::tma_load_2d(sa + A_BYTES, mW, full_bar(stage), kb * 128, n0);
+          ptx::bulk_load_1d(sa + C::OFF_SFA, q.sfa + ((long long)mt * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
+          ptx::bulk_load_1d(sa + C::OFF_SFB, q.sfw + ((long long)atom0 * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
+          ptx::bulk_load_1d(sa + C::OFF_SFB + SFA_BYTES, q.sfw + ((long long)atom1 * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -124,51 +162,58 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
   } else if (warp == 1) {
     // ===================== scale-factor copies + MMA issue =====================
     if (ptx::elect_one()) {
-      constexpr uint32_t idesc = ptx::make_idesc_nvfp4(BLOCK_M, BLOCK_N);
-      int stage = 0; uint32_t phase = 0, acc_phase = 0;
+      constexpr uint32_t idesc = ptx::make_idesc_nvfp4(BLOCK_M, BN);
+      int stage = 0, slot = 0, acc = 0;
+      uint32_t phase = 0, acc_phase = 0;
       for (int t = blockIdx.x; t < P.total_tiles; t += gridDim.x) {
         int prob, mt, nt;
         tile_of(t, prob, mt, nt);
         const int k_blocks = P.p[prob].k_blocks;
-        ptx::mbar_wait(tempty_bar, acc_phase ^ 1);                  // the epilogue has drained the accumulator
+        const uint32_t sfb_off = (uint32_t)(((nt * BN) & 127) >> 5);   // the tile's first W row inside its scale atom, in columns
+        ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1);             // the epilogue has drained this accumulator
         ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + acc * BN;
         for (int kb = 0; kb < k_blocks; ++kb) {
           ptx::mbar_wait(full_bar(stage), phase);
           ptx::tc_fence_after();
-          const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
-          const uint32_t tsf = tmem_base + TM_SF + stage * SF_COLS_PER_STAGE;
+          const uint32_t sa = smem_base + stage * C::STAGE_BYTES, sb = sa + A_BYTES;
+          // scale-factor slot in tensor memory: re-used every SF_SLOTS K blocks; the copy into it is ordered behind the
+          // MMAs that read its previous contents (tcgen05.cp and tcgen05.mma execute in issue order)
+          const uint32_t tsf = tmem_base + C::TM_SF + slot * SF_COLS_PER_SLOT;
 #pragma unroll
           for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
-            // scale factors of this K = 64 step: A rows 0-127 -> 4 columns, W rows 0-127 / 128-255 -> 4 + 4 columns
+            // scale factors of this K = 64 step: A rows 0-127 -> 4 columns, the two W atoms -> 4 + 4 columns
             const uint32_t sfa_t = tsf + k * 12, sfb_t = sfa_t + 4;
-            ptx::tmem_cp_32x128b_warpx4(sfa_t, ptx::make_smem_desc_noswizzle(sa + OFF_SFA + k * 512, 128, 128));
-            ptx::tmem_cp_32x128b_warpx4(sfb_t, ptx::make_smem_desc_noswizzle(sa + OFF_SFB + k * 512, 128, 128));
-            ptx::tmem_cp_32x128b_warpx4(sfb_t + 4, ptx::make_smem_desc_noswizzle(sa + OFF_SFB + SFA_BYTES + k * 512, 128, 128));
-            ptx::mma_nvfp4_ss(tmem_base, ptx::make_smem_desc(sa + k * 32, 16, 1024), ptx::make_smem_desc(sb + k * 32, 16, 1024), idesc,
-                              sfa_t, sfb_t, (kb | k) ? 1u : 0u);
+            ptx::tmem_cp_32x128b_warpx4(sfa_t, ptx::make_smem_desc_noswizzle(sa + C::OFF_SFA + k * 512, 128, 128));
+            ptx::tmem_cp_32x128b_warpx4(sfb_t, ptx::make_smem_desc_noswizzle(sa + C::OFF_SFB + k * 512, 128, 128));
+            ptx::tmem_cp_32x128b_warpx4(sfb_t + 4, ptx::make_smem_desc_noswizzle(sa + C::OFF_SFB + SFA_BYTES + k * 512, 128, 128));
+            ptx::mma_nvfp4_ss(d_tmem, ptx::make_smem_desc(sa + k * 32, 16, 1024), ptx::make_smem_desc(sb + k * 32, 16, 1024), idesc,
+                              sfa_t, sfb_t + sfb_off, (kb | k) ? 1u : 0u);
           }
           ptx::mma_commit(empty_bar(stage));
-          if (kb == k_blocks - 1) ptx::mma_commit(tfull_bar);
+          if (kb == k_blocks - 1) ptx::mma_commit(tfull_bar(acc));
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          if (++slot == C::SF_SLOTS) slot = 0;
         }
-        acc_phase ^= 1;
+        if (++acc == NACC) { acc = 0; acc_phase ^= 1; }
       }
     }
   } else if (warp >= 4) {
     // ===================== epilogue =====================
     const int q4 = warp & 3;                      // tensor-memory lane quarter of this warp
+    int acc = 0;
     uint32_t acc_phase = 0;
     for (int t = blockIdx.x; t < P.total_tiles; t += gridDim.x) {
       int prob, mt, nt;
       tile_of(t, prob, mt, nt);
       const NvProblem& q = P.p[prob];
       const long long r = (long long)mt * BLOCK_M + q4 * 32 + lane;
-      ptx::mbar_wait(tfull_bar, acc_phase);
+      ptx::mbar_wait(tfull_bar(acc), acc_phase);
       ptx::tc_fence_after();
-      const uint32_t taddr0 = tmem_base + ((uint32_t)(q4 * 32) << 16);
+      const uint32_t taddr0 = tmem_base + acc * BN + ((uint32_t)(q4 * 32) << 16);
 #pragma unroll 1
-      for (int ch = 0; ch < BLOCK_N / 32; ++ch) {
-        const int n0 = nt * BLOCK_N + ch * 32;
+      for (int ch = 0; ch < BN / 32; ++ch) {
+        const int n0 = nt * BN + ch * 32;
         uint32_t v[32];
         ptx::tmem_ld_32x32(taddr0 + ch * 32, v);
         ptx::tmem_ld_wait();
@@ -195,6 +240,25 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
             h.z = fmaf(gt.z, y[4 * g + 2], h.z); h.w = fmaf(gt.w, y[4 * g + 3], h.w);
             rp[g] = h;
           }
+        } else if (EPI == EPI_GELU_NVFP4) {
+          // u = GELU(y) is never stored: two 16-element blocks of the row become 2 E4M3 scales + 32 E2M1 codes (reading N3)
+          uint32_t packed[4], sfc[2];
+#pragma unroll
+          for (int b = 0; b < 2; ++b) {
+            float u[16], amax = 0.f;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) { u[i] = gelu_tanh_fast(y[16 * b + i]); amax = fmaxf(amax, fabsf(u[i])); }
+            const float sfv = e4m3_round(__fdiv_rn(amax, 6.f), &sfc[b]);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) u[i] = sfv > 0.f ? __fdiv_rn(u[i], sfv) : 0.f;
+            packed[2 * b] = e2m1x8(u);
+            packed[2 * b + 1] = e2m1x8(u + 8);
+          }
+          *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(q.out) + r * (q.N >> 1) + (n0 >> 1)) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
+          const int blk = n0 >> 4;                         // first of the two blocks (even): both scales sit in one 4-byte group
+          const long long atom = (r >> 7) * (q.N >> 6) + (blk >> 2);
+          *reinterpret_cast<uint16_t*>(q.out_sf + atom * 512 + (r & 31) * 16 + ((r & 127) >> 5) * 4 + (blk & 3)) =
+              (uint16_t)(sfc[0] | (sfc[1] << 8));
         } else {
           uint4* op = reinterpret_cast<uint4*>(q.out + r * q.N + n0);
 #pragma unroll
@@ -213,8 +277,8 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
       }
       ptx::tc_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(tempty_bar);
-      acc_phase ^= 1;
+      if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+      if (++acc == NACC) { acc = 0; acc_phase ^= 1; }
     }
   }
 
@@ -226,12 +290,51 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
 }  // namespace
 
 bool nvfp4_gemm_supported(const Nvfp4Problem& p) {
-  return p.M > 0 && p.N > 0 && p.K > 0 && p.M % BLOCK_M == 0 && p.N % BLOCK_N == 0 && p.K % BLOCK_K == 0 && p.a_codes && p.a_sf &&
-         p.w_codes && p.w_sf && p.w_scale && p.bias && spot_get_encode_tiled() != nullptr;
+  return p.M > 0 && p.N > 0 && p.K > 0 && p.M % BLOCK_M == 0 && (p.N % 192 == 0 || p.N % 256 == 0) && p.K % BLOCK_K == 0 && p.a_codes &&
+         p.a_sf && p.w_codes && p.w_sf && p.w_scale && p.bias && spot_get_encode_tiled() != nullptr;
 }
 
+namespace {
+
+template <int EPI, int BN>
+cudaError_t launch_one(const CUtensorMap* tm, const NvParams& P, int grid, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_nvfp4_kernel<EPI, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<BN>::SMEM_BYTES));
+    attr_set = true;
+  }
+  gemm_nvfp4_kernel<EPI, BN><<<grid, NUM_THREADS, Cfg<BN>::SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], P);
+  return cudaGetLastError();
+}
+
+template <int BN>
+cudaError_t launch_bn(int epi, const CUtensorMap* tm, const NvParams& P, int grid, cudaStream_t st) {
+  switch (epi) {
+    case EPI_BIAS: return launch_one<EPI_BIAS, BN>(tm, P, grid, st);
+    case EPI_BIAS_GELU: return launch_one<EPI_BIAS_GELU, BN>(tm, P, grid, st);
+    case EPI_GATE_RES: return launch_one<EPI_GATE_RES, BN>(tm, P, grid, st);
+    default: return launch_one<EPI_GELU_NVFP4, BN>(tm, P, grid, st);
+  }
+}
+
+}  // namespace
+
+// epi = EPI_BIAS_GELU with out_sf != NULL in every problem selects the fused GELU -> NVFP4 epilogue (out = codes [M, N / 2]).
 cudaError_t launch_gemm_nvfp4(Epilogue epi, const Nvfp4Problem* probs, int n_probs, int num_sms, cudaStream_t st) {
   if (n_probs < 1 || n_probs > 2 || (epi != EPI_BIAS && epi != EPI_BIAS_GELU && epi != EPI_GATE_RES)) return cudaErrorInvalidValue;
+  bool bn192 = true, fused = epi == EPI_BIAS_GELU;
+  for (int i = 0; i < n_probs; ++i) {
+    if (probs[i].M == 0) continue;
+    if (!nvfp4_gemm_supported(probs[i])) return cudaErrorInvalidValue;
+    if (probs[i].N % 192) bn192 = false;
+    if (!probs[i].out_sf) fused = false;
+  }
+  for (int i = 0; i < n_probs; ++i)
+    if (probs[i].M > 0 && !bn192 && probs[i].N % 256) return cudaErrorInvalidValue;
+  const int BN = bn192 ? 192 : 256;
+  if (fused)
+    for (int i = 0; i < n_probs; ++i)
+      if (probs[i].M > 0 && probs[i].N % 64) return cudaErrorInvalidValue;         // whole scale atoms along the output's K
   NvParams P;
   memset(&P, 0, sizeof(P));
   CUtensorMap tm[4];
@@ -240,16 +343,15 @@ cudaError_t launch_gemm_nvfp4(Epilogue epi, const Nvfp4Problem* probs, int n_pro
   for (int i = 0; i < n_probs; ++i) {
     const Nvfp4Problem& g = probs[i];
     if (g.M == 0) continue;
-    if (!nvfp4_gemm_supported(g)) return cudaErrorInvalidValue;
     if ((epi == EPI_GATE_RES) != (g.resid != nullptr) || (epi != EPI_GATE_RES && !g.out)) return cudaErrorInvalidValue;
     NvProblem& q = P.p[np];
-    q.m_tiles = g.M / BLOCK_M; q.n_tiles = g.N / BLOCK_N; q.k_blocks = g.K / BLOCK_K; q.tile_start = tiles; q.M = g.M; q.N = g.N;
+    q.m_tiles = g.M / BLOCK_M; q.n_tiles = g.N / BN; q.k_blocks = g.K / BLOCK_K; q.tile_start = tiles; q.M = g.M; q.N = g.N;
     q.sfa = (const uint8_t*)g.a_sf; q.sfw = (const uint8_t*)g.w_sf; q.w_scale = g.w_scale; q.bias = (const bf16*)g.bias;
-    q.out = (bf16*)g.out; q.gate = g.gate; q.resid = g.resid;
+    q.out = (bf16*)g.out; q.out_sf = (uint8_t*)g.out_sf; q.gate = g.gate; q.resid = g.resid;
     tiles += q.m_tiles * q.n_tiles;
     const uint64_t adims[2] = {(uint64_t)g.K / 2, (uint64_t)g.M}, wdims[2] = {(uint64_t)g.K / 2, (uint64_t)g.N};
     const uint64_t str[1] = {(uint64_t)g.K / 2};
-    const uint32_t abox[2] = {128, BLOCK_M}, wbox[2] = {128, BLOCK_N};
+    const uint32_t abox[2] = {128, BLOCK_M}, wbox[2] = {128, (uint32_t)BN};
     SPOT_CUDA_TRY(spot_make_tmap_u8(&tm[2 * np], g.a_codes, 2, adims, str, abox));
     SPOT_CUDA_TRY(spot_make_tmap_u8(&tm[2 * np + 1], g.w_codes, 2, wdims, str, wbox));
     ++np;
@@ -258,16 +360,7 @@ cudaError_t launch_gemm_nvfp4(Epilogue epi, const Nvfp4Problem* probs, int n_pro
   if (np == 1) { tm[2] = tm[0]; tm[3] = tm[1]; }
   P.n_probs = np;
   P.total_tiles = tiles;
-  static bool attr_set = false;
-  if (!attr_set) {
-    SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_nvfp4_kernel<EPI_BIAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
-    SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_nvfp4_kernel<EPI_BIAS_GELU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
-    SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_nvfp4_kernel<EPI_GATE_RES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
-    attr_set = true;
-  }
   const int grid = tiles < num_sms ? tiles : num_sms;
-  if (epi == EPI_BIAS) gemm_nvfp4_kernel<EPI_BIAS><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], P);
-  else if (epi == EPI_BIAS_GELU) gemm_nvfp4_kernel<EPI_BIAS_GELU><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], P);
-  else gemm_nvfp4_kernel<EPI_GATE_RES><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tm[0], tm[1], tm[2], tm[3], P);
-  return cudaGetLastError();
+  const int e = fused ? EPI_GELU_NVFP4 : (int)epi;
+  return bn192 ? launch_bn<192>(e, tm, P, grid, st) : launch_bn<256>(e, tm, P, grid, st);
 }

@@ -74,7 +74,8 @@ struct Nvfp4Problem {
   const float* w_scale;                      // [N] fp32
   const void* bias;                          // [N] bf16
   int M, N, K;
-  void* out;                                 // EPI_BIAS / EPI_BIAS_GELU: [M, N] bf16
+  void* out;                                 // EPI_BIAS / EPI_BIAS_GELU: [M, N] bf16; with out_sf: E2M1 codes of GELU(y) [M, N / 2]
+  void* out_sf;                              // EPI_BIAS_GELU only, optional: scale atoms of the output -> the epilogue quantises (fc2's operand)
   const float* gate;                         // EPI_GATE_RES: [N] fp32
   float* resid;                              // EPI_GATE_RES: [M, N] fp32 residual, updated in place
 };

@@ -79,10 +79,13 @@ def _linear_case(M, N, K, tid, epi):
 
 
 @pytest.mark.parametrize("epi", [0, 1, 2])
-@pytest.mark.parametrize("M,N,K", [(128, 256, 256), (256, 512, 1024), (384, 256, 3072), (1280, 768, 512)])
+@pytest.mark.parametrize("M,N,K", [(128, 256, 256), (256, 512, 1024), (384, 256, 3072), (1280, 768, 512), (256, 384, 512),
+                                   (512, 3072, 768)])
 def test_linear_nvfp4(epi, M, N, K):
     """kind::mxf4nvf4 block-scaled GEMM vs the oracle on the SAME codes: single tile, several K blocks (ring wrap), several
-    tiles per CTA.  fp32 accumulation of exactly representable products; bf16 outputs add one rounding."""
+    tiles per CTA; N = 256 / 512 take the 128 x 256 tiles (one accumulator), N = 768 / 384 / 3072 the 128 x 192 tiles (two
+    accumulators; odd tiles start 64 rows into a scale atom).  fp32 accumulation of exactly representable products; bf16
+    outputs add one rounding."""
     got, ref, exact = _linear_case(M, N, K, 1110, epi)
     err = rel_l2(got, ref)
     print(f"nvfp4 linear M={M} N={N} K={K} epi={epi}: rel-L2 vs nvfp4 oracle {err:.3e}")
@@ -95,6 +98,46 @@ def test_linear_nvfp4(epi, M, N, K):
         assert 0.05 < rel_l2(got, exact) < 0.25            # and the quantisation itself is what oracle/nvfp4.py says it is
     again = _linear_case(M, N, K, 1110, epi)[0]
     assert (again == got).all()                            # deterministic
+
+
+@pytest.mark.parametrize("M,N,K", [(256, 768, 512), (128, 512, 256), (384, 3072, 1024)])
+def test_linear_nvfp4_fused_gelu_quantiser(M, N, K):
+    """fc1's epilogue in the rollout: bias -> tanh-GELU -> NVFP4 codes + scales without ever storing u.  The oracle
+    quantises its own exact u; the CUDA side quantises tanh.approx-GELU of an fp32-accumulated value, so a code is allowed
+    to land on the NEIGHBOURING E2M1 value where u / sf sits within that difference of a rounding boundary: >= 99 % of the
+    codes identical, none further than one grid step away, block scales identical or adjacent E4M3 values."""
+    a = hash_normal(1130, M * K, 1.0, torch.bfloat16, "cuda").reshape(M, K)
+    w = hash_normal(1131, N * K, 0.05, torch.bfloat16, "cuda").reshape(N, K)
+    b = hash_normal(1132, N, 0.1, torch.bfloat16, "cuda")
+    ac, asf = spot.spot_nvfp4_quantize(a)
+    wc, wsf, ws = spot.spot_nvfp4_quantize_weight(w)
+    codes, sf = spot.spot_linear_nvfp4(ac, asf, wc, wsf, ws, b, spot.EPI_BIAS_GELU, quantize_out=True)
+    got_q, got_sf = _unpack(codes, sf, M, N)
+    wq, wsf64, s64 = nvfp4.quantize_weight(np64(w))
+    u = mmdit.gelu_tanh(nvfp4.linear_nvfp4(np64(a), wq, wsf64, s64, np64(b)))
+    ref_q, ref_sf = nvfp4.quantize_rows(u)
+    grid = np.array([0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0])
+    step = lambda v: np.searchsorted(grid, np.abs(v)) * np.sign(v)                # signed position on the E2M1 grid
+    same_sf = (got_sf == ref_sf).mean()
+    cmp = got_sf == ref_sf                                                        # compare codes where the block scale agrees
+    m = np.repeat(cmp, 16, axis=1)
+    same = (got_q[m] == ref_q[m]).mean()
+    far = np.abs(step(got_q[m]) - step(ref_q[m])).max()
+    deq = rel_l2(nvfp4.dequantize(got_q, got_sf), nvfp4.dequantize(ref_q, ref_sf))
+    print(f"fused GELU->NVFP4 M={M} N={N} K={K}: scales identical {same_sf:.4f}, codes identical {same:.4f} (max grid distance {far:.0f}), "
+          f"dequantised rel-L2 {deq:.3e}")
+    assert same_sf > 0.99 and same > 0.99 and far <= 1
+    assert np.abs(np.log2(np.where((got_sf > 0) & (ref_sf > 0), got_sf / np.where(ref_sf > 0, ref_sf, 1), 1.0))).max() <= 0.25   # adjacent E4M3 values at most
+    assert deq < 3e-2
+    # the two-step path (u rounded to bf16, then the quantiser kernel) differs from the fused one by the code flips that one
+    # bf16 rounding (2^-9) of the quantiser's input causes - measured 3.3e-2 here, in line with the amplification the oracle
+    # test measures; the fused epilogue is the one that matches the oracle
+    u_bf = spot.spot_linear_nvfp4(ac, asf, wc, wsf, ws, b, spot.EPI_BIAS_GELU)
+    c2, s2 = spot.spot_nvfp4_quantize(u_bf)
+    q2, sf2 = _unpack(c2, s2, M, N)
+    assert rel_l2(nvfp4.dequantize(q2, sf2), nvfp4.dequantize(got_q, got_sf)) < 6e-2
+    again = spot.spot_linear_nvfp4(ac, asf, wc, wsf, ws, b, spot.EPI_BIAS_GELU, quantize_out=True)
+    assert torch.equal(again[0], codes) and torch.equal(again[1], sf)
 
 
 def test_nvfp4_argument_errors():
