@@ -16,13 +16,14 @@
 // TWO 192-column accumulators (384 tensor-memory columns) + two 48-column scale-factor slots = 480 of 512, so the epilogue
 // of a tile overlaps the next tile's MMAs; a 192-row W tile starts 0 or 64 rows into a 128-row scale atom, so both atoms it
 // touches are copied and the MMA's scale address is offset by 0 or 2 columns.  Otherwise BN = 256 with ONE accumulator.
-// EPI_GELU_NVFP4 (fc1 in the rollout) does not write u at all: the epilogue thread owns a row and 32 consecutive columns =
-// two whole 16-element blocks, so it forms the block scales and E2M1 codes of u in registers and stores 16 bytes of codes
-// and 2 scale bytes - fc2's operand in the layout nvfp4.cu documents (reading N3 applied to the fp32 GELU value).
-#include <cuda_fp8.h>
+// EPI_GELU_NVFP4 (fc1 in the rollout) does not write u at all: the epilogue thread owns a row and, per step, 64 consecutive
+// columns = four whole 16-element blocks, so it forms the block scales and E2M1 codes of u in registers (nvfp4_math.cuh) and
+// stores 32 bytes of codes and 4 scale bytes - fc2's operand in the layout nvfp4.cu documents (reading N3 applied to the
+// fp32 GELU value).
 #include <string.h>
 
 #include "kernels.h"
+#include "nvfp4_math.cuh"
 #include "tcgen05.cuh"
 
 namespace {
@@ -68,26 +69,6 @@ __device__ __forceinline__ float gelu_tanh_fast(float x) {
   asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(inner));
   const float hx = 0.5f * x;
   return fmaf(hx, th, hx);
-}
-
-// nearest E4M3 value (RNE, saturating) of v as fp32, and its byte
-__device__ __forceinline__ float e4m3_round(float v, uint32_t* code) {
-  const __nv_fp8_storage_t c = __nv_cvt_float_to_fp8(v, __NV_SATFINITE, __NV_E4M3);
-  *code = (uint32_t)c;
-  return __half2float(__half(__nv_cvt_fp8_to_halfraw(c, __NV_E4M3)));
-}
-// eight fp32 -> eight E2M1 codes in one 32-bit word, element i in nibble i (RNE, ties to the even code, saturating)
-__device__ __forceinline__ uint32_t e2m1x8(const float* v) {
-  uint32_t r;
-  asm("{\n\t.reg .b8 b0, b1, b2, b3;\n\t"
-      "cvt.rn.satfinite.e2m1x2.f32 b0, %2, %1;\n\t"
-      "cvt.rn.satfinite.e2m1x2.f32 b1, %4, %3;\n\t"
-      "cvt.rn.satfinite.e2m1x2.f32 b2, %6, %5;\n\t"
-      "cvt.rn.satfinite.e2m1x2.f32 b3, %8, %7;\n\t"
-      "mov.b32 %0, {b0, b1, b2, b3};\n\t}\n"
-      : "=r"(r)
-      : "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]));
-  return r;
 }
 
 template <int EPI, int BN>
@@ -211,13 +192,11 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
       ptx::mbar_wait(tfull_bar(acc), acc_phase);
       ptx::tc_fence_after();
       const uint32_t taddr0 = tmem_base + acc * BN + ((uint32_t)(q4 * 32) << 16);
-#pragma unroll 1
-      for (int ch = 0; ch < BN / 32; ++ch) {
+      auto load_chunk = [&](int ch, float* y) {     // y[j] = acc[r, ch * 32 + j] * s_n + b_n
         const int n0 = nt * BN + ch * 32;
         uint32_t v[32];
         ptx::tmem_ld_32x32(taddr0 + ch * 32, v);
         ptx::tmem_ld_wait();
-        float y[32];
         const uint4* bp = reinterpret_cast<const uint4*>(q.bias + n0);
         const float4* sp = reinterpret_cast<const float4*>(q.w_scale + n0);
 #pragma unroll
@@ -229,49 +208,61 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
 #pragma unroll
           for (int j = 0; j < 8; ++j) y[g * 8 + j] = fmaf(__uint_as_float(v[g * 8 + j]), sc[j], __bfloat162float(bb[j]));
         }
-        if (EPI == EPI_GATE_RES) {
-          float4* rp = reinterpret_cast<float4*>(q.resid + r * q.N + n0);
-          const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
+      };
+      if (EPI == EPI_GELU_NVFP4) {
+        // u = GELU(y) is never stored: 64 columns of the row = four 16-element blocks = one 4-byte group of a scale atom
+        // and 32 bytes of codes (a whole sector), exactly what a thread of nvfp4_quantize_kernel writes (reading N3)
+#pragma unroll 1
+        for (int c2 = 0; c2 < BN / 64; ++c2) {
+          uint32_t packed[8], sfc[4];
 #pragma unroll
-          for (int g = 0; g < 8; ++g) {
-            float4 h = rp[g];
-            const float4 gt = __ldg(gp + g);
-            h.x = fmaf(gt.x, y[4 * g], h.x); h.y = fmaf(gt.y, y[4 * g + 1], h.y);
-            h.z = fmaf(gt.z, y[4 * g + 2], h.z); h.w = fmaf(gt.w, y[4 * g + 3], h.w);
-            rp[g] = h;
+          for (int h = 0; h < 2; ++h) {
+            float y[32];
+            load_chunk(2 * c2 + h, y);
+#pragma unroll
+            for (int i = 0; i < 32; ++i) y[i] = gelu_tanh_fast(y[i]);
+            nvfp4::quantize_block16(y, &sfc[2 * h], &packed[4 * h], &packed[4 * h + 1]);
+            nvfp4::quantize_block16(y + 16, &sfc[2 * h + 1], &packed[4 * h + 2], &packed[4 * h + 3]);
           }
-        } else if (EPI == EPI_GELU_NVFP4) {
-          // u = GELU(y) is never stored: two 16-element blocks of the row become 2 E4M3 scales + 32 E2M1 codes (reading N3)
-          uint32_t packed[4], sfc[2];
+          const int n0 = nt * BN + c2 * 64;
+          uint4* cp = reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(q.out) + r * (q.N >> 1) + (n0 >> 1));
+          cp[0] = make_uint4(packed[0], packed[1], packed[2], packed[3]);
+          cp[1] = make_uint4(packed[4], packed[5], packed[6], packed[7]);
+          const long long atom = (r >> 7) * (q.N >> 6) + (n0 >> 6);
+          *reinterpret_cast<uint32_t*>(q.out_sf + atom * 512 + (r & 31) * 16 + ((r & 127) >> 5) * 4) =
+              sfc[0] | (sfc[1] << 8) | (sfc[2] << 16) | (sfc[3] << 24);
+        }
+      } else {
+#pragma unroll 1
+        for (int ch = 0; ch < BN / 32; ++ch) {
+          const int n0 = nt * BN + ch * 32;
+          float y[32];
+          load_chunk(ch, y);
+          if (EPI == EPI_GATE_RES) {
+            float4* rp = reinterpret_cast<float4*>(q.resid + r * q.N + n0);
+            const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
 #pragma unroll
-          for (int b = 0; b < 2; ++b) {
-            float u[16], amax = 0.f;
+            for (int g = 0; g < 8; ++g) {
+              float4 h = rp[g];
+              const float4 gt = __ldg(gp + g);
+              h.x = fmaf(gt.x, y[4 * g], h.x); h.y = fmaf(gt.y, y[4 * g + 1], h.y);
+              h.z = fmaf(gt.z, y[4 * g + 2], h.z); h.w = fmaf(gt.w, y[4 * g + 3], h.w);
+              rp[g] = h;
+            }
+          } else {
+            uint4* op = reinterpret_cast<uint4*>(q.out + r * q.N + n0);
 #pragma unroll
-            for (int i = 0; i < 16; ++i) { u[i] = gelu_tanh_fast(y[16 * b + i]); amax = fmaxf(amax, fabsf(u[i])); }
-            const float sfv = e4m3_round(__fdiv_rn(amax, 6.f), &sfc[b]);
+            for (int g = 0; g < 4; ++g) {
+              float z[8];
 #pragma unroll
-            for (int i = 0; i < 16; ++i) u[i] = sfv > 0.f ? __fdiv_rn(u[i], sfv) : 0.f;
-            packed[2 * b] = e2m1x8(u);
-            packed[2 * b + 1] = e2m1x8(u + 8);
-          }
-          *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(q.out) + r * (q.N >> 1) + (n0 >> 1)) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
-          const int blk = n0 >> 4;                         // first of the two blocks (even): both scales sit in one 4-byte group
-          const long long atom = (r >> 7) * (q.N >> 6) + (blk >> 2);
-          *reinterpret_cast<uint16_t*>(q.out_sf + atom * 512 + (r & 31) * 16 + ((r & 127) >> 5) * 4 + (blk & 3)) =
-              (uint16_t)(sfc[0] | (sfc[1] << 8));
-        } else {
-          uint4* op = reinterpret_cast<uint4*>(q.out + r * q.N + n0);
-#pragma unroll
-          for (int g = 0; g < 4; ++g) {
-            float z[8];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) z[j] = EPI == EPI_BIAS_GELU ? gelu_tanh_fast(y[8 * g + j]) : y[8 * g + j];
-            uint4 pk;
-            __nv_bfloat162 p0 = __floats2bfloat162_rn(z[0], z[1]), p1 = __floats2bfloat162_rn(z[2], z[3]);
-            __nv_bfloat162 p2 = __floats2bfloat162_rn(z[4], z[5]), p3 = __floats2bfloat162_rn(z[6], z[7]);
-            pk.x = *reinterpret_cast<uint32_t*>(&p0); pk.y = *reinterpret_cast<uint32_t*>(&p1);
-            pk.z = *reinterpret_cast<uint32_t*>(&p2); pk.w = *reinterpret_cast<uint32_t*>(&p3);
-            op[g] = pk;
+              for (int j = 0; j < 8; ++j) z[j] = EPI == EPI_BIAS_GELU ? gelu_tanh_fast(y[8 * g + j]) : y[8 * g + j];
+              uint4 pk;
+              __nv_bfloat162 p0 = __floats2bfloat162_rn(z[0], z[1]), p1 = __floats2bfloat162_rn(z[2], z[3]);
+              __nv_bfloat162 p2 = __floats2bfloat162_rn(z[4], z[5]), p3 = __floats2bfloat162_rn(z[6], z[7]);
+              pk.x = *reinterpret_cast<uint32_t*>(&p0); pk.y = *reinterpret_cast<uint32_t*>(&p1);
+              pk.z = *reinterpret_cast<uint32_t*>(&p2); pk.w = *reinterpret_cast<uint32_t*>(&p3);
+              op[g] = pk;
+            }
           }
         }
       }
