@@ -68,6 +68,21 @@ spot_status spot_attention(spot_dtype dtype, spot_impl impl, const void *d_qkv, 
 spot_status spot_euler_update(float *d_x, const float *d_v, float dt, int n_seqs, int64_t elems, const float *d_probe,
                               float *d_rewards, float *d_partials, void *cuda_stream);
 
+/* spot_euler_update with the reward, for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): same kernels, same results bit for bit, but the partial-sum scratch is a
+ * static __device__ array inside the library (SPOT_STATIC_PARTIALS_MAX floats = 256 KiB, held by every GPU that loads the
+ * library until the process exits) instead of a caller buffer.  The call allocates nothing (no cudaMalloc / cudaFree).
+ *   d_x [n_seqs, elems] fp32 updated in place, d_v [n_seqs, elems], d_probe [elems], d_rewards [n_seqs] out; all required.
+ *   n_seqs * ceil(elems / 4096) > SPOT_STATIC_PARTIALS_MAX -> SPOT_ERR_WORKSPACE, nothing launched (n_seqs <= 65535 and
+ *   elems % 4 == 0 as for spot_euler_update, else SPOT_ERR_SHAPE).
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress, with that device current) and must be
+ * made outside stream capture; later calls are capture-safe.  All calls on a device share the array, which keeps the last
+ * call's partial sums: two calls that overlap on the GPU (different streams, no dependency) race on it - serialise them.
+ * Nothing needs clearing between calls (every slot is written before it is read). */
+#define SPOT_STATIC_PARTIALS_MAX 65536
+spot_status spot_euler_update_static(float *d_x, const float *d_v, float dt, int n_seqs, int64_t elems, const float *d_probe,
+                                     float *d_rewards, void *cuda_stream);
+
 /* A7 alone: per-prompt statistics and top/bottom-k selection of rewards that are already on the device (spot.h
  * spot_seed_rewards states the ordering rules).  This is the step every rank repeats after the all-gather of the reward
  * shards in the multi-GPU path.  d_rewards [n_prompts * seeds_per_prompt] fp32; d_stats

@@ -113,6 +113,7 @@ def load_library() -> C.CDLL:
         "spot_qk_norm_rope": [i32, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, f32, vp],
         "spot_attention": [i32, i32, vp, vp, i32, i32, i32, i32, vp],
         "spot_euler_update": [vp, vp, f32, i32, i64, vp, vp, vp, vp],
+        "spot_euler_update_static": [vp, vp, f32, i32, i64, vp, vp, vp],
         "spot_rope_table": [vp, vp, vp],
     }
     for name, args in sig.items():
@@ -589,6 +590,22 @@ def spot_euler_update(x: torch.Tensor, v: torch.Tensor, dt: float, probe: Option
         partials = torch.empty((B, (E + 4095) // 4096), dtype=torch.float32, device=x.device)
     _check(load_library().spot_euler_update(_ptr(x), _ptr(v), dt, B, E, _ptr(probe), _ptr(rewards), _ptr(partials), _stream()),
            "spot_euler_update")
+    return x, rewards
+
+
+STATIC_PARTIALS_MAX = 65536        # include/spot_kernels.h SPOT_STATIC_PARTIALS_MAX
+
+
+def spot_euler_update_static(x: torch.Tensor, v: torch.Tensor, dt: float, probe: torch.Tensor, rewards: torch.Tensor):
+    """spot_euler_update + reward with the library's static scratch: the call allocates nothing; `rewards` [B] fp32 is the
+    caller's output buffer."""
+    B = x.shape[0]
+    E = x.numel() // B
+    status = load_library().spot_euler_update_static(_ptr(x), _ptr(v), dt, B, E, _ptr(probe), _ptr(rewards), _stream())
+    if status == 5:          # SPOT_ERR_WORKSPACE: rejected before any launch
+        raise SpotError(status, f"spot_euler_update_static: n_seqs * ceil(elems / 4096) = {B * ((E + 4095) // 4096)} exceeds the "
+                                f"static scratch of {STATIC_PARTIALS_MAX} floats (use spot_euler_update with a caller buffer)")
+    _check(status, "spot_euler_update_static")
     return x, rewards
 
 

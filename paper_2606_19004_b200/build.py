@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libspot.so")
-SOURCES = ["api.cu", "noise.cu", "elementwise.cu", "gemm_simt.cu", "attn_simt.cu", "gemm_tcgen05.cu", "gemm_tcgen05_2cta.cu", "gemm_tcgen05_v3.cu", "teacache.cu", "sde.cu", "fp8.cu", "nvfp4.cu", "gemm_nvfp4.cu", "attn_tcgen05.cu", "attn_tcgen05_v3.cu", "planner.cpp"]
+SOURCES = ["api.cu", "noise.cu", "elementwise.cu", "euler_static.cu", "gemm_simt.cu", "attn_simt.cu", "gemm_tcgen05.cu", "gemm_tcgen05_2cta.cu", "gemm_tcgen05_v3.cu", "teacache.cu", "sde.cu", "fp8.cu", "nvfp4.cu", "gemm_nvfp4.cu", "attn_tcgen05.cu", "attn_tcgen05_v3.cu", "planner.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 
