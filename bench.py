@@ -546,6 +546,8 @@ def main():
                     help="after the timed region: one more rollout with an event pair around EVERY kernel launch (SPOT_OPT_TIMING = 2); "
                          "the line gains launch_gaps = share of a rollout's wall time in which no kernel of the library runs")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--graph", action="store_true",
+                    help="also capture one rollout into a CUDA graph and time its replays beside the eager launches (1 GPU)")
     ap.add_argument("--gemm-impl", type=int, default=0,
                     help="0 auto (CTA pair + TMA-store epilogue, K4 fused), 2 one-CTA tcgen05, 3 CTA pair with per-thread "
                          "epilogue, 4 as 0 with K4 as its own kernel (A/B testing)")
@@ -736,6 +738,34 @@ def main():
                 "idle_share": 1.0 - cg["gemm_ms"] / ms_step,
                 "how": "sum of CUDA-event durations around every kernel launch of one extra rollout, against ms_per_step of the timed region"}
 
+    graph = None
+    if args.graph and dist is None and not cached and not strong:
+        # SURVEY.md 3.2 "capturable as one CUDA graph per config": the same step(), captured once and replayed
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        g = torch.cuda.CUDAGraph()
+        t0 = time.perf_counter()
+        with torch.cuda.graph(g, stream=side):
+            step()
+        capture_s = time.perf_counter() - t0
+        eager_rewards = out["rewards"].clone()
+        g.replay()
+        sync_all()
+        ev0.record()
+        for _ in range(args.steps):
+            g.replay()
+        ev1.record()
+        sync_all()
+        g_ms = ev0.elapsed_time(ev1) / args.steps
+        ev0.record()
+        for _ in range(args.steps):
+            step()
+        ev1.record()
+        sync_all()
+        eager_ms = ev0.elapsed_time(ev1) / args.steps
+        graph = {"ms_per_step": g_ms, "eager_ms_per_step_back_to_back": eager_ms, "eager_over_graph": eager_ms / g_ms,
+                 "capture_s": capture_s, "same_rewards_as_eager": bool(torch.equal(out["rewards"], eager_rewards))}
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         nb = SAMPLE_BLOCKS
@@ -764,6 +794,8 @@ def main():
                 "cpu_baseline": cpu_baseline, "weight_gen_s": gen_s}
         if gaps:
             line["launch_gaps"] = gaps
+        if graph is not None:
+            line["cuda_graph"] = graph
         if nccl_log:
             line["nccl_log"] = os.path.relpath(nccl_log, ROOT)
         rk = lambda v: torch.argsort(torch.argsort(v)).double()

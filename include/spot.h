@@ -24,6 +24,13 @@
  *     is retrievable with spot_last_cuda_error().
  *   - Asynchrony: device work is enqueued on the caller's stream (a cudaStream_t passed as
  *     void*; NULL = the legacy default stream).  Only spot_explore_host synchronises.
+ *   - CUDA graphs: spot_noise_from_seeds, spot_dit_denoise, spot_seed_rewards and spot_explore (which chains the
+ *     three) enqueue only kernel launches and memsets and read no host pointer after they return (the
+ *     timestep grid travels as kernel arguments), so after ONE eager call with the same context and options
+ *     (which sets function attributes) a call may be captured into a CUDA graph and replayed while the context,
+ *     the workspace and the argument buffers stay alive; a replay reproduces the eager call bit for bit.  The
+ *     *_cached calls (one synchronisation per step), spot_explore_host and option SPOT_OPT_TIMING != 0 are not
+ *     capturable.
  *   - Determinism: same inputs => bit-identical outputs run to run; the result for sequence b does
  *     not depend on the batch size, its position in the batch, or the other sequences.
  *   - There is no CPU fallback: on a machine without an sm_100 device every compute call returns

@@ -649,7 +649,7 @@ spot_status denoise_core(spot_ctx* c, int P, int K, float* lat, const void* text
     if (probe) LK(c, launch_reward_partials(lat, probe, B, E, partials, st));
     return SPOT_OK;
   }
-  CK(c, cudaMemcpyAsync(ws + w.t_dev, h_t, (size_t)(T + 1) * 4, cudaMemcpyHostToDevice, st));
+  LK(c, launch_put_floats(h_t, T + 1, (float*)(ws + w.t_dev), st));   // by value: no host pointer outlives the call (CUDA-graph capturable)
   spot_status rs = conditioning(c, w, ws, T, st);
   if (rs != SPOT_OK) return rs;
   float* txt_h0 = (float*)(ws + w.txt_h0); float* h_img = (float*)(ws + w.h_img); float* h_txt = (float*)(ws + w.h_txt);

@@ -555,6 +555,13 @@ __global__ void fill_f32_kernel(float* __restrict__ p, float v, long long n) {
   if (i < n) p[i] = v;
 }
 
+// up to 64 host floats travel as KERNEL ARGUMENTS: no host pointer is read after the launch call returns, so a rollout
+// captured into a CUDA graph carries its timestep grid with it
+struct Floats64 { float v[64]; };
+__global__ void put_floats_kernel(Floats64 a, int n, float* __restrict__ p) {
+  if ((int)threadIdx.x < n) p[threadIdx.x] = a.v[threadIdx.x];
+}
+
 // out[t * stride_t + n] = acc[t, n] + acc[T + t, n] + bias[n]   (hi and lo halves of the split GEMM, then the bias)
 template <typename TB>
 __global__ void mod_combine_kernel(const float* __restrict__ acc, const TB* __restrict__ bias, int T, int N,
@@ -571,6 +578,18 @@ cudaError_t launch_split_hi_lo(const float* c, void* a_bf16, long long n, cudaSt
   if (n <= 0) return cudaSuccess;
   split_hi_lo_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c, (bf16*)a_bf16, n);
   return cudaGetLastError();
+}
+
+cudaError_t launch_put_floats(const float* h_src, int n, float* d_dst, cudaStream_t st) {
+  for (int i0 = 0; i0 < n; i0 += 64) {
+    Floats64 a;
+    const int m = n - i0 < 64 ? n - i0 : 64;
+    for (int i = 0; i < 64; ++i) a.v[i] = i < m ? h_src[i0 + i] : 0.f;
+    put_floats_kernel<<<1, 64, 0, st>>>(a, m, d_dst + i0);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 cudaError_t launch_fill_f32(float* p, float v, long long n, cudaStream_t st) {

@@ -14,6 +14,8 @@ cudaError_t launch_silu(const float* in, float* out, long long n, cudaStream_t s
 // K7 on the tensor cores: c = hi + lo (two bf16 rows per timestep) through the tcgen05 GEMM, then hi + lo + bias
 cudaError_t launch_split_hi_lo(const float* c, void* a_bf16, long long n, cudaStream_t st);
 cudaError_t launch_fill_f32(float* p, float v, long long n, cudaStream_t st);
+// n HOST floats -> device, passed by value as kernel arguments (64 per launch): capture-safe, unlike a copy from pageable memory
+cudaError_t launch_put_floats(const float* h_src, int n, float* d_dst, cudaStream_t st);
 cudaError_t launch_mod_combine(const float* acc, const void* bias_bf16, int T, int N, float* out, long long stride_t,
                                cudaStream_t st);
 

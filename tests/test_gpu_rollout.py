@@ -266,6 +266,39 @@ def test_cfg3_lite_rollout_bf16():
         assert out["top"][0, 0].item() == int(np.argmax(rew))
 
 
+def test_rollout_captures_into_a_cuda_graph_and_replays_bit_identically():
+    """SURVEY.md 3.2 "capturable as one CUDA graph per config": spot_explore (noise -> T velocity passes -> Euler -> reward ->
+    selection) launches only kernels and memsets, and no host pointer outlives the call (the timestep grid travels as kernel
+    arguments), so after one eager call (function attributes, the static scratch's address) the rollout is captured into a
+    graph and replayed: same bits as the eager call, also after the host-side timestep array has been freed and overwritten."""
+    import ctypes
+    import gc
+    s = CONFIGS[3].with_(n_blocks=2, seeds_per_prompt=2, n_steps=3, seeds=(5, 6))
+    w = device_weights(s)
+    ctx = spot.Context(s, w, max_seqs=2)
+    text, probe = make_text_emb(s, "cuda"), make_probe(s, "cuda")
+    ts = f32_timesteps(s)
+    seeds = _seeds(s.seeds)
+    out = spot.spot_explore(ctx, seeds, text, ts, probe, 1, 2, 1)
+    torch.cuda.synchronize()
+    ref = {k: v.clone() for k, v in out.items()}
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        spot.spot_explore(ctx, seeds, text, list(ts), probe, 1, 2, 1, out)
+    gc.collect()
+    junk = [(ctypes.c_float * 4)(7.0, 7.0, 7.0, 7.0) for _ in range(4096)]          # recycle the freed host arrays
+    for _ in range(2):
+        for v in out.values():
+            v.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        for k in ref:
+            assert torch.equal(out[k], ref[k]), k
+    del junk
+
+
 @pytest.mark.parametrize("world,wide", [(1, False), (3, False), (8, False), (4, True)])
 def test_sharded_exploration_is_bit_identical(world, wide):
     """sequences sharded over `world` ranks (run here one after the other on the one GPU - no rank
