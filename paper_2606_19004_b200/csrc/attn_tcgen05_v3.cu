@@ -23,6 +23,8 @@
 #include <cuda_fp8.h>
 #include <string.h>
 
+#include <stdlib.h>
+
 #include "kernels.h"
 #include "tcgen05.cuh"
 
@@ -65,7 +67,7 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 template <bool OUT8>
 __global__ void __launch_bounds__(ATT_THREADS, 1)
 attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, const __grid_constant__ CUtensorMap tm_out, int S, int H,
-                       int n_items, float scale_log2) {
+                       int n_items, float scale_log2, int kv_policy) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw_addr = ptx::smem_u32(smem_raw);
   const uint32_t base = (raw_addr + 1023u) & ~1023u;
@@ -122,6 +124,7 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, const __grid_
     //  of wrapping each one in a per-lane ELECT / BRA.U.ANY loop - see "single-thread issue paths" in tcgen05.cuh)
     if (ptx::elect_one()) {
       int it = 0;
+      const uint64_t pol_kv = ptx::l2_policy(kv_policy);   // K / V tiles are re-read by the item's other query tiles
       for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++it) {
         const int x = w % n_qt, head = (w / n_qt) % H, seq = w / (n_qt * H);
         const int q0 = x * (QT * BQ);
@@ -141,12 +144,12 @@ attn_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tm_qkv, const __grid_
           const uint32_t ph = (uint32_t)(g / KV_STAGES) & 1u;
           ptx::mbar_wait(k_empty(st), ph ^ 1);
           ptx::mbar_arrive_expect_tx(k_full(st), KV_TILE);
-          ptx::tma_load_3d(base + OFF_K + st * KV_TILE, &tm_qkv, k_full(st), col_k, j * BKV, seq);
-          ptx::tma_load_3d(base + OFF_K + st * KV_TILE + KV_SUB, &tm_qkv, k_full(st), col_k + 64, j * BKV, seq);
+          ptx::tma_load_3d_hint(base + OFF_K + st * KV_TILE, &tm_qkv, k_full(st), col_k, j * BKV, seq, pol_kv);
+          ptx::tma_load_3d_hint(base + OFF_K + st * KV_TILE + KV_SUB, &tm_qkv, k_full(st), col_k + 64, j * BKV, seq, pol_kv);
           ptx::mbar_wait(v_empty(st), ph ^ 1);
           ptx::mbar_arrive_expect_tx(v_full(st), KV_TILE);
-          ptx::tma_load_3d(base + OFF_V + st * KV_TILE, &tm_qkv, v_full(st), col_v, j * BKV, seq);
-          ptx::tma_load_3d(base + OFF_V + st * KV_TILE + KV_SUB, &tm_qkv, v_full(st), col_v + 64, j * BKV, seq);
+          ptx::tma_load_3d_hint(base + OFF_V + st * KV_TILE, &tm_qkv, v_full(st), col_v, j * BKV, seq, pol_kv);
+          ptx::tma_load_3d_hint(base + OFF_V + st * KV_TILE + KV_SUB, &tm_qkv, v_full(st), col_v + 64, j * BKV, seq, pol_kv);
         }
       }
     }
@@ -397,9 +400,11 @@ cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int
   }
   const long long items = (long long)((S + QT * BQ - 1) / (QT * BQ)) * H * B;
   if (items > 0x7fffffffLL / 128) return cudaErrorInvalidValue;
+  static int kv_policy = -1;                    // A/B only: SPOT_ATTN_L2_HINT = L2 policy of the K / V loads (tcgen05.cuh l2_policy)
+  if (kv_policy < 0) { const char* e = getenv("SPOT_ATTN_L2_HINT"); kv_policy = e ? atoi(e) : 0; }
   const int grid = (int)(items < num_sms ? items : num_sms);       // persistent: one CTA per SM walks the item list
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)DH);
-  if (out_e4m3) attn_tcgen05_v3_kernel<true><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, tmo, S, H, (int)items, scale_log2);
-  else attn_tcgen05_v3_kernel<false><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, tmo, S, H, (int)items, scale_log2);
+  if (out_e4m3) attn_tcgen05_v3_kernel<true><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, tmo, S, H, (int)items, scale_log2, kv_policy);
+  else attn_tcgen05_v3_kernel<false><<<grid, ATT_THREADS, ATT_SMEM, st>>>(tm, tmo, S, H, (int)items, scale_log2, kv_policy);
   return cudaGetLastError();
 }

@@ -20,6 +20,7 @@
 // columns = four whole 16-element blocks, so it forms the block scales and E2M1 codes of u in registers (nvfp4_math.cuh) and
 // stores 32 bytes of codes and 4 scale bytes - fc2's operand in the layout nvfp4.cu documents (reading N3 applied to the
 // fp32 GELU value).
+#include <stdlib.h>
 #include <string.h>
 
 #include "kernels.h"
@@ -60,6 +61,7 @@ struct NvProblem {
 struct NvParams {
   NvProblem p[2];
   int n_probs, total_tiles;
+  int l2_a, l2_w;           // L2 eviction priority of the code loads (tcgen05.cuh l2_policy)
 };
 
 __device__ __forceinline__ float gelu_tanh_fast(float x) {
@@ -118,6 +120,7 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
     // ===================== producer =====================
     if (ptx::elect_one()) {
       int stage = 0; uint32_t phase = 0;
+      const uint64_t pol_a = ptx::l2_policy(P.l2_a), pol_w = ptx::l2_policy(P.l2_w);
       for (int t = blockIdx.x; t < P.total_tiles; t += gridDim.x) {
         int prob, mt, nt;
         tile_of(t, prob, mt, nt);
@@ -131,8 +134,8 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
           ptx::mbar_wait(empty_bar(stage), phase ^ 1);
           ptx::mbar_arrive_expect_tx(full_bar(stage), C::TX_BYTES);
           const uint32_t sa = smem_base + stage * C::STAGE_BYTES;
-          ptx::tma_load_2d(sa, mA, full_bar(stage), kb * 128, mt * BLOCK_M);
-          ptx::tma_load_2d(sa + A_BYTES, mW, full_bar(stage), kb * 128, n0);
+          ptx::tma_load_2d_hint(sa, mA, full_bar(stage), kb * 128, mt * BLOCK_M, pol_a);
+          ptx::tma_load_2d_hint(sa + A_BYTES, mW, full_bar(stage), kb * 128, n0, pol_w);
           ptx::bulk_load_1d(sa + C::OFF_SFA, q.sfa + ((long long)mt * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
           ptx::bulk_load_1d(sa + C::OFF_SFB, q.sfw + ((long long)atom0 * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
           ptx::bulk_load_1d(sa + C::OFF_SFB + SFA_BYTES, q.sfw + ((long long)atom1 * ka + kb * 4) * 512, SFA_BYTES, full_bar(stage));
@@ -328,6 +331,11 @@ cudaError_t launch_gemm_nvfp4(Epilogue epi, const Nvfp4Problem* probs, int n_pro
       if (probs[i].M > 0 && probs[i].N % 64) return cudaErrorInvalidValue;         // whole scale atoms along the output's K
   NvParams P;
   memset(&P, 0, sizeof(P));
+  {
+    static int hint = -1;                         // A/B only: SPOT_NVFP4_L2_HINT = 10 * A-policy + W-policy
+    if (hint < 0) { const char* e = getenv("SPOT_NVFP4_L2_HINT"); hint = e ? atoi(e) : 0; }
+    P.l2_a = hint / 10; P.l2_w = hint % 10;
+  }
   CUtensorMap tm[4];
   memset(tm, 0, sizeof(tm));
   int tiles = 0, np = 0;

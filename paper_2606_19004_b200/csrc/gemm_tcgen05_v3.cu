@@ -62,6 +62,7 @@ struct V3Problem {
 struct V3Params {
   V3Problem p[2];
   int n_probs, total_tiles;
+  int l2_a, l2_w, l2_o;     // L2 eviction priority of the A / W loads and of the output stores / reductions (tcgen05.cuh l2_policy: 0 normal, 1 evict_last, 2 evict_first)
 };
 struct TileCoord { int prob, mt, nt; };
 
@@ -211,6 +212,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
     // UTCHMMA straight from uniform registers (see "single-thread issue paths" in tcgen05.cuh)
     if (ptx::elect_one()) {
       int stage = 0; uint32_t phase = 0;
+      const uint64_t pol_a = ptx::l2_policy(P.l2_a), pol_w = ptx::l2_policy(P.l2_w);
       for (int t = pair; t < P.total_tiles; t += n_pairs) {
         const TileCoord c = decode_tile(P, t);
         const V3Problem& q = P.p[c.prob];
@@ -223,8 +225,8 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
           ptx::mbar_wait(empty_bar(stage), phase ^ 1);
           const uint32_t leader_full = ptx::map_to_cta(full_bar(stage), 0);
           const uint32_t sa = smem_base + stage * STAGE_BYTES;
-          ptx::tma_load_3d_2cta(sa, mA, leader_full, kb * (FP8 ? 2 * BLOCK_K : BLOCK_K), r0, seq);
-          ptx::tma_load_2d_2cta(sa + A_BYTES, mW, leader_full, kb * (FP8 ? 2 * BLOCK_K : BLOCK_K), n0);
+          ptx::tma_load_3d_2cta_hint(sa, mA, leader_full, kb * (FP8 ? 2 * BLOCK_K : BLOCK_K), r0, seq, pol_a);
+          ptx::tma_load_2d_2cta_hint(sa + A_BYTES, mW, leader_full, kb * (FP8 ? 2 * BLOCK_K : BLOCK_K), n0, pol_w);
           // only the leader CTA arms its barrier, for the bytes of BOTH CTAs (see gemm_tcgen05_2cta.cu)
           if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
           if (++stage == NST) { stage = 0; phase ^= 1; }
@@ -302,6 +304,7 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
     if constexpr (EPI == EPI_QKV_ROPE && FP8) {
       if (pair < P.total_tiles) { ColConst first; load_colconst(pair, first); store_colconst(first); }
     }
+    const uint64_t pol_o = ptx::l2_policy(P.l2_o);
     for (int t = pair; t < P.total_tiles; t += n_pairs) {
       const TileCoord c = decode_tile(P, t);
       const V3Problem& q = P.p[c.prob];
@@ -318,8 +321,8 @@ gemm_tcgen05_v3_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_co
         __syncwarp();
         if (ptx::elect_one()) {                           // deterministic: the same lane every time (it owns the bulk groups)
           if (warp_ok) {
-            if (EPI == EPI_GATE_RES) ptx::tma_reduce_add_3d(mO, stg0 + buf * STG_BYTES, n0, row0, seq);
-            else ptx::tma_store_3d(mO, stg0 + buf * STG_BYTES, n0, row0, seq);
+            if (EPI == EPI_GATE_RES) ptx::tma_reduce_add_3d_hint(mO, stg0 + buf * STG_BYTES, n0, row0, seq, pol_o);
+            else ptx::tma_store_3d_hint(mO, stg0 + buf * STG_BYTES, n0, row0, seq, pol_o);
           }
           ptx::bulk_commit();
         }
@@ -584,6 +587,17 @@ cudaError_t launch_gemm_tcgen05_v3(Epilogue epi, const GemmProblem* probs, int n
   if (n_probs < 1 || n_probs > 2) return cudaErrorInvalidValue;
   V3Params P;
   memset(&P, 0, sizeof(P));
+  {
+    // L2 eviction priorities: both operands evict_last, outputs (stores and the residual reduce-add) evict_first.  A tile of
+    // A is re-read by the other N tiles of its raster group and a tile of W by the other M tiles, while an output line is
+    // never read again by this kernel; without the hints the 0.2-0.5 GB a launch writes push operand lines out.  Measured
+    // at config 3, same box, back to back, two rounds: 2469.5 / 2473.9 ms (no hints) -> 2414.2 / 2416.5 ms; A evict_first
+    // instead: 2651 ms and 2.2-4.1 GB of DRAM reads per launch (profiles/r2_gemm_l2.md).  SPOT_GEMM_L2_HINT =
+    // 100 * output + 10 * A + W policy (0 normal, 1 evict_last, 2 evict_first) overrides, for A/B timing only.
+    static int hint = -1;
+    if (hint < 0) { const char* e = getenv("SPOT_GEMM_L2_HINT"); hint = e ? atoi(e) : 211; }
+    P.l2_o = hint / 100; P.l2_a = hint / 10 % 10; P.l2_w = hint % 10;
+  }
   CUtensorMap tm[6];
   memset(tm, 0, sizeof(tm));
   int tiles = 0, np = 0;
