@@ -400,7 +400,9 @@ cudaError_t launch_attn_tcgen05_v3(const void* qkv, void* out, int B, int S, int
   }
   const long long items = (long long)((S + QT * BQ - 1) / (QT * BQ)) * H * B;
   if (items > 0x7fffffffLL / 128) return cudaErrorInvalidValue;
-  static int kv_policy = -1;                    // A/B only: SPOT_ATTN_L2_HINT = L2 policy of the K / V loads (tcgen05.cuh l2_policy)
+  // A/B only: SPOT_ATTN_L2_HINT = L2 policy of the K / V loads (tcgen05.cuh l2_policy).  Measured at config 3, two rounds:
+  // 2477 / 2480 / 2475 ms for normal / evict_last / evict_first - no effect, so the default stays normal.
+  static int kv_policy = -1;
   if (kv_policy < 0) { const char* e = getenv("SPOT_ATTN_L2_HINT"); kv_policy = e ? atoi(e) : 0; }
   const int grid = (int)(items < num_sms ? items : num_sms);       // persistent: one CTA per SM walks the item list
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)DH);

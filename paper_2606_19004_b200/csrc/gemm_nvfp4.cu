@@ -332,8 +332,10 @@ cudaError_t launch_gemm_nvfp4(Epilogue epi, const Nvfp4Problem* probs, int n_pro
   NvParams P;
   memset(&P, 0, sizeof(P));
   {
-    static int hint = -1;                         // A/B only: SPOT_NVFP4_L2_HINT = 10 * A-policy + W-policy
-    if (hint < 0) { const char* e = getenv("SPOT_NVFP4_L2_HINT"); hint = e ? atoi(e) : 0; }
+    // both operands evict_last, as in gemm_tcgen05_v3.cu: config-3 NVFP4 rollout 1353 -> 1323 ms, same box, two rounds
+    // (profiles/r2_gemm_l2.md).  SPOT_NVFP4_L2_HINT = 10 * A-policy + W-policy overrides, for A/B timing only.
+    static int hint = -1;
+    if (hint < 0) { const char* e = getenv("SPOT_NVFP4_L2_HINT"); hint = e ? atoi(e) : 11; }
     P.l2_a = hint / 10; P.l2_w = hint % 10;
   }
   CUtensorMap tm[4];
