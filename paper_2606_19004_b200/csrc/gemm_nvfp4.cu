@@ -16,10 +16,12 @@
 // TWO 192-column accumulators (384 tensor-memory columns) + two 48-column scale-factor slots = 480 of 512, so the epilogue
 // of a tile overlaps the next tile's MMAs; a 192-row W tile starts 0 or 64 rows into a 128-row scale atom, so both atoms it
 // touches are copied and the MMA's scale address is offset by 0 or 2 columns.  Otherwise BN = 256 with ONE accumulator.
-// EPI_GELU_NVFP4 (fc1 in the rollout) does not write u at all: the epilogue thread owns a row and, per step, 64 consecutive
-// columns = four whole 16-element blocks, so it forms the block scales and E2M1 codes of u in registers (nvfp4_math.cuh) and
-// stores 32 bytes of codes and 4 scale bytes - fc2's operand in the layout nvfp4.cu documents (reading N3 applied to the
-// fp32 GELU value).
+// EPI_GELU_NVFP4 (fc1 in the rollout) does not write u at all: the epilogue thread owns a row and, per 32-column chunk, two
+// whole 16-element blocks, so it forms the block scales and E2M1 codes of u in registers (nvfp4_math.cuh) and stores 16
+// bytes of codes and 2 scale bytes - fc2's operand in the layout nvfp4.cu documents (reading N3 applied to the fp32 GELU
+// value).
+// Where every M is a multiple of 256 and every N of 192 (the rollout's shapes) the CTA-PAIR kernel further down runs
+// instead (256 x 192 tiles, tcgen05.mma.cta_group::2); the one-CTA kernel is the fallback for other shapes.
 #include <stdlib.h>
 #include <string.h>
 
@@ -64,6 +66,9 @@ struct NvParams {
   int l2_a, l2_w;           // L2 eviction priority of the code loads (tcgen05.cuh l2_policy)
 };
 
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
 __device__ __forceinline__ float gelu_tanh_fast(float x) {
   const float k0 = 0.7978845608028654f, k1 = 0.7978845608028654f * 0.044715f;
   const float inner = x * fmaf(k1, x * x, k0);
@@ -71,6 +76,77 @@ __device__ __forceinline__ float gelu_tanh_fast(float x) {
   asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(inner));
   const float hx = 0.5f * x;
   return fmaf(hx, th, hx);
+}
+
+// y[j] = acc[r, ch * 32 + j] * s_n + b_n for one 32-column chunk of the thread's accumulator row
+template <int BN>
+__device__ __forceinline__ void load_chunk(const NvProblem& q, int nt, uint32_t taddr0, int ch, float* y) {
+  const int n0 = nt * BN + ch * 32;
+  uint32_t v[32];
+  ptx::tmem_ld_32x32(taddr0 + ch * 32, v);
+  ptx::tmem_ld_wait();
+  const uint4* bp = reinterpret_cast<const uint4*>(q.bias + n0);
+  const float4* sp = reinterpret_cast<const float4*>(q.w_scale + n0);
+#pragma unroll
+  for (int g = 0; g < 4; ++g) {
+    const uint4 braw = __ldg(bp + g);
+    const bf16* bb = reinterpret_cast<const bf16*>(&braw);
+    const float4 s0 = __ldg(sp + 2 * g), s1 = __ldg(sp + 2 * g + 1);
+    const float sc[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+#pragma unroll
+    for (int j = 0; j < 8; ++j) y[g * 8 + j] = fmaf(__uint_as_float(v[g * 8 + j]), sc[j], __bfloat162float(bb[j]));
+  }
+}
+
+// Epilogue of one tile for one thread: row r of the output, 32-column chunks [ch_lo, ch_hi) of N-tile nt, accumulator at
+// taddr0 (the thread's tensor-memory lane).  Shared by the one-CTA kernel (all BN / 32 chunks) and the CTA-pair kernel (two
+// warps per lane quarter, half of the chunks each).
+template <int EPI, int BN>
+__device__ __forceinline__ void epilogue_tile(const NvProblem& q, int nt, long long r, uint32_t taddr0, int ch_lo, int ch_hi) {
+#pragma unroll 1
+  for (int ch = ch_lo; ch < ch_hi; ++ch) {
+    const int n0 = nt * BN + ch * 32;
+    float y[32];
+    load_chunk<BN>(q, nt, taddr0, ch, y);
+    if (EPI == EPI_GATE_RES) {
+      float4* rp = reinterpret_cast<float4*>(q.resid + r * q.N + n0);
+      const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
+#pragma unroll
+      for (int g = 0; g < 8; ++g) {
+        float4 h = rp[g];
+        const float4 gt = __ldg(gp + g);
+        h.x = fmaf(gt.x, y[4 * g], h.x); h.y = fmaf(gt.y, y[4 * g + 1], h.y);
+        h.z = fmaf(gt.z, y[4 * g + 2], h.z); h.w = fmaf(gt.w, y[4 * g + 3], h.w);
+        rp[g] = h;
+      }
+    } else if (EPI == EPI_GELU_NVFP4) {
+      // u = GELU(y) is never stored: the chunk's two 16-element blocks become 2 E4M3 scales + 32 E2M1 codes (reading N3) -
+      // 16 bytes of codes and the two scale bytes of the row's 4-byte group in the scale atom nvfp4.cu documents
+      uint32_t packed[4], sfc[2];
+#pragma unroll
+      for (int i = 0; i < 32; ++i) y[i] = gelu_tanh_fast(y[i]);
+      nvfp4::quantize_block16(y, &sfc[0], &packed[0], &packed[1]);
+      nvfp4::quantize_block16(y + 16, &sfc[1], &packed[2], &packed[3]);
+      *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(q.out) + r * (q.N >> 1) + (n0 >> 1)) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
+      const int blk = n0 >> 4;                             // first of the chunk's two blocks (even)
+      const long long atom = (r >> 7) * (q.N >> 6) + (blk >> 2);
+      *reinterpret_cast<uint16_t*>(q.out_sf + atom * 512 + (r & 31) * 16 + ((r & 127) >> 5) * 4 + (blk & 3)) = (uint16_t)(sfc[0] | (sfc[1] << 8));
+    } else {
+      uint4* op = reinterpret_cast<uint4*>(q.out + r * q.N + n0);
+#pragma unroll
+      for (int g = 0; g < 4; ++g) {
+        float z[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) z[j] = EPI == EPI_BIAS_GELU ? gelu_tanh_fast(y[8 * g + j]) : y[8 * g + j];
+        uint4 pk;
+        __nv_bfloat162 p0 = __floats2bfloat162_rn(z[0], z[1]), p1 = __floats2bfloat162_rn(z[2], z[3]);
+        __nv_bfloat162 p2 = __floats2bfloat162_rn(z[4], z[5]), p3 = __floats2bfloat162_rn(z[6], z[7]);
+        pk.x = *reinterpret_cast<uint32_t*>(&p0); pk.y = *reinterpret_cast<uint32_t*>(&p1);
+        pk.z = *reinterpret_cast<uint32_t*>(&p2); pk.w = *reinterpret_cast<uint32_t*>(&p3);
+        op[g] = pk;
+      }
+    }
+  }
 }
 
 template <int EPI, int BN>
@@ -195,80 +271,7 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
       ptx::mbar_wait(tfull_bar(acc), acc_phase);
       ptx::tc_fence_after();
       const uint32_t taddr0 = tmem_base + acc * BN + ((uint32_t)(q4 * 32) << 16);
-      auto load_chunk = [&](int ch, float* y) {     // y[j] = acc[r, ch * 32 + j] * s_n + b_n
-        const int n0 = nt * BN + ch * 32;
-        uint32_t v[32];
-        ptx::tmem_ld_32x32(taddr0 + ch * 32, v);
-        ptx::tmem_ld_wait();
-        const uint4* bp = reinterpret_cast<const uint4*>(q.bias + n0);
-        const float4* sp = reinterpret_cast<const float4*>(q.w_scale + n0);
-#pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          const uint4 braw = __ldg(bp + g);
-          const bf16* bb = reinterpret_cast<const bf16*>(&braw);
-          const float4 s0 = __ldg(sp + 2 * g), s1 = __ldg(sp + 2 * g + 1);
-          const float sc[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
-#pragma unroll
-          for (int j = 0; j < 8; ++j) y[g * 8 + j] = fmaf(__uint_as_float(v[g * 8 + j]), sc[j], __bfloat162float(bb[j]));
-        }
-      };
-      if (EPI == EPI_GELU_NVFP4) {
-        // u = GELU(y) is never stored: 64 columns of the row = four 16-element blocks = one 4-byte group of a scale atom
-        // and 32 bytes of codes (a whole sector), exactly what a thread of nvfp4_quantize_kernel writes (reading N3)
-#pragma unroll 1
-        for (int c2 = 0; c2 < BN / 64; ++c2) {
-          uint32_t packed[8], sfc[4];
-#pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            float y[32];
-            load_chunk(2 * c2 + h, y);
-#pragma unroll
-            for (int i = 0; i < 32; ++i) y[i] = gelu_tanh_fast(y[i]);
-            nvfp4::quantize_block16(y, &sfc[2 * h], &packed[4 * h], &packed[4 * h + 1]);
-            nvfp4::quantize_block16(y + 16, &sfc[2 * h + 1], &packed[4 * h + 2], &packed[4 * h + 3]);
-          }
-          const int n0 = nt * BN + c2 * 64;
-          uint4* cp = reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(q.out) + r * (q.N >> 1) + (n0 >> 1));
-          cp[0] = make_uint4(packed[0], packed[1], packed[2], packed[3]);
-          cp[1] = make_uint4(packed[4], packed[5], packed[6], packed[7]);
-          const long long atom = (r >> 7) * (q.N >> 6) + (n0 >> 6);
-          *reinterpret_cast<uint32_t*>(q.out_sf + atom * 512 + (r & 31) * 16 + ((r & 127) >> 5) * 4) =
-              sfc[0] | (sfc[1] << 8) | (sfc[2] << 16) | (sfc[3] << 24);
-        }
-      } else {
-#pragma unroll 1
-        for (int ch = 0; ch < BN / 32; ++ch) {
-          const int n0 = nt * BN + ch * 32;
-          float y[32];
-          load_chunk(ch, y);
-          if (EPI == EPI_GATE_RES) {
-            float4* rp = reinterpret_cast<float4*>(q.resid + r * q.N + n0);
-            const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
-#pragma unroll
-            for (int g = 0; g < 8; ++g) {
-              float4 h = rp[g];
-              const float4 gt = __ldg(gp + g);
-              h.x = fmaf(gt.x, y[4 * g], h.x); h.y = fmaf(gt.y, y[4 * g + 1], h.y);
-              h.z = fmaf(gt.z, y[4 * g + 2], h.z); h.w = fmaf(gt.w, y[4 * g + 3], h.w);
-              rp[g] = h;
-            }
-          } else {
-            uint4* op = reinterpret_cast<uint4*>(q.out + r * q.N + n0);
-#pragma unroll
-            for (int g = 0; g < 4; ++g) {
-              float z[8];
-#pragma unroll
-              for (int j = 0; j < 8; ++j) z[j] = EPI == EPI_BIAS_GELU ? gelu_tanh_fast(y[8 * g + j]) : y[8 * g + j];
-              uint4 pk;
-              __nv_bfloat162 p0 = __floats2bfloat162_rn(z[0], z[1]), p1 = __floats2bfloat162_rn(z[2], z[3]);
-              __nv_bfloat162 p2 = __floats2bfloat162_rn(z[4], z[5]), p3 = __floats2bfloat162_rn(z[6], z[7]);
-              pk.x = *reinterpret_cast<uint32_t*>(&p0); pk.y = *reinterpret_cast<uint32_t*>(&p1);
-              pk.z = *reinterpret_cast<uint32_t*>(&p2); pk.w = *reinterpret_cast<uint32_t*>(&p3);
-              op[g] = pk;
-            }
-          }
-        }
-      }
+      epilogue_tile<EPI, BN>(q, nt, r, taddr0, 0, BN / 32);
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
@@ -279,6 +282,198 @@ gemm_nvfp4_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constan
   ptx::tc_fence_before();
   __syncthreads();
   if (warp == 2) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem_base, 512); }
+}
+
+
+// ------------------------------------------------------------------------------------------------------------------------
+// CTA-pair version (cluster of 2, tcgen05.mma.cta_group::2): one 256 x 192 tile per pair.  Each CTA stages its own 128 rows
+// of A, HALF of the W tile (96 rows), the scale factors of its A rows and the scale factors of ALL 192 W rows (its tensor
+// core multiplies its 128 rows by the whole tile width), i.e. 7 KB of operands per K = 64 step from shared memory instead of
+// the one-CTA tile's 10 KB - below the 96 cycles the FP4 math of the step takes.  Everything is loaded by TMA tensor loads
+// (.cta_group::2: completion bytes of both CTAs land on the LEADER's barrier); the scale-factor atoms through a linear
+// (unswizzled) map of the atom array seen as rows of 256 bytes.  The leader's elected thread issues tcgen05.cp / tcgen05.mma
+// for the pair; tcgen05.commit multicasts the stage release and the accumulator hand-over to both CTAs.
+namespace pair {
+constexpr int BN = 192, HALF_BN = 96, PAIR_M = 256, STAGES = 5, EPI_WARPS = 8, THREADS = 128 + EPI_WARPS * 32;
+constexpr uint32_t W_BYTES = HALF_BN * 128, OFF_W = A_BYTES, OFF_SFA = OFF_W + W_BYTES, OFF_SFB = OFF_SFA + SFA_BYTES;
+constexpr uint32_t STAGE_BYTES = OFF_SFB + SFB_BYTES;                  // 16384 + 12288 + 2048 + 4096 = 34816 = 34 x 1024
+constexpr uint32_t STG_BYTES = 32 * 128;                               // staging buffer of an epilogue warp: 32 rows x 32 fp32
+constexpr uint32_t OFF_STG = STAGES * STAGE_BYTES, OFF_BAR = OFF_STG + EPI_WARPS * STG_BYTES, SMEM_BYTES = OFF_BAR + 256 + 1024;
+constexpr uint32_t TM_SF = 2 * BN;
+static_assert(STAGE_BYTES % 1024 == 0 && SMEM_BYTES <= 232448, "shared memory plan");
+}  // namespace pair
+
+struct NvPairMaps { CUtensorMap a, w, sfa, sfw, resid; };
+
+template <int EPI>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(pair::THREADS, 1)
+gemm_nvfp4_pair_kernel(const __grid_constant__ NvPairMaps m0, const __grid_constant__ NvPairMaps m1, const NvParams P) {
+  using namespace pair;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + OFF_BAR;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + 2 + a); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
+  volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
+  const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
+  const uint32_t rank = __shfl_sync(0xffffffffu, ptx::cluster_ctarank(), 0);     // 0 = leader of the pair
+  const int pair_id = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&m0.a); ptx::prefetch_tmap(&m0.w); ptx::prefetch_tmap(&m0.sfa); ptx::prefetch_tmap(&m0.sfw);
+    if (P.n_probs > 1) { ptx::prefetch_tmap(&m1.a); ptx::prefetch_tmap(&m1.w); ptx::prefetch_tmap(&m1.sfa); ptx::prefetch_tmap(&m1.sfw); }
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    for (int a = 0; a < 2; ++a) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 2 * EPI_WARPS); }   // epilogue warps of both CTAs
+    ptx::fence_barrier_init();
+  }
+  if (warp == 2) { ptx::tmem_alloc_2cta(tmem_slot, 512); ptx::tmem_relinquish_2cta(); }
+  ptx::tc_fence_before();
+  ptx::cluster_sync();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot_ptr, 0);
+
+  auto tile_of = [&](int t, int& prob, int& mt, int& nt) {     // mt counts 256-row pair tiles
+    prob = (P.n_probs > 1 && t >= P.p[1].tile_start) ? 1 : 0;
+    const NvProblem& q = P.p[prob];
+    t -= q.tile_start;
+    const int per_group = 2 * q.n_tiles, g = t / per_group, first_m = 2 * g;
+    const int gm = min(2, q.m_tiles - first_m), r = t - g * per_group;
+    mt = first_m + r % gm;
+    nt = r / gm;
+  };
+
+  if (warp == 0) {
+    // ===================== TMA producer (both CTAs) =====================
+    if (ptx::elect_one()) {
+      int stage = 0; uint32_t phase = 0;
+      const uint64_t pol_a = ptx::l2_policy(P.l2_a), pol_w = ptx::l2_policy(P.l2_w);
+      for (int t = pair_id; t < P.total_tiles; t += n_pairs) {
+        int prob, mt, nt;
+        tile_of(t, prob, mt, nt);
+        const NvProblem& q = P.p[prob];
+        const NvPairMaps* M = prob ? &m1 : &m0;
+        const int ka = q.k_blocks * 4;                              // K / 64 atoms per 128 rows
+        const int row0 = mt * PAIR_M + (int)rank * BLOCK_M;         // this CTA's A rows
+        const int n0 = nt * BN;
+        const int atom0 = n0 >> 7, atom1 = min(atom0 + 1, ((q.N + 127) >> 7) - 1);
+        const int a_atom = (mt * 2 + (int)rank) * ka;
+        for (int kb = 0; kb < q.k_blocks; ++kb) {
+          ptx::mbar_wait(empty_bar(stage), phase ^ 1);
+          const uint32_t leader_full = ptx::map_to_cta(full_bar(stage), 0);
+          const uint32_t sa = smem_base + stage * STAGE_BYTES;
+          ptx::tma_load_2d_2cta_hint(sa, &M->a, leader_full, kb * 128, row0, pol_a);
+          ptx::tma_load_2d_2cta_hint(sa + OFF_W, &M->w, leader_full, kb * 128, n0 + (int)rank * HALF_BN, pol_w);
+          // scale-factor atoms: rows of 256 bytes, two per atom, four atoms (one K block) per load
+          ptx::tma_load_2d_2cta(sa + OFF_SFA, &M->sfa, leader_full, 0, 2 * (a_atom + kb * 4));
+          ptx::tma_load_2d_2cta(sa + OFF_SFB, &M->sfw, leader_full, 0, 2 * (atom0 * ka + kb * 4));
+          ptx::tma_load_2d_2cta(sa + OFF_SFB + SFA_BYTES, &M->sfw, leader_full, 0, 2 * (atom1 * ka + kb * 4));
+          if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2 * STAGE_BYTES);   // the leader arms for both CTAs
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== scale-factor copies + MMA issue (leader only; the peer runs the loop over zero tiles) =====================
+    if (ptx::elect_one()) {
+      const int my_tiles = rank == 0 ? P.total_tiles : 0;
+      constexpr uint32_t idesc = ptx::make_idesc_nvfp4(PAIR_M, BN);
+      int stage = 0, slot = 0, acc = 0;
+      uint32_t phase = 0, acc_phase = 0;
+      for (int t = pair_id; t < my_tiles; t += n_pairs) {
+        int prob, mt, nt;
+        tile_of(t, prob, mt, nt);
+        const int k_blocks = P.p[prob].k_blocks;
+        const uint32_t sfb_off = (uint32_t)(((nt * BN) & 127) >> 5);
+        ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + acc * BN;
+        for (int kb = 0; kb < k_blocks; ++kb) {
+          ptx::mbar_wait(full_bar(stage), phase);
+          ptx::tc_fence_after();
+          const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + OFF_W;
+          const uint32_t tsf = tmem_base + TM_SF + slot * SF_COLS_PER_SLOT;
+#pragma unroll
+          for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+            const uint32_t sfa_t = tsf + k * 12, sfb_t = sfa_t + 4;
+            ptx::tmem_cp_32x128b_warpx4_2cta(sfa_t, ptx::make_smem_desc_noswizzle(sa + OFF_SFA + k * 512, 128, 128));
+            ptx::tmem_cp_32x128b_warpx4_2cta(sfb_t, ptx::make_smem_desc_noswizzle(sa + OFF_SFB + k * 512, 128, 128));
+            ptx::tmem_cp_32x128b_warpx4_2cta(sfb_t + 4, ptx::make_smem_desc_noswizzle(sa + OFF_SFB + SFA_BYTES + k * 512, 128, 128));
+            ptx::mma_nvfp4_ss_2cta(d_tmem, ptx::make_smem_desc(sa + k * 32, 16, 1024), ptx::make_smem_desc(sb + k * 32, 16, 1024), idesc,
+                                   sfa_t, sfb_t + sfb_off, (kb | k) ? 1u : 0u);
+          }
+          ptx::mma_commit_2cta(empty_bar(stage));
+          if (kb == k_blocks - 1) ptx::mma_commit_2cta(tfull_bar(acc));
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          if (++slot == 2) slot = 0;
+        }
+        if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue (both CTAs, own 128 rows = own tensor-memory lanes) =====================
+    // EPI_WARPS / 4 warps per lane quarter, (BN / 32) / (EPI_WARPS / 4) 32-column chunks each: behind a mainloop that needs ~100 cycles per K = 64 step the
+    // epilogue sets the pace (measured with the epilogue switched off: fc1 0.254 ms, fc2 0.242 ms against 0.458 / 0.348 ms
+    // with four warps and per-thread residual updates; now 0.388 ms for the fused fc1 and 0.301 ms for fc2; twelve warps
+    // change nothing, and of fc1's remaining 0.13 ms the stores are 0.01, GELU 0.035 and the quantiser 0.03 ms).  EPI_GATE_RES leaves through shared memory and
+    // cp.reduce.async.bulk.tensor.add.f32 as in gemm_tcgen05_v3.cu: a thread owns a row, so its 16-byte global accesses
+    // touched 32 rows per instruction and kept the SM's request path to L2 70 % busy (ncu), in the way of the TMA loads.
+    const int q4 = warp & 3, half = (warp - 4) >> 2;
+    constexpr int CH = (BN / 32) / (EPI_WARPS / 4);            // 32-column chunks per warp
+    const int ch_lo = half * CH, ch_hi = ch_lo + CH;
+    const uint32_t stg = smem_base + OFF_STG + (uint32_t)(warp - 4) * STG_BYTES, row_off = (uint32_t)lane * 128, sw = (uint32_t)lane & 7;
+    const uint64_t pol_o = ptx::l2_policy(2);
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    for (int t = pair_id; t < P.total_tiles; t += n_pairs) {
+      int prob, mt, nt;
+      tile_of(t, prob, mt, nt);
+      const NvProblem& q = P.p[prob];
+      const int row0 = mt * PAIR_M + (int)rank * BLOCK_M + q4 * 32;       // first row of this warp
+      ptx::mbar_wait(tfull_bar(acc), acc_phase);
+      ptx::tc_fence_after();
+      const uint32_t taddr0 = tmem_base + acc * BN + ((uint32_t)(q4 * 32) << 16);
+      if (EPI == EPI_GATE_RES) {
+        const CUtensorMap* mR = prob ? &m1.resid : &m0.resid;
+#pragma unroll 1
+        for (int ch = ch_lo; ch < ch_hi; ++ch) {
+          const int n0 = nt * BN + ch * 32;
+          float y[32];
+          load_chunk<BN>(q, nt, taddr0, ch, y);
+          const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
+          ptx::bulk_wait_read<0>();                          // the TMA engine has read the previous chunk out of the buffer
+          __syncwarp();
+#pragma unroll
+          for (int g = 0; g < 8; ++g) {
+            const float4 gt = __ldg(gp + g);
+            st_shared_v4(stg + row_off + (((uint32_t)g ^ sw) << 4), __float_as_uint(gt.x * y[4 * g]), __float_as_uint(gt.y * y[4 * g + 1]),
+                         __float_as_uint(gt.z * y[4 * g + 2]), __float_as_uint(gt.w * y[4 * g + 3]));
+          }
+          ptx::fence_proxy_async_smem();
+          __syncwarp();
+          if (ptx::elect_one()) {                             // the same lane every time: it owns the bulk groups
+            ptx::tma_reduce_add_2d_hint(mR, stg, n0, row0, pol_o);
+            ptx::bulk_commit();
+          }
+        }
+      } else {
+        epilogue_tile<EPI, BN>(q, nt, (long long)row0 + lane, taddr0, ch_lo, ch_hi);
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive_cluster(ptx::map_to_cta(tempty_bar(acc), 0));
+      if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+    }
+    ptx::bulk_wait<0>();                                      // every reduction of this warp has completed
+  }
+
+  ptx::tc_fence_before();
+  ptx::cluster_sync();                                      // nobody of the pair still uses tensor memory or remote barriers
+  if (warp == 2) { ptx::tc_fence_after(); ptx::tmem_dealloc_2cta(tmem_base, 512); }
 }
 
 }  // namespace
@@ -311,6 +506,64 @@ cudaError_t launch_bn(int epi, const CUtensorMap* tm, const NvParams& P, int gri
   }
 }
 
+
+template <int EPI>
+cudaError_t launch_pair_one(const NvPairMaps* maps, const NvParams& P, int grid, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    SPOT_CUDA_TRY(cudaFuncSetAttribute(gemm_nvfp4_pair_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pair::SMEM_BYTES));
+    attr_set = true;
+  }
+  gemm_nvfp4_pair_kernel<EPI><<<grid, pair::THREADS, pair::SMEM_BYTES, st>>>(maps[0], maps[1], P);
+  return cudaGetLastError();
+}
+
+// CTA-pair launch: every problem has M % 256 == 0 and N % 192 == 0
+cudaError_t launch_pair(int e, const Nvfp4Problem* probs, int n_probs, NvParams P, int num_sms, cudaStream_t st) {
+  NvPairMaps maps[2];
+  memset(maps, 0, sizeof(maps));
+  int tiles = 0, np = 0;
+  for (int i = 0; i < n_probs; ++i) {
+    const Nvfp4Problem& g = probs[i];
+    if (g.M == 0) continue;
+    NvProblem& q = P.p[np];
+    q.m_tiles = g.M / pair::PAIR_M; q.n_tiles = g.N / pair::BN; q.k_blocks = g.K / BLOCK_K; q.tile_start = tiles; q.M = g.M; q.N = g.N;
+    q.sfa = (const uint8_t*)g.a_sf; q.sfw = (const uint8_t*)g.w_sf; q.w_scale = g.w_scale; q.bias = (const bf16*)g.bias;
+    q.out = (bf16*)g.out; q.out_sf = (uint8_t*)g.out_sf; q.gate = g.gate; q.resid = g.resid;
+    tiles += q.m_tiles * q.n_tiles;
+    const uint64_t adims[2] = {(uint64_t)g.K / 2, (uint64_t)g.M}, wdims[2] = {(uint64_t)g.K / 2, (uint64_t)g.N};
+    const uint64_t str[1] = {(uint64_t)g.K / 2};
+    const uint32_t abox[2] = {128, BLOCK_M}, wbox[2] = {128, (uint32_t)pair::HALF_BN};
+    SPOT_CUDA_TRY(spot_make_tmap_u8(&maps[np].a, g.a_codes, 2, adims, str, abox));
+    SPOT_CUDA_TRY(spot_make_tmap_u8(&maps[np].w, g.w_codes, 2, wdims, str, wbox));
+    // scale-factor atoms (512 bytes each, [rows / 128][K / 64]) as rows of 256 bytes; a box = 4 atoms = one K block
+    const uint64_t ka = (uint64_t)g.K / 64;
+    const uint64_t sadims[2] = {256, 2 * (uint64_t)(g.M / 128) * ka}, swdims[2] = {256, 2 * (uint64_t)((g.N + 127) / 128) * ka};
+    const uint64_t sstr[1] = {256};
+    const uint32_t sbox[2] = {256, 8};
+    SPOT_CUDA_TRY(spot_make_tmap_u8_linear(&maps[np].sfa, g.a_sf, 2, sadims, sstr, sbox));
+    SPOT_CUDA_TRY(spot_make_tmap_u8_linear(&maps[np].sfw, g.w_sf, 2, swdims, sstr, sbox));
+    if (g.resid) {                                  // fp32 residual [M, N]: boxes of 32 rows x 32 columns (128 bytes, swizzled)
+      const uint64_t rdims[2] = {(uint64_t)g.N, (uint64_t)g.M}, rstr[1] = {(uint64_t)g.N * 4};
+      const uint32_t rbox[2] = {32, 32};
+      SPOT_CUDA_TRY(spot_make_tmap_f32(&maps[np].resid, g.resid, 2, rdims, rstr, rbox));
+    }
+    ++np;
+  }
+  if (np == 0) return cudaSuccess;
+  if (np == 1) maps[1] = maps[0];
+  P.n_probs = np;
+  P.total_tiles = tiles;
+  const int pairs = num_sms / 2;
+  const int grid = 2 * (tiles < pairs ? tiles : pairs);
+  switch (e) {
+    case EPI_BIAS: return launch_pair_one<EPI_BIAS>(maps, P, grid, st);
+    case EPI_BIAS_GELU: return launch_pair_one<EPI_BIAS_GELU>(maps, P, grid, st);
+    case EPI_GATE_RES: return launch_pair_one<EPI_GATE_RES>(maps, P, grid, st);
+    default: return launch_pair_one<EPI_GELU_NVFP4>(maps, P, grid, st);
+  }
+}
+
 }  // namespace
 
 // epi = EPI_BIAS_GELU with out_sf != NULL in every problem selects the fused GELU -> NVFP4 epilogue (out = codes [M, N / 2]).
@@ -337,6 +590,19 @@ cudaError_t launch_gemm_nvfp4(Epilogue epi, const Nvfp4Problem* probs, int n_pro
     static int hint = -1;
     if (hint < 0) { const char* e = getenv("SPOT_NVFP4_L2_HINT"); hint = e ? atoi(e) : 11; }
     P.l2_a = hint / 10; P.l2_w = hint % 10;
+  }
+  {
+    // CTA pairs (256 x 192 tiles) wherever the shapes allow; SPOT_NVFP4_IMPL = 1 keeps the one-CTA kernel (A/B timing only)
+    static int impl = -1;
+    if (impl < 0) { const char* e = getenv("SPOT_NVFP4_IMPL"); impl = e ? atoi(e) : 0; }
+    bool pair_ok = bn192 && impl != 1;
+    for (int i = 0; i < n_probs; ++i) {
+      const Nvfp4Problem& g = probs[i];
+      if (g.M == 0) continue;
+      if ((epi == EPI_GATE_RES) != (g.resid != nullptr) || (epi != EPI_GATE_RES && !g.out)) return cudaErrorInvalidValue;
+      if (g.M % pair::PAIR_M) pair_ok = false;
+    }
+    if (pair_ok) return launch_pair(fused ? EPI_GELU_NVFP4 : (int)epi, probs, n_probs, P, num_sms, st);
   }
   CUtensorMap tm[4];
   memset(tm, 0, sizeof(tm));

@@ -229,7 +229,7 @@ spot_encode_tiled_fn spot_get_encode_tiled() {
 }
 
 static cudaError_t make_tmap(CUtensorMap* out, CUtensorMapDataType dt, const void* base, int rank, const uint64_t* dims,
-                             const uint64_t* strides_bytes, const uint32_t* box) {
+                             const uint64_t* strides_bytes, const uint32_t* box, bool swizzle = true) {
   spot_encode_tiled_fn enc = spot_get_encode_tiled();
   if (!enc) return cudaErrorNotSupported;
   cuuint64_t gdim[5], gstr[5];
@@ -237,7 +237,8 @@ static cudaError_t make_tmap(CUtensorMap* out, CUtensorMapDataType dt, const voi
   for (int i = 0; i < rank; ++i) { gdim[i] = dims[i]; bx[i] = box[i]; es[i] = 1; }
   for (int i = 0; i + 1 < rank; ++i) gstr[i] = strides_bytes[i];
   CUresult r = enc(out, dt, (cuuint32_t)rank, const_cast<void*>(base), gdim, gstr, bx, es,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
@@ -250,6 +251,11 @@ cudaError_t spot_make_tmap_bf16(CUtensorMap* out, const void* base, int rank, co
 cudaError_t spot_make_tmap_u8(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
                               const uint64_t* strides_bytes, const uint32_t* box) {
   return make_tmap(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, base, rank, dims, strides_bytes, box);
+}
+
+cudaError_t spot_make_tmap_u8_linear(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
+                                     const uint64_t* strides_bytes, const uint32_t* box) {
+  return make_tmap(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, base, rank, dims, strides_bytes, box, false);
 }
 
 cudaError_t spot_make_tmap_f32(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,

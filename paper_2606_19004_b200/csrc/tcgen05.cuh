@@ -228,6 +228,9 @@ cudaError_t spot_make_tmap_f32(CUtensorMap* out, const void* base, int rank, con
 // one-byte element tensor (E4M3 operands of the FP8 variant), 128-byte swizzle
 cudaError_t spot_make_tmap_u8(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
                               const uint64_t* strides_bytes, const uint32_t* box);
+// as spot_make_tmap_u8 without the 128-byte swizzle: the box lands in shared memory row after row (inner box <= 256 bytes)
+cudaError_t spot_make_tmap_u8_linear(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
+                                     const uint64_t* strides_bytes, const uint32_t* box);
 
 // ---- TMA stores (shared -> global through a tensor map), bulk async-groups ---------------------------------
 namespace ptx {
@@ -254,6 +257,12 @@ __device__ __forceinline__ void tma_reduce_add_3d_hint(const CUtensorMap* m, uin
   asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group.L2::cache_hint [%0, {%2, %3, %4}], [%1], %5;" ::"l"(
                    reinterpret_cast<uint64_t>(m)),
                "r"(src), "r"(c0), "r"(c1), "r"(c2), "l"(policy)
+               : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_2d_hint(const CUtensorMap* m, uint32_t src, int c0, int c1, uint64_t policy) {
+  asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group.L2::cache_hint [%0, {%2, %3}], [%1], %4;" ::"l"(
+                   reinterpret_cast<uint64_t>(m)),
+               "r"(src), "r"(c0), "r"(c1), "l"(policy)
                : "memory");
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
@@ -345,6 +354,19 @@ __device__ __forceinline__ void mma_f8_ss_2cta(uint32_t d_tmem, uint64_t a_desc,
       "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::2.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(d_tmem),
       "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// block-scaled E2M1 MMA and the scale-factor copy for a CTA pair: issued by the leader, each CTA reads ITS OWN shared memory
+// at the descriptor's offset (A rows / half of B's rows / scale factors) and writes ITS OWN tensor memory
+__device__ __forceinline__ void tmem_cp_32x128b_warpx4_2cta(uint32_t taddr, uint64_t sdesc) {
+  asm volatile("tcgen05.cp.cta_group::2.32x128b.warpx4 [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+__device__ __forceinline__ void mma_nvfp4_ss_2cta(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t sfa,
+                                                  uint32_t sfb, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::mxf4nvf4.block_scale.block16 [%0], %1, %2, %3, [%5], [%6], p;\n\t}\n" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(sfa), "r"(sfb)
       : "memory");
 }
 // arrive on the barrier at the same shared-memory offset in both CTAs of the pair once all prior MMAs are done

@@ -80,11 +80,12 @@ def _linear_case(M, N, K, tid, epi):
 
 @pytest.mark.parametrize("epi", [0, 1, 2])
 @pytest.mark.parametrize("M,N,K", [(128, 256, 256), (256, 512, 1024), (384, 256, 3072), (1280, 768, 512), (256, 384, 512),
-                                   (512, 3072, 768)])
+                                   (512, 3072, 768), (384, 768, 512), (128, 384, 2048), (768, 384, 3072)])
 def test_linear_nvfp4(epi, M, N, K):
     """kind::mxf4nvf4 block-scaled GEMM vs the oracle on the SAME codes: single tile, several K blocks (ring wrap), several
-    tiles per CTA; N = 256 / 512 take the 128 x 256 tiles (one accumulator), N = 768 / 384 / 3072 the 128 x 192 tiles (two
-    accumulators; odd tiles start 64 rows into a scale atom).  fp32 accumulation of exactly representable products; bf16
+    tiles per CTA; N = 256 / 512 take the 128 x 256 tiles (one accumulator), N = 768 / 384 / 3072 the 192-column tiles
+    (two accumulators; odd tiles start 64 rows into a scale atom): CTA pairs on 256 x 192 where M is a multiple of 256
+    (M = 256, 512, 768, 1280), the one-CTA 128 x 192 kernel otherwise (M = 384, 128).  fp32 accumulation of exactly representable products; bf16
     outputs add one rounding."""
     got, ref, exact = _linear_case(M, N, K, 1110, epi)
     err = rel_l2(got, ref)
