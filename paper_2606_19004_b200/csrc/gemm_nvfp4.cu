@@ -78,20 +78,24 @@ __device__ __forceinline__ float gelu_tanh_fast(float x) {
   return fmaf(hx, th, hx);
 }
 
-// y[j] = acc[r, ch * 32 + j] * s_n + b_n for one 32-column chunk of the thread's accumulator row
+// y[j] = acc[r, ch * 32 + j] * s_n + b_n for one 32-column chunk of the thread's accumulator row.  The tensor-memory load
+// of the NEXT chunk is issued as soon as this chunk's values have left v (chunk_finish), so its latency - several hundred
+// cycles while the MMAs of the next tile keep tensor memory busy - runs under the arithmetic of this chunk.
+__device__ __forceinline__ void chunk_issue(uint32_t taddr0, int ch, uint32_t (&v)[32]) { ptx::tmem_ld_32x32(taddr0 + ch * 32, v); }
 template <int BN>
-__device__ __forceinline__ void load_chunk(const NvProblem& q, int nt, uint32_t taddr0, int ch, float* y) {
+__device__ __forceinline__ void chunk_finish(const NvProblem& q, int nt, int ch, const uint32_t* v, float* y) {
   const int n0 = nt * BN + ch * 32;
-  uint32_t v[32];
-  ptx::tmem_ld_32x32(taddr0 + ch * 32, v);
-  ptx::tmem_ld_wait();
   const uint4* bp = reinterpret_cast<const uint4*>(q.bias + n0);
   const float4* sp = reinterpret_cast<const float4*>(q.w_scale + n0);
+  uint4 braw[4];
+  float4 sraw[8];
+#pragma unroll
+  for (int g = 0; g < 4; ++g) { braw[g] = __ldg(bp + g); sraw[2 * g] = __ldg(sp + 2 * g); sraw[2 * g + 1] = __ldg(sp + 2 * g + 1); }
+  ptx::tmem_ld_wait();
 #pragma unroll
   for (int g = 0; g < 4; ++g) {
-    const uint4 braw = __ldg(bp + g);
-    const bf16* bb = reinterpret_cast<const bf16*>(&braw);
-    const float4 s0 = __ldg(sp + 2 * g), s1 = __ldg(sp + 2 * g + 1);
+    const bf16* bb = reinterpret_cast<const bf16*>(&braw[g]);
+    const float4 s0 = sraw[2 * g], s1 = sraw[2 * g + 1];
     const float sc[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
 #pragma unroll
     for (int j = 0; j < 8; ++j) y[g * 8 + j] = fmaf(__uint_as_float(v[g * 8 + j]), sc[j], __bfloat162float(bb[j]));
@@ -103,11 +107,14 @@ __device__ __forceinline__ void load_chunk(const NvProblem& q, int nt, uint32_t 
 // warps per lane quarter, half of the chunks each).
 template <int EPI, int BN>
 __device__ __forceinline__ void epilogue_tile(const NvProblem& q, int nt, long long r, uint32_t taddr0, int ch_lo, int ch_hi) {
+  uint32_t v[32];
+  chunk_issue(taddr0, ch_lo, v);
 #pragma unroll 1
   for (int ch = ch_lo; ch < ch_hi; ++ch) {
     const int n0 = nt * BN + ch * 32;
     float y[32];
-    load_chunk<BN>(q, nt, taddr0, ch, y);
+    chunk_finish<BN>(q, nt, ch, v, y);
+    if (ch + 1 < ch_hi) chunk_issue(taddr0, ch + 1, v);
     if (EPI == EPI_GATE_RES) {
       float4* rp = reinterpret_cast<float4*>(q.resid + r * q.N + n0);
       const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
@@ -439,11 +446,14 @@ gemm_nvfp4_pair_kernel(const __grid_constant__ NvPairMaps m0, const __grid_const
       const uint32_t taddr0 = tmem_base + acc * BN + ((uint32_t)(q4 * 32) << 16);
       if (EPI == EPI_GATE_RES) {
         const CUtensorMap* mR = prob ? &m1.resid : &m0.resid;
+        uint32_t v[32];
+        chunk_issue(taddr0, ch_lo, v);
 #pragma unroll 1
         for (int ch = ch_lo; ch < ch_hi; ++ch) {
           const int n0 = nt * BN + ch * 32;
           float y[32];
-          load_chunk<BN>(q, nt, taddr0, ch, y);
+          chunk_finish<BN>(q, nt, ch, v, y);
+          if (ch + 1 < ch_hi) chunk_issue(taddr0, ch + 1, v);
           const float4* gp = reinterpret_cast<const float4*>(q.gate + n0);
           ptx::bulk_wait_read<0>();                          // the TMA engine has read the previous chunk out of the buffer
           __syncwarp();
