@@ -42,6 +42,13 @@ def test_option_constants_match_the_header():
         assert getattr(binding, name[len("SPOT_"):]) == value, name
 
 
+def test_static_scratch_limit_matches_the_header():
+    """binding.STATIC_PARTIALS_MAX is SPOT_STATIC_PARTIALS_MAX of include/spot_kernels.h (spot_euler_update_static)."""
+    text = open(os.path.join(ROOT, "include", "spot_kernels.h")).read()
+    m = re.search(r"#define\s+SPOT_STATIC_PARTIALS_MAX\s+(\d+)", text)
+    assert m and int(m.group(1)) == binding.STATIC_PARTIALS_MAX == 65536
+
+
 def _cfg_struct(s, **over):
     kw = dict(n_blocks=s.n_blocks, hidden=s.hidden, n_heads=s.n_heads, head_dim=s.head_dim, mlp_hidden=s.mlp_hidden,
               grid_h=s.grid_h, grid_w=s.grid_w, n_txt=s.n_txt, latent_ch=s.latent_ch, txt_dim=s.txt_dim,
