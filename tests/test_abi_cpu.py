@@ -93,6 +93,12 @@ def test_kernel_calls_reject_bad_arguments(lib):
     assert lib.spot_ln_modulate(0, p, 4, 100, p, p, 1e-6, p, None) == 2                # D % 128
     assert lib.spot_attention(0, 0, p, p, 1, 8, 1, 48, None) == 2                      # head_dim
     assert lib.spot_euler_update(p, p, 0.1, 1, 6, None, None, None, None) == 2
+    f = lib.spot_euler_update_static                                                  # the no-allocation variant (static scratch)
+    assert f(p, p, 0.1, 1, 6, p, p, None) == 2                                         # elems % 4
+    assert f(p, p, 0.1, 70000, 8, p, p, None) == 2                                     # sequences ride on gridDim.y
+    assert f(p, p, 0.1, 1, 8, None, p, None) == 1                                      # probe and rewards are required
+    assert f(p, p, 0.1, 40000, 8192, p, p, None) == 5                                  # 80000 partial sums > 65536: rejected before any launch
+    assert f(p, p, 0.1, 0, 8, p, p, None) == 0
     if not torch.cuda.is_available():
         assert lib.spot_ln_modulate(0, p, 4, 128, p, p, 1e-6, p, None) == 6
 
