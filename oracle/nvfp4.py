@@ -78,6 +78,14 @@ def linear_nvfp4(x: Array, wq: Array, wsf: Array, s: Array, b: Array) -> Array:
     return (dequantize(xq, xsf) @ dequantize(wq, wsf).T) * s + b
 
 
+def linear_nvfp4_deq(x: Array, w_deq: Array, s: Array, b: Array) -> Array:
+    """linear_nvfp4 with dequantize(wq, wsf) formed once by the caller (tests/golden/make_cfg3_golden.py keeps it per block:
+    an E2M1 value times an E4M3 scale has a 5-bit significand, so even a bf16 copy holds it exactly).  Same arithmetic, same
+    result bit for bit (pinned in tests/test_oracle_nvfp4.py)."""
+    xq, xsf = quantize_rows(x)
+    return (dequantize(xq, xsf) @ w_deq.T) * s + b
+
+
 MLP_LINEARS = ("fc1", "fc2")
 
 

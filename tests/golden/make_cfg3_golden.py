@@ -6,6 +6,7 @@ path.  Cost: ~40 min to generate the 20.4 G weights on 8 cores + ~15 min of fp64
     python tests/golden/make_cfg3_golden.py [--blocks L] [--steps T] [--seed S] [--out NAME]
     python tests/golden/make_cfg3_golden.py --config 5 --prompt 7 --seed 229 --out cfg5_p7     (config 5, prompt 7)
     python tests/golden/make_cfg3_golden.py --precision fp8 --out cfg3_seed0_fp8               (FP8 variant, oracle/fp8.py)
+    python tests/golden/make_cfg3_golden.py --precision nvfp4 --out cfg3_seed0_nvfp4 --workers 8 (NVFP4 variant, oracle/nvfp4.py)
     python tests/golden/make_cfg3_golden.py --config 4 --seed 0 --out cfg4_seed0 --weight-cache /tmp/spot_weights
     python tests/golden/make_cfg3_golden.py --config 5 --prompt 7 --seeds 224:240 --out cfg5_p7_a --weight-cache /tmp/spot_weights
 
@@ -24,7 +25,7 @@ import torch
 ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 sys.path.insert(0, ROOT)
 
-from oracle import fp8, mmdit, philox, rollout  # noqa: E402
+from oracle import fp8, mmdit, nvfp4, philox, rollout  # noqa: E402
 from synth import CONFIGS, make_probe, make_text_emb, tensor_checksum  # noqa: E402
 from synth.manifest import make_block_weights, make_global_weights  # noqa: E402
 
@@ -65,6 +66,45 @@ class BlockSource:
         return bw
 
 
+def nvfp4_prepare_block(bw, cache_dir, b):
+    """Reading N1 for one block: fc1 / fc2 quantised with oracle/nvfp4.py and kept DEQUANTISED in bf16 (exact: an E2M1 value
+    times an E4M3 scale has a 5-bit significand) with their fp64 channel scales; qkv / out quantised with oracle/fp8.py and
+    kept as 1-byte E4M3 tensors.  The bf16 copies of the eight Linears are dropped.  With a cache directory the result is
+    stored there (written by --prep-workers processes ahead of the rollout)."""
+    f = os.path.join(cache_dir, f"nv_block{b:02d}.pt") if cache_dir else None
+    if f and os.path.exists(f):
+        small, q = torch.load(f, weights_only=True)
+        return small, q
+    bw = dict(bw)
+    q = {}
+    for st in ("img", "txt"):
+        for ln in fp8.BLOCK_LINEARS:
+            wfull = np64(bw.pop(f"{st}.{ln}_w"))
+            if ln in nvfp4.MLP_LINEARS:
+                wq, wsf, sc = nvfp4.quantize_weight(wfull)
+                q[f"{st}.{ln}"] = (torch.from_numpy(nvfp4.dequantize(wq, wsf)).to(torch.bfloat16), torch.from_numpy(sc))
+            else:
+                wq, sc = fp8.quantize_weight(wfull)
+                q[f"{st}.{ln}"] = (torch.from_numpy(wq).to(torch.float8_e4m3fn), torch.from_numpy(sc))
+    small = {k: v.clone() for k, v in bw.items()}
+    if f:
+        torch.save((small, q), f + ".tmp")
+        os.replace(f + ".tmp", f)
+    return small, q
+
+
+def _prep_worker(args):
+    config, n_blocks, cache_dir, b = args
+    torch.set_num_threads(2)
+    s = CONFIGS[config]
+    if n_blocks is not None:
+        s = s.with_(n_blocks=n_blocks)
+    src = BlockSource(s, cache_dir, keep_in_ram=False)
+    bw = src.get(b)                                        # generates + stores the bf16 block and its checksums
+    nvfp4_prepare_block(bw, cache_dir, b)
+    return b
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--blocks", type=int, default=None)
@@ -75,10 +115,13 @@ def main():
     ap.add_argument("--out", default="cfg3_seed0")
     ap.add_argument("--config", type=int, default=3, choices=[3, 4, 5])
     ap.add_argument("--prompt", type=int, default=0)
-    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp8"],
-                    help="fp8: the low-precision exploration variant as oracle/fp8.py states it (DESIGN.md section 13)")
+    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp8", "nvfp4"],
+                    help="fp8 / nvfp4: the low-precision exploration variants as oracle/fp8.py / oracle/nvfp4.py state them "
+                         "(DESIGN.md sections 13, 13b)")
     ap.add_argument("--workers", type=int, default=1, help="host threads: over the sequences with --seeds (BLAS is then "
                     "limited to one thread per call), else over attention heads / row blocks (oracle.mmdit.set_workers)")
+    ap.add_argument("--prep-workers", type=int, default=0, help="nvfp4 with --weight-cache: processes that generate and "
+                    "quantise the blocks ahead of the rollout")
     ap.add_argument("--weight-cache", default=None, help="directory (outside the repository) for the generated bf16 blocks")
     a = ap.parse_args()
     s = CONFIGS[a.config]
@@ -91,11 +134,20 @@ def main():
     here = os.path.dirname(os.path.abspath(__file__))
     t0 = time.time()
     gw = make_global_weights(s)
-    src = BlockSource(s, a.weight_cache, keep_in_ram=a.weight_cache is None or a.precision == "fp8")
+    lowp = a.precision in ("fp8", "nvfp4")
+    src = BlockSource(s, a.weight_cache, keep_in_ram=a.weight_cache is None or lowp)
     qblocks = {}
-    if a.weight_cache is None or a.precision == "fp8":
+    if a.precision == "nvfp4" and a.weight_cache and a.prep_workers > 1:
+        import multiprocessing as mp
+        with mp.get_context("spawn").Pool(a.prep_workers) as pool:
+            for b in pool.imap_unordered(_prep_worker, [(a.config, a.blocks, a.weight_cache, b) for b in range(s.n_blocks)]):
+                print(f"block {b} prepared ({time.time() - t0:.0f} s)", flush=True)
+    if a.weight_cache is None or lowp:
         for b in range(s.n_blocks):
             bw = src.get(b)
+            if a.precision == "nvfp4":
+                bw, qblocks[b] = nvfp4_prepare_block(bw, a.weight_cache, b)
+                src.ram[b] = bw
             if a.precision == "fp8":
                 # quantise once with the oracle's quantiser and keep the codes as 1-byte tensors (exact: the values are
                 # E4M3-representable); the bf16 copies of the four Linears are dropped (20 GB instead of 40.8 GB)
@@ -134,8 +186,17 @@ def main():
             return fp8.linear_fp8(x, wq8.to(torch.float64).numpy(), sc, np64(src.get(bi)[f"{name}_b"]))
         return lin
 
+    def nvfp4_lin(bi):                                     # the `lin` hook of oracle/nvfp4.py (block_lin), weights widened per call
+        def lin(x, name):
+            ent = qblocks[bi][name]
+            bias = np64(src.get(bi)[f"{name}_b"])
+            if name.split(".")[1] in nvfp4.MLP_LINEARS:
+                return nvfp4.linear_nvfp4_deq(x, ent[0].to(torch.float64).numpy(), ent[1].numpy(), bias)
+            return fp8.linear_fp8(x, ent[0].to(torch.float64).numpy(), ent[1].numpy(), bias)
+        return lin
+
     kw = dict(n_heads=s.n_heads, cos=cos, sin=sin, ln_eps=s.ln_eps, rms_eps=s.rms_eps,
-              block_lin=fp8_lin if a.precision == "fp8" else None)
+              block_lin=fp8_lin if a.precision == "fp8" else nvfp4_lin if a.precision == "nvfp4" else None)
 
     if a.workers > 1 and not multi:
         mmdit.set_workers(a.workers)

@@ -158,6 +158,50 @@ def test_cfg3_full_size_fp8_against_golden(full_model):
     assert rho >= 0.8                                              # PAPER.md:340 rank-fidelity criterion
 
 
+def test_cfg3_full_size_nvfp4_against_golden(full_model):
+    """The NVFP4 exploration variant (fc1 / fc2 on 4-bit block-scaled operands, QKV / out-proj in FP8) at config 3's full
+    size against oracle/nvfp4.py's result for one seed (tests/golden/cfg3_seed0_nvfp4*, written by make_cfg3_golden.py
+    --precision nvfp4).  Criterion N6: a 4-bit quantiser re-rounds every value near a code boundary
+    when its input moves, so the CUDA path is judged against the variant's OWN distance from the exact path - on x_T - x_0,
+    rel-L2(CUDA, oracle variant) < rel-L2(oracle variant, oracle bf16-weights path) - plus the rank criterion of
+    PAPER.md:340 against the bf16 rollout."""
+    s, w = full_model
+    meta, lat_ref = _load_golden("cfg3_seed0_nvfp4")
+    meta_bf, lat_exact = _load_golden("cfg3_seed0")
+    assert meta["precision"] == "nvfp4" and meta["n_blocks"] == s.n_blocks and meta["n_steps"] == s.n_steps
+    assert meta["seed"] == meta_bf["seed"]
+    text, probe = make_text_emb(s, "cuda"), make_probe(s, "cuda")
+    _check_weights(meta, w, text, probe)
+    ctx = spot.Context(s, w, max_seqs=s.n_seqs)
+    ts = f32_timesteps(s)
+    K = s.seeds_per_prompt
+    bf = spot.spot_explore(ctx, _seeds(s.seeds), text, ts, probe, 1, K, K // 2)
+    rew_bf = np64(bf["rewards"]).copy()
+    ctx.enable_nvfp4(True)
+    try:
+        out = spot.spot_explore(ctx, _seeds(s.seeds), text, ts, probe, 1, K, K // 2)
+        torch.cuda.synchronize()
+    finally:
+        ctx.enable_nvfp4(False)
+    i = list(s.seeds).index(meta["seed"])
+    x0 = _x0(s, meta["seed"])
+    got = np64(out["latents"][i])
+    d_cuda = rel_l2(got - x0, lat_ref - x0)                     # CUDA variant vs oracle variant, on what the model contributed
+    d_var = rel_l2(lat_ref - x0, lat_exact - x0)                # the variant's own distance from the exact path
+    rew = np64(out["rewards"])
+    scale = max(np.abs(rew).max(), 1e-30)
+    e_rew = abs(rew[i] - meta["reward"]) / scale
+    v_rew = abs(meta["reward"] - meta_bf["reward"]) / scale
+    rank = lambda a: np.argsort(np.argsort(a))
+    rho = np.corrcoef(rank(rew), rank(rew_bf))[0, 1]
+    print(f"cfg3 full size NVFP4, seed {meta['seed']}: x_T - x_0 rel-L2 vs nvfp4 oracle {d_cuda:.3e}, the oracle variant vs the exact "
+          f"path {d_var:.3e} (ratio {d_cuda / d_var:.2f}); latents rel-L2 {rel_l2(got, lat_ref):.3e}; reward {rew[i]:.6f} vs oracle "
+          f"{meta['reward']:.6f} ({e_rew:.3e} of the batch's reward scale; variant vs exact {v_rew:.3e}); Spearman with the bf16 "
+          f"rollout {rho:.3f}")
+    assert d_cuda < d_var                                        # criterion N6 for a rollout
+    assert rho >= 0.8                                             # PAPER.md:340 rank-fidelity criterion
+
+
 def test_cfg5_prompt_independence_and_golden(full_model):
     """Config 5 (8 prompts x 32 seeds): a prompt group inside the 256-sequence batch is bit-identical to the same
     group run alone; one seed of prompt 7 is compared with the stored oracle result when present."""

@@ -71,6 +71,12 @@ def test_weight_quantisation_and_linear():
         ref += (xq[:, sl] @ q[:, sl].T) * xsf[:, blk:blk + 1] * sf[:, blk][None, :]
     assert np.abs(y - (ref * s + b)).max() < 1e-12
     assert 0.08 < rel_l2(y - b, x @ w.T) < 0.2                             # one mantissa bit on both operands
+    # the form the full-size golden script uses: dequantised weights formed once, held EXACTLY by a bf16 copy
+    import torch
+    wd = nvfp4.dequantize(q, sf)
+    wd_bf16 = torch.from_numpy(wd).to(torch.bfloat16).to(torch.float64).numpy()
+    assert (wd_bf16 == wd).all()
+    assert (nvfp4.linear_nvfp4_deq(x, wd_bf16, s, b) == y).all()
 
 
 def test_block_nvfp4_is_close_and_mixed_with_fp8():
